@@ -1,0 +1,137 @@
+/* qe_hpsi.h -- C ABI of libqe_hpsi.so: H|psi> for plane-wave pseudopotential Kohn-Sham on one NVIDIA B200.
+ *
+ * What the library computes.  The paper (PAPER.md, arXiv:2104.10502) names the operation -- "Hamiltonian
+ * builds (i.e. the application of the one-particle Hamiltonian to molecular orbitals and Bloch states)",
+ * PAPER.md:L105 section III -- and its three terms -- "local-potential, pseudopotential, kinetic-energy
+ * contributions to the Hamiltonian", section III.C -- plus "generation of plane waves and of
+ * their mapping to FFT grids", PAPER.md:L176 (vi).  It prints no formula; BASELINE.json's north_star fixes
+ *
+ *     (H psi)(G) = |k+G|^2 psi(G) + sum_G' V(G-G') psi(G') + sum_a sum_ij beta_ai(G) D^a_ij <beta_aj|psi>
+ *
+ * in Rydberg atomic units (lengths bohr, energies Ry), with V(G-G') the 3-D DFT coefficient of the supplied
+ * real-space array V(r) at the cyclically wrapped index difference.  The library is a
+ * self-contained object with a flat API in the sense of PAPER.md:L112/L152/L156, callable as the external
+ * H builder of an iterative eigensolver; the caller owns streams and synchronisation
+ * (PAPER.md:L134-136).
+ *
+ * Conventions shared by all calls
+ *   - `at[9]`: lattice vectors a_1,a_2,a_3 as rows (row-major 3x3), bohr.  Reciprocal rows b_j, a_i.b_j = 2 pi d_ij.
+ *   - `xk[3]`: Cartesian k in bohr^-1.  `nr[3]`: FFT grid N1,N2,N3; every N_j must factor into 2,3,5.
+ *   - Miller triple n, G = sum n_j b_j; wrapped index i_j = n_j mod N_j; linear index idx = (i1*N2+i2)*N3+i3.
+ *   - The sphere {G : |k+G|^2 <= ecutwfc} (inclusive) is ordered by ASCENDING idx ("canonical order"); psi,
+ *     hpsi and beta rows are indexed by position ig in that order.
+ *   - complex128 = interleaved (re,im) doubles.  psi/hpsi: band-major [nbands][ld], beta: [nproj][ldbeta].
+ *   - psi(r) = sum_G c(G) exp(+i(k+G).r): sphere -> grid uses the un-normalised exp(+) DFT, grid -> sphere the
+ *     exp(-) DFT with 1/N.
+ *   - "dev" pointers are CUDA device pointers on the current device, "host" pointers ordinary host memory.
+ *   - Every function returns 0 (QE_HPSI_OK) or a negative qe_hpsi_status; none throws, aborts or exits.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns QE_HPSI_ECUDA.
+ */
+#ifndef QE_HPSI_H
+#define QE_HPSI_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qe_hpsi_handle* qe_hpsi_t;
+
+typedef enum {
+  QE_HPSI_OK = 0,
+  QE_HPSI_EINVAL = -1, /* null pointer, negative size, ld < npw, psi aliases hpsi, bad block table        */
+  QE_HPSI_EGRID = -2,  /* N_j has a prime factor other than 2,3,5, exceeds QE_HPSI_MAX_N, or is smaller  */
+                       /* than the sphere's index extent along j (the sphere itself would wrap)          */
+  QE_HPSI_ENOMEM = -3, /* host or device allocation failed                                               */
+  QE_HPSI_ECUDA = -4,  /* CUDA runtime error; the cudaError_t is returned by qe_hpsi_last_cuda_error     */
+  QE_HPSI_ESTATE = -5  /* handle is NULL / destroyed                                                     */
+} qe_hpsi_status;
+
+/* flags for qe_hpsi_create */
+#define QE_HPSI_BORROW_BETA 1u   /* use beta_dev in place (caller keeps it alive and unchanged) instead of copying */
+#define QE_HPSI_GENERIC_FFT 2u   /* (testing) use only radices 2,3,4,5 in the FFT passes                           */
+
+#define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */
+
+/* a0, stand-alone (PAPER.md:L176 (vi)).  Canonical sphere for a cell / k / cutoff / grid before any handle
+ * exists, so that the caller can lay out psi and beta.  Two-call pattern: with miller_host == NULL only
+ * *npw is written; otherwise miller_host[3*npw] (host, int32, triples n1,n2,n3 in canonical order) is filled
+ * and must hold at least 3 * (*npw as returned by the first call) entries.  Runs kernel a0 on the current
+ * device and synchronises. */
+int qe_hpsi_gsphere(const double at[9], const double xk[3], double ecutwfc, const int nr[3],
+                    int64_t* npw, int32_t* miller_host);
+
+/* Build a handle (once per k-point / potential update).
+ *   vr_dev     [N1][N2][N3] real FP64 local potential V(r) in Ry, i3 contiguous, r = sum (i_j/N_j) a_j.  COPIED
+ *              (pre-scaled by 1/N).
+ *   nproj      total number of projectors (0 allowed: kinetic + local only; beta/blocks then ignored).
+ *   beta_dev   complex128 [nproj][ldbeta], ldbeta >= npw, canonical G order.  Copied unless QE_HPSI_BORROW_BETA.
+ *   nblocks, blk_off_host[nblocks+1]   atoms: block a owns projectors blk_off[a] .. blk_off[a+1]-1;
+ *              blk_off[0] = 0, strictly increasing, blk_off[nblocks] = nproj.
+ *   d_host     the real symmetric D^a blocks packed one after another, block a row-major nh_a x nh_a
+ *              (nh_a = blk_off[a+1]-blk_off[a]), Ry.  COPIED.
+ *   max_batch  largest number of bands processed as one internal chunk (workspace is sized for it), >= 1.
+ *   cuda_stream  cudaStream_t (NULL = default stream) on which create's device work is enqueued; create
+ *              synchronises that stream before returning.
+ * On failure *out = NULL. */
+int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc, const double xk[3], const int nr[3],
+                   const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                   const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
+                   void* cuda_stream);
+
+/* The hot path (steps a1-a8 of DESIGN.md): hpsi[b][0..npw) = (H psi_b) for b < nbands.
+ *   psi_dev  [nbands][ldpsi] complex128 (read only), hpsi_dev [nbands][ldhpsi] complex128 (overwritten, not
+ *   accumulated; entries ig >= npw of each row untouched).  ldpsi, ldhpsi >= npw.  The two arrays must not
+ *   overlap.  Any nbands >= 0; internally processed in chunks of at most max_batch bands; the result for a
+ *   band does not depend on which other bands are in the call.
+ * Asynchronous: all work is enqueued on cuda_stream, no host synchronisation, no device->host traffic.  Only
+ * argument errors are reported synchronously.  One in-flight apply per handle (the workspace is shared). */
+int qe_hpsi_apply(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+                  void* cuda_stream);
+
+/* End-to-end variant with HOST buffers (pinned memory recommended): per internal chunk copies psi host->device,
+ * applies H, copies hpsi device->host, overlapping copies with compute on internal streams.  Returns after
+ * the last copy has completed (synchronous).  Same layouts and rules as qe_hpsi_apply. */
+int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldpsi, void* hpsi_host, int64_t ldhpsi,
+                       int nbands);
+
+/* Frees everything the handle owns.  NULL is a no-op.  The caller must have synchronised every stream that
+ * used the handle. */
+int qe_hpsi_destroy(qe_hpsi_t h);
+
+/* ---- accessors (needed for the bit-exact map check, the roofline report and diagnostics) ---- */
+int64_t qe_hpsi_npw(qe_hpsi_t h);            /* sphere size, or a negative status                               */
+int64_t qe_hpsi_nsticks(qe_hpsi_t h);        /* S: (i1,i2) columns holding >= 1 sphere point                    */
+int64_t qe_hpsi_nplanes(qe_hpsi_t h);        /* P: i1 planes holding >= 1 sphere point                          */
+/* Copies the device-built maps into caller DEVICE arrays (any may be NULL): miller [npw][3] int32,
+ * fft_index [npw] int32, g2kin [npw] float64.  Enqueued on cuda_stream. */
+int qe_hpsi_get_maps(qe_hpsi_t h, int32_t* miller_dev, int32_t* fftidx_dev, double* g2kin_dev, void* cuda_stream);
+/* Stage access for tests: becp = beta^H psi (a6) and dbecp = D becp (a7) of the LAST chunk applied, as
+ * complex128 [nproj][nb_last] band-contiguous, into caller DEVICE arrays (either may be NULL). */
+int qe_hpsi_get_becp(qe_hpsi_t h, void* becp_dev, void* dbecp_dev, void* cuda_stream);
+/* Number of kernel launches qe_hpsi_apply enqueues for nbands bands (for the benchmark's gpu_launches). */
+int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands);
+/* info[0..15]: npw, S, P, fft band chunk, split-K count, workspace bytes, then per axis j=0..2 the number of
+ * FFT passes, then zero padding.  For the roofline report. */
+int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);
+const char* qe_hpsi_strerror(int status);
+int qe_hpsi_last_cuda_error(qe_hpsi_t h);    /* cudaError_t of the last QE_HPSI_ECUDA (0 if none)               */
+
+/* Measurement helper (not on the hot path): runs register-resident FP64 DMMA (mma.sync m8n8k4.f64) and DFMA
+ * loops on every SM for about `millis` ms each and returns the achieved TFLOP/s.  bench.py uses the DMMA
+ * figure as the measured FP64 tensor peak of the box.  Synchronises the device. */
+int qe_hpsi_probe_fp64(double millis, double* dmma_tflops, double* dfma_tflops);
+
+/* Stand-alone stage entry points for tests and micro-benchmarks (same kernels the hot path launches):
+ *   qe_hpsi_fft_local: hpsi = g2kin*psi + local term only (a1-a5), ignoring projectors.
+ *   qe_hpsi_nonlocal:  hpsi += beta D beta^H psi (a6-a8) on top of the caller's hpsi contents. */
+int qe_hpsi_fft_local(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+                      void* cuda_stream);
+int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+                     void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QE_HPSI_H */

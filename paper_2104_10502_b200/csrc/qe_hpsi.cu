@@ -1,0 +1,1029 @@
+// qe_hpsi.cu -- C ABI of libqe_hpsi.so (include/qe_hpsi.h): handle, plan, G-sphere maps (a0) and the launch
+// sequence of the hot path (a1-a8).  No torch types, no cuFFT / cuBLAS: every step runs in this library's kernels.
+// PAPER.md:L105 (the operation), L224-226 (the three terms), L176 (vi) (sphere + FFT mapping); formulas and
+// readings: DESIGN.md sections 2-3.
+#include "../../include/qe_hpsi.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fft_kernels.cuh"
+#include "zgemm_kernels.cuh"
+
+using namespace qehpsi;
+
+namespace {
+
+constexpr double TWO_PI = 6.283185307179586;
+constexpr int NUM_SMS_FALLBACK = 148;
+
+// ZGEMM tile configuration (see zgemm_kernels.cuh)
+constexpr int ZG_BM = 128, ZG_BN = 64, ZG_WM = 4, ZG_WN = 2, ZG_NSTAGE = 4;
+constexpr int ZG_NT = ZG_WM * ZG_WN * 32;
+constexpr size_t BECP_SMEM = (size_t)ZG_NSTAGE * (ZG_BM + ZG_BN) * ZG_BK * sizeof(double2);
+constexpr size_t VNL_SMEM = (size_t)ZG_NSTAGE * (ZG_BK * (ZG_BM + 2) + ZG_BN * ZG_BK) * sizeof(double2);
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+};
+
+}  // namespace
+
+struct qe_hpsi_handle {
+  int device = 0;
+  int num_sms = NUM_SMS_FALLBACK;
+  int last_cuda = 0;
+  // geometry
+  int nr[3] = {0, 0, 0};
+  int ldz = 0;
+  int npw = 0, S = 0, P = 0;
+  // maps (device)
+  int* miller = nullptr;   // [npw][3]
+  int* fftidx = nullptr;   // [npw]
+  double* g2kin = nullptr; // [npw]
+  int *stick_start = nullptr, *stick_i2 = nullptr, *plane_stick = nullptr, *plane_i1 = nullptr, *pw_pos = nullptr;
+  double* vs = nullptr;    // V(r)/N  [N1][N2][ldz]
+  double2* tw[3] = {nullptr, nullptr, nullptr};
+  FftGeom geom{};
+  size_t smem_z = 0, smem_y = 0, smem_x = 0;
+  int fft_nb = 1;  // bands per FFT sub-chunk (workspace kept L2-sized)
+  int x_split = 1;
+  double2 *w1 = nullptr, *w2 = nullptr;
+  // nonlocal
+  int nproj = 0;
+  const double2* beta = nullptr;  // borrowed or owned
+  double2* beta_own = nullptr;
+  long long ldbeta = 0;
+  int *proj_blk0 = nullptr, *proj_nh = nullptr;
+  long long* proj_doff = nullptr;
+  double* dpk = nullptr;
+  int max_batch = 0;
+  int ldc = 0, ldp = 0;
+  int nsplit = 1, kchunk = 0;
+  double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
+  int nb_last = 0;
+  size_t workspace_bytes = 0;
+  // apply_host staging
+  double2* hbuf_psi[2] = {nullptr, nullptr};
+  double2* hbuf_h[2] = {nullptr, nullptr};
+  long long ldint = 0;
+  cudaStream_t st_in = nullptr, st_comp = nullptr, st_out = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+#define CU_TRY(h, expr)                                   \
+  do {                                                    \
+    cudaError_t e__ = (expr);                             \
+    if (e__ != cudaSuccess) {                             \
+      if (h) (h)->last_cuda = (int)e__;                   \
+      g_last_cuda = (int)e__;                             \
+      return QE_HPSI_ECUDA;                               \
+    }                                                     \
+  } while (0)
+
+int g_last_cuda = 0;
+
+// ---------------------------------------------------------------------------------------------------------
+// host geometry: reciprocal lattice and fractional k with a FIXED operation order so
+// that the sphere test is reproducible bit for bit (compiled with -ffp-contract=off on the host side)
+// ---------------------------------------------------------------------------------------------------------
+struct SphereGeom {
+  double b[3][3];
+  double kap[3];
+  double ecut;
+  int n1, n2, n3;
+};
+
+void host_recip(const double at[9], double b[3][3], double* vol) {
+  const double* a[3] = {at, at + 3, at + 6};
+  double c[3][3];
+  auto cross = [](const double* u, const double* v, double* o) {
+    o[0] = u[1] * v[2] - u[2] * v[1];
+    o[1] = u[2] * v[0] - u[0] * v[2];
+    o[2] = u[0] * v[1] - u[1] * v[0];
+  };
+  cross(a[1], a[2], c[0]);
+  cross(a[2], a[0], c[1]);
+  cross(a[0], a[1], c[2]);
+  volatile double t0 = a[0][0] * c[0][0], t1 = a[0][1] * c[0][1], t2 = a[0][2] * c[0][2];
+  volatile double s = t0 + t1;
+  *vol = s + t2;
+  for (int j = 0; j < 3; ++j)
+    for (int k = 0; k < 3; ++k) {
+      volatile double num = TWO_PI * c[j][k];
+      b[j][k] = num / *vol;
+    }
+}
+void host_kfrac(const double at[9], const double xk[3], double kap[3]) {
+  for (int j = 0; j < 3; ++j) {
+    volatile double t0 = at[3 * j] * xk[0], t1 = at[3 * j + 1] * xk[1], t2 = at[3 * j + 2] * xk[2];
+    volatile double s = t0 + t1;
+    volatile double s2 = s + t2;
+    kap[j] = s2 / TWO_PI;
+  }
+}
+
+bool factor_235(int n) {
+  if (n < 1) return false;
+  for (int p : {2, 3, 5})
+    while (n % p == 0) n /= p;
+  return n == 1;
+}
+
+// fewest passes, then smallest largest radix; radices sorted descending
+void plan_radices(int n, bool generic, std::vector<int>* best) {
+  static const int fast_set[] = {16, 12, 10, 9, 8, 6, 5, 4, 3, 2};
+  static const int gen_set[] = {5, 4, 3, 2};
+  const int* set = generic ? gen_set : fast_set;
+  const int nset = generic ? 4 : 10;
+  std::vector<int> cur;
+  best->clear();
+  bool have = false;
+  struct Rec {
+    const int* set;
+    int nset;
+    std::vector<int>* cur;
+    std::vector<int>* best;
+    bool* have;
+    void go(int rem, int maxr) {
+      if (rem == 1) {
+        bool better = !*have || cur->size() < best->size();
+        if (!better && cur->size() == best->size()) {
+          int mc = 0, mb = 0;
+          for (int r : *cur) mc = std::max(mc, r);
+          for (int r : *best) mb = std::max(mb, r);
+          better = mc < mb;
+        }
+        if (better) {
+          *best = *cur;
+          *have = true;
+        }
+        return;
+      }
+      if (*have && cur->size() + 1 > best->size()) return;
+      for (int i = 0; i < nset; ++i) {
+        int r = set[i];
+        if (r > maxr || rem % r) continue;
+        cur->push_back(r);
+        go(rem / r, r);
+        cur->pop_back();
+      }
+    }
+  } rec{set, nset, &cur, best, &have};
+  if (n == 1) return;
+  rec.go(n, 16);
+}
+
+// exp(+2 pi i k / n) in long double with exact quadrant reduction
+void host_twiddles(int n, std::vector<double2>* out) {
+  out->resize(n);
+  const long double pi = 3.14159265358979323846264338327950288L;
+  for (int k = 0; k < n; ++k) {
+    int q = (8 * k + n) / (2 * n);
+    int num = 4 * k - q * n;
+    long double d = pi * (long double)num / (long double)(2 * n);
+    long double c = num == 0 ? 1.0L : cosl(d), s = num == 0 ? 0.0L : sinl(d);
+    long double re, im;
+    switch (q & 3) {
+      case 0: re = c; im = s; break;
+      case 1: re = -s; im = c; break;
+      case 2: re = -c; im = -s; break;
+      default: re = s; im = -c; break;
+    }
+    (*out)[k] = make_double2((double)re, (double)im);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a0: sphere enumeration kernels.  Each CTA of 256 threads owns 1024 consecutive linear indices (4 per thread,
+// consecutive), so a block-ordered compaction keeps ascending idx = the canonical order.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int SPH_NT = 256, SPH_PER = 4;
+
+__device__ __forceinline__ int signed_idx(int i, int n) { return i >= (n + 1) / 2 ? i - n : i; }
+
+__device__ __forceinline__ bool sphere_test(const SphereGeom& g, long long idx, int m[3], double* q2out) {
+  const int i3 = (int)(idx % g.n3);
+  const long long t = idx / g.n3;
+  const int i2 = (int)(t % g.n2), i1 = (int)(t / g.n2);
+  m[0] = signed_idx(i1, g.n1);
+  m[1] = signed_idx(i2, g.n2);
+  m[2] = signed_idx(i3, g.n3);
+  const double x1 = __dadd_rn((double)m[0], g.kap[0]);
+  const double x2 = __dadd_rn((double)m[1], g.kap[1]);
+  const double x3 = __dadd_rn((double)m[2], g.kap[2]);
+  double q[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+    q[c] = __dadd_rn(__dadd_rn(__dmul_rn(x1, g.b[0][c]), __dmul_rn(x2, g.b[1][c])), __dmul_rn(x3, g.b[2][c]));
+  const double q2 = __dadd_rn(__dadd_rn(__dmul_rn(q[0], q[0]), __dmul_rn(q[1], q[1])), __dmul_rn(q[2], q[2]));
+  *q2out = q2;
+  return q2 <= g.ecut;
+}
+
+__global__ void __launch_bounds__(SPH_NT) k_sphere_count(SphereGeom g, long long ntot, int* __restrict__ counts) {
+  const long long base = ((long long)blockIdx.x * SPH_NT + threadIdx.x) * SPH_PER;
+  int cnt = 0;
+#pragma unroll
+  for (int e = 0; e < SPH_PER; ++e) {
+    int m[3];
+    double q2;
+    if (base + e < ntot && sphere_test(g, base + e, m, &q2)) ++cnt;
+  }
+  __shared__ int wsum[SPH_NT / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+  if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = cnt;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int s = 0;
+    for (int w = 0; w < SPH_NT / 32; ++w) s += wsum[w];
+    counts[blockIdx.x] = s;
+  }
+}
+
+__global__ void __launch_bounds__(SPH_NT) k_sphere_fill(SphereGeom g, long long ntot, const int* __restrict__ offsets,
+                                                        int* __restrict__ miller, int* __restrict__ fftidx,
+                                                        double* __restrict__ g2kin) {
+  const long long base = ((long long)blockIdx.x * SPH_NT + threadIdx.x) * SPH_PER;
+  int m[SPH_PER][3];
+  double q2[SPH_PER];
+  bool in[SPH_PER];
+  int cnt = 0;
+#pragma unroll
+  for (int e = 0; e < SPH_PER; ++e) {
+    in[e] = base + e < ntot && sphere_test(g, base + e, m[e], &q2[e]);
+    cnt += in[e] ? 1 : 0;
+  }
+  // exclusive scan of cnt over the block
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  __shared__ int wsum[SPH_NT / 32];
+  if (lane == 31) wsum[warp] = incl;
+  __syncthreads();
+  int woff = 0;
+  for (int w = 0; w < warp; ++w) woff += wsum[w];
+  int pos = offsets[blockIdx.x] + woff + incl - cnt;
+#pragma unroll
+  for (int e = 0; e < SPH_PER; ++e) {
+    if (in[e]) {
+      miller[3 * (size_t)pos + 0] = m[e][0];
+      miller[3 * (size_t)pos + 1] = m[e][1];
+      miller[3 * (size_t)pos + 2] = m[e][2];
+      fftidx[pos] = (int)(base + e);
+      g2kin[pos] = q2[e];
+      ++pos;
+    }
+  }
+}
+
+// V(r) -> V(r)/N in the padded [N1][N2][ldz] layout
+__global__ void k_scale_pad_v(const double* __restrict__ vr, double* __restrict__ vs, int n3, int ldz, long long rows,
+                              double scale) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= rows * ldz) return;
+  const long long r = i / ldz;
+  const int z = (int)(i - r * ldz);
+  vs[i] = z < n3 ? vr[r * n3 + z] * scale : 0.0;
+}
+
+struct SphereOut {
+  int npw = 0;
+  int* miller = nullptr;
+  int* fftidx = nullptr;
+  double* g2kin = nullptr;
+};
+
+void free_sphere(SphereOut* s) {
+  cudaFree(s->miller);
+  cudaFree(s->fftidx);
+  cudaFree(s->g2kin);
+  *s = SphereOut{};
+}
+
+int validate_grid(const double at[9], const double xk[3], double ecutwfc, const int nr[3], SphereGeom* sg) {
+  if (!at || !xk || !nr) return QE_HPSI_EINVAL;
+  if (!(ecutwfc >= 0.0) || !std::isfinite(ecutwfc)) return QE_HPSI_EINVAL;
+  double vol;
+  host_recip(at, sg->b, &vol);
+  if (!(std::fabs(vol) > 0.0) || !std::isfinite(vol)) return QE_HPSI_EINVAL;
+  host_kfrac(at, xk, sg->kap);
+  sg->ecut = ecutwfc;
+  sg->n1 = nr[0];
+  sg->n2 = nr[1];
+  sg->n3 = nr[2];
+  for (int j = 0; j < 3; ++j) {
+    if (nr[j] < 1 || nr[j] > QE_HPSI_MAX_N || !factor_235(nr[j])) return QE_HPSI_EGRID;
+    // |n_j + kappa_j| <= sqrt(ecut) |a_j| / 2 pi for every sphere point: the sphere must fit the box unwrapped
+    const double* a = at + 3 * j;
+    const double alen = std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+    const double ext = std::sqrt(ecutwfc) * alen / TWO_PI;
+    const int nmax = (int)std::floor(ext + std::fabs(sg->kap[j]) + 1e-9);
+    if (nr[j] < 2 * nmax + 1) return QE_HPSI_EGRID;
+  }
+  return QE_HPSI_OK;
+}
+
+int build_sphere(const SphereGeom& sg, cudaStream_t st, SphereOut* out) {
+  qe_hpsi_handle* h = nullptr;
+  const long long ntot = (long long)sg.n1 * sg.n2 * sg.n3;
+  const int nblk = (int)((ntot + SPH_NT * SPH_PER - 1) / (SPH_NT * SPH_PER));
+  int* d_counts = nullptr;
+  CU_TRY(h, cudaMalloc(&d_counts, sizeof(int) * (size_t)nblk));
+  k_sphere_count<<<nblk, SPH_NT, 0, st>>>(sg, ntot, d_counts);
+  std::vector<int> counts(nblk);
+  cudaError_t e = cudaMemcpyAsync(counts.data(), d_counts, sizeof(int) * (size_t)nblk, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) {
+    cudaFree(d_counts);
+    g_last_cuda = (int)e;
+    return QE_HPSI_ECUDA;
+  }
+  long long tot = 0;
+  for (int i = 0; i < nblk; ++i) {
+    int c = counts[i];
+    counts[i] = (int)tot;
+    tot += c;
+  }
+  out->npw = (int)tot;
+  const size_t n = (size_t)std::max<long long>(tot, 1);
+  e = cudaMalloc(&out->miller, sizeof(int) * 3 * n);
+  if (e == cudaSuccess) e = cudaMalloc(&out->fftidx, sizeof(int) * n);
+  if (e == cudaSuccess) e = cudaMalloc(&out->g2kin, sizeof(double) * n);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_counts, counts.data(), sizeof(int) * (size_t)nblk, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) {
+    k_sphere_fill<<<nblk, SPH_NT, 0, st>>>(sg, ntot, d_counts, out->miller, out->fftidx, out->g2kin);
+    e = cudaStreamSynchronize(st);
+  }
+  cudaFree(d_counts);
+  if (e != cudaSuccess) {
+    free_sphere(out);
+    g_last_cuda = (int)e;
+    return e == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA;
+  }
+  return QE_HPSI_OK;
+}
+
+template <typename T>
+cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t st) {
+  cudaError_t e = cudaMalloc(dst, sizeof(T) * std::max<size_t>(v.size(), 1));
+  if (e != cudaSuccess) return e;
+  if (!v.empty()) e = cudaMemcpyAsync(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice, st);
+  return e;
+}
+
+bool g_attr_done = false;
+cudaError_t set_kernel_attrs() {
+  if (g_attr_done) return cudaSuccess;
+  int dev = 0, optin = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+#define SET_SMEM(k)                                                                     \
+  e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);      \
+  if (e != cudaSuccess) return e;
+  SET_SMEM(k_scatter_zinv);
+  SET_SMEM(k_yinv);
+  SET_SMEM(k_x_vmul);
+  SET_SMEM(k_yfwd);
+  SET_SMEM(k_zfwd_gather);
+  SET_SMEM((k_becp<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE>));
+  SET_SMEM((k_vnl_add<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE>));
+#undef SET_SMEM
+  g_attr_done = true;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+// =========================================================================================================
+// C ABI
+// =========================================================================================================
+
+extern "C" const char* qe_hpsi_strerror(int status) {
+  switch (status) {
+    case QE_HPSI_OK: return "ok";
+    case QE_HPSI_EINVAL: return "invalid argument";
+    case QE_HPSI_EGRID: return "unsupported FFT grid (factors other than 2,3,5, too large, or smaller than the sphere)";
+    case QE_HPSI_ENOMEM: return "out of memory";
+    case QE_HPSI_ECUDA: return "CUDA error (see qe_hpsi_last_cuda_error)";
+    case QE_HPSI_ESTATE: return "invalid handle";
+    default: return "unknown status";
+  }
+}
+
+extern "C" int qe_hpsi_last_cuda_error(qe_hpsi_t h) { return h ? h->last_cuda : g_last_cuda; }
+
+extern "C" int qe_hpsi_gsphere(const double at[9], const double xk[3], double ecutwfc, const int nr[3], int64_t* npw,
+                               int32_t* miller_host) {
+  if (!npw) return QE_HPSI_EINVAL;
+  SphereGeom sg;
+  int rc = validate_grid(at, xk, ecutwfc, nr, &sg);
+  if (rc) return rc;
+  SphereOut so;
+  rc = build_sphere(sg, nullptr, &so);
+  if (rc) return rc;
+  *npw = so.npw;
+  if (miller_host && so.npw > 0) {
+    cudaError_t e = cudaMemcpy(miller_host, so.miller, sizeof(int) * 3 * (size_t)so.npw, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) {
+      free_sphere(&so);
+      g_last_cuda = (int)e;
+      return QE_HPSI_ECUDA;
+    }
+  }
+  free_sphere(&so);
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
+  if (!h) return QE_HPSI_OK;
+  cudaFree(h->miller);
+  cudaFree(h->fftidx);
+  cudaFree(h->g2kin);
+  cudaFree(h->stick_start);
+  cudaFree(h->stick_i2);
+  cudaFree(h->plane_stick);
+  cudaFree(h->plane_i1);
+  cudaFree(h->pw_pos);
+  cudaFree(h->vs);
+  for (int j = 0; j < 3; ++j) cudaFree(h->tw[j]);
+  cudaFree(h->w1);
+  cudaFree(h->w2);
+  cudaFree(h->beta_own);
+  cudaFree(h->proj_blk0);
+  cudaFree(h->proj_nh);
+  cudaFree(h->proj_doff);
+  cudaFree(h->dpk);
+  cudaFree(h->partial);
+  cudaFree(h->becp);
+  cudaFree(h->dbecp);
+  cudaFree(h->dbT);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(h->hbuf_psi[i]);
+    cudaFree(h->hbuf_h[i]);
+    if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+    if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
+    if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
+  }
+  if (h->st_in) cudaStreamDestroy(h->st_in);
+  if (h->st_comp) cudaStreamDestroy(h->st_comp);
+  if (h->st_out) cudaStreamDestroy(h->st_out);
+  delete h;
+  return QE_HPSI_OK;
+}
+
+namespace {
+
+int env_int(const char* name, int dflt) {
+  const char* s = std::getenv(name);
+  if (!s || !*s) return dflt;
+  return std::atoi(s);
+}
+
+// choose the split-K count of a6 so that (M tiles x N tiles x nsplit) fills whole waves of CTAs
+void choose_split(qe_hpsi_handle* h) {
+  const int ntile = ((h->nproj + ZG_BM - 1) / ZG_BM) * ((h->max_batch + ZG_BN - 1) / ZG_BN);
+  const int ksmax = std::max(1, h->npw / 512);
+  int best = 1;
+  double best_score = -1.0;
+  for (int ks = 1; ks <= std::min(ksmax, 1024); ++ks) {
+    const long long ctas = (long long)ntile * ks;
+    const long long waves = (ctas + h->num_sms - 1) / h->num_sms;
+    double eff = (double)ctas / (double)(waves * h->num_sms);
+    if (waves < 2) eff *= 0.5 + 0.25 * (double)ctas / h->num_sms;  // prefer at least two waves when K allows
+    const double score = eff - 1e-4 * ks;  // ties -> fewer splits (less partial traffic)
+    if (score > best_score) {
+      best_score = score;
+      best = ks;
+    }
+    if (waves >= 16 && eff > 0.97) break;
+  }
+  int kchunk = (h->npw + best - 1) / best;
+  kchunk = (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK;
+  if (kchunk < ZG_BK) kchunk = ZG_BK;
+  h->kchunk = kchunk;
+  h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+}
+
+}  // namespace
+
+extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc, const double xk[3], const int nr[3],
+                              const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                              const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
+                              void* cuda_stream) {
+  if (!out) return QE_HPSI_EINVAL;
+  *out = nullptr;
+  if (!vr_dev || nproj < 0 || max_batch < 1) return QE_HPSI_EINVAL;
+  SphereGeom sg;
+  int rc = validate_grid(at, xk, ecutwfc, nr, &sg);
+  if (rc) return rc;
+  long long d_total = 0;
+  if (nproj > 0) {
+    if (!beta_dev || !blk_off_host || !d_host || nblocks < 1) return QE_HPSI_EINVAL;
+    if (blk_off_host[0] != 0 || blk_off_host[nblocks] != nproj) return QE_HPSI_EINVAL;
+    for (int a = 0; a < nblocks; ++a) {
+      const long long nh = (long long)blk_off_host[a + 1] - blk_off_host[a];
+      if (nh <= 0) return QE_HPSI_EINVAL;
+      d_total += nh * nh;
+    }
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  qe_hpsi_handle* h = new (std::nothrow) qe_hpsi_handle();
+  if (!h) return QE_HPSI_ENOMEM;
+#define CR_TRY(expr)                                                             \
+  do {                                                                           \
+    cudaError_t e__ = (expr);                                                    \
+    if (e__ != cudaSuccess) {                                                    \
+      g_last_cuda = (int)e__;                                                    \
+      qe_hpsi_destroy(h);                                                        \
+      return e__ == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA;  \
+    }                                                                            \
+  } while (0)
+  CR_TRY(cudaGetDevice(&h->device));
+  CR_TRY(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device));
+  CR_TRY(set_kernel_attrs());
+  for (int j = 0; j < 3; ++j) h->nr[j] = nr[j];
+  h->ldz = (nr[2] + 7) / 8 * 8;
+  h->max_batch = max_batch;
+  h->nproj = nproj;
+
+  // ---- a0: sphere maps --------------------------------------------------------------------------------
+  SphereOut so;
+  rc = build_sphere(sg, st, &so);
+  if (rc) {
+    qe_hpsi_destroy(h);
+    return rc;
+  }
+  h->npw = so.npw;
+  h->miller = so.miller;
+  h->fftidx = so.fftidx;
+  h->g2kin = so.g2kin;
+  if (nproj > 0 && ldbeta < h->npw) {
+    qe_hpsi_destroy(h);
+    return QE_HPSI_EINVAL;
+  }
+  std::vector<int> idx((size_t)h->npw);
+  if (h->npw) CR_TRY(cudaMemcpy(idx.data(), h->fftidx, sizeof(int) * (size_t)h->npw, cudaMemcpyDeviceToHost));
+  // sticks ((i1,i2) columns) and populated planes, in canonical order
+  std::vector<int> stick_start, stick_i2, plane_stick, plane_i1, pw_pos((size_t)h->npw);
+  {
+    const int n2 = nr[1], n3 = nr[2];
+    int last_col = -1, last_plane = -1;
+    for (int ig = 0; ig < h->npw; ++ig) {
+      const int col = idx[ig] / n3, i3 = idx[ig] - col * n3;
+      if (col != last_col) {
+        const int i1 = col / n2;
+        if (i1 != last_plane) {
+          plane_stick.push_back((int)stick_start.size());
+          plane_i1.push_back(i1);
+          last_plane = i1;
+        }
+        stick_start.push_back(ig);
+        stick_i2.push_back(col - i1 * n2);
+        last_col = col;
+      }
+      const int c = ((int)stick_start.size() - 1) % FFT_C;
+      pw_pos[ig] = i3 * FFT_C + (c ^ (i3 & 7));
+    }
+    h->S = (int)stick_start.size();
+    h->P = (int)plane_i1.size();
+    stick_start.push_back(h->npw);
+    plane_stick.push_back(h->S);
+  }
+  CR_TRY(upload(&h->stick_start, stick_start, st));
+  CR_TRY(upload(&h->stick_i2, stick_i2, st));
+  CR_TRY(upload(&h->plane_stick, plane_stick, st));
+  CR_TRY(upload(&h->plane_i1, plane_i1, st));
+  CR_TRY(upload(&h->pw_pos, pw_pos, st));
+
+  // ---- FFT plan ---------------------------------------------------------------------------------------
+  FftGeom& g = h->geom;
+  g.n1 = nr[0];
+  g.n2 = nr[1];
+  g.n3 = nr[2];
+  g.ldz = h->ldz;
+  g.npw = h->npw;
+  g.S = h->S;
+  g.P = h->P;
+  g.ntz = (nr[2] + FFT_C - 1) / FFT_C;
+  g.stick_start = h->stick_start;
+  g.stick_i2 = h->stick_i2;
+  g.plane_stick = h->plane_stick;
+  g.plane_i1 = h->plane_i1;
+  g.pw_pos = h->pw_pos;
+  g.g2kin = h->g2kin;
+  FftAxis* axes[3] = {&g.ax1, &g.ax2, &g.ax3};
+  for (int j = 0; j < 3; ++j) {
+    std::vector<int> rad;
+    plan_radices(nr[j], (flags & QE_HPSI_GENERIC_FFT) != 0, &rad);
+    if ((int)rad.size() > FFT_MAX_PASS) {
+      qe_hpsi_destroy(h);
+      return QE_HPSI_EGRID;
+    }
+    axes[j]->n = nr[j];
+    axes[j]->npass = (int)rad.size();
+    for (size_t p = 0; p < rad.size(); ++p) axes[j]->radix[p] = rad[p];
+    std::vector<double2> tw;
+    host_twiddles(nr[j], &tw);
+    CR_TRY(upload(&h->tw[j], tw, st));
+    axes[j]->tw = h->tw[j];
+  }
+  h->smem_z = 2 * (size_t)nr[2] * FFT_C * sizeof(double2);
+  h->smem_y = 2 * (size_t)nr[1] * FFT_C * sizeof(double2);
+  h->smem_x = 2 * (size_t)nr[0] * FFT_C * sizeof(double2) + (size_t)nr[0] * FFT_C * sizeof(double);
+
+  // V(r)/N in the padded layout
+  {
+    const long long rows = (long long)nr[0] * nr[1];
+    CR_TRY(cudaMalloc(&h->vs, sizeof(double) * (size_t)rows * h->ldz));
+    const long long tot = rows * h->ldz;
+    const double scale = 1.0 / ((double)nr[0] * (double)nr[1] * (double)nr[2]);
+    k_scale_pad_v<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(vr_dev, h->vs, nr[2], h->ldz, rows, scale);
+    CR_TRY(cudaGetLastError());
+    g.vs = h->vs;
+  }
+
+  // FFT workspace: sub-chunks of fft_nb bands sized to stay L2-resident between passes
+  {
+    const size_t per_band = ((size_t)h->S + (size_t)h->P * nr[1]) * h->ldz * sizeof(double2);
+    const size_t budget = (size_t)env_int("QE_HPSI_FFT_L2_MB", 48) << 20;
+    long long nbf = per_band ? (long long)(budget / per_band) : max_batch;
+    nbf = std::max<long long>(1, std::min<long long>(nbf, max_batch));
+    const int forced = env_int("QE_HPSI_FFT_NB", 0);
+    if (forced > 0) nbf = std::min(forced, max_batch);
+    h->fft_nb = (int)nbf;
+    CR_TRY(cudaMalloc(&h->w1, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2))));
+    CR_TRY(cudaMalloc(&h->w2, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2))));
+    h->workspace_bytes += (size_t)h->fft_nb * per_band;
+    // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
+    // gridDim.y only as far as needed to give every SM a few CTAs
+    const long long xt = (long long)nr[1] * g.ntz;
+    int split = (int)std::min<long long>(h->fft_nb, std::max<long long>(1, (4LL * h->num_sms + xt - 1) / xt));
+    h->x_split = std::max(1, split);
+  }
+
+  // ---- nonlocal ---------------------------------------------------------------------------------------
+  if (nproj > 0) {
+    if (flags & QE_HPSI_BORROW_BETA) {
+      h->beta = static_cast<const double2*>(beta_dev);
+      h->ldbeta = ldbeta;
+    } else {
+      h->ldbeta = ((long long)h->npw + 7) / 8 * 8;
+      CR_TRY(cudaMalloc(&h->beta_own, sizeof(double2) * (size_t)nproj * h->ldbeta));
+      CR_TRY(cudaMemsetAsync(h->beta_own, 0, sizeof(double2) * (size_t)nproj * h->ldbeta, st));
+      CR_TRY(cudaMemcpy2DAsync(h->beta_own, sizeof(double2) * h->ldbeta, beta_dev, sizeof(double2) * (size_t)ldbeta,
+                               sizeof(double2) * (size_t)h->npw, (size_t)nproj, cudaMemcpyDeviceToDevice, st));
+      h->beta = h->beta_own;
+    }
+    std::vector<int> blk0((size_t)nproj), nhv((size_t)nproj);
+    std::vector<long long> doff((size_t)nproj);
+    long long off = 0;
+    for (int a = 0; a < nblocks; ++a) {
+      const int q0 = blk_off_host[a], nh = blk_off_host[a + 1] - q0;
+      for (int i = 0; i < nh; ++i) {
+        blk0[q0 + i] = q0;
+        nhv[q0 + i] = nh;
+        doff[q0 + i] = off + (long long)i * nh;
+      }
+      off += (long long)nh * nh;
+    }
+    std::vector<double> dv(d_host, d_host + d_total);
+    CR_TRY(upload(&h->proj_blk0, blk0, st));
+    CR_TRY(upload(&h->proj_nh, nhv, st));
+    CR_TRY(upload(&h->proj_doff, doff, st));
+    CR_TRY(upload(&h->dpk, dv, st));
+    h->ldc = (max_batch + 1) / 2 * 2;
+    h->ldp = (nproj + 7) / 8 * 8;
+    choose_split(h);
+    const int forced = env_int("QE_HPSI_NSPLIT", 0);
+    if (forced > 0) {
+      int kchunk = (h->npw + forced - 1) / forced;
+      kchunk = std::max(ZG_BK, (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK);
+      h->kchunk = kchunk;
+      h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+    }
+    const size_t pc = (size_t)nproj * h->ldc * sizeof(double2);
+    CR_TRY(cudaMalloc(&h->partial, pc * h->nsplit));
+    CR_TRY(cudaMalloc(&h->becp, pc));
+    CR_TRY(cudaMalloc(&h->dbecp, pc));
+    CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
+    CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
+    h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
+  }
+  CR_TRY(cudaStreamSynchronize(st));
+#undef CR_TRY
+  *out = h;
+  return QE_HPSI_OK;
+}
+
+namespace {
+
+int check_apply_args(qe_hpsi_t h, const void* psi, int64_t ldpsi, void* hpsi, int64_t ldhpsi, int nbands) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nbands < 0) return QE_HPSI_EINVAL;
+  if (nbands == 0) return QE_HPSI_OK;
+  if (!psi || !hpsi || ldpsi < h->npw || ldhpsi < h->npw) return QE_HPSI_EINVAL;
+  const char* a0 = static_cast<const char*>(psi);
+  const char* a1 = a0 + ((size_t)(nbands - 1) * ldpsi + h->npw) * sizeof(double2);
+  const char* b0 = static_cast<const char*>(hpsi);
+  const char* b1 = b0 + ((size_t)(nbands - 1) * ldhpsi + h->npw) * sizeof(double2);
+  if (a0 < b1 && b0 < a1) return QE_HPSI_EINVAL;
+  return QE_HPSI_OK;
+}
+
+// a1-a5 for nb bands (nb <= max_batch), processed in sub-chunks of fft_nb bands
+int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const FftGeom& g = h->geom;
+  if (h->npw == 0) return QE_HPSI_OK;
+  const unsigned zt = (unsigned)((g.S + FFT_C - 1) / FFT_C);
+  const unsigned yt = (unsigned)(g.P * g.ntz);
+  const unsigned xt = (unsigned)(g.n2 * g.ntz);
+  for (int b0 = 0; b0 < nb; b0 += h->fft_nb) {
+    const int n = std::min(h->fft_nb, nb - b0);
+    const double2* p = psi + (size_t)b0 * ldpsi;
+    double2* o = hpsi + (size_t)b0 * ldh;
+    k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
+    k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
+    k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
+    k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
+    k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
+  }
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// a6-a7 for nb bands: becp, dbecp, dbT
+int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
+  const int mt = (h->nproj + ZG_BM - 1) / ZG_BM, nt = (nb + ZG_BN - 1) / ZG_BN;
+  k_becp<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE><<<dim3(mt * nt, h->nsplit), ZG_NT, BECP_SMEM, st>>>(
+      h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb, h->npw, h->kchunk, h->partial, h->ldc);
+  const dim3 rg((nb + 127) / 128, h->nproj);
+  k_becp_reduce<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->becp);
+  k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
+                            h->dbT, h->ldp);
+  h->nb_last = nb;
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// a8
+int launch_vnl_add(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const int mt = (h->npw + ZG_BM - 1) / ZG_BM, nt = (nb + ZG_BN - 1) / ZG_BN;
+  if (mt == 0) return QE_HPSI_OK;
+  k_vnl_add<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE><<<(unsigned)(mt * nt), ZG_NT, VNL_SMEM, st>>>(
+      h->beta, h->ldbeta, h->nproj, h->npw, h->dbT, h->ldp, nb, hpsi, ldh);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi, long long ldh, int nb, cudaStream_t st,
+                bool local, bool nonlocal) {
+  int rc = QE_HPSI_OK;
+  if (nonlocal && h->nproj > 0 && h->npw > 0) {
+    rc = launch_becp(h, psi, ldpsi, nb, st);
+    if (rc) return rc;
+  }
+  if (local) {
+    rc = launch_local(h, psi, ldpsi, hpsi, ldh, nb, st);
+    if (rc) return rc;
+  }
+  if (nonlocal && h->nproj > 0 && h->npw > 0) rc = launch_vnl_add(h, hpsi, ldh, nb, st);
+  return rc;
+}
+
+int apply_impl(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+               void* cuda_stream, bool local, bool nonlocal) {
+  int rc = check_apply_args(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands);
+  if (rc || nbands == 0) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const double2* psi = static_cast<const double2*>(psi_dev);
+  double2* hpsi = static_cast<double2*>(hpsi_dev);
+  for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
+    const int nb = std::min(h->max_batch, nbands - b0);
+    rc = apply_chunk(h, psi + (size_t)b0 * ldpsi, ldpsi, hpsi + (size_t)b0 * ldhpsi, ldhpsi, nb, st, local, nonlocal);
+    if (rc) return rc;
+  }
+  return QE_HPSI_OK;
+}
+
+}  // namespace
+
+extern "C" int qe_hpsi_apply(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+                             void* cuda_stream) {
+  return apply_impl(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands, cuda_stream, true, true);
+}
+extern "C" int qe_hpsi_fft_local(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
+                                 int nbands, void* cuda_stream) {
+  return apply_impl(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands, cuda_stream, true, false);
+}
+extern "C" int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
+                                int nbands, void* cuda_stream) {
+  return apply_impl(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands, cuda_stream, false, true);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// end-to-end variant with host buffers: H2D copy of chunk i+1 and D2H copy of chunk i-1 overlap the compute
+// of chunk i (three internal streams, two staging buffers each for psi and hpsi)
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldpsi, void* hpsi_host, int64_t ldhpsi,
+                                  int nbands) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nbands < 0) return QE_HPSI_EINVAL;
+  if (nbands == 0) return QE_HPSI_OK;
+  if (!psi_host || !hpsi_host || ldpsi < h->npw || ldhpsi < h->npw) return QE_HPSI_EINVAL;
+  if (!h->st_comp) {
+    h->ldint = ((long long)h->npw + 7) / 8 * 8;
+    const size_t bytes = std::max<size_t>(16, (size_t)h->max_batch * h->ldint * sizeof(double2));
+    for (int i = 0; i < 2; ++i) {
+      CU_TRY(h, cudaMalloc(&h->hbuf_psi[i], bytes));
+      CU_TRY(h, cudaMalloc(&h->hbuf_h[i], bytes));
+      CU_TRY(h, cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
+      CU_TRY(h, cudaEventCreateWithFlags(&h->ev_comp[i], cudaEventDisableTiming));
+      CU_TRY(h, cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming));
+    }
+    CU_TRY(h, cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking));
+    CU_TRY(h, cudaStreamCreateWithFlags(&h->st_out, cudaStreamNonBlocking));
+    CU_TRY(h, cudaStreamCreateWithFlags(&h->st_comp, cudaStreamNonBlocking));
+  }
+  const double2* psi = static_cast<const double2*>(psi_host);
+  double2* hpsi = static_cast<double2*>(hpsi_host);
+  const size_t width = sizeof(double2) * (size_t)h->npw;
+  int ci = 0;
+  for (int b0 = 0; b0 < nbands; b0 += h->max_batch, ++ci) {
+    const int nb = std::min(h->max_batch, nbands - b0);
+    const int u = ci & 1;
+    if (ci >= 2) CU_TRY(h, cudaStreamWaitEvent(h->st_in, h->ev_comp[u], 0));  // compute of chunk ci-2 read psi buf u
+    if (width)
+      CU_TRY(h, cudaMemcpy2DAsync(h->hbuf_psi[u], sizeof(double2) * h->ldint, psi + (size_t)b0 * ldpsi,
+                                  sizeof(double2) * (size_t)ldpsi, width, (size_t)nb, cudaMemcpyHostToDevice, h->st_in));
+    CU_TRY(h, cudaEventRecord(h->ev_in[u], h->st_in));
+    CU_TRY(h, cudaStreamWaitEvent(h->st_comp, h->ev_in[u], 0));
+    if (ci >= 2) CU_TRY(h, cudaStreamWaitEvent(h->st_comp, h->ev_out[u], 0));  // D2H of chunk ci-2 read hpsi buf u
+    int rc = apply_chunk(h, h->hbuf_psi[u], h->ldint, h->hbuf_h[u], h->ldint, nb, h->st_comp, true, true);
+    if (rc) return rc;
+    CU_TRY(h, cudaEventRecord(h->ev_comp[u], h->st_comp));
+    CU_TRY(h, cudaStreamWaitEvent(h->st_out, h->ev_comp[u], 0));
+    if (width)
+      CU_TRY(h, cudaMemcpy2DAsync(hpsi + (size_t)b0 * ldhpsi, sizeof(double2) * (size_t)ldhpsi, h->hbuf_h[u],
+                                  sizeof(double2) * h->ldint, width, (size_t)nb, cudaMemcpyDeviceToHost, h->st_out));
+    CU_TRY(h, cudaEventRecord(h->ev_out[u], h->st_out));
+  }
+  CU_TRY(h, cudaStreamSynchronize(h->st_out));
+  CU_TRY(h, cudaStreamSynchronize(h->st_comp));
+  return QE_HPSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// accessors
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int64_t qe_hpsi_npw(qe_hpsi_t h) { return h ? h->npw : (int64_t)QE_HPSI_ESTATE; }
+extern "C" int64_t qe_hpsi_nsticks(qe_hpsi_t h) { return h ? h->S : (int64_t)QE_HPSI_ESTATE; }
+extern "C" int64_t qe_hpsi_nplanes(qe_hpsi_t h) { return h ? h->P : (int64_t)QE_HPSI_ESTATE; }
+
+extern "C" int qe_hpsi_get_maps(qe_hpsi_t h, int32_t* miller_dev, int32_t* fftidx_dev, double* g2kin_dev,
+                                void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t n = (size_t)h->npw;
+  if (n == 0) return QE_HPSI_OK;
+  if (miller_dev) CU_TRY(h, cudaMemcpyAsync(miller_dev, h->miller, sizeof(int) * 3 * n, cudaMemcpyDeviceToDevice, st));
+  if (fftidx_dev) CU_TRY(h, cudaMemcpyAsync(fftidx_dev, h->fftidx, sizeof(int) * n, cudaMemcpyDeviceToDevice, st));
+  if (g2kin_dev) CU_TRY(h, cudaMemcpyAsync(g2kin_dev, h->g2kin, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_get_becp(qe_hpsi_t h, void* becp_dev, void* dbecp_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (h->nproj == 0 || h->nb_last == 0) return QE_HPSI_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t w = sizeof(double2) * (size_t)h->nb_last, sp = sizeof(double2) * (size_t)h->ldc;
+  if (becp_dev) CU_TRY(h, cudaMemcpy2DAsync(becp_dev, w, h->becp, sp, w, (size_t)h->nproj, cudaMemcpyDeviceToDevice, st));
+  if (dbecp_dev) CU_TRY(h, cudaMemcpy2DAsync(dbecp_dev, w, h->dbecp, sp, w, (size_t)h->nproj, cudaMemcpyDeviceToDevice, st));
+  return QE_HPSI_OK;
+}
+
+extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nbands <= 0 || h->npw == 0) return 0;
+  int64_t total = 0;
+  for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
+    const int nb = std::min(h->max_batch, nbands - b0);
+    total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
+    if (h->nproj > 0) total += 4;
+  }
+  return total;
+}
+
+extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!info) return QE_HPSI_EINVAL;
+  for (int i = 0; i < 16; ++i) info[i] = 0;
+  info[0] = h->npw;
+  info[1] = h->S;
+  info[2] = h->P;
+  info[3] = h->fft_nb;
+  info[4] = h->nsplit;
+  info[5] = (int64_t)h->workspace_bytes;
+  info[6] = h->geom.ax1.npass;
+  info[7] = h->geom.ax2.npass;
+  info[8] = h->geom.ax3.npass;
+  info[9] = h->kchunk;
+  info[10] = h->x_split;
+  info[11] = h->num_sms;
+  return QE_HPSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// FP64 peak probe (measurement helper for the roofline denominator; not on the hot path)
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+__global__ void __launch_bounds__(256) k_probe_dmma(double* out, int iters, double a, double b) {
+  double c[32][2];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) {
+    c[i][0] = (double)i;
+    c[i][1] = (double)threadIdx.x;
+  }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 32; ++i) dmma884(c[i][0], c[i][1], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) s += c[i][0] + c[i][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void __launch_bounds__(1024) k_probe_dfma(double* out, int iters, double a, double b) {
+  double x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = threadIdx.x * 1e-3 + i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += x[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+extern "C" int qe_hpsi_probe_fp64(double millis, double* dmma_tflops, double* dfma_tflops) {
+  qe_hpsi_handle* h = nullptr;
+  int dev = 0, nsm = 0;
+  CU_TRY(h, cudaGetDevice(&dev));
+  CU_TRY(h, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  double* out = nullptr;
+  CU_TRY(h, cudaMalloc(&out, sizeof(double) * (size_t)nsm * 1024));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  int rc = QE_HPSI_OK;
+  for (int which = 0; which < 2 && rc == QE_HPSI_OK; ++which) {
+    const int iters = which == 0 ? 4000 : 16000;
+    const double flop_per_launch =
+        which == 0 ? 2.0 * 256 * 32 * iters * 8.0 * nsm : 2.0 * 16 * iters * 1024.0 * nsm;
+    double best = 0.0, spent = 0.0;
+    for (int rep = 0; rep < 1000 && (rep < 3 || spent < millis); ++rep) {
+      cudaEventRecord(e0);
+      if (which == 0)
+        k_probe_dmma<<<nsm, 256>>>(out, iters, 1.0000001, 1e-9);
+      else
+        k_probe_dfma<<<nsm, 1024>>>(out, iters, 1.0000001, 1e-9);
+      cudaEventRecord(e1);
+      cudaError_t e = cudaEventSynchronize(e1);
+      if (e != cudaSuccess) {
+        g_last_cuda = (int)e;
+        rc = QE_HPSI_ECUDA;
+        break;
+      }
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      spent += ms;
+      if (rep >= 1) best = std::max(best, flop_per_launch / (ms * 1e-3) * 1e-12);
+    }
+    if (which == 0 && dmma_tflops) *dmma_tflops = best;
+    if (which == 1 && dfma_tflops) *dfma_tflops = best;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  return rc;
+}

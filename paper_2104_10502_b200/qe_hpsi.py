@@ -1,0 +1,255 @@
+"""ctypes binding of libqe_hpsi.so (include/qe_hpsi.h). Argument marshalling only: every step of H|psi> runs in
+the library's CUDA kernels. PyTorch supplies device memory and streams. There is NO fallback: if the shared
+library is missing or cannot be loaded, importing callers get a RuntimeError.
+
+Function names mirror the C ABI (qe_hpsi_gsphere, qe_hpsi_create, qe_hpsi_apply, ...); `Hpsi` is a small RAII
+convenience around a handle.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libqe_hpsi.so")
+
+QE_HPSI_OK, QE_HPSI_EINVAL, QE_HPSI_EGRID, QE_HPSI_ENOMEM, QE_HPSI_ECUDA, QE_HPSI_ESTATE = 0, -1, -2, -3, -4, -5
+QE_HPSI_BORROW_BETA = 1
+QE_HPSI_GENERIC_FFT = 2
+QE_HPSI_MAX_N = 720
+
+_c = ctypes
+_vp, _i64, _i32, _dbl = _c.c_void_p, _c.c_int64, _c.c_int, _c.c_double
+_pd, _pi32, _pi64 = _c.POINTER(_c.c_double), _c.POINTER(_c.c_int32), _c.POINTER(_c.c_int64)
+
+# name -> (restype, argtypes); the single source the loader and the symbol test use
+SIGNATURES = {
+    "qe_hpsi_gsphere": (_i32, [_pd, _pd, _dbl, _pi32, _pi64, _pi32]),
+    "qe_hpsi_create": (_i32, [_c.POINTER(_vp), _pd, _dbl, _pd, _pi32, _vp, _i32, _vp, _i64, _i32, _pi32, _pd, _i32,
+                              _c.c_uint, _vp]),
+    "qe_hpsi_apply": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
+    "qe_hpsi_apply_host": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32]),
+    "qe_hpsi_destroy": (_i32, [_vp]),
+    "qe_hpsi_npw": (_i64, [_vp]),
+    "qe_hpsi_nsticks": (_i64, [_vp]),
+    "qe_hpsi_nplanes": (_i64, [_vp]),
+    "qe_hpsi_get_maps": (_i32, [_vp, _vp, _vp, _vp, _vp]),
+    "qe_hpsi_get_becp": (_i32, [_vp, _vp, _vp, _vp]),
+    "qe_hpsi_launch_count": (_i64, [_vp, _i32]),
+    "qe_hpsi_info": (_i32, [_vp, _pi64]),
+    "qe_hpsi_strerror": (_c.c_char_p, [_i32]),
+    "qe_hpsi_last_cuda_error": (_i32, [_vp]),
+    "qe_hpsi_probe_fp64": (_i32, [_dbl, _pd, _pd]),
+    "qe_hpsi_fft_local": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
+    "qe_hpsi_nonlocal": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
+}
+
+_lib = None
+
+
+def load_library():
+    """dlopen libqe_hpsi.so (built by paper_2104_10502_b200.build). Fails loudly; never falls back."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2104_10502_b200.build` (nvcc, sm_100a). "
+                           "There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)  # AttributeError if the symbol is not exported
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class QeHpsiError(RuntimeError):
+    def __init__(self, status, cuda=0):
+        msg = load_library().qe_hpsi_strerror(int(status)).decode()
+        super().__init__(f"qe_hpsi status {status}: {msg}" + (f" (cudaError {cuda})" if cuda else ""))
+        self.status = int(status)
+        self.cuda = int(cuda)
+
+
+def _check(rc, handle=None):
+    if rc != 0:
+        raise QeHpsiError(rc, load_library().qe_hpsi_last_cuda_error(handle))
+
+
+def _darr(x, n):
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.float64).reshape(-1))
+    assert a.size == n
+    return a, a.ctypes.data_as(_pd)
+
+
+def _iarr(x, n):
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.int32).reshape(-1))
+    assert a.size == n
+    return a, a.ctypes.data_as(_pi32)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return _vp(stream.cuda_stream)
+
+
+def qe_hpsi_gsphere(at, xk, ecutwfc, nr) -> np.ndarray:
+    """Canonical sphere: int32 Miller triples [npw, 3] (host), ascending FFT linear index."""
+    lib = load_library()
+    _a, pa = _darr(at, 9)
+    _k, pk = _darr(xk, 3)
+    _n, pn = _iarr(nr, 3)
+    npw = _c.c_int64(0)
+    _check(lib.qe_hpsi_gsphere(pa, pk, float(ecutwfc), pn, _c.byref(npw), None))
+    mil = np.zeros((max(npw.value, 0), 3), dtype=np.int32)
+    if npw.value > 0:
+        _check(lib.qe_hpsi_gsphere(pa, pk, float(ecutwfc), pn, _c.byref(npw), mil.ctypes.data_as(_pi32)))
+    return mil
+
+
+def qe_hpsi_probe_fp64(millis=200.0):
+    """(DMMA TFLOP/s, DFMA TFLOP/s) measured on the current device."""
+    lib = load_library()
+    a, b = _c.c_double(0), _c.c_double(0)
+    _check(lib.qe_hpsi_probe_fp64(float(millis), _c.byref(a), _c.byref(b)))
+    return a.value, b.value
+
+
+class Hpsi:
+    """One handle = one (cell, k, cutoff, grid, V(r), projectors, D). See include/qe_hpsi.h for the contract."""
+
+    def __init__(self, at, ecutwfc, xk, nr, vr: torch.Tensor, beta: torch.Tensor | None = None, blk_off=None,
+                 dblocks=None, max_batch: int = 128, flags: int = 0, stream=None):
+        lib = load_library()
+        self._lib = lib
+        self._h = _vp(None)
+        assert vr.is_cuda and vr.dtype == torch.float64 and vr.is_contiguous()
+        assert tuple(vr.shape) == tuple(int(x) for x in nr)
+        _a, pa = _darr(at, 9)
+        _k, pk = _darr(xk, 3)
+        _n, pn = _iarr(nr, 3)
+        nproj = 0 if beta is None else int(beta.shape[0])
+        if nproj:
+            assert beta.is_cuda and beta.dtype == torch.complex128 and beta.stride(1) == 1
+            ldbeta = int(beta.stride(0)) if beta.shape[0] > 1 else int(beta.shape[1])
+            blk = np.ascontiguousarray(np.asarray(blk_off, dtype=np.int32))
+            dpk = np.ascontiguousarray(np.concatenate([np.asarray(d, dtype=np.float64).reshape(-1) for d in dblocks]))
+            pb, nblocks = blk.ctypes.data_as(_pi32), blk.size - 1
+            pdk = dpk.ctypes.data_as(_pd)
+            bptr = _vp(beta.data_ptr())
+        else:
+            ldbeta, pb, nblocks, pdk, bptr = 0, None, 0, None, _vp(None)
+        self._keep = (vr, beta) if (flags & QE_HPSI_BORROW_BETA) else None
+        rc = lib.qe_hpsi_create(_c.byref(self._h), pa, float(ecutwfc), pk, pn, _vp(vr.data_ptr()), nproj, bptr,
+                                ldbeta, nblocks, pb, pdk, int(max_batch), int(flags), _stream_ptr(stream))
+        _check(rc)
+        self.npw = int(lib.qe_hpsi_npw(self._h))
+        self.nproj = nproj
+        self.max_batch = int(max_batch)
+
+    # -- hot path ----------------------------------------------------------------------------------------
+    def _call(self, fn, psi, hpsi, stream):
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.dim() == 2 and psi.stride(1) == 1
+        nb = int(psi.shape[0])
+        if hpsi is None:
+            hpsi = torch.zeros_like(psi)
+        assert hpsi.is_cuda and hpsi.dtype == torch.complex128 and hpsi.shape[0] == nb and hpsi.stride(1) == 1
+        ldp = int(psi.stride(0)) if nb > 1 else int(psi.shape[1])
+        ldh = int(hpsi.stride(0)) if nb > 1 else int(hpsi.shape[1])
+        _check(fn(self._h, _vp(psi.data_ptr()), ldp, _vp(hpsi.data_ptr()), ldh, nb, _stream_ptr(stream)), self._h)
+        return hpsi
+
+    def apply(self, psi, hpsi=None, stream=None):
+        """qe_hpsi_apply: hpsi[b][:npw] = H psi[b] (asynchronous on `stream`)."""
+        return self._call(self._lib.qe_hpsi_apply, psi, hpsi, stream)
+
+    def fft_local(self, psi, hpsi=None, stream=None):
+        return self._call(self._lib.qe_hpsi_fft_local, psi, hpsi, stream)
+
+    def nonlocal_add(self, psi, hpsi, stream=None):
+        return self._call(self._lib.qe_hpsi_nonlocal, psi, hpsi, stream)
+
+    def apply_host(self, psi_host: torch.Tensor, hpsi_host: torch.Tensor):
+        """qe_hpsi_apply_host: host (pinned) buffers, copies inside the call, synchronous."""
+        assert (not psi_host.is_cuda) and (not hpsi_host.is_cuda)
+        assert psi_host.dtype == torch.complex128 and hpsi_host.dtype == torch.complex128
+        nb = int(psi_host.shape[0])
+        ldp = int(psi_host.stride(0)) if nb > 1 else int(psi_host.shape[1])
+        ldh = int(hpsi_host.stride(0)) if nb > 1 else int(hpsi_host.shape[1])
+        _check(self._lib.qe_hpsi_apply_host(self._h, _vp(psi_host.data_ptr()), ldp, _vp(hpsi_host.data_ptr()), ldh, nb),
+               self._h)
+        return hpsi_host
+
+    # -- accessors ---------------------------------------------------------------------------------------
+    def maps(self):
+        """(miller [npw,3] int32, fft_index [npw] int32, g2kin [npw] float64) as CUDA tensors."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        mil = torch.empty((self.npw, 3), dtype=torch.int32, device=dev)
+        idx = torch.empty((self.npw,), dtype=torch.int32, device=dev)
+        g2 = torch.empty((self.npw,), dtype=torch.float64, device=dev)
+        _check(self._lib.qe_hpsi_get_maps(self._h, _vp(mil.data_ptr()), _vp(idx.data_ptr()), _vp(g2.data_ptr()),
+                                          _stream_ptr(None)), self._h)
+        return mil, idx, g2
+
+    def becp(self, nb):
+        """(becp, dbecp) [nproj, nb] complex128 of the last chunk applied (nb must be that chunk's band count)."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        a = torch.empty((self.nproj, nb), dtype=torch.complex128, device=dev)
+        b = torch.empty((self.nproj, nb), dtype=torch.complex128, device=dev)
+        _check(self._lib.qe_hpsi_get_becp(self._h, _vp(a.data_ptr()), _vp(b.data_ptr()), _stream_ptr(None)), self._h)
+        return a, b
+
+    def info(self) -> dict:
+        buf = (_c.c_int64 * 16)()
+        _check(self._lib.qe_hpsi_info(self._h, buf), self._h)
+        keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
+                "x_split", "num_sms"]
+        return {k: int(buf[i]) for i, k in enumerate(keys)}
+
+    def launch_count(self, nbands) -> int:
+        return int(self._lib.qe_hpsi_launch_count(self._h, int(nbands)))
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value is not None:
+            self._lib.qe_hpsi_destroy(self._h)
+            self._h = _vp(None)
+        self._keep = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def from_workload(wl, max_batch=None, flags=0, device="cuda", beta=None):
+    """Build every input of a BASELINE.json workload on the GPU with the seeded generators (inputs.py) and the
+    library's own sphere, and create a handle. Returns (Hpsi, dict of inputs)."""
+    from . import inputs
+
+    wl = inputs.get_workload(wl)
+    mil = qe_hpsi_gsphere(wl.at, wl.xk, wl.ecutwfc, wl.nr)
+    npw = mil.shape[0]
+    ld = inputs.pad8(npw)
+    vr = inputs.gen_vloc(wl, device="cpu").to(device)  # input generation only (CPU FFT); not the product path
+    atoms = inputs.gen_atoms(wl)
+    mil_d = torch.as_tensor(mil, device=device)
+    if wl.nproj:
+        if beta is None:
+            beta = torch.zeros((wl.nproj, ld), dtype=torch.complex128, device=device)
+            step = 16
+            for a0 in range(0, wl.natoms, step):
+                na = min(step, wl.natoms - a0)
+                inputs.gen_beta(wl, mil_d, atoms, a0, na, ld=ld, device=device, out=beta[a0 * wl.nh:(a0 + na) * wl.nh])
+        blk = np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh
+        db = inputs.gen_dblocks(wl)
+    else:
+        beta, blk, db = None, None, None
+    mb = wl.batch if max_batch is None else max_batch
+    h = Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr, beta, blk, db, max_batch=mb, flags=flags)
+    return h, dict(wl=wl, miller=mil, miller_dev=mil_d, ld=ld, vr=vr, atoms=atoms, beta=beta, dblocks=db)

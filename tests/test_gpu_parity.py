@@ -1,0 +1,194 @@
+"""GPU parity: libqe_hpsi.so (through the C ABI / ctypes binding) against the CPU oracle, element by element, on
+the same seeded inputs. Tolerance: relative L2 error <= 1e-11 per band (BASELINE.json north_star); index maps
+bit-exact. PAPER.md:L105, L224-226, L176 (vi); readings in DESIGN.md section 3."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import hpsi_oracle as orc
+from paper_2104_10502_b200 import inputs, qe_hpsi
+from tests import _gpu
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+TINY = ["T1_general_k", "T2_radix5", "T2b_radix5_20", "T3_aliased", "T4_noproj", "T5_odd_bands"]
+
+
+@pytest.mark.parametrize("cfg", TINY + [0, 1, 2, 3, 4])
+def test_maps_bit_exact(cfg):
+    wl = inputs.get_workload(cfg)
+    sp = _gpu.oracle_sphere(wl)
+    mil = qe_hpsi.qe_hpsi_gsphere(wl.at, wl.xk, wl.ecutwfc, wl.nr)
+    assert mil.dtype == np.int32 and np.array_equal(mil, sp["miller"])
+    vr = torch.zeros(tuple(wl.nr), dtype=torch.float64, device="cuda")
+    h = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr, max_batch=1)
+    m2, idx, g2 = h.maps()
+    assert np.array_equal(m2.cpu().numpy(), sp["miller"])
+    assert np.array_equal(idx.cpu().numpy(), sp["fft_index"])
+    assert np.array_equal(g2.cpu().numpy().view(np.int64), sp["g2kin"].view(np.int64)), "g2kin must match bit for bit"
+    info = h.info()
+    n3 = wl.nr[2]
+    assert info["S"] == np.unique(sp["fft_index"].astype(np.int64) // n3).size
+    assert info["P"] == np.unique(sp["fft_index"].astype(np.int64) // (n3 * wl.nr[1])).size
+    h.destroy()
+
+
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT])
+@pytest.mark.parametrize("cfg", TINY + [0])
+def test_small_cases_against_dense_h(cfg, flags):
+    """Level A (dense H from the definition) on every tiny case and config 0; both radix plans."""
+    h, inp = _gpu.make(cfg, flags=flags)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    hpsi = torch.full_like(psi, 7.0)  # sentinel: pad columns must stay untouched, the rest overwritten
+    h.apply(psi, hpsi)
+    torch.cuda.synchronize()
+    beta = inp["beta"][:, :npw].cpu().numpy() if wl.nproj else None
+    hd = orc.dense_h(sp["miller"], sp["g2kin"], tuple(wl.nr), inp["vr"].cpu().numpy(), beta, inp["dblocks"])
+    ref = orc.hpsi_dense(hd, psi[:, :npw].cpu().numpy())
+    got = hpsi.cpu().numpy()
+    err = _gpu.rel_l2(got[:, :npw], ref)
+    assert err.max() <= TOL, err
+    assert np.all(got[:, npw:] == 7.0)
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T5_odd_bands", 0])
+def test_stages_local_and_becp(cfg):
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    ph = psi[:, :npw].cpu().numpy()
+    loc_ref, vnl_ref = _gpu.oracle_hpsi(inp, sp, ph, parts=True)
+    loc = h.fft_local(psi)
+    torch.cuda.synchronize()
+    assert _gpu.rel_l2(loc.cpu().numpy()[:, :npw], loc_ref).max() <= TOL
+    out = h.nonlocal_add(psi, loc.clone())
+    becp, dbecp = h.becp(wl.nbands)
+    torch.cuda.synchronize()
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    bref = orc.becp_of(beta, ph)
+    assert np.abs(becp.cpu().numpy() - bref).max() <= 1e-13 * max(1.0, np.abs(bref).max())
+    dref = orc.dbecp_of(inp["dblocks"], bref)
+    assert np.abs(dbecp.cpu().numpy() - dref).max() <= 1e-13 * max(1.0, np.abs(dref).max())
+    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], loc_ref + vnl_ref).max() <= TOL
+    h.destroy()
+
+
+def test_closed_form_plane_wave_in_constant_potential():
+    """north_star invariant straight on the GPU path: psi = delta_G0, V = V0 -> (|k+G0|^2 + V0) delta."""
+    wl = inputs.get_workload(0)
+    v0 = 0.625
+    vr = torch.full(tuple(wl.nr), v0, dtype=torch.float64, device="cuda")
+    h = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr, max_batch=4)
+    _, _, g2 = h.maps()
+    npw = h.npw
+    picks = [0, 1, npw // 2, npw - 1]
+    psi = torch.zeros((4, npw), dtype=torch.complex128, device="cuda")
+    for b, g in enumerate(picks):
+        psi[b, g] = 1.0 - 0.5j
+    out = h.apply(psi)
+    ref = torch.zeros_like(psi)
+    for b, g in enumerate(picks):
+        ref[b, g] = (g2[g] + v0) * psi[b, g]
+    assert float((out - ref).abs().max()) <= 1e-13
+    h.destroy()
+
+
+def test_batch_composition_and_chunking_do_not_change_bits():
+    """A band's result must not depend on which other bands share the call (reading 13)."""
+    h, inp = _gpu.make(0, max_batch=5)  # 16 bands -> chunks 5,5,5,1
+    psi = _gpu.gen_psi_dev(inp, 0, 16)
+    full = h.apply(psi).clone()
+    one = torch.stack([h.apply(psi[b:b + 1].contiguous())[0] for b in (0, 7, 15)])
+    torch.cuda.synchronize()
+    assert torch.equal(full[[0, 7, 15]].view(torch.float64), one.view(torch.float64))
+    h.destroy()
+
+
+def test_config1_all_bands():
+    h, inp = _gpu.make(1)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    out = h.apply(psi)
+    torch.cuda.synchronize()
+    ref = _gpu.oracle_hpsi(inp, sp, psi[:, :h.npw].cpu().numpy())
+    err = _gpu.rel_l2(out.cpu().numpy()[:, :h.npw], ref)
+    assert err.max() <= TOL, err.max()
+    # Level A' (definition, sampled rows) at full scale, no FFT of psi involved
+    rows = inputs.aux_choice(wl.seed, 3, h.npw, 16)
+    bands = [0, 63, 127]
+    vt = orc.vloc_coeffs(inp["vr"].cpu().numpy())
+    beta = inp["beta"][:, :h.npw].cpu().numpy()
+    ap = orc.hpsi_rows(rows, sp["miller"], sp["g2kin"], tuple(wl.nr), vt, psi[bands, :h.npw].cpu().numpy(), beta,
+                       inp["dblocks"])
+    got = out.cpu().numpy()[bands][:, rows]
+    assert np.abs(got - ap).max() <= 1e-12 * np.abs(ref).max()
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_sampled_bands(cfg):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (batch = wl.batch, beta borrowed):
+    Level B oracle on sampled bands + a Hermitian probe <phi|H psi_b> = <H phi|psi_b> covering every band of the
+    batch at the cost of one extra oracle application."""
+    h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    nb = wl.batch
+    band0 = wl.nbands - nb  # last batch
+    psi = _gpu.gen_psi_dev(inp, band0, nb)
+    out = h.apply(psi)
+    torch.cuda.synchronize()
+    sample = sorted({0, nb - 1, nb // 2 + 1})
+    phi = inputs.aux_normal_complex(wl.seed, 99, npw).numpy()
+    phi /= np.linalg.norm(phi)
+    x = np.concatenate([psi[sample, :npw].cpu().numpy(), phi[None]])
+    ref = _gpu.oracle_hpsi(inp, sp, x)
+    err = _gpu.rel_l2(out[sample, :npw].cpu().numpy(), ref[:-1])
+    assert err.max() <= TOL, err
+    hphi = torch.as_tensor(ref[-1], device="cuda")
+    lhs = (torch.as_tensor(phi, device="cuda").conj()[None] * out[:, :npw]).sum(1)
+    rhs = (hphi.conj()[None] * psi[:, :npw]).sum(1)
+    scale = float(torch.linalg.vector_norm(out[:, :npw], dim=1).max())
+    assert float((lhs - rhs).abs().max()) <= 1e-11 * scale
+    h.destroy()
+
+
+def test_apply_host_matches_device_path():
+    h, inp = _gpu.make(0, max_batch=6)
+    psi = _gpu.gen_psi_dev(inp, 0, 16)
+    dev = h.apply(psi).cpu()
+    ph = psi.cpu().pin_memory()
+    hh = torch.zeros_like(ph).pin_memory()
+    h.apply_host(ph, hh)
+    assert torch.equal(hh[:, :h.npw].view(torch.float64), dev[:, :h.npw].view(torch.float64))
+    h.destroy()
+
+
+def test_argument_errors():
+    wl = inputs.get_workload("T2_radix5")
+    vr = torch.zeros(tuple(wl.nr), dtype=torch.float64, device="cuda")
+    with pytest.raises(qe_hpsi.QeHpsiError) as e:
+        qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, (14, 15, 15), torch.zeros((14, 15, 15), dtype=torch.float64, device="cuda"))
+    assert e.value.status == qe_hpsi.QE_HPSI_EGRID  # 14 = 2*7
+    with pytest.raises(qe_hpsi.QeHpsiError) as e:
+        qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, (5, 15, 15), torch.zeros((5, 15, 15), dtype=torch.float64, device="cuda"))
+    assert e.value.status == qe_hpsi.QE_HPSI_EGRID  # sphere wider than the box
+    h = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr, max_batch=2)
+    psi = torch.zeros((2, h.npw), dtype=torch.complex128, device="cuda")
+    with pytest.raises(qe_hpsi.QeHpsiError) as e:
+        h.apply(psi, psi)  # aliasing
+    assert e.value.status == qe_hpsi.QE_HPSI_EINVAL
+    with pytest.raises(qe_hpsi.QeHpsiError) as e:
+        h.apply(psi[:, :h.npw - 1].contiguous())  # ld < npw
+    assert e.value.status == qe_hpsi.QE_HPSI_EINVAL
+    out = h.apply(torch.zeros((0, h.npw), dtype=torch.complex128, device="cuda"))  # empty input is fine
+    assert out.shape[0] == 0
+    h.destroy()
