@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py -- H|psi> band-applications/s on B200 (BASELINE.json metric), with roofline and CPU-oracle baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (a1-a8) over all `nbands` bands of the workload, applied in calls of
+`batch` bands (config 4: 1024 bands as 8 calls of 128). `value` = bands/s with psi/hpsi resident in HBM; `e2e` =
+the same through qe_hpsi_apply_host with pinned HOST buffers (H2D of psi and D2H of hpsi inside the timed region).
+Default workload: config 4 (the configuration north_star's target is quoted on; fits one GPU). Inputs are seeded
+synthetic data. N > 1 (torchrun): every rank runs the same workload on its own bands
+(k-point-pool style sharding, no data-path collective): weak scaling, max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "hpsi_band_applications_per_s"
+UNIT = "bands/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--detail", action="store_true", help="extra pass with per-FFT-kernel events (stderr table)")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# clocks sampling during the timed region
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# roofline model (DESIGN.md section 6 / SURVEY.md 8(d)): algorithmic bytes and flops per band
+# ---------------------------------------------------------------------------------------------------------
+def model(wl, info):
+    npw, S, P = info["npw"], info["S"], info["P"]
+    n1, n2, n3 = wl.nr
+    b_fft = 16.0 * (3 * npw + 4 * S * n3 + 4 * P * n2 * n3) + 8.0 * n1 * n2 * n3 / wl.batch
+    b_beta = 2 * 16.0 * wl.nproj * npw / wl.batch
+    f_proj = 2 * 8.0 * wl.nproj * npw
+    return dict(b_fft=b_fft, b_beta=b_beta, f_proj=f_proj)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json", d
+    return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+def committed_traffic(cfg, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture (profiles/traffic.json)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f)
+    return d.get(f"cfg{cfg}", {}).get(kernel)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands on the host cores, on a bounded sample
+# ---------------------------------------------------------------------------------------------------------
+def oracle_sample_time(wl, nbands_sample=2, atoms_sample=16):
+    """Times oracle Level B (hpsi_dual) on `nbands_sample` bands of the workload. The local+kinetic part runs on
+    the full grid; the nonlocal part runs on the first `atoms_sample` atoms and its time is scaled by
+    natoms/atoms_sample (config 4's beta is 25 GB; the oracle's cost is linear in the number of atoms).
+    Returns (seconds per band extrapolated to the full workload, description, threads)."""
+    from oracle import hpsi_oracle as orc
+    from paper_2104_10502_b200 import inputs
+
+    sp = orc.gsphere(wl.at, wl.xk, wl.ecutwfc, wl.nr)
+    vr = inputs.gen_vloc(wl).numpy()
+    atoms = inputs.gen_atoms(wl)
+    na = min(atoms_sample, wl.natoms)
+    beta = inputs.gen_beta(wl, sp["miller"], atoms, 0, na).numpy() if na else None
+    db = inputs.gen_dblocks(wl)[:na] if na else None
+    psi = inputs.gen_psi(wl, sp["miller"], 0, nbands_sample).numpy()
+    t0 = time.perf_counter()
+    orc.hpsi_dual(sp["fft_index"], sp["g2kin"], tuple(wl.nr), vr, psi, None, None)
+    t_loc = time.perf_counter() - t0
+    t_nl = 0.0
+    if na:
+        t0 = time.perf_counter()
+        orc.vnl_psi(beta, db, psi)
+        t_nl = (time.perf_counter() - t0) * (wl.natoms / na)
+    per_band = (t_loc + t_nl) / nbands_sample
+    desc = (f"oracle Level B on {nbands_sample} bands of {wl.name}: local+kinetic on the full {wl.nr} grid, "
+            f"nonlocal on {na}/{wl.natoms} atoms scaled linearly")
+    return per_band, desc, torch.get_num_threads()
+
+
+def run_reference(args, wl, rank):
+    if rank != 0:
+        return
+    times = []
+    desc, cores = "", 0
+    for i in range(args.warmup + args.steps):
+        per_band, desc, cores = oracle_sample_time(wl)
+        if i >= args.warmup:
+            times.append(per_band)
+    per_band = float(np.mean(times))
+    val = 1.0 / per_band
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": per_band * wl.nbands * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "nbands": wl.nbands, "batch": wl.batch, "grid": list(wl.nr), "nproj": wl.nproj},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    from paper_2104_10502_b200 import inputs
+
+    wl = inputs.get_workload(args.config)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, wl, rank)
+        return
+
+    from paper_2104_10502_b200 import qe_hpsi
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the H|psi> path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # ---- inputs, resident in HBM ---------------------------------------------------------------------
+    t_setup = time.perf_counter()
+    h, inp = qe_hpsi.from_workload(wl, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
+    info = h.info()
+    npw, ld = h.npw, inp["ld"]
+    nb, batch = wl.nbands, wl.batch
+    psi = torch.empty((nb, ld), dtype=torch.complex128, device="cuda")
+    for b0 in range(0, nb, batch):  # rank r applies H to its own bands (band keys offset by rank * nbands)
+        psi[b0:b0 + batch] = inputs.gen_psi(wl, inp["miller_dev"], rank * nb + b0, min(batch, nb - b0), ld=ld, device="cuda")
+    hpsi = torch.zeros_like(psi)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t_setup
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for b0 in range(0, nb, batch):
+            h.apply(psi[b0:b0 + batch], hpsi[b0:b0 + batch], stream)
+
+    # inputs per step (psi 6.3 GB + beta 25 GB at config 4) exceed the 126 MB L2; for small configs flush L2
+    flush = None
+    if (psi.numel() * 16 + (inp["beta"].numel() * 16 if inp["beta"] is not None else 0)) < (512 << 20):
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    h.profile(1)
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for k in range(args.steps):
+        if flush is not None:
+            flush.fill_(k)
+        evs[k][0].record(stream)
+        step()
+        evs[k][1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    prof = h.profile_read()
+    h.profile(0)
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * nb / (ms_per_step * 1e-3)
+
+    # ---- e2e through the host-buffer entry point ------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        ph = torch.empty((nb, ld), dtype=torch.complex128).pin_memory()
+        hh = torch.empty((nb, ld), dtype=torch.complex128).pin_memory()
+        ph.copy_(psi)
+        for _ in range(2):
+            h.apply_host(ph, hh)
+        barrier()
+        t0 = time.perf_counter()
+        ne = max(2, min(args.steps, 3))
+        for _ in range(ne):
+            h.apply_host(ph, hh)  # synchronous: returns after the last D2H copy
+        t_e2e = (time.perf_counter() - t0) / ne
+        if dist is not None:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        # the e2e result must be the device path's result
+        assert torch.equal(hh[:, :npw].view(torch.float64), hpsi[:, :npw].cpu().view(torch.float64)), "e2e != device path"
+        e2e = {"value": world * nb / t_e2e, "unit": UNIT, "h2d_bytes_per_step": nb * npw * 16,
+               "d2h_bytes_per_step": nb * npw * 16, "ms_per_step": t_e2e * 1e3}
+        del ph, hh
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline --------------------------------------------------------------------------------------
+    m = model(wl, info)
+    hbm_peak, peak_src, mp = peaks()
+    dmma, dfma = qe_hpsi.qe_hpsi_probe_fp64(300.0)
+    chunks_per_step = (nb + batch - 1) // batch
+    stage = {k: (v[0] / max(v[1], 1), v[1]) for k, v in prof.items()}  # avg ms per span
+    t_becp, t_vnl, t_fft = stage["a6_becp"][0], stage["a8_vnl_add"][0], stage["a1_a5_fft_chain"][0]
+    flops_launch = 8.0 * wl.nproj * npw * min(batch, nb)  # per ZGEMM launch (one chunk)
+    roof_t = max((m["b_fft"] + m["b_beta"]) / (hbm_peak * 1e9), m["f_proj"] / (dmma * 1e12))  # s per band
+    if wl.nproj and t_vnl + t_becp > t_fft:
+        kname, t_k = ("k_vnl_add", t_vnl) if t_vnl >= t_becp else ("k_becp", t_becp)
+        ach = flops_launch / (t_k * 1e-3) * 1e-12
+        roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
+                    "traffic": committed_traffic(args.config, kname), "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-resident "
+                    "loop measured live by qe_hpsi_probe_fp64; MEASURED_PEAKS.json has no FP64 entry",
+                    "ms_per_launch": t_k, "flops_per_launch": flops_launch}
+    else:
+        bytes_launch = m["b_fft"] * min(batch, nb)
+        ach = bytes_launch / (t_fft * 1e-3) * 1e-9
+        roofline = {"bound": "hbm", "kernel": "a1-a5 FFT chain (5 kernels per sub-chunk)", "achieved": ach, "peak": hbm_peak,
+                    "unit": "GB/s", "frac": ach / hbm_peak, "traffic": committed_traffic(args.config, "fft_chain"),
+                    "peak_source": peak_src, "ms_per_launch": t_fft, "bytes_per_launch": bytes_launch}
+    stages = {"a6_becp_ms": t_becp, "a7_ms": stage["a7_reduce_dmul"][0], "a1_a5_fft_ms": t_fft, "a8_vnl_add_ms": t_vnl,
+              "per": f"chunk of {min(batch, nb)} bands", "chunks_per_step": chunks_per_step,
+              "becp_tflops": flops_launch / (t_becp * 1e-3) * 1e-12 if t_becp else None,
+              "vnl_tflops": flops_launch / (t_vnl * 1e-3) * 1e-12 if t_vnl else None,
+              "fft_algorithmic_gbs": m["b_fft"] * min(batch, nb) / (t_fft * 1e-3) * 1e-9 if t_fft else None}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        per_band, desc, cores = oracle_sample_time(wl)
+        cpu = {"value": 1.0 / per_band, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": wl.name, "nbands": nb, "batch": batch, "grid": list(wl.nr), "npw": npw, "nproj": wl.nproj,
+                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["nsplit"],
+                       "l2": "inputs per step exceed L2" if flush is None else "L2 flushed (256 MB write) between steps",
+                       "sharding": "bands / k-point pools per rank, no collective"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": h.launch_count(batch) * chunks_per_step * args.steps if nb % batch == 0
+            else sum(h.launch_count(min(batch, nb - b0)) for b0 in range(0, nb, batch)) * args.steps,
+            "roofline": roofline,
+            "combined_roofline": {"bands_per_s": 1.0 / roof_t, "frac": value / world * roof_t, "hbm_gbs": hbm_peak,
+                                  "fp64_tensor_tflops": dmma, "fp64_dfma_tflops": dfma, "bytes_per_band": m["b_fft"] + m["b_beta"],
+                                  "proj_flops_per_band": m["f_proj"], "note": "max(bytes/HBM, projector flops/FP64 tensor) per band"},
+            "stages": stages, "cpu_baseline": cpu, "setup_s": t_setup}
+    print(json.dumps(line), flush=True)
+
+    if args.detail:
+        h.profile(2)
+        step()
+        torch.cuda.synchronize()
+        d = h.profile_read()
+        h.profile(0)
+        for k, (ms, cnt) in d.items():
+            if cnt:
+                sys.stderr.write(f"{k:18s} total {ms:10.3f} ms over {cnt} spans\n")
+    h.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -118,6 +118,14 @@ int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);
 const char* qe_hpsi_strerror(int status);
 int qe_hpsi_last_cuda_error(qe_hpsi_t h);    /* cudaError_t of the last QE_HPSI_ECUDA (0 if none)               */
 
+/* Stage timing for the roofline report.  mode 0 = off (default; apply records no events), 1 = CUDA events around
+ * a6 (slot 0), a7 (slot 1), the whole a1-a5 chain (slot 2) and a8 (slot 3) of every chunk, 2 = additionally
+ * around each of the five FFT kernels a1..a5 (slots 4..8; slot 2 is then not recorded).  Events are recorded
+ * on the stream passed to apply.  qe_hpsi_profile resets the accumulators; qe_hpsi_profile_read synchronises
+ * the pending events and returns, per slot, the summed milliseconds and the number of spans. */
+int qe_hpsi_profile(qe_hpsi_t h, int mode);
+int qe_hpsi_profile_read(qe_hpsi_t h, double ms[16], int64_t count[16]);
+
 /* Measurement helper (not on the hot path): runs register-resident FP64 DMMA (mma.sync m8n8k4.f64) and DFMA
  * loops on every SM for about `millis` ms each and returns the achieved TFLOP/s.  bench.py uses the DMMA
  * figure as the measured FP64 tensor peak of the box.  Synchronises the device. */

@@ -77,6 +77,17 @@ struct qe_hpsi_handle {
   long long ldint = 0;
   cudaStream_t st_in = nullptr, st_comp = nullptr, st_out = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+  // optional stage timing (qe_hpsi_profile): CUDA events recorded around stages on the caller's stream
+  int prof_mode = 0;
+  std::vector<cudaEvent_t> prof_pool;
+  size_t prof_used = 0;
+  struct ProfSpan {
+    size_t e0, e1;
+    int slot;
+  };
+  std::vector<ProfSpan> prof_spans;
+  double prof_ms[16] = {0};
+  long long prof_cnt[16] = {0};
 };
 
 namespace {
@@ -92,6 +103,46 @@ namespace {
   } while (0)
 
 int g_last_cuda = 0;
+
+// ---- stage timing helpers ---------------------------------------------------------------------------------
+enum { SLOT_BECP = 0, SLOT_DMUL = 1, SLOT_FFT = 2, SLOT_VNL = 3, SLOT_A1 = 4, SLOT_A2 = 5, SLOT_A3 = 6, SLOT_A4 = 7, SLOT_A5 = 8 };
+
+void prof_drain(qe_hpsi_handle* h) {
+  if (h->prof_spans.empty()) {
+    h->prof_used = 0;
+    return;
+  }
+  cudaEventSynchronize(h->prof_pool[h->prof_spans.back().e1]);
+  for (const auto& sp : h->prof_spans) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, h->prof_pool[sp.e0], h->prof_pool[sp.e1]) == cudaSuccess) {
+      h->prof_ms[sp.slot] += ms;
+      h->prof_cnt[sp.slot] += 1;
+    }
+  }
+  h->prof_spans.clear();
+  h->prof_used = 0;
+}
+// returns the index of a freshly recorded event, or (size_t)-1 when timing is off
+size_t prof_mark(qe_hpsi_handle* h, cudaStream_t st) {
+  if (!h->prof_mode) return (size_t)-1;
+  if (h->prof_used == h->prof_pool.size()) {
+    if (h->prof_pool.size() >= 16384) {
+      prof_drain(h);
+    } else {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) return (size_t)-1;
+      h->prof_pool.push_back(e);
+    }
+  }
+  const size_t i = h->prof_used++;
+  cudaEventRecord(h->prof_pool[i], st);
+  return i;
+}
+void prof_span(qe_hpsi_handle* h, size_t e0, size_t e1, int slot) {
+  if (e0 == (size_t)-1 || e1 == (size_t)-1 || e1 < e0) return;
+  h->prof_spans.push_back({e0, e1, slot});
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // host geometry: reciprocal lattice and fractional k with a FIXED operation order so
@@ -482,6 +533,7 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
     if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
     if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
   }
+  for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
   if (h->st_in) cudaStreamDestroy(h->st_in);
   if (h->st_comp) cudaStreamDestroy(h->st_comp);
   if (h->st_out) cudaStreamDestroy(h->st_out);
@@ -759,11 +811,27 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     const int n = std::min(h->fft_nb, nb - b0);
     const double2* p = psi + (size_t)b0 * ldpsi;
     double2* o = hpsi + (size_t)b0 * ldh;
+    const bool fine = h->prof_mode == 2;
+    size_t m0 = fine ? prof_mark(h, st) : (size_t)-1;
     k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
+    size_t m1 = fine ? prof_mark(h, st) : (size_t)-1;
     k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
+    size_t m2 = fine ? prof_mark(h, st) : (size_t)-1;
     k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
+    size_t m3 = fine ? prof_mark(h, st) : (size_t)-1;
     k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
+    size_t m4 = fine ? prof_mark(h, st) : (size_t)-1;
     k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
+    if (fine) {
+      size_t m5 = prof_mark(h, st);
+      if (m5 != (size_t)-1 && m5 > m0) {  // a drain in between would have reset the indices
+        prof_span(h, m0, m1, SLOT_A1);
+        prof_span(h, m1, m2, SLOT_A2);
+        prof_span(h, m2, m3, SLOT_A3);
+        prof_span(h, m3, m4, SLOT_A4);
+        prof_span(h, m4, m5, SLOT_A5);
+      }
+    }
   }
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
@@ -772,12 +840,16 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const int mt = (h->nproj + ZG_BM - 1) / ZG_BM, nt = (nb + ZG_BN - 1) / ZG_BN;
+  const size_t t0 = prof_mark(h, st);
   k_becp<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE><<<dim3(mt * nt, h->nsplit), ZG_NT, BECP_SMEM, st>>>(
       h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb, h->npw, h->kchunk, h->partial, h->ldc);
+  const size_t t1 = prof_mark(h, st);
+  prof_span(h, t0, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
   k_becp_reduce<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->becp);
   k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
                             h->dbT, h->ldp);
+  prof_span(h, t1, prof_mark(h, st), SLOT_DMUL);
   h->nb_last = nb;
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
@@ -796,15 +868,23 @@ int launch_vnl_add(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream
 int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi, long long ldh, int nb, cudaStream_t st,
                 bool local, bool nonlocal) {
   int rc = QE_HPSI_OK;
-  if (nonlocal && h->nproj > 0 && h->npw > 0) {
+  const bool nl = nonlocal && h->nproj > 0 && h->npw > 0;
+  if (h->prof_mode && h->prof_used + 16 > 16384) prof_drain(h);
+  if (nl) {
     rc = launch_becp(h, psi, ldpsi, nb, st);
     if (rc) return rc;
   }
   if (local) {
+    const size_t t0 = h->prof_mode == 1 ? prof_mark(h, st) : (size_t)-1;
     rc = launch_local(h, psi, ldpsi, hpsi, ldh, nb, st);
     if (rc) return rc;
+    if (h->prof_mode == 1) prof_span(h, t0, prof_mark(h, st), SLOT_FFT);
   }
-  if (nonlocal && h->nproj > 0 && h->npw > 0) rc = launch_vnl_add(h, hpsi, ldh, nb, st);
+  if (nl) {
+    const size_t t0 = prof_mark(h, st);
+    rc = launch_vnl_add(h, hpsi, ldh, nb, st);
+    prof_span(h, t0, prof_mark(h, st), SLOT_VNL);
+  }
   return rc;
 }
 
@@ -947,6 +1027,28 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[9] = h->kchunk;
   info[10] = h->x_split;
   info[11] = h->num_sms;
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_profile(qe_hpsi_t h, int mode) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (mode < 0 || mode > 2) return QE_HPSI_EINVAL;
+  prof_drain(h);
+  for (int i = 0; i < 16; ++i) {
+    h->prof_ms[i] = 0.0;
+    h->prof_cnt[i] = 0;
+  }
+  h->prof_mode = mode;
+  return QE_HPSI_OK;
+}
+extern "C" int qe_hpsi_profile_read(qe_hpsi_t h, double ms[16], int64_t count[16]) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!ms || !count) return QE_HPSI_EINVAL;
+  prof_drain(h);
+  for (int i = 0; i < 16; ++i) {
+    ms[i] = h->prof_ms[i];
+    count[i] = h->prof_cnt[i];
+  }
   return QE_HPSI_OK;
 }
 

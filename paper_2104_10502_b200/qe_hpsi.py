@@ -43,6 +43,8 @@ SIGNATURES = {
     "qe_hpsi_strerror": (_c.c_char_p, [_i32]),
     "qe_hpsi_last_cuda_error": (_i32, [_vp]),
     "qe_hpsi_probe_fp64": (_i32, [_dbl, _pd, _pd]),
+    "qe_hpsi_profile": (_i32, [_vp, _i32]),
+    "qe_hpsi_profile_read": (_i32, [_vp, _pd, _pi64]),
     "qe_hpsi_fft_local": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
     "qe_hpsi_nonlocal": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
 }
@@ -210,6 +212,20 @@ class Hpsi:
         keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
                 "x_split", "num_sms"]
         return {k: int(buf[i]) for i, k in enumerate(keys)}
+
+    PROFILE_SLOTS = ["a6_becp", "a7_reduce_dmul", "a1_a5_fft_chain", "a8_vnl_add", "a1_scatter_zinv", "a2_yinv",
+                     "a3_x_vmul", "a4_yfwd", "a5_zfwd_gather"]
+
+    def profile(self, mode: int):
+        """qe_hpsi_profile: 0 off, 1 stage events, 2 per-FFT-kernel events. Resets the accumulators."""
+        _check(self._lib.qe_hpsi_profile(self._h, int(mode)), self._h)
+
+    def profile_read(self) -> dict:
+        """{slot name: (total ms, spans)} accumulated since the last profile() call (synchronises)."""
+        ms = (_c.c_double * 16)()
+        cnt = (_c.c_int64 * 16)()
+        _check(self._lib.qe_hpsi_profile_read(self._h, ms, cnt), self._h)
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(self.PROFILE_SLOTS)}
 
     def launch_count(self, nbands) -> int:
         return int(self._lib.qe_hpsi_launch_count(self._h, int(nbands)))
