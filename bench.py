@@ -195,7 +195,7 @@ def main():
         run_reference(args, wl, rank)
         return
 
-    from paper_2104_10502_b200 import qe_hpsi
+    from paper_2104_10502_b200 import qe_hpsi, sharding
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the H|psi> path has no CPU fallback")
@@ -212,16 +212,18 @@ def main():
     npw, ld = h.npw, inp["ld"]
     nb, batch = wl.nbands, wl.batch
     psi = torch.empty((nb, ld), dtype=torch.complex128, device="cuda")
-    for b0 in range(0, nb, batch):  # rank r applies H to its own bands (band keys offset by rank * nbands)
-        psi[b0:b0 + batch] = inputs.gen_psi(wl, inp["miller_dev"], rank * nb + b0, min(batch, nb - b0), ld=ld, device="cuda")
+    band0, _ = sharding.weak_band_range(rank, nb)  # rank r applies H to its own bands (keys rank*nb ...)
+    calls = sharding.batches(nb, batch)
+    for b0, n in calls:
+        psi[b0:b0 + n] = inputs.gen_psi(wl, inp["miller_dev"], band0 + b0, n, ld=ld, device="cuda")
     hpsi = torch.zeros_like(psi)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
     stream = torch.cuda.current_stream()
 
     def step():
-        for b0 in range(0, nb, batch):
-            h.apply(psi[b0:b0 + batch], hpsi[b0:b0 + batch], stream)
+        for b0, n in calls:
+            h.apply(psi[b0:b0 + n], hpsi[b0:b0 + n], stream)
 
     # inputs per step (psi 6.3 GB + beta 25 GB at config 4) exceed the 126 MB L2; for small configs flush L2
     flush = None
@@ -253,12 +255,9 @@ def main():
     total_ms = float(sum(step_ms))
     prof = h.profile_read()
     h.profile(0)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * nb / (ms_per_step * 1e-3)
+    value = sharding.aggregate_bands_per_s(world, nb, ms_per_step)
 
     # ---- e2e through the host-buffer entry point ------------------------------------------------------
     e2e = None
@@ -274,10 +273,7 @@ def main():
         for _ in range(ne):
             h.apply_host(ph, hh)  # synchronous: returns after the last D2H copy
         t_e2e = (time.perf_counter() - t0) / ne
-        if dist is not None:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = sharding.max_over_ranks(t_e2e, dist, "cuda")
         # the e2e result must be the device path's result
         assert torch.equal(hh[:, :npw].view(torch.float64), hpsi[:, :npw].cpu().view(torch.float64)), "e2e != device path"
         e2e = {"value": world * nb / t_e2e, "unit": UNIT, "h2d_bytes_per_step": nb * npw * 16,
