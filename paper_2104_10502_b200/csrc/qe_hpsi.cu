@@ -24,11 +24,16 @@ namespace {
 constexpr double TWO_PI = 6.283185307179586;
 constexpr int NUM_SMS_FALLBACK = 148;
 
-// ZGEMM tile configuration (see zgemm_kernels.cuh)
-constexpr int ZG_BM = 128, ZG_BN = 64, ZG_WM = 4, ZG_WN = 2, ZG_NSTAGE = 4;
-constexpr int ZG_NT = ZG_WM * ZG_WN * 32;
-constexpr size_t BECP_SMEM = (size_t)ZG_NSTAGE * (ZG_BM + ZG_BN) * ZG_BK * sizeof(double2);
-constexpr size_t VNL_SMEM = (size_t)ZG_NSTAGE * (ZG_BK * (ZG_BM + 2) + ZG_BN * ZG_BK) * sizeof(double2);
+// ZGEMM tile configurations (see zgemm_kernels.cuh): BM, BN, warps along M, warps along N, BK, pipeline stages.
+// Variant 0 is the product default; the others exist for tuning runs (env QE_HPSI_ZG_VARIANT).
+using ZgV0 = ZgCfg<64, 64, 2, 4, 16, 4>;
+using ZgV1 = ZgCfg<64, 64, 4, 4, 16, 4>;
+using ZgV2 = ZgCfg<128, 32, 4, 2, 16, 4>;
+using ZgV3 = ZgCfg<64, 64, 2, 4, 8, 6>;
+constexpr int ZG_NVARIANT = 4;
+constexpr int ZG_BM_TAB[ZG_NVARIANT] = {64, 64, 128, 64};
+constexpr int ZG_BN_TAB[ZG_NVARIANT] = {64, 64, 32, 64};
+constexpr int ZG_BK_TAB[ZG_NVARIANT] = {16, 16, 16, 8};
 
 struct DevBuf {
   void* p = nullptr;
@@ -68,6 +73,7 @@ struct qe_hpsi_handle {
   int max_batch = 0;
   int ldc = 0, ldp = 0;
   int nsplit = 1, kchunk = 0;
+  int zg_variant = 0;
   double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
   int nb_last = 0;
   size_t workspace_bytes = 0;
@@ -454,8 +460,14 @@ cudaError_t set_kernel_attrs() {
   SET_SMEM(k_x_vmul);
   SET_SMEM(k_yfwd);
   SET_SMEM(k_zfwd_gather);
-  SET_SMEM((k_becp<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE>));
-  SET_SMEM((k_vnl_add<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE>));
+  SET_SMEM(k_becp<ZgV0>);
+  SET_SMEM(k_vnl_add<ZgV0>);
+  SET_SMEM(k_becp<ZgV1>);
+  SET_SMEM(k_vnl_add<ZgV1>);
+  SET_SMEM(k_becp<ZgV2>);
+  SET_SMEM(k_vnl_add<ZgV2>);
+  SET_SMEM(k_becp<ZgV3>);
+  SET_SMEM(k_vnl_add<ZgV3>);
 #undef SET_SMEM
   g_attr_done = true;
   return cudaSuccess;
@@ -551,6 +563,7 @@ int env_int(const char* name, int dflt) {
 
 // choose the split-K count of a6 so that (M tiles x N tiles x nsplit) fills whole waves of CTAs
 void choose_split(qe_hpsi_handle* h) {
+  const int ZG_BM = ZG_BM_TAB[h->zg_variant], ZG_BN = ZG_BN_TAB[h->zg_variant], ZG_BK = ZG_BK_TAB[h->zg_variant];
   const int ntile = ((h->nproj + ZG_BM - 1) / ZG_BM) * ((h->max_batch + ZG_BN - 1) / ZG_BN);
   const int ksmax = std::max(1, h->npw / 512);
   int best = 1;
@@ -763,9 +776,11 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     CR_TRY(upload(&h->dpk, dv, st));
     h->ldc = (max_batch + 1) / 2 * 2;
     h->ldp = (nproj + 7) / 8 * 8;
+    h->zg_variant = std::min(std::max(env_int("QE_HPSI_ZG_VARIANT", 0), 0), ZG_NVARIANT - 1);
     choose_split(h);
     const int forced = env_int("QE_HPSI_NSPLIT", 0);
     if (forced > 0) {
+      const int ZG_BK = ZG_BK_TAB[h->zg_variant];
       int kchunk = (h->npw + forced - 1) / forced;
       kchunk = std::max(ZG_BK, (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK);
       h->kchunk = kchunk;
@@ -837,12 +852,29 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
   return QE_HPSI_OK;
 }
 
+template <class Cfg>
+void becp_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
+  const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  k_becp<Cfg><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
+                                                                         h->npw, h->kchunk, h->partial, h->ldc);
+}
+template <class Cfg>
+void vnl_launch(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  if (mt == 0) return;
+  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->dbT, h->ldp,
+                                                                    nb, hpsi, ldh);
+}
+
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
-  const int mt = (h->nproj + ZG_BM - 1) / ZG_BM, nt = (nb + ZG_BN - 1) / ZG_BN;
   const size_t t0 = prof_mark(h, st);
-  k_becp<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE><<<dim3(mt * nt, h->nsplit), ZG_NT, BECP_SMEM, st>>>(
-      h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb, h->npw, h->kchunk, h->partial, h->ldc);
+  switch (h->zg_variant) {
+    case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st); break;
+    case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st); break;
+    case 3: becp_launch<ZgV3>(h, psi, ldpsi, nb, st); break;
+    default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st); break;
+  }
   const size_t t1 = prof_mark(h, st);
   prof_span(h, t0, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
@@ -857,10 +889,12 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 
 // a8
 int launch_vnl_add(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
-  const int mt = (h->npw + ZG_BM - 1) / ZG_BM, nt = (nb + ZG_BN - 1) / ZG_BN;
-  if (mt == 0) return QE_HPSI_OK;
-  k_vnl_add<ZG_BM, ZG_BN, ZG_WM, ZG_WN, ZG_NSTAGE><<<(unsigned)(mt * nt), ZG_NT, VNL_SMEM, st>>>(
-      h->beta, h->ldbeta, h->nproj, h->npw, h->dbT, h->ldp, nb, hpsi, ldh);
+  switch (h->zg_variant) {
+    case 1: vnl_launch<ZgV1>(h, hpsi, ldh, nb, st); break;
+    case 2: vnl_launch<ZgV2>(h, hpsi, ldh, nb, st); break;
+    case 3: vnl_launch<ZgV3>(h, hpsi, ldh, nb, st); break;
+    default: vnl_launch<ZgV0>(h, hpsi, ldh, nb, st); break;
+  }
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
 }

@@ -1,12 +1,18 @@
 // zgemm_kernels.cuh -- the nonlocal (pseudopotential) term as FP64 tensor-core contractions (steps a6-a8 of
-// DESIGN.md section 2; "pseudopotential ... contributions to the Hamiltonian", done with GEMM
+// DESIGN.md section 5; "pseudopotential ... contributions to the Hamiltonian", done with GEMM
 // in the paper's port).
 //   a6 k_becp     : partial[ks][p][b] = sum_{ig in K-slice ks} conj(beta[p][ig]) psi[b][ig]     (split-K ZGEMM)
 //   a7 k_becp_reduce / k_dmul : becp = sum_ks partial (fixed order); dbecpT[b][p] = sum_j D^a_ij becp[a,j][b]
 //   a8 k_vnl_add  : hpsi[b][ig] += sum_p beta[p][ig] dbecpT[b][p]                                 (ZGEMM)
 // FP64 tensor math on sm_100a exists only as warp-level mma.sync (DMMA.8x8x4 in SASS; there is no tcgen05 /
 // TMEM path for f64), so the tiles are fed by cp.async multi-stage pipelines into bank-conflict-free shared
-// memory layouts and each warp owns a 32x32 complex accumulator tile (4 real DMMAs per complex 8x8x4 block).
+// memory layouts.
+//
+// Complex product = "3M" (Karatsuba) form: with P = sum ar*br, Q = sum ai*bi, R = sum (ar+ai)*(br+bi),
+//   sum a*b       = (P - Q) + i (R - P - Q)
+//   sum conj(a)*b = (P + Q) + i (R' - P + Q),   R' = sum (ar-ai)*(br+bi)
+// i.e. three real DMMAs per complex 8x8x4 block instead of four; the fragment sums cost one DADD per loaded
+// element.  Normwise error stays O(eps*sqrt(K)) (tolerance).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -28,29 +34,58 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N));
 }
 
-constexpr int ZG_BK = 8;  // complex k per pipeline stage (two DMMA k-steps)
+// K-contiguous operand tile: rows of BK complex; 16-byte column kc of odd rows is XOR-ed with 4 so that a
+// fragment load (quarter warp = 2 rows x 4 k) touches 8 distinct 16-byte bank groups.
+template <int BK>
+__device__ __forceinline__ int swz_k(int row, int kc) {
+  return row * BK + (kc ^ ((row & 1) << 2));
+}
 
-// rows of 8 complex (128 B), K contiguous; the two 64-byte halves of odd rows are swapped so that the fragment
-// load (8 lanes = 2 rows x 4 k) touches 8 distinct 16-byte bank groups.
-__device__ __forceinline__ int swz_k8(int row, int kc) { return row * 8 + (kc ^ ((row & 1) << 2)); }
-
-template <int BM, int BN, int WM, int WN, int NSTAGE>
+template <int BM_, int BN_, int WM_, int WN_, int BK_, int NSTAGE_>
 struct ZgCfg {
+  static constexpr int BM = BM_, BN = BN_, WM = WM_, WN = WN_, BK = BK_, NSTAGE = NSTAGE_;
   static constexpr int NT = WM * WN * 32;
   static constexpr int TM = BM / WM / 8;  // 8-row blocks per warp along M
   static constexpr int TN = BN / WN / 8;
-  static_assert(BM % (WM * 8) == 0 && BN % (WN * 8) == 0, "tile shape");
+  static constexpr int KSTEPS = BK / 4;
+  static constexpr int LDA_M = BM + 2;  // row stride of an M-contiguous [k][m] tile: (2k + m) mod 8 distinct per quarter warp
+  static constexpr size_t SMEM_BECP = (size_t)NSTAGE * (BM + BN) * BK * sizeof(double2);
+  static constexpr size_t SMEM_VNL = (size_t)NSTAGE * (BK * LDA_M + BN * BK) * sizeof(double2);
+  static_assert(BM % (WM * 8) == 0 && BN % (WN * 8) == 0 && BK % 4 == 0 && BK >= 8, "tile shape");
 };
+
+// one k4 step of the 3M product on a TM x TN grid of 8x8 blocks
+template <int TM, int TN, bool CONJ_A>
+__device__ __forceinline__ void mma3m(double (&P)[TM][TN][2], double (&Q)[TM][TN][2], double (&R)[TM][TN][2],
+                                      const double2 (&af)[TM], const double2 (&bf)[TN]) {
+  double as[TM], bs[TN];
+#pragma unroll
+  for (int i = 0; i < TM; ++i) as[i] = CONJ_A ? af[i].x - af[i].y : af[i].x + af[i].y;
+#pragma unroll
+  for (int j = 0; j < TN; ++j) bs[j] = bf[j].x + bf[j].y;
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) dmma884(P[i][j][0], P[i][j][1], af[i].x, bf[j].x);
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) dmma884(Q[i][j][0], Q[i][j][1], af[i].y, bf[j].y);
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) dmma884(R[i][j][0], R[i][j][1], as[i], bs[j]);
+}
 
 // a6 ------------------------------------------------------------------------------------------------------
 // C[p][b] = sum_k conj(A[p][k]) B[b][k] over k in [ks*kchunk, min(npw,(ks+1)*kchunk)); A = beta, B = psi.
-template <int BM, int BN, int WM, int WN, int NSTAGE>
-__global__ void __launch_bounds__(WM* WN * 32, 1)
+template <class Cfg>
+__global__ void __launch_bounds__(Cfg::NT, 1)
     k_becp(const double2* __restrict__ beta, long long ldb, int nproj, const double2* __restrict__ psi, long long ldpsi,
            int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc) {
-  using Cfg = ZgCfg<BM, BN, WM, WN, NSTAGE>;
-  constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN;
-  constexpr int STAGE = (BM + BN) * ZG_BK;  // complex elements per stage
+  constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
+  constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS;
+  constexpr int STAGE = (BM + BN) * BK;  // complex elements per stage
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* sm = reinterpret_cast<double2*>(smem_raw);
 
@@ -60,33 +95,36 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
   const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
   const int ks = blockIdx.y;
   const int kb = ks * kchunk, ke = min(npw, kb + kchunk);
-  const int nkt = (ke - kb + ZG_BK - 1) / ZG_BK;
+  const int nkt = (ke - kb + BK - 1) / BK;
 
   auto load_stage = [&](int kt, int st) {
     double2* As = sm + st * STAGE;
-    double2* Bs = As + BM * ZG_BK;
-    const int k0 = kb + kt * ZG_BK;
-    for (int id = tid; id < (BM + BN) * ZG_BK; id += NT) {
-      const int kc = id & 7;
-      const int r = id >> 3;
+    double2* Bs = As + BM * BK;
+    const int k0 = kb + kt * BK;
+#pragma unroll
+    for (int id = tid; id < (BM + BN) * BK; id += NT) {
+      const int kc = id % BK;
+      const int r = id / BK;
       const bool kok = (k0 + kc) < ke;
       if (r < BM) {
         const int p = m0 + r;
         const bool ok = kok && p < nproj;
-        cp_async16(&As[swz_k8(r, kc)], ok ? &beta[(size_t)p * ldb + k0 + kc] : beta, ok);
+        cp_async16(&As[swz_k<BK>(r, kc)], ok ? &beta[(size_t)p * ldb + k0 + kc] : beta, ok);
       } else {
         const int rb = r - BM, b = n0 + rb;
         const bool ok = kok && b < nb;
-        cp_async16(&Bs[swz_k8(rb, kc)], ok ? &psi[(size_t)b * ldpsi + k0 + kc] : psi, ok);
+        cp_async16(&Bs[swz_k<BK>(rb, kc)], ok ? &psi[(size_t)b * ldpsi + k0 + kc] : psi, ok);
       }
     }
   };
 
-  double cre[TM][TN][2], cim[TM][TN][2];
+  double P[TM][TN][2], Q[TM][TN][2], R[TM][TN][2];
 #pragma unroll
   for (int i = 0; i < TM; ++i)
 #pragma unroll
-    for (int j = 0; j < TN; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+    for (int j = 0; j < TN; ++j)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
 
 #pragma unroll
   for (int s = 0; s < NSTAGE - 1; ++s) {
@@ -100,30 +138,25 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
     if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, (kt + NSTAGE - 1) % NSTAGE);
     cp_async_commit();
     const double2* As = sm + (kt % NSTAGE) * STAGE;
-    const double2* Bs = As + BM * ZG_BK;
+    const double2* Bs = As + BM * BK;
+    double2 af[2][TM], bf[2][TN];
 #pragma unroll
-    for (int kk = 0; kk < 2; ++kk) {
-      double2 af[TM], bf[TN];
+    for (int i = 0; i < TM; ++i) af[0][i] = As[swz_k<BK>(wm0 + i * 8 + fr, fk)];
 #pragma unroll
-      for (int i = 0; i < TM; ++i) af[i] = As[swz_k8(wm0 + i * 8 + fr, kk * 4 + fk)];
+    for (int j = 0; j < TN; ++j) bf[0][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, fk)];
 #pragma unroll
-      for (int j = 0; j < TN; ++j) bf[j] = Bs[swz_k8(wn0 + j * 8 + fr, kk * 4 + fk)];
+    for (int kk = 0; kk < KSTEPS; ++kk) {
+      if (kk + 1 < KSTEPS) {
 #pragma unroll
-      for (int i = 0; i < TM; ++i) {
-        const double ar = af[i].x, ai = af[i].y, nai = -af[i].y;
+        for (int i = 0; i < TM; ++i) af[(kk + 1) & 1][i] = As[swz_k<BK>(wm0 + i * 8 + fr, (kk + 1) * 4 + fk)];
 #pragma unroll
-        for (int j = 0; j < TN; ++j) {
-          // conj(a) b = (ar br + ai bi) + i (ar bi - ai br)
-          dmma884(cre[i][j][0], cre[i][j][1], ar, bf[j].x);
-          dmma884(cim[i][j][0], cim[i][j][1], ar, bf[j].y);
-          dmma884(cre[i][j][0], cre[i][j][1], ai, bf[j].y);
-          dmma884(cim[i][j][0], cim[i][j][1], nai, bf[j].x);
-        }
+        for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
+      mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
     }
   }
   cp_async_wait<0>();
-  // C fragment: row = lane/4, columns 2*(lane%4) + {0,1}
+  // C fragment: row = lane/4, columns 2*(lane%4) + {0,1};  conj(a) b = (P + Q) + i (R - P + Q)
   double2* out = partial + (size_t)ks * nproj * ldc;
 #pragma unroll
   for (int i = 0; i < TM; ++i) {
@@ -131,9 +164,11 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
     if (p >= nproj) continue;
 #pragma unroll
     for (int j = 0; j < TN; ++j) {
-      const int b = n0 + wn0 + j * 8 + 2 * fk;
-      if (b < nb) out[(size_t)p * ldc + b] = make_double2(cre[i][j][0], cim[i][j][0]);
-      if (b + 1 < nb) out[(size_t)p * ldc + b + 1] = make_double2(cre[i][j][1], cim[i][j][1]);
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int b = n0 + wn0 + j * 8 + 2 * fk + e;
+        if (b < nb) out[(size_t)p * ldc + b] = make_double2(P[i][j][e] + Q[i][j][e], (R[i][j][e] - P[i][j][e]) + Q[i][j][e]);
+      }
     }
   }
 }
@@ -175,14 +210,13 @@ __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int
 
 // a8 ------------------------------------------------------------------------------------------------------
 // hpsi[b][g] += sum_p A[p][g] B[b][p];  A = beta ([p][g], g contiguous: "M-major"), B = dbT ([b][p], p contiguous)
-template <int BM, int BN, int WM, int WN, int NSTAGE>
-__global__ void __launch_bounds__(WM* WN * 32, 1)
+template <class Cfg>
+__global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_add(const double2* __restrict__ beta, long long ldb, int nproj, int npw, const double2* __restrict__ dbT,
               int ldp, int nb, double2* __restrict__ hpsi, long long ldh) {
-  using Cfg = ZgCfg<BM, BN, WM, WN, NSTAGE>;
-  constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN;
-  constexpr int LDA = BM + 2;  // row stride (complex) of the [k][g] tile: (2k + g) mod 8 distinct in a fragment load
-  constexpr int STAGE = ZG_BK * LDA + BN * ZG_BK;
+  constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
+  constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS, LDA = Cfg::LDA_M;
+  constexpr int STAGE = BK * LDA + BN * BK;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* sm = reinterpret_cast<double2*>(smem_raw);
 
@@ -190,31 +224,35 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
   const int wm0 = (warp / WN) * (BM / WM), wn0 = (warp % WN) * (BN / WN);
   const int ntn = (nb + BN - 1) / BN;
   const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
-  const int nkt = (nproj + ZG_BK - 1) / ZG_BK;
+  const int nkt = (nproj + BK - 1) / BK;
 
   auto load_stage = [&](int kt, int st) {
     double2* As = sm + st * STAGE;
-    double2* Bs = As + ZG_BK * LDA;
-    const int k0 = kt * ZG_BK;
-    for (int id = tid; id < ZG_BK * BM; id += NT) {
+    double2* Bs = As + BK * LDA;
+    const int k0 = kt * BK;
+#pragma unroll
+    for (int id = tid; id < BK * BM; id += NT) {
       const int gc = id % BM, r = id / BM;
       const int p = k0 + r, gg = m0 + gc;
       const bool ok = p < nproj && gg < npw;
       cp_async16(&As[r * LDA + gc], ok ? &beta[(size_t)p * ldb + gg] : beta, ok);
     }
-    for (int id = tid; id < BN * ZG_BK; id += NT) {
-      const int kc = id & 7, r = id >> 3;
+#pragma unroll
+    for (int id = tid; id < BN * BK; id += NT) {
+      const int kc = id % BK, r = id / BK;
       const int b = n0 + r;
       const bool ok = b < nb && (k0 + kc) < nproj;
-      cp_async16(&Bs[swz_k8(r, kc)], ok ? &dbT[(size_t)b * ldp + k0 + kc] : dbT, ok);
+      cp_async16(&Bs[swz_k<BK>(r, kc)], ok ? &dbT[(size_t)b * ldp + k0 + kc] : dbT, ok);
     }
   };
 
-  double cre[TM][TN][2], cim[TM][TN][2];
+  double P[TM][TN][2], Q[TM][TN][2], R[TM][TN][2];
 #pragma unroll
   for (int i = 0; i < TM; ++i)
 #pragma unroll
-    for (int j = 0; j < TN; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+    for (int j = 0; j < TN; ++j)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
 
 #pragma unroll
   for (int s = 0; s < NSTAGE - 1; ++s) {
@@ -228,29 +266,25 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
     if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, (kt + NSTAGE - 1) % NSTAGE);
     cp_async_commit();
     const double2* As = sm + (kt % NSTAGE) * STAGE;
-    const double2* Bs = As + ZG_BK * LDA;
+    const double2* Bs = As + BK * LDA;
+    double2 af[2][TM], bf[2][TN];
 #pragma unroll
-    for (int kk = 0; kk < 2; ++kk) {
-      double2 af[TM], bf[TN];
+    for (int i = 0; i < TM; ++i) af[0][i] = As[fk * LDA + wm0 + i * 8 + fr];
 #pragma unroll
-      for (int i = 0; i < TM; ++i) af[i] = As[(kk * 4 + fk) * LDA + wm0 + i * 8 + fr];
+    for (int j = 0; j < TN; ++j) bf[0][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, fk)];
 #pragma unroll
-      for (int j = 0; j < TN; ++j) bf[j] = Bs[swz_k8(wn0 + j * 8 + fr, kk * 4 + fk)];
+    for (int kk = 0; kk < KSTEPS; ++kk) {
+      if (kk + 1 < KSTEPS) {
 #pragma unroll
-      for (int j = 0; j < TN; ++j) {
-        const double br = bf[j].x, bi = bf[j].y, nbi = -bf[j].y;
+        for (int i = 0; i < TM; ++i) af[(kk + 1) & 1][i] = As[((kk + 1) * 4 + fk) * LDA + wm0 + i * 8 + fr];
 #pragma unroll
-        for (int i = 0; i < TM; ++i) {
-          // a b = (ar br - ai bi) + i (ar bi + ai br)
-          dmma884(cre[i][j][0], cre[i][j][1], af[i].x, br);
-          dmma884(cim[i][j][0], cim[i][j][1], af[i].x, bi);
-          dmma884(cre[i][j][0], cre[i][j][1], af[i].y, nbi);
-          dmma884(cim[i][j][0], cim[i][j][1], af[i].y, br);
-        }
+        for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
+      mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
     }
   }
   cp_async_wait<0>();
+  // a b = (P - Q) + i (R - P - Q)
 #pragma unroll
   for (int i = 0; i < TM; ++i) {
     const int gg = m0 + wm0 + i * 8 + fr;
@@ -263,8 +297,8 @@ __global__ void __launch_bounds__(WM* WN * 32, 1)
         if (b < nb) {
           double2* h = &hpsi[(size_t)b * ldh + gg];
           double2 v = *h;
-          v.x += cre[i][j][e];
-          v.y += cim[i][j][e];
+          v.x += P[i][j][e] - Q[i][j][e];
+          v.y += (R[i][j][e] - P[i][j][e]) - Q[i][j][e];
           *h = v;
         }
       }
