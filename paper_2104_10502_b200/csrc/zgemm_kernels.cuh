@@ -97,24 +97,44 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   const int kb = ks * kchunk, ke = min(npw, kb + kchunk);
   const int nkt = (ke - kb + BK - 1) / BK;
 
-  auto load_stage = [&](int kt, int st) {
-    double2* As = sm + st * STAGE;
-    double2* Bs = As + BM * BK;
-    const int k0 = kb + kt * BK;
+  // Per-thread copy plan, fixed for the whole K loop: thread owns 16-byte column kc of rows r0, r0+RPT, ...
+  // (A rows first, then B rows); only the k offset advances, so a stage costs one compare plus the cp.asyncs.
+  constexpr int RPT = NT / BK, NA = BM / RPT, NB = BN / RPT;
+  static_assert(NT % BK == 0 && BM % RPT == 0 && BN % RPT == 0 && RPT % 2 == 0, "copy plan");
+  const int ckc = tid % BK, cr0 = tid / BK;
+  const double2* asrc[NA];
+  const double2* bsrc[NB];
+  unsigned rowok = 0;
 #pragma unroll
-    for (int id = tid; id < (BM + BN) * BK; id += NT) {
-      const int kc = id % BK;
-      const int r = id / BK;
-      const bool kok = (k0 + kc) < ke;
-      if (r < BM) {
-        const int p = m0 + r;
-        const bool ok = kok && p < nproj;
-        cp_async16(&As[swz_k<BK>(r, kc)], ok ? &beta[(size_t)p * ldb + k0 + kc] : beta, ok);
-      } else {
-        const int rb = r - BM, b = n0 + rb;
-        const bool ok = kok && b < nb;
-        cp_async16(&Bs[swz_k<BK>(rb, kc)], ok ? &psi[(size_t)b * ldpsi + k0 + kc] : psi, ok);
-      }
+  for (int n = 0; n < NA; ++n) {
+    const int p = m0 + cr0 + n * RPT;
+    const bool ok = p < nproj;
+    rowok |= ok ? (1u << n) : 0u;
+    asrc[n] = beta + (size_t)(ok ? p : 0) * ldb + kb + ckc;
+  }
+#pragma unroll
+  for (int n = 0; n < NB; ++n) {
+    const int b = n0 + cr0 + n * RPT;
+    const bool ok = b < nb;
+    rowok |= ok ? (1u << (NA + n)) : 0u;
+    bsrc[n] = psi + (size_t)(ok ? b : 0) * ldpsi + kb + ckc;
+  }
+  const unsigned cdst = static_cast<unsigned>(__cvta_generic_to_shared(sm + swz_k<BK>(cr0, ckc)));
+  auto load_stage = [&](int kt, int st) {
+    const int koff = kt * BK;
+    const bool kok = (kb + koff + ckc) < ke;
+    const unsigned d0 = cdst + (unsigned)(st * STAGE * (int)sizeof(double2));
+#pragma unroll
+    for (int n = 0; n < NA; ++n) {
+      const int sz = (kok && ((rowok >> n) & 1u)) ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d0 + (unsigned)(n * RPT * BK * 16)),
+                   "l"(asrc[n] + koff), "r"(sz));
+    }
+#pragma unroll
+    for (int n = 0; n < NB; ++n) {
+      const int sz = (kok && ((rowok >> (NA + n)) & 1u)) ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d0 + (unsigned)((BM + n * RPT) * BK * 16)),
+                   "l"(bsrc[n] + koff), "r"(sz));
     }
   };
 
@@ -132,12 +152,11 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     cp_async_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
+  int st_c = 0, st_l = NSTAGE - 1;  // stage being consumed / stage being refilled
   for (int kt = 0; kt < nkt; ++kt) {
     cp_async_wait<NSTAGE - 2>();
     __syncthreads();
-    if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, (kt + NSTAGE - 1) % NSTAGE);
-    cp_async_commit();
-    const double2* As = sm + (kt % NSTAGE) * STAGE;
+    const double2* As = sm + st_c * STAGE;
     const double2* Bs = As + BM * BK;
     double2 af[2][TM], bf[2][TN];
 #pragma unroll
@@ -153,7 +172,13 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
       mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
+      if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
+        if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
+        cp_async_commit();
+      }
     }
+    st_c = (st_c + 1 == NSTAGE) ? 0 : st_c + 1;
+    st_l = (st_l + 1 == NSTAGE) ? 0 : st_l + 1;
   }
   cp_async_wait<0>();
   // C fragment: row = lane/4, columns 2*(lane%4) + {0,1};  conj(a) b = (P + Q) + i (R - P + Q)
@@ -226,23 +251,43 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
   const int nkt = (nproj + BK - 1) / BK;
 
+  // Per-thread copy plan (see k_becp).  A tile [BK][LDA]: thread owns column gc of rows ra, ra+RPA, ...; B tile
+  // [BN][BK]: column ckc of rows cr0, cr0+RPT, ...
+  constexpr int RPA = NT / BM, NA = BK / RPA, RPT = NT / BK, NB = BN / RPT;
+  static_assert(NT % BM == 0 && BK % RPA == 0 && NT % BK == 0 && BN % RPT == 0 && RPT % 2 == 0, "copy plan");
+  const int gc = tid % BM, ra = tid / BM;
+  const bool gok = (m0 + gc) < npw;
+  const double2* asrc = beta + (size_t)ra * ldb + (gok ? m0 + gc : 0);
+  const size_t astep = (size_t)RPA * ldb;
+  const unsigned adst = static_cast<unsigned>(__cvta_generic_to_shared(sm + ra * LDA + gc));
+  const int ckc = tid % BK, cr0 = tid / BK;
+  const double2* bsrc[NB];
+  unsigned rowok = 0;
+#pragma unroll
+  for (int n = 0; n < NB; ++n) {
+    const int b = n0 + cr0 + n * RPT;
+    const bool ok = b < nb;
+    rowok |= ok ? (1u << n) : 0u;
+    bsrc[n] = dbT + (size_t)(ok ? b : 0) * ldp + ckc;
+  }
+  const unsigned bdst = static_cast<unsigned>(__cvta_generic_to_shared(sm + BK * LDA + swz_k<BK>(cr0, ckc)));
   auto load_stage = [&](int kt, int st) {
-    double2* As = sm + st * STAGE;
-    double2* Bs = As + BK * LDA;
     const int k0 = kt * BK;
+    const unsigned soff = (unsigned)(st * STAGE * (int)sizeof(double2));
+    const double2* ap = asrc + (size_t)k0 * ldb;
 #pragma unroll
-    for (int id = tid; id < BK * BM; id += NT) {
-      const int gc = id % BM, r = id / BM;
-      const int p = k0 + r, gg = m0 + gc;
-      const bool ok = p < nproj && gg < npw;
-      cp_async16(&As[r * LDA + gc], ok ? &beta[(size_t)p * ldb + gg] : beta, ok);
+    for (int n = 0; n < NA; ++n) {
+      const bool ok = gok && (k0 + ra + n * RPA) < nproj;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(adst + soff + (unsigned)(n * RPA * LDA * 16)),
+                   "l"(ok ? ap : beta), "r"(ok ? 16 : 0));
+      ap += astep;
     }
+    const bool kok = (k0 + ckc) < nproj;
 #pragma unroll
-    for (int id = tid; id < BN * BK; id += NT) {
-      const int kc = id % BK, r = id / BK;
-      const int b = n0 + r;
-      const bool ok = b < nb && (k0 + kc) < nproj;
-      cp_async16(&Bs[swz_k<BK>(r, kc)], ok ? &dbT[(size_t)b * ldp + k0 + kc] : dbT, ok);
+    for (int n = 0; n < NB; ++n) {
+      const int sz = (kok && ((rowok >> n) & 1u)) ? 16 : 0;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(bdst + soff + (unsigned)(n * RPT * BK * 16)),
+                   "l"(bsrc[n] + k0), "r"(sz));
     }
   };
 
@@ -260,12 +305,11 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     cp_async_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
+  int st_c = 0, st_l = NSTAGE - 1;  // stage being consumed / stage being refilled
   for (int kt = 0; kt < nkt; ++kt) {
     cp_async_wait<NSTAGE - 2>();
     __syncthreads();
-    if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, (kt + NSTAGE - 1) % NSTAGE);
-    cp_async_commit();
-    const double2* As = sm + (kt % NSTAGE) * STAGE;
+    const double2* As = sm + st_c * STAGE;
     const double2* Bs = As + BK * LDA;
     double2 af[2][TM], bf[2][TN];
 #pragma unroll
@@ -281,7 +325,13 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
       mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
+      if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
+        if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
+        cp_async_commit();
+      }
     }
+    st_c = (st_c + 1 == NSTAGE) ? 0 : st_c + 1;
+    st_l = (st_l + 1 == NSTAGE) ? 0 : st_l + 1;
   }
   cp_async_wait<0>();
   // a b = (P - Q) + i (R - P - Q)
