@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "fft_kernels.cuh"
+#include "fft2p_kernels.cuh"
 #include "zgemm_kernels.cuh"
 
 using namespace qehpsi;
@@ -62,6 +63,11 @@ struct qe_hpsi_handle {
   int fft_nb = 1;  // bands per FFT sub-chunk (workspace kept L2-sized)
   int x_split = 1;
   double2 *w1 = nullptr, *w2 = nullptr;
+  // fast two-pass FFT path (fft2p_kernels.cuh): used when every grid dimension has a table entry
+  const Fft2pEntry* f2p[3] = {nullptr, nullptr, nullptr};  // per axis j = 0..2 (N1, N2, N3)
+  Fft2pGeom g2p{};
+  int *stick_lo = nullptr, *stick_hi = nullptr, *col_of = nullptr, *plane_of = nullptr;
+  size_t smem_x2p = 0;
   // nonlocal
   int nproj = 0;
   const double2* beta = nullptr;  // borrowed or owned
@@ -525,6 +531,10 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->plane_stick);
   cudaFree(h->plane_i1);
   cudaFree(h->pw_pos);
+  cudaFree(h->stick_lo);
+  cudaFree(h->stick_hi);
+  cudaFree(h->col_of);
+  cudaFree(h->plane_of);
   cudaFree(h->vs);
   for (int j = 0; j < 3; ++j) cudaFree(h->tw[j]);
   cudaFree(h->w1);
@@ -677,6 +687,36 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   CR_TRY(upload(&h->plane_stick, plane_stick, st));
   CR_TRY(upload(&h->plane_i1, plane_i1, st));
   CR_TRY(upload(&h->pw_pos, pw_pos, st));
+  // tables of the fast two-pass path: signed i3 range of every stick (its sphere points are one interval, the
+  // sphere being convex), stick index of every (plane, i2) column, populated-plane index of every i1
+  bool sticks_are_intervals = true;
+  {
+    const int n1 = nr[0], n2 = nr[1], n3 = nr[2];
+    std::vector<int> lo((size_t)h->S), hi((size_t)h->S), col_of((size_t)h->P * n2, -1), plane_of((size_t)n1, -1);
+    for (int s_ = 0; s_ < h->S; ++s_) {
+      int l = n3, u = -n3;
+      for (int ig = stick_start[s_]; ig < stick_start[s_ + 1]; ++ig) {
+        const int i3 = idx[ig] % n3, m3 = i3 >= (n3 + 1) / 2 ? i3 - n3 : i3;
+        l = std::min(l, m3);
+        u = std::max(u, m3);
+      }
+      lo[s_] = l;
+      hi[s_] = u;
+      if (u - l + 1 != stick_start[s_ + 1] - stick_start[s_]) sticks_are_intervals = false;
+    }
+    for (int p_ = 0; p_ < h->P; ++p_) {
+      plane_of[plane_i1[p_]] = p_;
+      for (int s_ = plane_stick[p_]; s_ < plane_stick[p_ + 1]; ++s_) col_of[(size_t)p_ * n2 + stick_i2[s_]] = s_;
+    }
+    CR_TRY(upload(&h->stick_lo, lo, st));
+    CR_TRY(upload(&h->stick_hi, hi, st));
+    CR_TRY(upload(&h->col_of, col_of, st));
+    CR_TRY(upload(&h->plane_of, plane_of, st));
+    h->g2p.stick_lo = h->stick_lo;
+    h->g2p.stick_hi = h->stick_hi;
+    h->g2p.col_of = h->col_of;
+    h->g2p.plane_of = h->plane_of;
+  }
 
   // ---- FFT plan ---------------------------------------------------------------------------------------
   FftGeom& g = h->geom;
@@ -714,6 +754,15 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   h->smem_y = 2 * (size_t)nr[1] * FFT_C * sizeof(double2);
   h->smem_x = 2 * (size_t)nr[0] * FFT_C * sizeof(double2) + (size_t)nr[0] * FFT_C * sizeof(double);
 
+  if (!(flags & QE_HPSI_GENERIC_FFT) && sticks_are_intervals && env_int("QE_HPSI_FFT2P", 1)) {
+    const Fft2pEntry* e[3] = {fft2p_find(nr[0]), fft2p_find(nr[1]), fft2p_find(nr[2])};
+    if (e[0] && e[1] && e[2]) {
+      for (int j = 0; j < 3; ++j) h->f2p[j] = e[j];
+      h->smem_x2p = e[0]->rb > 1 ? 2 * (size_t)nr[0] * FFT_C * sizeof(double2) : 0;
+      CR_TRY(cudaFuncSetAttribute((const void*)e[0]->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_x2p));
+    }
+  }
+
   // V(r)/N in the padded layout
   {
     const long long rows = (long long)nr[0] * nr[1];
@@ -736,6 +785,9 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     h->fft_nb = (int)nbf;
     CR_TRY(cudaMalloc(&h->w1, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2))));
     CR_TRY(cudaMalloc(&h->w2, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2))));
+    // pad columns i3 in [N3, ldz) are carried through the y and x passes of the fast path: keep them finite
+    CR_TRY(cudaMemsetAsync(h->w1, 0, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2)), st));
+    CR_TRY(cudaMemsetAsync(h->w2, 0, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2)), st));
     h->workspace_bytes += (size_t)h->fft_nb * per_band;
     // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
     // gridDim.y only as far as needed to give every SM a few CTAs
@@ -827,16 +879,33 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     const double2* p = psi + (size_t)b0 * ldpsi;
     double2* o = hpsi + (size_t)b0 * ldh;
     const bool fine = h->prof_mode == 2;
+    const bool fast = h->f2p[0] != nullptr;
+    const Fft2pEntry *ex = h->f2p[0], *ey = h->f2p[1], *ez = h->f2p[2];
     size_t m0 = fine ? prof_mark(h, st) : (size_t)-1;
-    k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
+    if (fast)
+      ez->zinv<<<dim3(zt, n), ez->ra * FFT_C, 0, st>>>(g, h->g2p, p, ldpsi, h->w1);
+    else
+      k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
     size_t m1 = fine ? prof_mark(h, st) : (size_t)-1;
-    k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
+    if (fast)
+      ey->yinv<<<dim3(yt, n), ey->ra * FFT_C, 0, st>>>(g, h->g2p, h->w1, h->w2);
+    else
+      k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
     size_t m2 = fine ? prof_mark(h, st) : (size_t)-1;
-    k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
+    if (fast)
+      ex->x<<<dim3(xt, std::min(n, h->x_split)), ex->ra * FFT_C, h->smem_x2p, st>>>(g, h->g2p, h->w2, n);
+    else
+      k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
     size_t m3 = fine ? prof_mark(h, st) : (size_t)-1;
-    k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
+    if (fast)
+      ey->yfwd<<<dim3(yt, n), ey->ra * FFT_C, 0, st>>>(g, h->g2p, h->w2, h->w1);
+    else
+      k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
     size_t m4 = fine ? prof_mark(h, st) : (size_t)-1;
-    k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
+    if (fast)
+      ez->zfwd<<<dim3(zt, n), ez->ra * FFT_C, 0, st>>>(g, h->g2p, h->w1, p, ldpsi, o, ldh);
+    else
+      k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
     if (fine) {
       size_t m5 = prof_mark(h, st);
       if (m5 != (size_t)-1 && m5 > m0) {  // a drain in between would have reset the indices
@@ -1061,6 +1130,7 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[9] = h->kchunk;
   info[10] = h->x_split;
   info[11] = h->num_sms;
+  info[12] = h->f2p[0] ? 1 : 0;
   return QE_HPSI_OK;
 }
 
