@@ -60,7 +60,7 @@ struct qe_hpsi_handle {
   double2* tw[3] = {nullptr, nullptr, nullptr};
   FftGeom geom{};
   size_t smem_z = 0, smem_y = 0, smem_x = 0;
-  int fft_nb = 1;  // bands per FFT sub-chunk (workspace kept L2-sized)
+  int fft_nb = 1;  // bands per FFT sub-chunk
   int x_split = 1;
   double2 *w1 = nullptr, *w2 = nullptr;
   // fast two-pass FFT path (fft2p_kernels.cuh): used when every grid dimension has a table entry
@@ -774,10 +774,12 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     g.vs = h->vs;
   }
 
-  // FFT workspace: sub-chunks of fft_nb bands sized to stay L2-resident between passes
+  // FFT workspace: sub-chunks of fft_nb bands (workspace budget QE_HPSI_FFT_WS_MB, default 2.5 GB)
   {
     const size_t per_band = ((size_t)h->S + (size_t)h->P * nr[1]) * h->ldz * sizeof(double2);
-    const size_t budget = (size_t)env_int("QE_HPSI_FFT_L2_MB", 48) << 20;
+    // Measured on B200 (profiles/r1b): the chain gets faster with more bands per launch up to ~32 (fewer partial
+    // waves, V(r) reused across the bands of a sub-chunk in a3); L2 residency of one band's workspace is worth less.
+    const size_t budget = (size_t)env_int("QE_HPSI_FFT_WS_MB", 2560) << 20;
     long long nbf = per_band ? (long long)(budget / per_band) : max_batch;
     nbf = std::max<long long>(1, std::min<long long>(nbf, max_batch));
     const int forced = env_int("QE_HPSI_FFT_NB", 0);
