@@ -321,30 +321,33 @@ using K2pX = void (*)(FftGeom, Fft2pGeom, double2*, int);
 
 struct Fft2pEntry {
   int n, ra, rb;
+  int nthreads;    // CTA size of all five kernels
+  size_t smem_zy;  // dynamic shared memory of the z and y kernels (0: static tiles)
+  size_t smem_x;   // dynamic shared memory of the x kernel
   K2pZinv zinv;
   K2pZfwd zfwd;
   K2pY yinv, yfwd;
   K2pX x;
 };
 
-#define QE_FFT2P_ENTRY(RA, RB)                                                                              \
-  {                                                                                                         \
-    (RA) * (RB), RA, RB, k2p_scatter_zinv<RA, RB>, k2p_zfwd_gather<RA, RB>, k2p_yinv<RA, RB>, k2p_yfwd<RA, RB>, \
-        k2p_x_vmul<RA, RB>                                                                                  \
+#define QE_FFT2P_ENTRY(RA, RB)                                                                                  \
+  {                                                                                                             \
+    (RA) * (RB), RA, RB, (RA) * FFT_C, 0, (RB) > 1 ? 2 * (size_t)(RA) * (RB) * FFT_C * sizeof(double2) : 0,     \
+        k2p_scatter_zinv<RA, RB>, k2p_zfwd_gather<RA, RB>, k2p_yinv<RA, RB>, k2p_yfwd<RA, RB>, k2p_x_vmul<RA, RB> \
   }
 
 static const Fft2pEntry kFft2pTable[] = {
     QE_FFT2P_ENTRY(8, 1),   QE_FFT2P_ENTRY(9, 1),   QE_FFT2P_ENTRY(10, 1),  QE_FFT2P_ENTRY(12, 1),  QE_FFT2P_ENTRY(15, 1),
     QE_FFT2P_ENTRY(16, 1),  QE_FFT2P_ENTRY(6, 3),   QE_FFT2P_ENTRY(5, 4),   QE_FFT2P_ENTRY(6, 6),   QE_FFT2P_ENTRY(8, 6),
     QE_FFT2P_ENTRY(8, 8),   QE_FFT2P_ENTRY(9, 8),   QE_FFT2P_ENTRY(10, 8),  QE_FFT2P_ENTRY(12, 8),  QE_FFT2P_ENTRY(10, 10),
-    QE_FFT2P_ENTRY(12, 9),  QE_FFT2P_ENTRY(12, 10), QE_FFT2P_ENTRY(25, 5),  QE_FFT2P_ENTRY(16, 8),  QE_FFT2P_ENTRY(12, 12),
-    QE_FFT2P_ENTRY(16, 10), QE_FFT2P_ENTRY(15, 12), QE_FFT2P_ENTRY(16, 12), QE_FFT2P_ENTRY(16, 15), QE_FFT2P_ENTRY(16, 16),
+    QE_FFT2P_ENTRY(12, 9),  QE_FFT2P_ENTRY(12, 10), QE_FFT2P_ENTRY(16, 8),  QE_FFT2P_ENTRY(12, 12), QE_FFT2P_ENTRY(16, 10),
+    QE_FFT2P_ENTRY(15, 12), QE_FFT2P_ENTRY(16, 12), QE_FFT2P_ENTRY(16, 15), QE_FFT2P_ENTRY(16, 16),
 };
 #undef QE_FFT2P_ENTRY
 
-inline const Fft2pEntry* fft2p_find(int n) {
-  for (const Fft2pEntry& e : kFft2pTable)
-    if (e.n == n) return &e;
+inline const Fft2pEntry* fft2p_find_in(const Fft2pEntry* tab, size_t cnt, int n) {
+  for (size_t i = 0; i < cnt; ++i)
+    if (tab[i].n == n) return &tab[i];
   return nullptr;
 }
 

@@ -15,7 +15,7 @@
 #include <vector>
 
 #include "fft_kernels.cuh"
-#include "fft2p_kernels.cuh"
+#include "fft3p_kernels.cuh"
 #include "zgemm_kernels.cuh"
 
 using namespace qehpsi;
@@ -31,10 +31,12 @@ using ZgV0 = ZgCfg<64, 64, 2, 4, 16, 4>;
 using ZgV1 = ZgCfg<64, 64, 4, 4, 16, 4>;
 using ZgV2 = ZgCfg<128, 32, 4, 2, 16, 4>;
 using ZgV3 = ZgCfg<64, 64, 2, 4, 8, 6>;
-constexpr int ZG_NVARIANT = 4;
-constexpr int ZG_BM_TAB[ZG_NVARIANT] = {64, 64, 128, 64};
-constexpr int ZG_BN_TAB[ZG_NVARIANT] = {64, 64, 32, 64};
-constexpr int ZG_BK_TAB[ZG_NVARIANT] = {16, 16, 16, 8};
+using ZgV4 = ZgCfg<64, 64, 2, 4, 32, 3>;
+using ZgV5 = ZgCfg<64, 64, 2, 4, 16, 6>;
+constexpr int ZG_NVARIANT = 6;
+constexpr int ZG_BM_TAB[ZG_NVARIANT] = {64, 64, 128, 64, 64, 64};
+constexpr int ZG_BN_TAB[ZG_NVARIANT] = {64, 64, 32, 64, 64, 64};
+constexpr int ZG_BK_TAB[ZG_NVARIANT] = {16, 16, 16, 8, 32, 16};
 
 struct DevBuf {
   void* p = nullptr;
@@ -474,6 +476,10 @@ cudaError_t set_kernel_attrs() {
   SET_SMEM(k_vnl_add<ZgV2>);
   SET_SMEM(k_becp<ZgV3>);
   SET_SMEM(k_vnl_add<ZgV3>);
+  SET_SMEM(k_becp<ZgV4>);
+  SET_SMEM(k_vnl_add<ZgV4>);
+  SET_SMEM(k_becp<ZgV5>);
+  SET_SMEM(k_vnl_add<ZgV5>);
 #undef SET_SMEM
   g_attr_done = true;
   return cudaSuccess;
@@ -755,11 +761,19 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   h->smem_x = 2 * (size_t)nr[0] * FFT_C * sizeof(double2) + (size_t)nr[0] * FFT_C * sizeof(double);
 
   if (!(flags & QE_HPSI_GENERIC_FFT) && sticks_are_intervals && env_int("QE_HPSI_FFT2P", 1)) {
-    const Fft2pEntry* e[3] = {fft2p_find(nr[0]), fft2p_find(nr[1]), fft2p_find(nr[2])};
+    const int p3 = env_int("QE_HPSI_FFT3P", 0);  // bit j set: prefer the three-pass plan on axis j (tuning knob)
+    const Fft2pEntry* e[3] = {fft2p_find(nr[0], p3 & 1), fft2p_find(nr[1], p3 & 2), fft2p_find(nr[2], p3 & 4)};
     if (e[0] && e[1] && e[2]) {
       for (int j = 0; j < 3; ++j) h->f2p[j] = e[j];
-      h->smem_x2p = e[0]->rb > 1 ? 2 * (size_t)nr[0] * FFT_C * sizeof(double2) : 0;
-      CR_TRY(cudaFuncSetAttribute((const void*)e[0]->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_x2p));
+      h->smem_x2p = e[0]->smem_x;
+      CR_TRY(cudaFuncSetAttribute((const void*)e[0]->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e[0]->smem_x));
+      for (int j = 1; j < 3; ++j) {
+        if (!e[j]->smem_zy) continue;
+        const void* fns[2] = {j == 1 ? (const void*)e[j]->yinv : (const void*)e[j]->zinv,
+                              j == 1 ? (const void*)e[j]->yfwd : (const void*)e[j]->zfwd};
+        for (const void* fn : fns)
+          CR_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e[j]->smem_zy));
+      }
     }
   }
 
@@ -885,27 +899,27 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     const Fft2pEntry *ex = h->f2p[0], *ey = h->f2p[1], *ez = h->f2p[2];
     size_t m0 = fine ? prof_mark(h, st) : (size_t)-1;
     if (fast)
-      ez->zinv<<<dim3(zt, n), ez->ra * FFT_C, 0, st>>>(g, h->g2p, p, ldpsi, h->w1);
+      ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
     else
       k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
     size_t m1 = fine ? prof_mark(h, st) : (size_t)-1;
     if (fast)
-      ey->yinv<<<dim3(yt, n), ey->ra * FFT_C, 0, st>>>(g, h->g2p, h->w1, h->w2);
+      ey->yinv<<<dim3(yt, n), ey->nthreads, ey->smem_zy, st>>>(g, h->g2p, h->w1, h->w2);
     else
       k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
     size_t m2 = fine ? prof_mark(h, st) : (size_t)-1;
     if (fast)
-      ex->x<<<dim3(xt, std::min(n, h->x_split)), ex->ra * FFT_C, h->smem_x2p, st>>>(g, h->g2p, h->w2, n);
+      ex->x<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_x2p, st>>>(g, h->g2p, h->w2, n);
     else
       k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
     size_t m3 = fine ? prof_mark(h, st) : (size_t)-1;
     if (fast)
-      ey->yfwd<<<dim3(yt, n), ey->ra * FFT_C, 0, st>>>(g, h->g2p, h->w2, h->w1);
+      ey->yfwd<<<dim3(yt, n), ey->nthreads, ey->smem_zy, st>>>(g, h->g2p, h->w2, h->w1);
     else
       k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
     size_t m4 = fine ? prof_mark(h, st) : (size_t)-1;
     if (fast)
-      ez->zfwd<<<dim3(zt, n), ez->ra * FFT_C, 0, st>>>(g, h->g2p, h->w1, p, ldpsi, o, ldh);
+      ez->zfwd<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, h->w1, p, ldpsi, o, ldh);
     else
       k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
     if (fine) {
@@ -944,6 +958,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st); break;
     case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st); break;
     case 3: becp_launch<ZgV3>(h, psi, ldpsi, nb, st); break;
+    case 4: becp_launch<ZgV4>(h, psi, ldpsi, nb, st); break;
+    case 5: becp_launch<ZgV5>(h, psi, ldpsi, nb, st); break;
     default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st); break;
   }
   const size_t t1 = prof_mark(h, st);
@@ -964,6 +980,8 @@ int launch_vnl_add(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream
     case 1: vnl_launch<ZgV1>(h, hpsi, ldh, nb, st); break;
     case 2: vnl_launch<ZgV2>(h, hpsi, ldh, nb, st); break;
     case 3: vnl_launch<ZgV3>(h, hpsi, ldh, nb, st); break;
+    case 4: vnl_launch<ZgV4>(h, hpsi, ldh, nb, st); break;
+    case 5: vnl_launch<ZgV5>(h, hpsi, ldh, nb, st); break;
     default: vnl_launch<ZgV0>(h, hpsi, ldh, nb, st); break;
   }
   CU_TRY(h, cudaGetLastError());

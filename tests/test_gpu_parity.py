@@ -192,3 +192,43 @@ def test_argument_errors():
     out = h.apply(torch.zeros((0, h.npw), dtype=torch.complex128, device="cuda"))  # empty input is fine
     assert out.shape[0] == 0
     h.destroy()
+
+
+# every FFT length with a fast-path plan (two-pass: fft2p_kernels.cuh, three-pass: fft3p_kernels.cuh) plus a few
+# lengths that only the generic multi-pass plan serves, each placed on each of the three axes in turn
+FFT2P_LENGTHS = [8, 9, 10, 12, 15, 16, 18, 20, 36, 48, 64, 72, 80, 96, 100, 108, 120, 128, 144, 160, 180, 192, 240, 256]
+FFT3P_LENGTHS = [125, 150, 200, 216, 250, 288, 300, 320, 360, 384]
+GENERIC_LENGTHS = [24, 45, 135, 243]
+
+
+@pytest.mark.parametrize("n", FFT2P_LENGTHS + FFT3P_LENGTHS + GENERIC_LENGTHS)
+def test_local_term_for_every_fft_length(n):
+    """Local + kinetic term (nproj = 0) on anisotropic cells whose grid is (n, 9, 10), (9, n, 10), (9, 10, n) with the
+    sphere using the full index range of every axis, against oracle Level B on the same arrays."""
+    ecut = 4.0
+    gen = torch.Generator().manual_seed(1000 + n)
+    for axis in range(3):
+        nr = [9, 10, 12][axis:] + [9, 10, 12][:axis]
+        nr = [nr[0], nr[1], nr[2]]
+        nr[axis] = n
+        at = np.zeros((3, 3))
+        for j in range(3):
+            nmax = (nr[j] - 1) // 2
+            at[j, j] = 2.0 * np.pi * (nmax + 0.4) / np.sqrt(ecut)
+        xk = np.array([0.0, 0.0, 0.0]) if axis == 0 else 0.02 * 2 * np.pi / at.diagonal() * np.array([1.0, -2.0, 1.5])
+        sp = orc.gsphere(at, xk, ecut, nr)
+        npw = sp["miller"].shape[0]
+        assert npw > 0
+        vr = torch.randn(tuple(nr), dtype=torch.float64, generator=gen)
+        nb = 3
+        ld = inputs.pad8(npw)
+        psi = torch.zeros((nb, ld), dtype=torch.complex128)
+        psi[:, :npw] = torch.randn((nb, npw), dtype=torch.complex128, generator=gen)
+        h = qe_hpsi.Hpsi(at, ecut, xk, nr, vr.cuda(), max_batch=2)  # 3 bands through chunks of 2 and 1
+        assert h.npw == npw
+        out = h.apply(psi.cuda())
+        torch.cuda.synchronize()
+        ref = orc.hpsi_dual(sp["fft_index"], sp["g2kin"], tuple(nr), vr.numpy(), psi[:, :npw].numpy(), None, None)
+        err = _gpu.rel_l2(out.cpu().numpy()[:, :npw], ref)
+        assert err.max() <= TOL, (n, axis, nr, err)
+        h.destroy()
