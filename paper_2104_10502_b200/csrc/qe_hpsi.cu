@@ -90,6 +90,10 @@ struct qe_hpsi_handle {
   double2* hbuf_h[2] = {nullptr, nullptr};
   long long ldint = 0;
   cudaStream_t st_in = nullptr, st_comp = nullptr, st_out = nullptr;
+  // optional overlap of the FFT chain with the projector ZGEMM (QE_HPSI_OVERLAP)
+  int overlap = 0;
+  cudaStream_t st_fft = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   // optional stage timing (qe_hpsi_profile): CUDA events recorded around stages on the caller's stream
   int prof_mode = 0;
@@ -564,6 +568,9 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
   if (h->st_in) cudaStreamDestroy(h->st_in);
   if (h->st_comp) cudaStreamDestroy(h->st_comp);
+  if (h->st_fft) cudaStreamDestroy(h->st_fft);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->st_out) cudaStreamDestroy(h->st_out);
   delete h;
   return QE_HPSI_OK;
@@ -812,6 +819,13 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     h->x_split = std::max(1, split);
   }
 
+  h->overlap = env_int("QE_HPSI_OVERLAP", 0);
+  if (h->overlap) {
+    CR_TRY(cudaStreamCreateWithFlags(&h->st_fft, cudaStreamNonBlocking));
+    CR_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    CR_TRY(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+  }
+
   // ---- nonlocal ---------------------------------------------------------------------------------------
   if (nproj > 0) {
     if (flags & QE_HPSI_BORROW_BETA) {
@@ -993,11 +1007,23 @@ int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi,
   int rc = QE_HPSI_OK;
   const bool nl = nonlocal && h->nproj > 0 && h->npw > 0;
   if (h->prof_mode && h->prof_used + 16 > 16384) prof_drain(h);
+  // a6-a7 and a1-a5 are independent (both only read psi): with QE_HPSI_OVERLAP=1 the FFT chain runs on an internal
+  // stream forked from the caller's stream while the projector ZGEMM runs on the caller's stream; joined before a8.
+  const bool fork = nl && local && h->overlap && h->st_fft && !h->prof_mode;
+  if (fork) {
+    CU_TRY(h, cudaEventRecord(h->ev_fork, st));
+    CU_TRY(h, cudaStreamWaitEvent(h->st_fft, h->ev_fork, 0));
+    rc = launch_local(h, psi, ldpsi, hpsi, ldh, nb, h->st_fft);
+    if (rc) return rc;
+    CU_TRY(h, cudaEventRecord(h->ev_join, h->st_fft));
+  }
   if (nl) {
     rc = launch_becp(h, psi, ldpsi, nb, st);
     if (rc) return rc;
   }
-  if (local) {
+  if (fork) {
+    CU_TRY(h, cudaStreamWaitEvent(st, h->ev_join, 0));
+  } else if (local) {
     const size_t t0 = h->prof_mode == 1 ? prof_mark(h, st) : (size_t)-1;
     rc = launch_local(h, psi, ldpsi, hpsi, ldh, nb, st);
     if (rc) return rc;
