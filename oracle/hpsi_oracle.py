@@ -33,7 +33,10 @@ Three levels:
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed forms (single plane wave in constant V0; cosine
 potential shift; rank-1 projector), FFT round trip / Parseval / naive O(n^2) DFT, Hermiticity, translation
 covariance, time reversal at k=0, linearity, A == A' == B on tiny cases, independently enumerated npw counts
-(tests/golden/npw_counts.txt from SURVEY.md 8 table). Nothing here is "parity unpinned".
+(tests/golden/npw_counts.txt from SURVEY.md 8 table). The functions of the "next" rows at the end of the file
+(`spsi_of`, `overlap_of`, `psi_r`, `density_of`) are pinned in tests/test_oracle_next.py (rank-1 closed form, brute-force
+loops, Hermiticity, single / two plane-wave closed forms, Parseval, explicit DFT matrices). Nothing here is "parity
+unpinned".
 """
 from __future__ import annotations
 
@@ -262,3 +265,42 @@ def rel_l2(x, ref):
     num = np.sqrt((d.real**2 + d.imag**2).sum(-1))
     den = np.sqrt((r.real**2 + r.imag**2).sum(-1))
     return np.asarray(num / den, dtype=np.float64)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# Rows marked "next" in SURVEY.md 8(f): overlap operator S, reduced matrices of the Davidson step, charge density
+# ("application of the overlap operator", "charge density generation"; iterative diagonaliser
+# calling H|psi> and S|psi>).  The paper prints no formula; these are the textbook
+# definitions in the conventions fixed above (DESIGN.md section 2 items 18-20).
+# ----------------------------------------------------------------------------------------------------------
+
+
+def spsi_of(beta, qblocks, psi):
+    """NEXT-2: S psi = psi + sum_a sum_ij beta_ai(G) q^a_ij <beta_aj|psi>  (ultrasoft/PAW overlap operator with
+    per-atom real symmetric q blocks [nat,nh,nh]).  psi [nb,npw] -> [nb,npw]."""
+    return psi + vnl_psi(beta, qblocks, psi)
+
+
+def overlap_of(a, b):
+    """NEXT-3: reduced matrix M[i][j] = <a_i|b_j> = sum_G conj(a[i][G]) b[j][G].  a [na,npw], b [nb,npw] -> [na,nb].
+    With a = psi, b = H psi (S psi) this is the projected Hamiltonian (overlap) of the Davidson step."""
+    return np.conj(a) @ b.T
+
+
+def psi_r(fft_index, nr, psi_b):
+    """psi(r_i) = sum_G c(G) exp(+2 pi i n.i/N) on the full grid for one band (un-normalised inverse DFT,
+    reading 4 of DESIGN.md section 2; the Bloch phase has modulus 1 and drops out of |psi(r)|^2)."""
+    n = int(nr[0]) * int(nr[1]) * int(nr[2])
+    box = np.zeros(n, dtype=np.complex128)
+    box[fft_index] = psi_b
+    return np.fft.ifftn(box.reshape(nr)) * n
+
+
+def density_of(fft_index, nr, psi, occ, scale):
+    """NEXT-4: rho(r_i) = scale * sum_b occ[b] |psi_b(r_i)|^2 on the [N1,N2,N3] grid (scale = 1/Omega gives
+    electrons per bohr^3 for normalised bands)."""
+    rho = np.zeros(tuple(int(x) for x in nr), dtype=np.float64)
+    for b in range(psi.shape[0]):
+        pr = psi_r(fft_index, nr, psi[b])
+        rho += occ[b] * (pr.real**2 + pr.imag**2)
+    return scale * rho
