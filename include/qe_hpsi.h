@@ -139,6 +139,34 @@ int qe_hpsi_fft_local(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hps
 int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
                      void* cuda_stream);
 
+/* ---- rows SURVEY.md 8(f) marks "next": same kernels and tables as the hot path ---------------------------- */
+
+/* NEXT-2, overlap operator of ultrasoft/PAW pseudopotentials ("application of the overlap operator",
+ * PAPER.md:L226): S = 1 + sum_a sum_ij |beta_ai> q^a_ij <beta_aj|.
+ * qe_hpsi_set_s stores the real symmetric q^a blocks (packed exactly like d_host of qe_hpsi_create; COPIED;
+ * synchronises).  qe_hpsi_apply_hs computes hpsi = H psi and spsi = S psi in one call: becp = beta^H psi (a6) is
+ * computed once and shared; spsi[b][0..npw) is overwritten, entries >= npw untouched; spsi must not overlap psi or
+ * hpsi.  hpsi_dev may be NULL (S psi only).  Without projectors S = 1.  QE_HPSI_ESTATE if set_s was never called
+ * on a handle that has projectors.  Asynchronous on cuda_stream like qe_hpsi_apply. */
+int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host);
+int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, void* spsi_dev,
+                     int64_t ldspsi, int nbands, void* cuda_stream);
+
+/* NEXT-3, reduced matrices of the iterative diagonaliser: out[i][j] = <a_i|b_j> =
+ * sum_G conj(a[i][G]) b[j][G] over the npw sphere entries, i < na, j < nb.  a_dev [na][lda], b_dev [nb][ldb]
+ * complex128 (may be the same array), out_dev [na][ldo] complex128, ldo >= nb (entries j >= nb untouched).  Runs the
+ * split-K DMMA kernel of step a6 with a fixed-order reduction (bit-reproducible).  Asynchronous on cuda_stream. */
+int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb,
+                    void* out_dev, int64_t ldo, void* cuda_stream);
+
+/* NEXT-4, charge density ("charge density generation"):
+ *   rho[i1][i2][i3] += scale * sum_b occ[b] |psi_b(r_i)|^2,  psi_b(r_i) = sum_G psi[b][G] exp(+2 pi i n.i/N)
+ * using steps a1-a2 of the hot path and the inverse half of a3.  rho_dev is a dense [N1][N2][N3] FP64 DEVICE array
+ * that is ACCUMULATED into (zero it first for a fresh density); occ_dev [nbands] FP64 on the device.
+ * Asynchronous on cuda_stream; bit-reproducible (each grid point is owned by one thread, bands summed in order). */
+int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, int nbands, const double* occ_dev, double scale,
+                    double* rho_dev, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

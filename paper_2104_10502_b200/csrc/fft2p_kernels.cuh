@@ -311,6 +311,67 @@ __global__ void __launch_bounds__(RA* FFT_C) k2p_x_vmul(FftGeom g, Fft2pGeom t, 
   }
 }
 
+// NEXT-4 (charge density) ----------------------------------------------------------------------
+// inverse FFT along i1 exactly as the first half of a3, then rho[i1][i2][i3] += scale * sum_b occ[b] |psi_b(r)|^2.
+// One CTA owns its (i2, i3 tile) pencils for all bands of the launch (gridDim.y must be 1): no atomics, fixed order.
+template <int RA, int RB>
+__global__ void __launch_bounds__(RA* FFT_C) k2p_x_rho(FftGeom g, Fft2pGeom t, const double2* __restrict__ w2, int nb,
+                                                       const double* __restrict__ occ, double scale,
+                                                       double* __restrict__ rho) {
+  constexpr int N = RA * RB;
+  constexpr int NV = RB > 1 ? RB : RA;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double2* tile1 = reinterpret_cast<double2*>(smem_raw);
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const int i2 = blockIdx.x / g.ntz;
+  const int z = (blockIdx.x - i2 * g.ntz) * FFT_C + c;
+  const double2 zero = make_double2(0.0, 0.0);
+  const size_t pstride = (size_t)g.n2 * g.ldz;
+  int pl[RA];
+  if (j < RB) {
+#pragma unroll
+    for (int q = 0; q < RA; ++q) pl[q] = __ldg(&t.plane_of[j + q * RB]);
+  }
+  double acc[NV];
+#pragma unroll
+  for (int q = 0; q < NV; ++q) acc[q] = 0.0;
+  for (int b = 0; b < nb; ++b) {
+    const double f = __ldg(&occ[b]);
+    const double2* in = w2 + ((size_t)b * g.P * g.n2 + i2) * g.ldz + z;
+    if constexpr (RB > 1) {
+      if (j < RB) {
+        double2 v[RA];
+#pragma unroll
+        for (int q = 0; q < RA; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * pstride] : zero;
+        pass_a_store<RA, +1>(v, tile1, j, c);
+      }
+      __syncthreads();
+      double2 u[RB];
+      pass_b_load<RA, RB, +1>(tile1, g.ax1.tw, j, c, u);
+#pragma unroll
+      for (int q = 0; q < RB; ++q) acc[q] += f * (u[q].x * u[q].x + u[q].y * u[q].y);
+      __syncthreads();  // the next band's first pass overwrites tile1
+    } else {
+      if (j < 1) {
+        double2 v[RA];
+#pragma unroll
+        for (int q = 0; q < RA; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * pstride] : zero;
+        Dft<RA, +1>::run(v);
+#pragma unroll
+        for (int q = 0; q < RA; ++q) acc[q] += f * (v[q].x * v[q].x + v[q].y * v[q].y);
+      }
+    }
+  }
+  if (z < g.n3 && (RB > 1 || j < 1)) {
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      const int i1 = RB > 1 ? j + q * RA : q;
+      double* r = rho + ((size_t)i1 * g.n2 + i2) * g.n3 + z;
+      *r += scale * acc[q];
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // dispatch: one entry per supported length N = RA * RB
 // ---------------------------------------------------------------------------------------------------------
@@ -318,6 +379,7 @@ using K2pZinv = void (*)(FftGeom, Fft2pGeom, const double2*, long long, double2*
 using K2pZfwd = void (*)(FftGeom, Fft2pGeom, const double2*, const double2*, long long, double2*, long long);
 using K2pY = void (*)(FftGeom, Fft2pGeom, const double2*, double2*);
 using K2pX = void (*)(FftGeom, Fft2pGeom, double2*, int);
+using K2pRho = void (*)(FftGeom, Fft2pGeom, const double2*, int, const double*, double, double*);
 
 struct Fft2pEntry {
   int n, ra, rb;
@@ -328,12 +390,14 @@ struct Fft2pEntry {
   K2pZfwd zfwd;
   K2pY yinv, yfwd;
   K2pX x;
+  K2pRho rho;      // NEXT-4: x-inverse + density accumulation (dynamic shared memory: smem_x / 2)
 };
 
 #define QE_FFT2P_ENTRY(RA, RB)                                                                                  \
   {                                                                                                             \
     (RA) * (RB), RA, RB, (RA) * FFT_C, 0, (RB) > 1 ? 2 * (size_t)(RA) * (RB) * FFT_C * sizeof(double2) : 0,     \
-        k2p_scatter_zinv<RA, RB>, k2p_zfwd_gather<RA, RB>, k2p_yinv<RA, RB>, k2p_yfwd<RA, RB>, k2p_x_vmul<RA, RB> \
+        k2p_scatter_zinv<RA, RB>, k2p_zfwd_gather<RA, RB>, k2p_yinv<RA, RB>, k2p_yfwd<RA, RB>, k2p_x_vmul<RA, RB>, \
+        k2p_x_rho<RA, RB>                                                                                        \
   }
 
 static const Fft2pEntry kFft2pTable[] = {

@@ -263,6 +263,59 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_x_vmul(FftGeom g, Fft2
   }
 }
 
+// NEXT-4 (charge density): inverse (R1,R2,R3) along i1, rho += scale * sum_b occ[b] |psi_b(r)|^2 (see k2p_x_rho)
+template <int R1, int R2, int R3>
+__global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_x_rho(FftGeom g, Fft2pGeom t, const double2* __restrict__ w2, int nb,
+                                                               const double* __restrict__ occ, double scale,
+                                                               double* __restrict__ rho) {
+  using P = P3<R1, R2, R3>;
+  constexpr int N = P::N;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double2* tA = reinterpret_cast<double2*>(smem_raw);
+  double2* tB = tA + N * FFT_C;
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const int i2 = blockIdx.x / g.ntz;
+  const int z = (blockIdx.x - i2 * g.ntz) * FFT_C + c;
+  const double2 zero = make_double2(0.0, 0.0);
+  const size_t pstride = (size_t)g.n2 * g.ldz;
+  int pl[R1];
+  if (j < P::T1) {
+#pragma unroll
+    for (int q = 0; q < R1; ++q) pl[q] = __ldg(&t.plane_of[j + q * P::T1]);
+  }
+  double acc[R3];
+#pragma unroll
+  for (int q = 0; q < R3; ++q) acc[q] = 0.0;
+  for (int b = 0; b < nb; ++b) {
+    const double f = __ldg(&occ[b]);
+    const double2* in = w2 + ((size_t)b * g.P * g.n2 + i2) * g.ldz + z;
+    if (j < P::T1) {
+      double2 v[R1];
+#pragma unroll
+      for (int q = 0; q < R1; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * pstride] : zero;
+      pass_a_store<R1, +1>(v, tA, j, c);
+    }
+    __syncthreads();
+    if (j < P::T2) pass_mid<R2, +1>(tA, tB, g.ax1.tw, N, R1, j, c);
+    __syncthreads();
+    if (j < P::T3) {
+      double2 u[R3];
+      pass_b_load<P::T3, R3, +1>(tB, g.ax1.tw, j, c, u);
+#pragma unroll
+      for (int q = 0; q < R3; ++q) acc[q] += f * (u[q].x * u[q].x + u[q].y * u[q].y);
+    }
+    // next band: tile A is rewritten before the first barrier (last read before the second barrier above: safe);
+    // tile B is rewritten after the next band's first barrier, i.e. after every thread has left this read
+  }
+  if (z < g.n3 && j < P::T3) {
+#pragma unroll
+    for (int q = 0; q < R3; ++q) {
+      double* r = rho + ((size_t)(j + q * P::T3) * g.n2 + i2) * g.n3 + z;
+      *r += scale * acc[q];
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // dispatch: lengths served by the three-pass plan (ra = R1, rb = R2*R3 in the shared entry type)
 // ---------------------------------------------------------------------------------------------------------
@@ -270,7 +323,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_x_vmul(FftGeom g, Fft2
   {                                                                                                                \
     (R1) * (R2) * (R3), R1, (R2) * (R3), P3<R1, R2, R3>::NT, P3<R1, R2, R3>::SMEM, P3<R1, R2, R3>::SMEM,            \
         k3p_scatter_zinv<R1, R2, R3>, k3p_zfwd_gather<R1, R2, R3>, k3p_yinv<R1, R2, R3>, k3p_yfwd<R1, R2, R3>,      \
-        k3p_x_vmul<R1, R2, R3>                                                                                     \
+        k3p_x_vmul<R1, R2, R3>, k3p_x_rho<R1, R2, R3>                                                              \
   }
 
 static const Fft2pEntry kFft3pTable[] = {

@@ -126,6 +126,41 @@ __global__ void __launch_bounds__(FFT_NT) k_x_vmul(FftGeom g, double2* __restric
   }
 }
 
+// NEXT-4 (charge density), generic plan: inverse FFT along i1, rho += scale * sum_b occ[b] |psi_b(r)|^2.
+// Dynamic shared memory: two [N1][FFT_C] tiles.  gridDim.y must be 1 (one CTA owns its pencils: no atomics).
+__global__ void __launch_bounds__(FFT_NT) k_x_rho(FftGeom g, const double2* __restrict__ w2, int nb,
+                                                  const double* __restrict__ occ, double scale, double* __restrict__ rho) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double2* bufA = reinterpret_cast<double2*>(smem_raw);
+  double2* bufB = bufA + g.n1 * FFT_C;
+  const int tid = threadIdx.x;
+  const int i2 = blockIdx.x / g.ntz;
+  const int z0 = (blockIdx.x - i2 * g.ntz) * FFT_C;
+  const int tile = g.n1 * FFT_C;
+  const size_t pstride = (size_t)g.n2 * g.ldz;
+  for (int b = 0; b < nb; ++b) {
+    const double f = scale * __ldg(&occ[b]);
+    tile_zero(bufA, tile, tid);
+    __syncthreads();
+    const double2* in = w2 + ((size_t)b * g.P * g.n2 + i2) * g.ldz + z0;
+    for (int idx = tid; idx < g.P * FFT_C; idx += FFT_NT) {
+      const int c = idx & (FFT_C - 1), pi = idx / FFT_C;
+      if (z0 + c < g.n3) bufA[fft_phys(__ldg(&g.plane_i1[pi]), c)] = in[pi * pstride + c];
+    }
+    __syncthreads();
+    const double2* r = fft_tile<+1>(bufA, bufB, g.ax1, tid, FFT_NT);
+    for (int idx = tid; idx < tile; idx += FFT_NT) {  // the same thread owns the same grid points for every band
+      const int c = idx & (FFT_C - 1), n = idx / FFT_C;
+      if (z0 + c < g.n3) {
+        const double2 x = r[fft_phys(n, c)];
+        double* o = rho + ((size_t)n * g.n2 + i2) * g.n3 + z0 + c;
+        *o += f * (x.x * x.x + x.y * x.y);
+      }
+    }
+    __syncthreads();
+  }
+}
+
 // a4 ------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(FFT_NT) k_yfwd(FftGeom g, const double2* __restrict__ w2, double2* __restrict__ w1) {
   extern __shared__ __align__(16) unsigned char smem_raw[];

@@ -83,6 +83,14 @@ struct qe_hpsi_handle {
   int nsplit = 1, kchunk = 0;
   int zg_variant = 0;
   double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
+  // NEXT-2: overlap operator S (q blocks packed like D; qbecp/qbT mirror dbecp/dbT)
+  long long d_total = 0;
+  double* qpk = nullptr;
+  double2 *qbecp = nullptr, *qbT = nullptr;
+  // NEXT-3: split-K workspace of qe_hpsi_overlap (grown on demand)
+  double2* ovl_partial = nullptr;
+  size_t ovl_cap = 0;
+  bool rho_attr_done = false;
   int nb_last = 0;
   size_t workspace_bytes = 0;
   // apply_host staging
@@ -470,6 +478,7 @@ cudaError_t set_kernel_attrs() {
   SET_SMEM(k_scatter_zinv);
   SET_SMEM(k_yinv);
   SET_SMEM(k_x_vmul);
+  SET_SMEM(k_x_rho);
   SET_SMEM(k_yfwd);
   SET_SMEM(k_zfwd_gather);
   SET_SMEM(k_becp<ZgV0>);
@@ -558,6 +567,10 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->becp);
   cudaFree(h->dbecp);
   cudaFree(h->dbT);
+  cudaFree(h->qpk);
+  cudaFree(h->qbecp);
+  cudaFree(h->qbT);
+  cudaFree(h->ovl_partial);
   for (int i = 0; i < 2; ++i) {
     cudaFree(h->hbuf_psi[i]);
     cudaFree(h->hbuf_h[i]);
@@ -851,6 +864,7 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
       }
       off += (long long)nh * nh;
     }
+    h->d_total = d_total;
     std::vector<double> dv(d_host, d_host + d_total);
     CR_TRY(upload(&h->proj_blk0, blk0, st));
     CR_TRY(upload(&h->proj_nh, nhv, st));
@@ -958,10 +972,10 @@ void becp_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaS
                                                                          h->npw, h->kchunk, h->partial, h->ldc);
 }
 template <class Cfg>
-void vnl_launch(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
   if (mt == 0) return;
-  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->dbT, h->ldp,
+  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT, h->ldp,
                                                                     nb, hpsi, ldh);
 }
 
@@ -989,14 +1003,14 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 }
 
 // a8
-int launch_vnl_add(qe_hpsi_t h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   switch (h->zg_variant) {
-    case 1: vnl_launch<ZgV1>(h, hpsi, ldh, nb, st); break;
-    case 2: vnl_launch<ZgV2>(h, hpsi, ldh, nb, st); break;
-    case 3: vnl_launch<ZgV3>(h, hpsi, ldh, nb, st); break;
-    case 4: vnl_launch<ZgV4>(h, hpsi, ldh, nb, st); break;
-    case 5: vnl_launch<ZgV5>(h, hpsi, ldh, nb, st); break;
-    default: vnl_launch<ZgV0>(h, hpsi, ldh, nb, st); break;
+    case 1: vnl_launch<ZgV1>(h, bT, hpsi, ldh, nb, st); break;
+    case 2: vnl_launch<ZgV2>(h, bT, hpsi, ldh, nb, st); break;
+    case 3: vnl_launch<ZgV3>(h, bT, hpsi, ldh, nb, st); break;
+    case 4: vnl_launch<ZgV4>(h, bT, hpsi, ldh, nb, st); break;
+    case 5: vnl_launch<ZgV5>(h, bT, hpsi, ldh, nb, st); break;
+    default: vnl_launch<ZgV0>(h, bT, hpsi, ldh, nb, st); break;
   }
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
@@ -1031,7 +1045,7 @@ int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi,
   }
   if (nl) {
     const size_t t0 = prof_mark(h, st);
-    rc = launch_vnl_add(h, hpsi, ldh, nb, st);
+    rc = launch_vnl_add(h, h->dbT, hpsi, ldh, nb, st);
     prof_span(h, t0, prof_mark(h, st), SLOT_VNL);
   }
   return rc;
@@ -1065,6 +1079,168 @@ extern "C" int qe_hpsi_fft_local(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi
 extern "C" int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
                                 int nbands, void* cuda_stream) {
   return apply_impl(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands, cuda_stream, false, true);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-2: overlap operator S = 1 + beta q beta^H, sharing becp with H (include/qe_hpsi.h)
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (h->nproj == 0) return QE_HPSI_OK;
+  if (!q_host) return QE_HPSI_EINVAL;
+  CU_TRY(h, cudaSetDevice(h->device));
+  if (!h->qpk) {
+    const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2);
+    CU_TRY(h, cudaMalloc(&h->qpk, sizeof(double) * (size_t)std::max<long long>(h->d_total, 1)));
+    CU_TRY(h, cudaMalloc(&h->qbecp, pc));
+    CU_TRY(h, cudaMalloc(&h->qbT, (size_t)h->max_batch * h->ldp * sizeof(double2)));
+    CU_TRY(h, cudaMemset(h->qbT, 0, (size_t)h->max_batch * h->ldp * sizeof(double2)));
+    h->workspace_bytes += pc + (size_t)h->max_batch * h->ldp * sizeof(double2);
+  }
+  CU_TRY(h, cudaMemcpy(h->qpk, q_host, sizeof(double) * (size_t)h->d_total, cudaMemcpyHostToDevice));
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
+                                void* spsi_dev, int64_t ldspsi, int nbands, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!spsi_dev) return QE_HPSI_EINVAL;
+  int rc = check_apply_args(h, psi_dev, ldpsi, spsi_dev, ldspsi, nbands);
+  if (rc) return rc;
+  if (hpsi_dev) {
+    rc = check_apply_args(h, psi_dev, ldpsi, hpsi_dev, ldhpsi, nbands);
+    if (rc) return rc;
+    rc = check_apply_args(h, hpsi_dev, ldhpsi, spsi_dev, ldspsi, nbands);  // hpsi and spsi must not overlap either
+    if (rc) return rc;
+  }
+  if (nbands == 0) return QE_HPSI_OK;
+  const bool nl = h->nproj > 0 && h->npw > 0;
+  if (nl && !h->qpk) return QE_HPSI_ESTATE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const double2* psi = static_cast<const double2*>(psi_dev);
+  double2* hpsi = static_cast<double2*>(hpsi_dev);
+  double2* spsi = static_cast<double2*>(spsi_dev);
+  for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
+    const int nb = std::min(h->max_batch, nbands - b0);
+    const double2* p = psi + (size_t)b0 * ldpsi;
+    double2* sp = spsi + (size_t)b0 * ldspsi;
+    if (nl) {
+      rc = launch_becp(h, p, ldpsi, nb, st);  // becp, dbecp = D becp, dbT
+      if (rc) return rc;
+      const dim3 rg((nb + 127) / 128, h->nproj);
+      k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->qpk, h->qbecp,
+                                h->qbT, h->ldp);  // qbecp = q becp, qbT
+    }
+    if (hpsi) {
+      double2* hp = hpsi + (size_t)b0 * ldhpsi;
+      rc = launch_local(h, p, ldpsi, hp, ldhpsi, nb, st);
+      if (rc) return rc;
+      if (nl) {
+        rc = launch_vnl_add(h, h->dbT, hp, ldhpsi, nb, st);
+        if (rc) return rc;
+      }
+    }
+    if (h->npw > 0)
+      CU_TRY(h, cudaMemcpy2DAsync(sp, sizeof(double2) * (size_t)ldspsi, p, sizeof(double2) * (size_t)ldpsi,
+                                  sizeof(double2) * (size_t)h->npw, (size_t)nb, cudaMemcpyDeviceToDevice, st));
+    if (nl) {
+      rc = launch_vnl_add(h, h->qbT, sp, ldspsi, nb, st);  // spsi = psi + beta (q becp)
+      if (rc) return rc;
+    }
+  }
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-3: reduced matrices out[i][j] = <a_i|b_j> with the split-K DMMA kernel of a6
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb,
+                               int nb, void* out_dev, int64_t ldo, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (na < 0 || nb < 0) return QE_HPSI_EINVAL;
+  if (na == 0 || nb == 0) return QE_HPSI_OK;
+  if (!a_dev || !b_dev || !out_dev || lda < h->npw || ldb < h->npw || ldo < nb) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const double2* a = static_cast<const double2*>(a_dev);
+  const double2* b = static_cast<const double2*>(b_dev);
+  double2* out = static_cast<double2*>(out_dev);
+  if (h->npw == 0) {
+    CU_TRY(h, cudaMemset2DAsync(out, sizeof(double2) * (size_t)ldo, 0, sizeof(double2) * (size_t)nb, (size_t)na, st));
+    return QE_HPSI_OK;
+  }
+  CU_TRY(h, set_kernel_attrs());
+  // K slices depend on npw only, so an element's bits do not depend on how many rows/columns the call has
+  constexpr int MA = 512, NB = 128, LDC = 128;
+  const int ns0 = std::max(1, std::min(32, h->npw / 2048));
+  int kchunk = (h->npw + ns0 - 1) / ns0;
+  kchunk = std::max(ZgV0::BK, (kchunk + ZgV0::BK - 1) / ZgV0::BK * ZgV0::BK);
+  const int ns = std::max(1, (h->npw + kchunk - 1) / kchunk);
+  const size_t need = sizeof(double2) * (size_t)ns * (size_t)std::min(na, MA) * LDC;
+  if (need > h->ovl_cap) {
+    CU_TRY(h, cudaStreamSynchronize(st));  // an earlier call on this stream may still read the old buffer
+    cudaFree(h->ovl_partial);
+    h->ovl_partial = nullptr;
+    h->ovl_cap = 0;
+    const size_t cap = sizeof(double2) * (size_t)ns * MA * LDC;
+    cudaError_t e = cudaMalloc(&h->ovl_partial, cap);
+    if (e != cudaSuccess) {
+      h->last_cuda = (int)e;
+      return e == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA;
+    }
+    h->ovl_cap = cap;
+  }
+  for (int a0 = 0; a0 < na; a0 += MA) {
+    const int ma = std::min(MA, na - a0);
+    for (int b0 = 0; b0 < nb; b0 += NB) {
+      const int nbc = std::min(NB, nb - b0);
+      const int mt = (ma + ZgV0::BM - 1) / ZgV0::BM, nt = (nbc + ZgV0::BN - 1) / ZgV0::BN;
+      k_becp<ZgV0><<<dim3(mt * nt, ns), ZgV0::NT, ZgV0::SMEM_BECP, st>>>(a + (size_t)a0 * lda, lda, ma, b + (size_t)b0 * ldb,
+                                                                         ldb, nbc, h->npw, kchunk, h->ovl_partial, LDC);
+      k_ovl_reduce<<<dim3((nbc + 127) / 128, ma), 128, 0, st>>>(h->ovl_partial, ns, ma, LDC, nbc,
+                                                                out + (size_t)a0 * ldo + b0, ldo);
+    }
+  }
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-4: charge density rho += scale * sum_b occ[b] |psi_b(r)|^2 from steps a1, a2 and the inverse half of a3
+// ---------------------------------------------------------------------------------------------------------
+extern "C" int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, int nbands, const double* occ_dev,
+                               double scale, double* rho_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nbands < 0) return QE_HPSI_EINVAL;
+  if (nbands == 0 || h->npw == 0) return QE_HPSI_OK;
+  if (!psi_dev || !occ_dev || !rho_dev || ldpsi < h->npw) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const double2* psi = static_cast<const double2*>(psi_dev);
+  const FftGeom& g = h->geom;
+  const unsigned zt = (unsigned)((g.S + FFT_C - 1) / FFT_C);
+  const unsigned yt = (unsigned)(g.P * g.ntz);
+  const unsigned xt = (unsigned)(g.n2 * g.ntz);
+  const bool fast = h->f2p[0] != nullptr;
+  const Fft2pEntry *ex = h->f2p[0], *ey = h->f2p[1], *ez = h->f2p[2];
+  if (fast && !h->rho_attr_done) {
+    CU_TRY(h, cudaFuncSetAttribute((const void*)ex->rho, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ex->smem_x));
+    h->rho_attr_done = true;
+  }
+  for (int b0 = 0; b0 < nbands; b0 += h->fft_nb) {
+    const int n = std::min(h->fft_nb, nbands - b0);
+    const double2* p = psi + (size_t)b0 * ldpsi;
+    if (fast) {
+      ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
+      ey->yinv<<<dim3(yt, n), ey->nthreads, ey->smem_zy, st>>>(g, h->g2p, h->w1, h->w2);
+      ex->rho<<<dim3(xt, 1), ex->nthreads, ex->smem_x, st>>>(g, h->g2p, h->w2, n, occ_dev + b0, scale, rho_dev);
+    } else {
+      k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
+      k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
+      k_x_rho<<<dim3(xt, 1), FFT_NT, h->smem_x, st>>>(g, h->w2, n, occ_dev + b0, scale, rho_dev);
+    }
+  }
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------

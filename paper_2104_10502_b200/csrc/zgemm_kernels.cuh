@@ -213,6 +213,20 @@ __global__ void k_becp_reduce(const double2* __restrict__ partial, int nsplit, i
   }
   becp[(size_t)p * ldc + b] = make_double2(re, im);
 }
+// NEXT-3 (reduced matrices <a_i|b_j>): out[i][j] = sum_ks partial[ks][i][j], ks ascending, with its own row stride
+__global__ void k_ovl_reduce(const double2* __restrict__ partial, int nsplit, int na, int ldc, int nb,
+                             double2* __restrict__ out, long long ldo) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (b >= nb) return;
+  double re = 0.0, im = 0.0;
+  for (int ks = 0; ks < nsplit; ++ks) {
+    const double2 v = partial[((size_t)ks * na + p) * ldc + b];
+    re += v.x;
+    im += v.y;
+  }
+  out[(size_t)p * ldo + b] = make_double2(re, im);
+}
 // dbecp[p][b] = sum_j D[p][j] becp[blk_start(p)+j][b]; written both as dbecp[p][b] and transposed dbT[b][p]
 __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int nb, const int* __restrict__ proj_blk0,
                        const int* __restrict__ proj_nh, const long long* __restrict__ proj_doff,

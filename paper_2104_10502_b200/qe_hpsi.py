@@ -47,6 +47,10 @@ SIGNATURES = {
     "qe_hpsi_profile_read": (_i32, [_vp, _pd, _pi64]),
     "qe_hpsi_fft_local": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
     "qe_hpsi_nonlocal": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
+    "qe_hpsi_set_s": (_i32, [_vp, _pd]),
+    "qe_hpsi_apply_hs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i64, _i32, _vp]),
+    "qe_hpsi_overlap": (_i32, [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _vp, _i64, _vp]),
+    "qe_hpsi_density": (_i32, [_vp, _vp, _i64, _i32, _vp, _dbl, _vp, _vp]),
 }
 
 _lib = None
@@ -186,6 +190,54 @@ class Hpsi:
         _check(self._lib.qe_hpsi_apply_host(self._h, _vp(psi_host.data_ptr()), ldp, _vp(hpsi_host.data_ptr()), ldh, nb),
                self._h)
         return hpsi_host
+
+    # -- rows marked "next" in SURVEY.md 8(f) ------------------------------------------------------------
+    def set_s(self, qblocks):
+        """qe_hpsi_set_s: per-atom real symmetric q blocks of the overlap operator (same packing as D)."""
+        qpk = np.ascontiguousarray(np.concatenate([np.asarray(q, dtype=np.float64).reshape(-1) for q in qblocks])) \
+            if self.nproj else np.zeros(1)
+        self._nq = qpk.size
+        _check(self._lib.qe_hpsi_set_s(self._h, qpk.ctypes.data_as(_pd)), self._h)
+
+    def apply_hs(self, psi, hpsi=None, spsi=None, stream=None, want_h=True):
+        """qe_hpsi_apply_hs: (H psi, S psi) with becp shared; want_h=False computes S psi only (returns (None, spsi))."""
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.dim() == 2 and psi.stride(1) == 1
+        nb = int(psi.shape[0])
+        if spsi is None:
+            spsi = torch.zeros_like(psi)
+        if want_h and hpsi is None:
+            hpsi = torch.zeros_like(psi)
+        ld = lambda t: int(t.stride(0)) if nb > 1 else int(t.shape[1])
+        hp = _vp(hpsi.data_ptr()) if want_h else _vp(None)
+        _check(self._lib.qe_hpsi_apply_hs(self._h, _vp(psi.data_ptr()), ld(psi), hp, ld(hpsi) if want_h else 0,
+                                          _vp(spsi.data_ptr()), ld(spsi), nb, _stream_ptr(stream)), self._h)
+        return (hpsi if want_h else None), spsi
+
+    def overlap(self, a, b, out=None, stream=None):
+        """qe_hpsi_overlap: out[i][j] = <a_i|b_j> over the npw sphere entries; a [na, ld], b [nb, ld] complex128."""
+        for t in (a, b):
+            assert t.is_cuda and t.dtype == torch.complex128 and t.dim() == 2 and t.stride(1) == 1
+        na, nb = int(a.shape[0]), int(b.shape[0])
+        if out is None:
+            out = torch.zeros((na, nb), dtype=torch.complex128, device=a.device)
+        assert out.is_cuda and out.dtype == torch.complex128 and out.stride(1) == 1
+        lda = int(a.stride(0)) if na > 1 else int(a.shape[1])
+        ldb = int(b.stride(0)) if nb > 1 else int(b.shape[1])
+        ldo = int(out.stride(0)) if na > 1 else int(out.shape[1])
+        _check(self._lib.qe_hpsi_overlap(self._h, _vp(a.data_ptr()), lda, na, _vp(b.data_ptr()), ldb, nb,
+                                         _vp(out.data_ptr()), ldo, _stream_ptr(stream)), self._h)
+        return out
+
+    def density(self, psi, occ, scale, rho, stream=None):
+        """qe_hpsi_density: rho[N1,N2,N3] += scale * sum_b occ[b] |psi_b(r)|^2 (rho, occ: CUDA float64 tensors)."""
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.dim() == 2 and psi.stride(1) == 1
+        nb = int(psi.shape[0])
+        assert occ.is_cuda and occ.dtype == torch.float64 and occ.numel() == nb and occ.is_contiguous()
+        assert rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous()
+        ldp = int(psi.stride(0)) if nb > 1 else int(psi.shape[1])
+        _check(self._lib.qe_hpsi_density(self._h, _vp(psi.data_ptr()), ldp, nb, _vp(occ.data_ptr()), float(scale),
+                                         _vp(rho.data_ptr()), _stream_ptr(stream)), self._h)
+        return rho
 
     # -- accessors ---------------------------------------------------------------------------------------
     def maps(self):

@@ -1,0 +1,143 @@
+"""GPU parity for the rows SURVEY.md 8(f) marks "next" -- S|psi> (NEXT-2), reduced matrices (NEXT-3), charge density
+(NEXT-4) -- through the C ABI against the oracle (oracle/hpsi_oracle.py: spsi_of, overlap_of, density_of) on the same
+seeded inputs.  PAPER.md:L226 ("application of the overlap operator", "charge density generation"), L162/L168."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import hpsi_oracle as orc
+from paper_2104_10502_b200 import inputs, qe_hpsi
+from tests import _gpu
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def _qblocks(wl, seed):
+    rng = np.random.default_rng(seed)
+    q = rng.uniform(-1.0, 1.0, (wl.natoms, wl.nh, wl.nh))
+    return 0.5 * (q + q.transpose(0, 2, 1))
+
+
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
+def test_apply_hs_against_oracle(cfg):
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    nb = min(wl.nbands, 24)
+    psi = _gpu.gen_psi_dev(inp, 0, nb)
+    q = _qblocks(wl, 17)
+    h.set_s(q)
+    hpsi = torch.full_like(psi, 3.0)
+    spsi = torch.full_like(psi, 5.0)
+    h.apply_hs(psi, hpsi, spsi)
+    torch.cuda.synchronize()
+    ph = psi[:, :npw].cpu().numpy()
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    href = _gpu.oracle_hpsi(inp, sp, ph)
+    sref = orc.spsi_of(beta, q, ph)
+    assert _gpu.rel_l2(hpsi.cpu().numpy()[:, :npw], href).max() <= TOL
+    assert _gpu.rel_l2(spsi.cpu().numpy()[:, :npw], sref).max() <= TOL
+    assert np.all(spsi.cpu().numpy()[:, npw:] == 5.0) and np.all(hpsi.cpu().numpy()[:, npw:] == 3.0)
+    # H psi from apply_hs is the H psi of apply, bit for bit; S psi alone equals S psi of the joint call
+    h2 = h.apply(psi)
+    _, s2 = h.apply_hs(psi, want_h=False)
+    torch.cuda.synchronize()
+    assert torch.equal(h2[:, :npw].view(torch.float64), hpsi[:, :npw].view(torch.float64))
+    assert torch.equal(s2[:, :npw].view(torch.float64), spsi[:, :npw].view(torch.float64))
+    h.destroy()
+
+
+def test_apply_hs_without_projectors_and_state_errors():
+    h, inp = _gpu.make("T4_noproj")
+    psi = _gpu.gen_psi_dev(inp, 0, 3)
+    _, s = h.apply_hs(psi, want_h=False)  # no projectors: S = 1, no set_s needed
+    torch.cuda.synchronize()
+    assert torch.equal(s[:, :h.npw].view(torch.float64), psi[:, :h.npw].view(torch.float64))
+    h.destroy()
+    h, inp = _gpu.make("T1_general_k")
+    psi = _gpu.gen_psi_dev(inp, 0, 2)
+    with pytest.raises(qe_hpsi.QeHpsiError):
+        h.apply_hs(psi)  # projectors but set_s never called
+    h.set_s(_qblocks(inp["wl"], 1))
+    with pytest.raises(qe_hpsi.QeHpsiError):
+        h.apply_hs(psi, psi.clone(), psi)  # spsi aliases psi
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg,na,nb", [("T1_general_k", 5, 7), (0, 16, 16), (1, 128, 128), (1, 130, 61)])
+def test_overlap_against_oracle(cfg, na, nb):
+    h, inp = _gpu.make(cfg)
+    npw = h.npw
+    a = _gpu.gen_psi_dev(inp, 0, na)
+    b = h.apply(_gpu.gen_psi_dev(inp, 100, nb))  # b = H psi: the projected Hamiltonian of the Davidson step
+    out = torch.full((na, nb + 3), 9.0, dtype=torch.complex128, device="cuda")
+    h.overlap(a, b, out[:, :nb])
+    torch.cuda.synchronize()
+    ref = orc.overlap_of(a[:, :npw].cpu().numpy(), b[:, :npw].cpu().numpy())
+    got = out.cpu().numpy()
+    scale = np.sqrt((np.abs(a[:, :npw].cpu().numpy()) ** 2).sum(1))[:, None] * np.sqrt((np.abs(b[:, :npw].cpu().numpy()) ** 2).sum(1))[None, :]
+    assert (np.abs(got[:, :nb] - ref) / scale).max() <= 1e-13  # |<a|b> error| <= 1e-13 |a||b|
+    assert np.all(got[:, nb:] == 9.0)
+    # an element's bits do not depend on the shape of the call
+    o2 = h.overlap(a[:3], b[:2])
+    torch.cuda.synchronize()
+    assert torch.equal(o2.view(torch.float64), out[:3, :2].contiguous().view(torch.float64))
+    h.destroy()
+
+
+def test_overlap_of_psi_with_hpsi_is_hermitian_on_gpu():
+    h, inp = _gpu.make(0)
+    psi = _gpu.gen_psi_dev(inp, 0, 16)
+    hm = h.overlap(psi, h.apply(psi)).cpu().numpy()
+    assert np.abs(hm - hm.conj().T).max() <= 1e-12 * np.abs(hm).max()
+    h.destroy()
+
+
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT])
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T2b_radix5_20", "T3_aliased", "T5_odd_bands", 0])
+def test_density_against_oracle(cfg, flags):
+    h, inp = _gpu.make(cfg, flags=flags, max_batch=5)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    nb = min(wl.nbands, 7)
+    psi = _gpu.gen_psi_dev(inp, 0, nb)
+    occ = torch.linspace(2.0, 0.25, nb, dtype=torch.float64, device="cuda")
+    rho = torch.full(tuple(wl.nr), 0.125, dtype=torch.float64, device="cuda")  # accumulated into
+    scale = 1.0 / wl.omega
+    h.density(psi, occ, scale, rho)
+    torch.cuda.synchronize()
+    ref = 0.125 + orc.density_of(sp["fft_index"], tuple(wl.nr), psi[:, :npw].cpu().numpy(), occ.cpu().numpy(), scale)
+    got = rho.cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_density_full_size_properties_and_sampled_points(cfg):
+    """Full-size configs: Parseval (mean of rho = scale * sum occ |c|^2) and sampled grid points evaluated one by
+    one from the definition psi(r) = sum_G c(G) exp(2 pi i n.i/N)."""
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    npw = h.npw
+    nb = 8
+    psi = _gpu.gen_psi_dev(inp, 0, nb)
+    occ = torch.linspace(2.0, 1.0, nb, dtype=torch.float64, device="cuda")
+    rho = torch.zeros(tuple(wl.nr), dtype=torch.float64, device="cuda")
+    h.density(psi, occ, 1.0, rho)
+    torch.cuda.synchronize()
+    ph = psi[:, :npw].cpu().numpy()
+    tot = float((occ.cpu().numpy() * (np.abs(ph) ** 2).sum(1)).sum())
+    assert abs(rho.mean().item() - tot) <= 1e-12 * tot
+    assert rho.min().item() >= 0.0
+    mil = inp["miller"].astype(np.float64)
+    rng = np.random.default_rng(3)
+    nr = np.array(wl.nr)
+    for _ in range(6):
+        i = rng.integers(0, nr)
+        phase = np.exp(2j * np.pi * (mil @ (i / nr)))
+        val = float((occ.cpu().numpy() * np.abs(ph @ phase) ** 2).sum())
+        assert abs(rho[i[0], i[1], i[2]].item() - val) <= 1e-11 * max(val, tot)
+    h.destroy()
