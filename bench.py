@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--detail", action="store_true", help="extra pass with per-FFT-kernel events (stderr table)")
+    ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows (apply_hs, overlap, density): "
+                    "adds a next_rows object to the JSON line")
     return ap.parse_args()
 
 
@@ -160,6 +162,51 @@ def oracle_sample_time(wl, nbands_sample=2, atoms_sample=16):
     desc = (f"oracle Level B on {nbands_sample} bands of {wl.name}: local+kinetic on the full {wl.nr} grid, "
             f"nonlocal on {na}/{wl.natoms} atoms scaled linearly")
     return per_band, desc, torch.get_num_threads()
+
+
+def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
+    """CUDA-event timings of the rows SURVEY.md 8(f) marks next, on one chunk of `batch` bands of the workload:
+    qe_hpsi_apply_hs (H psi and S psi), qe_hpsi_overlap (<psi|H psi>, batch x batch), qe_hpsi_density."""
+    nb = min(batch, psi.shape[0])
+    p, hp = psi[:nb], hpsi[:nb]
+    sp = torch.empty_like(p)
+    out = {}
+
+    def ev_time(fn, reps=3):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    if wl.nproj:
+        rng = np.random.default_rng(7)
+        q = rng.uniform(-1, 1, (wl.natoms, wl.nh, wl.nh))
+        h.set_s(0.5 * (q + q.transpose(0, 2, 1)))
+    ms = ev_time(lambda: h.apply_hs(p, hp, sp))
+    fl = 3 * 8.0 * wl.nproj * npw * nb  # a6 once + a8 twice
+    out["apply_hs"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "proj_tflops": fl / ms * 1e-9 if wl.nproj else None,
+                       "bound": "tensor", "frac_of_dmma_peak": fl / ms * 1e-9 / dmma if wl.nproj else None}
+    m = torch.empty((nb, nb), dtype=torch.complex128, device="cuda")
+    ms = ev_time(lambda: h.overlap(p, hp, m))
+    fl = 8.0 * nb * nb * npw
+    by = 2 * 16.0 * nb * npw
+    out["overlap"] = {"ms": ms, "shape": [nb, nb, npw], "tflops": fl / ms * 1e-9, "gbs": by / ms * 1e-6,
+                      "bound": "hbm" if by / (hbm_peak * 1e9) > fl / (dmma * 1e12) else "tensor",
+                      "frac": max(by / (hbm_peak * 1e9), fl / (dmma * 1e12)) / (ms * 1e-3)}
+    occ = torch.full((nb,), 2.0, dtype=torch.float64, device="cuda")
+    rho = torch.zeros(tuple(wl.nr), dtype=torch.float64, device="cuda")
+    ms = ev_time(lambda: h.density(p, occ, 1.0 / wl.omega, rho))
+    n1, n2, n3 = wl.nr
+    info = h.info()
+    by = nb * 16.0 * (npw + 2 * info["S"] * n3 + 2 * info["P"] * n2 * n3) + 16.0 * n1 * n2 * n3 * -(-nb // info["fft_nb"])
+    out["density"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "algorithmic_gbs": by / ms * 1e-6, "bound": "hbm",
+                      "frac": by / ms * 1e-6 / hbm_peak}
+    return out
 
 
 def run_reference(args, wl, rank):
@@ -302,7 +349,10 @@ def main():
         roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
                     "traffic": committed_traffic(args.config, kname), "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-resident "
                     "loop measured live by qe_hpsi_probe_fp64; MEASURED_PEAKS.json has no FP64 entry",
-                    "ms_per_launch": t_k, "flops_per_launch": flops_launch}
+                    "ms_per_launch": t_k, "flops_per_launch": flops_launch,
+                    "executed_dmma_frac": ach / dmma * 0.75,
+                    "note": "achieved counts the algorithmic 8 flops per complex MAC; the 3M product executes 6, so frac can "
+                            "exceed 1 (DESIGN.md section 6); executed_dmma_frac = frac x 0.75 is the pipe utilisation"}
     else:
         bytes_launch = m["b_fft"] * min(batch, nb)
         ach = bytes_launch / (t_fft * 1e-3) * 1e-9
@@ -334,6 +384,8 @@ def main():
                                   "fp64_tensor_tflops": dmma, "fp64_dfma_tflops": dfma, "bytes_per_band": m["b_fft"] + m["b_beta"],
                                   "proj_flops_per_band": m["f_proj"], "note": "max(bytes/HBM, projector flops/FP64 tensor) per band"},
             "stages": stages, "cpu_baseline": cpu, "setup_s": t_setup}
+    if args.next:
+        line["next_rows"] = time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak)
     print(json.dumps(line), flush=True)
 
     if args.detail:
