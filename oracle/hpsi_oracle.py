@@ -304,3 +304,40 @@ def density_of(fft_index, nr, psi, occ, scale):
         pr = psi_r(fft_index, nr, psi[b])
         rho += occ[b] * (pr.real**2 + pr.imag**2)
     return scale * rho
+
+
+# ----------------------------------------------------------------------------------------------------------
+# NEXT-1: Gamma-only path (k = 0, real wavefunctions; the paper ports "Gamma-point specific algorithms" for every
+# kernel).  Only the half sphere is stored: c(-G) = conj(c(G)).  The oracle is the definition: expand
+# to the full sphere, apply the full-sphere H, restrict (DESIGN.md section 2 item 21).
+# ----------------------------------------------------------------------------------------------------------
+
+
+def gamma_half(miller):
+    """Half sphere of a k = 0 sphere in canonical order: keep G = (n1,n2,n3) with n1 > 0, or n1 == 0 and n2 > 0, or
+    n1 == n2 == 0 and n3 >= 0 (G = 0 included), in the order they have in the full sphere.
+    Returns (idx_plus [ngw] positions of G in the full sphere, idx_minus [ngw] positions of -G)."""
+    m = np.asarray(miller, dtype=np.int64)
+    keep = (m[:, 0] > 0) | ((m[:, 0] == 0) & (m[:, 1] > 0)) | ((m[:, 0] == 0) & (m[:, 1] == 0) & (m[:, 2] >= 0))
+    idx_plus = np.nonzero(keep)[0]
+    pos = {tuple(v): i for i, v in enumerate(m.tolist())}
+    idx_minus = np.array([pos[(-a, -b, -c)] for a, b, c in m[idx_plus].tolist()], dtype=np.int64)
+    return idx_plus, idx_minus
+
+
+def gamma_expand(x_half, idx_plus, idx_minus, npw):
+    """[nb, ngw] half-sphere coefficients -> [nb, npw] full sphere with x(-G) = conj(x(G)) (G = 0 kept as given)."""
+    full = np.zeros((x_half.shape[0], npw), dtype=np.complex128)
+    full[:, idx_minus] = np.conj(x_half)
+    full[:, idx_plus] = x_half
+    return full
+
+
+def hpsi_gamma(miller, fft_index, g2kin, nr, vr, psi_half, beta_half=None, dblocks=None):
+    """(H psi) on the half sphere for real wavefunctions: expand psi and beta to the full sphere (Hermitian
+    completion), apply Level B, restrict to the half sphere.  psi_half [nb, ngw] with Im psi(G=0) = 0."""
+    ip, im = gamma_half(miller)
+    npw = np.asarray(miller).shape[0]
+    psi = gamma_expand(psi_half, ip, im, npw)
+    beta = gamma_expand(beta_half, ip, im, npw) if beta_half is not None and beta_half.shape[0] else None
+    return hpsi_dual(fft_index, g2kin, nr, vr, psi, beta, dblocks)[:, ip]

@@ -146,3 +146,66 @@ def test_psi_r_matches_explicit_dft():
     box = np.zeros(nr, complex)
     box.reshape(-1)[sp["fft_index"]] = psi
     np.testing.assert_allclose(orc.psi_r(sp["fft_index"], nr, psi), orc.dft3_explicit(box, +1), atol=1e-12)
+
+
+# ---- Gamma-only path (NEXT-1) ---------------------------------------------------------------------------------------
+def _gamma_problem(cfg, nb=3):
+    """k = 0 tiny case: half-sphere psi / beta with real G = 0 components (inputs of a real-wavefunction calculation)."""
+    pr = problem(cfg)
+    assert np.all(np.asarray(pr["wl"].xk) == 0.0)
+    ip, im = orc.gamma_half(pr["miller"])
+    psi_h = pr["psi"][:nb, ip].copy()
+    psi_h[:, 0] = psi_h[:, 0].real
+    beta_h = pr["beta"][:, ip].copy()
+    beta_h[:, 0] = beta_h[:, 0].real
+    return pr, ip, im, psi_h, beta_h
+
+
+def test_gamma_half_is_a_partition_of_the_sphere():
+    pr = problem("T2_radix5")
+    m = pr["miller"].astype(int)
+    ip, im = orc.gamma_half(m)
+    npw = m.shape[0]
+    assert ip[0] == 0 and tuple(m[0]) == (0, 0, 0) and im[0] == 0  # G = 0 first, its own negative
+    assert np.all(np.diff(ip) > 0)  # canonical order preserved
+    np.testing.assert_array_equal(m[im], -m[ip])
+    both = np.concatenate([ip, im[1:]])
+    assert both.size == npw and np.array_equal(np.sort(both), np.arange(npw))  # each G exactly once
+    assert 2 * ip.size - 1 == npw
+    # brute force of the half rule on every sphere point
+    for i, (a, b, c) in enumerate(m.tolist()):
+        assert (i in set(ip.tolist())) == ((a, b, c) > (0, 0, -1) and (a > 0 or (a == 0 and (b > 0 or (b == 0 and c >= 0)))))
+
+
+@pytest.mark.parametrize("cfg", ["T2_radix5", "T2b_radix5_20", "T3_aliased", 0])
+def test_gamma_expansion_gives_real_psi_and_closed_result(cfg):
+    pr, ip, im, psi_h, beta_h = _gamma_problem(cfg)
+    npw = pr["miller"].shape[0]
+    full = orc.gamma_expand(psi_h, ip, im, npw)
+    for b in range(full.shape[0]):
+        assert np.abs(orc.psi_r(pr["fft_index"], pr["nr"], full[b]).imag).max() < 1e-12  # psi(r) is real
+    beta_f = orc.gamma_expand(beta_h, ip, im, npw)
+    hf = orc.hpsi_dual(pr["fft_index"], pr["g2kin"], pr["nr"], pr["vr"], full, beta_f, pr["dblocks"])
+    # H of a real field with real V and Hermitian-completed projectors is a real field: h(-G) = conj(h(G))
+    np.testing.assert_allclose(hf[:, im], np.conj(hf[:, ip]), atol=1e-12 * np.abs(hf).max())
+    # becp is real
+    assert np.abs(orc.becp_of(beta_f, full).imag).max() < 1e-13
+    got = orc.hpsi_gamma(pr["miller"], pr["fft_index"], pr["g2kin"], pr["nr"], pr["vr"], psi_h, beta_h, pr["dblocks"])
+    np.testing.assert_array_equal(got, hf[:, ip])
+    # and it is the dense-H (Level A, explicit DFT matrices) result restricted to the half sphere
+    hd = orc.dense_h(pr["miller"], pr["g2kin"], pr["nr"], pr["vr"], beta_f, pr["dblocks"])
+    np.testing.assert_allclose(got, orc.hpsi_dense(hd, full)[:, ip], atol=1e-11 * np.abs(got).max())
+
+
+def test_gamma_single_plane_wave_pair_in_constant_potential():
+    """psi = c e^{iGr} + conj(c) e^{-iGr} (a real cosine) in V0 without projectors: H psi = (|G|^2 + V0) psi."""
+    pr, ip, im, psi_h, _ = _gamma_problem("T2_radix5", nb=1)
+    psi_h[:] = 0.0
+    g = ip.size // 2
+    psi_h[0, g] = 0.3 - 0.7j
+    v0 = 0.83
+    vr = np.full(pr["nr"], v0)
+    got = orc.hpsi_gamma(pr["miller"], pr["fft_index"], pr["g2kin"], pr["nr"], vr, psi_h)
+    ref = np.zeros_like(psi_h)
+    ref[0, g] = (pr["g2kin"][ip[g]] + v0) * psi_h[0, g]
+    np.testing.assert_allclose(got, ref, atol=1e-13)
