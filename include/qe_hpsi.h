@@ -167,6 +167,22 @@ int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const v
 int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, int nbands, const double* occ_dev, double scale,
                     double* rho_dev, void* cuda_stream);
 
+/* NEXT-1, Gamma-only path ("Gamma-point specific algorithms"): k = 0 and real wavefunctions, so only
+ * the half sphere is stored, c(-G) = conj(c(G)).  Half rule: G = n1 b1 + n2 b2 + n3 b3 is kept if n1 > 0, or n1 == 0 and
+ * n2 > 0, or n1 == n2 == 0 and n3 >= 0; order = the order those G have in the canonical full sphere (G = 0 first).
+ * psi, hpsi and beta are complex128 arrays over the ngw half-sphere entries with Im(x[G=0]) = 0; beta(-G) = conj(beta(G))
+ * is implied (projector functions real in real space).  The library transforms two bands per complex FFT and contracts
+ * the projectors as real matrices over the 2*ngw real components.  Arguments as qe_hpsi_create / qe_hpsi_apply (no k). */
+typedef struct qe_hpsi_gamma_handle* qe_hpsi_gamma_t;
+int qe_hpsi_gamma_gsphere(const double at[9], double ecutwfc, const int nr[3], int64_t* ngw, int32_t* miller_host);
+int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], double ecutwfc, const int nr[3], const double* vr_dev,
+                         int nproj, const void* beta_dev, int64_t ldbeta, int nblocks, const int32_t* blk_off_host,
+                         const double* d_host, int max_batch, unsigned flags, void* cuda_stream);
+int qe_hpsi_gamma_apply(qe_hpsi_gamma_t g, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
+                        void* cuda_stream);
+int64_t qe_hpsi_gamma_ngw(qe_hpsi_gamma_t g);
+int qe_hpsi_gamma_destroy(qe_hpsi_gamma_t g);
+
 #ifdef __cplusplus
 }
 #endif

@@ -91,6 +91,8 @@ struct qe_hpsi_handle {
   double2* ovl_partial = nullptr;
   size_t ovl_cap = 0;
   bool rho_attr_done = false;
+  // NEXT-1: this handle is the half-sphere nonlocal part of a Gamma-only handle (real becp, two real DMMAs per block)
+  bool gamma = false;
   int nb_last = 0;
   size_t workspace_bytes = 0;
   // apply_host staging
@@ -493,6 +495,10 @@ cudaError_t set_kernel_attrs() {
   SET_SMEM(k_vnl_add<ZgV4>);
   SET_SMEM(k_becp<ZgV5>);
   SET_SMEM(k_vnl_add<ZgV5>);
+  e = cudaFuncSetAttribute(k_becp<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
 #undef SET_SMEM
   g_attr_done = true;
   return cudaSuccess;
@@ -621,6 +627,69 @@ void choose_split(qe_hpsi_handle* h) {
   if (kchunk < ZG_BK) kchunk = ZG_BK;
   h->kchunk = kchunk;
   h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+}
+
+// nonlocal state of a handle whose npw is already set (K dimension of a6 / M dimension of a8): beta (copied or
+// borrowed), D tables, split-K plan and workspaces.  Shared by qe_hpsi_create and qe_hpsi_gamma_create.
+cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                           const int32_t* blk_off_host, const double* d_host, long long d_total, int max_batch,
+                           unsigned flags, cudaStream_t st) {
+#define CR_TRY(expr)                     \
+  do {                                   \
+    cudaError_t e__ = (expr);            \
+    if (e__ != cudaSuccess) return e__;  \
+  } while (0)
+
+    if (flags & QE_HPSI_BORROW_BETA) {
+      h->beta = static_cast<const double2*>(beta_dev);
+      h->ldbeta = ldbeta;
+    } else {
+      h->ldbeta = ((long long)h->npw + 7) / 8 * 8;
+      CR_TRY(cudaMalloc(&h->beta_own, sizeof(double2) * (size_t)nproj * h->ldbeta));
+      CR_TRY(cudaMemsetAsync(h->beta_own, 0, sizeof(double2) * (size_t)nproj * h->ldbeta, st));
+      CR_TRY(cudaMemcpy2DAsync(h->beta_own, sizeof(double2) * h->ldbeta, beta_dev, sizeof(double2) * (size_t)ldbeta,
+                               sizeof(double2) * (size_t)h->npw, (size_t)nproj, cudaMemcpyDeviceToDevice, st));
+      h->beta = h->beta_own;
+    }
+    std::vector<int> blk0((size_t)nproj), nhv((size_t)nproj);
+    std::vector<long long> doff((size_t)nproj);
+    long long off = 0;
+    for (int a = 0; a < nblocks; ++a) {
+      const int q0 = blk_off_host[a], nh = blk_off_host[a + 1] - q0;
+      for (int i = 0; i < nh; ++i) {
+        blk0[q0 + i] = q0;
+        nhv[q0 + i] = nh;
+        doff[q0 + i] = off + (long long)i * nh;
+      }
+      off += (long long)nh * nh;
+    }
+    h->d_total = d_total;
+    std::vector<double> dv(d_host, d_host + d_total);
+    CR_TRY(upload(&h->proj_blk0, blk0, st));
+    CR_TRY(upload(&h->proj_nh, nhv, st));
+    CR_TRY(upload(&h->proj_doff, doff, st));
+    CR_TRY(upload(&h->dpk, dv, st));
+    h->ldc = (max_batch + 1) / 2 * 2;
+    h->ldp = (nproj + 7) / 8 * 8;
+    h->zg_variant = std::min(std::max(env_int("QE_HPSI_ZG_VARIANT", 0), 0), ZG_NVARIANT - 1);
+    choose_split(h);
+    const int forced = env_int("QE_HPSI_NSPLIT", 0);
+    if (forced > 0) {
+      const int ZG_BK = ZG_BK_TAB[h->zg_variant];
+      int kchunk = (h->npw + forced - 1) / forced;
+      kchunk = std::max(ZG_BK, (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK);
+      h->kchunk = kchunk;
+      h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+    }
+    const size_t pc = (size_t)nproj * h->ldc * sizeof(double2);
+    CR_TRY(cudaMalloc(&h->partial, pc * h->nsplit));
+    CR_TRY(cudaMalloc(&h->becp, pc));
+    CR_TRY(cudaMalloc(&h->dbecp, pc));
+    CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
+    CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
+    h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
+  #undef CR_TRY
+  return cudaSuccess;
 }
 
 }  // namespace
@@ -840,56 +909,8 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   }
 
   // ---- nonlocal ---------------------------------------------------------------------------------------
-  if (nproj > 0) {
-    if (flags & QE_HPSI_BORROW_BETA) {
-      h->beta = static_cast<const double2*>(beta_dev);
-      h->ldbeta = ldbeta;
-    } else {
-      h->ldbeta = ((long long)h->npw + 7) / 8 * 8;
-      CR_TRY(cudaMalloc(&h->beta_own, sizeof(double2) * (size_t)nproj * h->ldbeta));
-      CR_TRY(cudaMemsetAsync(h->beta_own, 0, sizeof(double2) * (size_t)nproj * h->ldbeta, st));
-      CR_TRY(cudaMemcpy2DAsync(h->beta_own, sizeof(double2) * h->ldbeta, beta_dev, sizeof(double2) * (size_t)ldbeta,
-                               sizeof(double2) * (size_t)h->npw, (size_t)nproj, cudaMemcpyDeviceToDevice, st));
-      h->beta = h->beta_own;
-    }
-    std::vector<int> blk0((size_t)nproj), nhv((size_t)nproj);
-    std::vector<long long> doff((size_t)nproj);
-    long long off = 0;
-    for (int a = 0; a < nblocks; ++a) {
-      const int q0 = blk_off_host[a], nh = blk_off_host[a + 1] - q0;
-      for (int i = 0; i < nh; ++i) {
-        blk0[q0 + i] = q0;
-        nhv[q0 + i] = nh;
-        doff[q0 + i] = off + (long long)i * nh;
-      }
-      off += (long long)nh * nh;
-    }
-    h->d_total = d_total;
-    std::vector<double> dv(d_host, d_host + d_total);
-    CR_TRY(upload(&h->proj_blk0, blk0, st));
-    CR_TRY(upload(&h->proj_nh, nhv, st));
-    CR_TRY(upload(&h->proj_doff, doff, st));
-    CR_TRY(upload(&h->dpk, dv, st));
-    h->ldc = (max_batch + 1) / 2 * 2;
-    h->ldp = (nproj + 7) / 8 * 8;
-    h->zg_variant = std::min(std::max(env_int("QE_HPSI_ZG_VARIANT", 0), 0), ZG_NVARIANT - 1);
-    choose_split(h);
-    const int forced = env_int("QE_HPSI_NSPLIT", 0);
-    if (forced > 0) {
-      const int ZG_BK = ZG_BK_TAB[h->zg_variant];
-      int kchunk = (h->npw + forced - 1) / forced;
-      kchunk = std::max(ZG_BK, (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK);
-      h->kchunk = kchunk;
-      h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
-    }
-    const size_t pc = (size_t)nproj * h->ldc * sizeof(double2);
-    CR_TRY(cudaMalloc(&h->partial, pc * h->nsplit));
-    CR_TRY(cudaMalloc(&h->becp, pc));
-    CR_TRY(cudaMalloc(&h->dbecp, pc));
-    CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
-    CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
-    h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
-  }
+  if (nproj > 0)
+    CR_TRY(setup_nonlocal(h, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
   CR_TRY(cudaStreamSynchronize(st));
 #undef CR_TRY
   *out = h;
@@ -982,6 +1003,12 @@ void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, in
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const size_t t0 = prof_mark(h, st);
+  if (h->gamma) {
+    using Cfg = ZgV0;
+    const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+    k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
+                                                                                 h->npw, h->kchunk, h->partial, h->ldc);
+  } else
   switch (h->zg_variant) {
     case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st); break;
     case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st); break;
@@ -993,7 +1020,11 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
   const size_t t1 = prof_mark(h, st);
   prof_span(h, t0, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
-  k_becp_reduce<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->becp);
+  if (h->gamma)
+    k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->beta, h->ldbeta, psi, ldpsi,
+                                            h->becp);
+  else
+    k_becp_reduce<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->becp);
   k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
                             h->dbT, h->ldp);
   prof_span(h, t1, prof_mark(h, st), SLOT_DMUL);
@@ -1004,6 +1035,13 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 
 // a8
 int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  if (h->gamma) {
+    using Cfg = ZgV0;
+    const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+    if (mt > 0)
+      k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
+                                                                                h->ldp, nb, hpsi, ldh);
+  } else
   switch (h->zg_variant) {
     case 1: vnl_launch<ZgV1>(h, bT, hpsi, ldh, nb, st); break;
     case 2: vnl_launch<ZgV2>(h, bT, hpsi, ldh, nb, st); break;
@@ -1237,6 +1275,229 @@ extern "C" int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, 
       k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
       k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
       k_x_rho<<<dim3(xt, 1), FFT_NT, h->smem_x, st>>>(g, h->w2, n, occ_dev + b0, scale, rho_dev);
+    }
+  }
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-1: Gamma-only path (k = 0, real wavefunctions, half sphere; "Gamma-point specific algorithms").
+// A Gamma handle = a full-sphere local handle (nproj = 0) that transforms TWO real bands per complex FFT
+// (Phi = c1 + i c2 on the full sphere), a half-sphere nonlocal handle (real becp, two real DMMAs per 8x8x4 block)
+// and the index maps of G / -G.
+// ---------------------------------------------------------------------------------------------------------
+struct qe_hpsi_gamma_handle {
+  qe_hpsi_handle* loc = nullptr;  // full sphere, local + kinetic only, max_batch = pairs
+  qe_hpsi_handle* nl = nullptr;   // npw = ngw: nonlocal part only (may be null: no projectors)
+  int ngw = 0, npw = 0, max_batch = 0, pairs = 0;
+  long long ldf = 0;              // row stride of phi / hphi
+  int *idx_plus = nullptr, *idx_minus = nullptr;  // [ngw] positions of G and -G in the full sphere
+  double2 *phi = nullptr, *hphi = nullptr;        // [pairs][ldf]
+};
+
+namespace {
+
+// does the Miller triple belong to the half sphere?  (n1 > 0) or (n1 == 0 and n2 > 0) or (n1 == n2 == 0 and n3 >= 0)
+inline bool gamma_keep(const int* m) { return m[0] > 0 || (m[0] == 0 && (m[1] > 0 || (m[1] == 0 && m[2] >= 0))); }
+
+// Phi[pair][G] = c1(G) + i c2(G), Phi[pair][-G] = conj(c1(G)) + i conj(c2(G)); band 2*pair+1 missing -> zero
+__global__ void k_gamma_merge(const double2* __restrict__ psi, long long ldpsi, int nb, const int* __restrict__ idx_plus,
+                              const int* __restrict__ idx_minus, int ngw, double2* __restrict__ phi, long long ldf) {
+  const int ig = blockIdx.x * blockDim.x + threadIdx.x;
+  const int pr = blockIdx.y;
+  if (ig >= ngw) return;
+  const int b1 = 2 * pr, b2 = 2 * pr + 1;
+  const double2 c1 = psi[(size_t)b1 * ldpsi + ig];
+  const double2 c2 = b2 < nb ? psi[(size_t)b2 * ldpsi + ig] : make_double2(0.0, 0.0);
+  double2* row = phi + (size_t)pr * ldf;
+  const int ip = idx_plus[ig], im = idx_minus[ig];
+  if (im != ip) row[im] = make_double2(c1.x + c2.y, c2.x - c1.y);  // conj(c1) + i conj(c2)
+  row[ip] = make_double2(c1.x - c2.y, c1.y + c2.x);                // c1 + i c2
+}
+// h1(G) = (X + conj(Y))/2, h2(G) = (X - conj(Y))/(2i) with X = Phi'(G), Y = Phi'(-G)
+__global__ void k_gamma_split(const double2* __restrict__ hphi, long long ldf, const int* __restrict__ idx_plus,
+                              const int* __restrict__ idx_minus, int ngw, double2* __restrict__ hpsi, long long ldh, int nb) {
+  const int ig = blockIdx.x * blockDim.x + threadIdx.x;
+  const int pr = blockIdx.y;
+  if (ig >= ngw) return;
+  const double2* row = hphi + (size_t)pr * ldf;
+  const double2 x = row[idx_plus[ig]], y = row[idx_minus[ig]];
+  const int b1 = 2 * pr, b2 = 2 * pr + 1;
+  hpsi[(size_t)b1 * ldh + ig] = make_double2(0.5 * (x.x + y.x), 0.5 * (x.y - y.y));
+  if (b2 < nb) hpsi[(size_t)b2 * ldh + ig] = make_double2(0.5 * (x.y + y.y), 0.5 * (y.x - x.x));
+}
+
+}  // namespace
+
+extern "C" int qe_hpsi_gamma_gsphere(const double at[9], double ecutwfc, const int nr[3], int64_t* ngw,
+                                     int32_t* miller_host) {
+  if (!ngw) return QE_HPSI_EINVAL;
+  const double xk[3] = {0.0, 0.0, 0.0};
+  int64_t npw = 0;
+  int rc = qe_hpsi_gsphere(at, xk, ecutwfc, nr, &npw, nullptr);
+  if (rc) return rc;
+  std::vector<int32_t> mil((size_t)std::max<int64_t>(npw, 1) * 3);
+  rc = qe_hpsi_gsphere(at, xk, ecutwfc, nr, &npw, mil.data());
+  if (rc) return rc;
+  int64_t n = 0;
+  for (int64_t i = 0; i < npw; ++i)
+    if (gamma_keep(&mil[3 * i])) {
+      if (miller_host) {
+        miller_host[3 * n] = mil[3 * i];
+        miller_host[3 * n + 1] = mil[3 * i + 1];
+        miller_host[3 * n + 2] = mil[3 * i + 2];
+      }
+      ++n;
+    }
+  *ngw = n;
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_gamma_destroy(qe_hpsi_gamma_t g) {
+  if (!g) return QE_HPSI_OK;
+  qe_hpsi_destroy(g->loc);
+  qe_hpsi_destroy(g->nl);
+  cudaFree(g->idx_plus);
+  cudaFree(g->idx_minus);
+  cudaFree(g->phi);
+  cudaFree(g->hphi);
+  delete g;
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], double ecutwfc, const int nr[3],
+                                    const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                                    const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
+                                    void* cuda_stream) {
+  if (!out) return QE_HPSI_EINVAL;
+  *out = nullptr;
+  if (!vr_dev || nproj < 0 || max_batch < 1) return QE_HPSI_EINVAL;
+  long long d_total = 0;
+  if (nproj > 0) {
+    if (!beta_dev || !blk_off_host || !d_host || nblocks < 1) return QE_HPSI_EINVAL;
+    if (blk_off_host[0] != 0 || blk_off_host[nblocks] != nproj) return QE_HPSI_EINVAL;
+    for (int a = 0; a < nblocks; ++a) {
+      const long long nh = (long long)blk_off_host[a + 1] - blk_off_host[a];
+      if (nh <= 0) return QE_HPSI_EINVAL;
+      d_total += nh * nh;
+    }
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  qe_hpsi_gamma_handle* g = new (std::nothrow) qe_hpsi_gamma_handle();
+  if (!g) return QE_HPSI_ENOMEM;
+  g->max_batch = max_batch;
+  g->pairs = (max_batch + 1) / 2;
+  const double xk[3] = {0.0, 0.0, 0.0};
+  int rc = qe_hpsi_create(&g->loc, at, ecutwfc, xk, nr, vr_dev, 0, nullptr, 0, 0, nullptr, nullptr, g->pairs,
+                          flags & QE_HPSI_GENERIC_FFT, cuda_stream);
+  if (rc) {
+    delete g;
+    return rc;
+  }
+  g->npw = g->loc->npw;
+#define CG_TRY(expr)                                                           \
+  do {                                                                         \
+    cudaError_t e__ = (expr);                                                  \
+    if (e__ != cudaSuccess) {                                                  \
+      g_last_cuda = (int)e__;                                                  \
+      qe_hpsi_gamma_destroy(g);                                                \
+      return e__ == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA; \
+    }                                                                          \
+  } while (0)
+  // half-sphere maps from the device-built full sphere (host side: integer work, once per handle)
+  std::vector<int> mil((size_t)std::max(g->npw, 1) * 3), fidx((size_t)std::max(g->npw, 1));
+  if (g->npw) {
+    CG_TRY(cudaMemcpy(mil.data(), g->loc->miller, sizeof(int) * 3 * (size_t)g->npw, cudaMemcpyDeviceToHost));
+    CG_TRY(cudaMemcpy(fidx.data(), g->loc->fftidx, sizeof(int) * (size_t)g->npw, cudaMemcpyDeviceToHost));
+  }
+  std::vector<int> ip, im;
+  for (int i = 0; i < g->npw; ++i) {
+    if (!gamma_keep(&mil[3 * (size_t)i])) continue;
+    // position of -G: wrapped linear index of the negated triple, binary search in the ascending fft_index
+    long long lin = 0;
+    for (int j = 0; j < 3; ++j) {
+      const int n = -mil[3 * (size_t)i + j];
+      lin = lin * nr[j] + ((n % nr[j]) + nr[j]) % nr[j];
+    }
+    auto it = std::lower_bound(fidx.begin(), fidx.begin() + g->npw, (int)lin);
+    if (it == fidx.begin() + g->npw || *it != (int)lin) {  // cannot happen for a k = 0 sphere
+      qe_hpsi_gamma_destroy(g);
+      return QE_HPSI_ESTATE;
+    }
+    ip.push_back(i);
+    im.push_back((int)(it - fidx.begin()));
+  }
+  g->ngw = (int)ip.size();
+  if (nproj > 0 && ldbeta < g->ngw) {
+    qe_hpsi_gamma_destroy(g);
+    return QE_HPSI_EINVAL;
+  }
+  CG_TRY(upload(&g->idx_plus, ip, st));
+  CG_TRY(upload(&g->idx_minus, im, st));
+  g->ldf = ((long long)g->npw + 7) / 8 * 8;
+  const size_t fb = sizeof(double2) * (size_t)g->pairs * (size_t)std::max<long long>(g->ldf, 1);
+  CG_TRY(cudaMalloc(&g->phi, fb));
+  CG_TRY(cudaMalloc(&g->hphi, fb));
+  CG_TRY(cudaMemsetAsync(g->phi, 0, fb, st));
+  CG_TRY(cudaMemsetAsync(g->hphi, 0, fb, st));
+  if (nproj > 0 && g->ngw > 0) {
+    g->nl = new (std::nothrow) qe_hpsi_handle();
+    if (!g->nl) {
+      qe_hpsi_gamma_destroy(g);
+      return QE_HPSI_ENOMEM;
+    }
+    g->nl->device = g->loc->device;
+    g->nl->num_sms = g->loc->num_sms;
+    g->nl->npw = g->ngw;
+    g->nl->nproj = nproj;
+    g->nl->max_batch = max_batch;
+    g->nl->gamma = true;
+    CG_TRY(set_kernel_attrs());
+    CG_TRY(setup_nonlocal(g->nl, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
+  }
+  CG_TRY(cudaStreamSynchronize(st));
+#undef CG_TRY
+  *out = g;
+  return QE_HPSI_OK;
+}
+
+extern "C" int64_t qe_hpsi_gamma_ngw(qe_hpsi_gamma_t g) { return g ? g->ngw : (int64_t)QE_HPSI_ESTATE; }
+
+extern "C" int qe_hpsi_gamma_apply(qe_hpsi_gamma_t g, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
+                                   int nbands, void* cuda_stream) {
+  if (!g) return QE_HPSI_ESTATE;
+  if (nbands < 0) return QE_HPSI_EINVAL;
+  if (nbands == 0 || g->ngw == 0) return QE_HPSI_OK;
+  if (!psi_dev || !hpsi_dev || ldpsi < g->ngw || ldhpsi < g->ngw) return QE_HPSI_EINVAL;
+  {
+    const char* a0 = static_cast<const char*>(psi_dev);
+    const char* a1 = a0 + ((size_t)(nbands - 1) * ldpsi + g->ngw) * sizeof(double2);
+    const char* b0 = static_cast<const char*>(hpsi_dev);
+    const char* b1 = b0 + ((size_t)(nbands - 1) * ldhpsi + g->ngw) * sizeof(double2);
+    if (a0 < b1 && b0 < a1) return QE_HPSI_EINVAL;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const double2* psi = static_cast<const double2*>(psi_dev);
+  double2* hpsi = static_cast<double2*>(hpsi_dev);
+  qe_hpsi_handle* h = g->loc;
+  for (int b0 = 0; b0 < nbands; b0 += g->max_batch) {
+    const int nb = std::min(g->max_batch, nbands - b0);
+    const int pairs = (nb + 1) / 2;
+    const double2* p = psi + (size_t)b0 * ldpsi;
+    double2* o = hpsi + (size_t)b0 * ldhpsi;
+    if (g->nl) {
+      const int rc = launch_becp(g->nl, p, ldpsi, nb, st);  // real becp over the half sphere, dbecp = D becp
+      if (rc) return rc;
+    }
+    const dim3 grid((g->ngw + 255) / 256, pairs);
+    k_gamma_merge<<<grid, 256, 0, st>>>(p, ldpsi, nb, g->idx_plus, g->idx_minus, g->ngw, g->phi, g->ldf);
+    int rc = launch_local(h, g->phi, g->ldf, g->hphi, g->ldf, pairs, st);  // a1-a5 on pairs of bands, kinetic included
+    if (rc) return rc;
+    k_gamma_split<<<grid, 256, 0, st>>>(g->hphi, g->ldf, g->idx_plus, g->idx_minus, g->ngw, o, ldhpsi, nb);
+    if (g->nl) {
+      rc = launch_vnl_add(g->nl, g->nl->dbT, o, ldhpsi, nb, st);
+      if (rc) return rc;
     }
   }
   CU_TRY(h, cudaGetLastError());

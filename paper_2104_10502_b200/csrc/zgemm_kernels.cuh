@@ -77,9 +77,26 @@ __device__ __forceinline__ void mma3m(double (&P)[TM][TN][2], double (&Q)[TM][TN
     for (int j = 0; j < TN; ++j) dmma884(R[i][j][0], R[i][j][1], as[i], bs[j]);
 }
 
+// Gamma-only variants (NEXT-1: real wavefunctions, c(-G) = conj c(G), half sphere).  A complex element is read as
+// two consecutive reals, so the contraction over the 2*ngw real components needs two real DMMAs per block:
+//   becp (real)  : sum_k (ar*br + ai*bi)            -> P += ar*br, Q += ai*bi, result P + Q
+//   vnl_add      : out.re += sum_p ar*d, out.im += sum_p ai*d with real d = B.re -> P += ar*br, Q += ai*br
+template <int TM, int TN, bool B_IMAG>
+__device__ __forceinline__ void mma2r(double (&P)[TM][TN][2], double (&Q)[TM][TN][2], const double2 (&af)[TM],
+                                      const double2 (&bf)[TN]) {
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) dmma884(P[i][j][0], P[i][j][1], af[i].x, bf[j].x);
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) dmma884(Q[i][j][0], Q[i][j][1], af[i].y, B_IMAG ? bf[j].y : bf[j].x);
+}
+
 // a6 ------------------------------------------------------------------------------------------------------
 // C[p][b] = sum_k conj(A[p][k]) B[b][k] over k in [ks*kchunk, min(npw,(ks+1)*kchunk)); A = beta, B = psi.
-template <class Cfg>
+template <class Cfg, bool GAMMA = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_becp(const double2* __restrict__ beta, long long ldb, int nproj, const double2* __restrict__ psi, long long ldpsi,
            int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc) {
@@ -171,7 +188,10 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
-      mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
+      if constexpr (GAMMA)
+        mma2r<TM, TN, true>(P, Q, af[kk & 1], bf[kk & 1]);
+      else
+        mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
       if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
         if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
         cp_async_commit();
@@ -192,7 +212,9 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int b = n0 + wn0 + j * 8 + 2 * fk + e;
-        if (b < nb) out[(size_t)p * ldc + b] = make_double2(P[i][j][e] + Q[i][j][e], (R[i][j][e] - P[i][j][e]) + Q[i][j][e]);
+        if (b < nb)
+          out[(size_t)p * ldc + b] = GAMMA ? make_double2(P[i][j][e] + Q[i][j][e], 0.0)
+                                           : make_double2(P[i][j][e] + Q[i][j][e], (R[i][j][e] - P[i][j][e]) + Q[i][j][e]);
       }
     }
   }
@@ -212,6 +234,19 @@ __global__ void k_becp_reduce(const double2* __restrict__ partial, int nsplit, i
     im += v.y;
   }
   becp[(size_t)p * ldc + b] = make_double2(re, im);
+}
+// Gamma-only a7: becp[p][b] = 2 * sum_ks partial[ks][p][b].re - beta[p][0].re * psi[b][0].re  (the G = 0 term of the
+// half sphere must count once, not twice; real result stored as (re, 0))
+__global__ void k_becp_reduce_gamma(const double2* __restrict__ partial, int nsplit, int nproj, int ldc, int nb,
+                                    const double2* __restrict__ beta, long long ldb, const double2* __restrict__ psi,
+                                    long long ldpsi, double2* __restrict__ becp) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (b >= nb) return;
+  double re = 0.0;
+  for (int ks = 0; ks < nsplit; ++ks) re += partial[((size_t)ks * nproj + p) * ldc + b].x;
+  const double2 b0 = beta[(size_t)p * ldb], c0 = psi[(size_t)b * ldpsi];
+  becp[(size_t)p * ldc + b] = make_double2(2.0 * re - (b0.x * c0.x + b0.y * c0.y), 0.0);
 }
 // NEXT-3 (reduced matrices <a_i|b_j>): out[i][j] = sum_ks partial[ks][i][j], ks ascending, with its own row stride
 __global__ void k_ovl_reduce(const double2* __restrict__ partial, int nsplit, int na, int ldc, int nb,
@@ -249,7 +284,7 @@ __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int
 
 // a8 ------------------------------------------------------------------------------------------------------
 // hpsi[b][g] += sum_p A[p][g] B[b][p];  A = beta ([p][g], g contiguous: "M-major"), B = dbT ([b][p], p contiguous)
-template <class Cfg>
+template <class Cfg, bool GAMMA = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_add(const double2* __restrict__ beta, long long ldb, int nproj, int npw, const double2* __restrict__ dbT,
               int ldp, int nb, double2* __restrict__ hpsi, long long ldh) {
@@ -338,7 +373,10 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
-      mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
+      if constexpr (GAMMA)
+        mma2r<TM, TN, false>(P, Q, af[kk & 1], bf[kk & 1]);
+      else
+        mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
       if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
         if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
         cp_async_commit();
@@ -361,8 +399,13 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         if (b < nb) {
           double2* h = &hpsi[(size_t)b * ldh + gg];
           double2 v = *h;
-          v.x += P[i][j][e] - Q[i][j][e];
-          v.y += (R[i][j][e] - P[i][j][e]) - Q[i][j][e];
+          if constexpr (GAMMA) {
+            v.x += P[i][j][e];
+            v.y += Q[i][j][e];
+          } else {
+            v.x += P[i][j][e] - Q[i][j][e];
+            v.y += (R[i][j][e] - P[i][j][e]) - Q[i][j][e];
+          }
           *h = v;
         }
       }

@@ -51,6 +51,12 @@ SIGNATURES = {
     "qe_hpsi_apply_hs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i64, _i32, _vp]),
     "qe_hpsi_overlap": (_i32, [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _vp, _i64, _vp]),
     "qe_hpsi_density": (_i32, [_vp, _vp, _i64, _i32, _vp, _dbl, _vp, _vp]),
+    "qe_hpsi_gamma_gsphere": (_i32, [_pd, _dbl, _pi32, _pi64, _pi32]),
+    "qe_hpsi_gamma_create": (_i32, [_c.POINTER(_vp), _pd, _dbl, _pi32, _vp, _i32, _vp, _i64, _i32, _pi32, _pd, _i32,
+                                    _c.c_uint, _vp]),
+    "qe_hpsi_gamma_apply": (_i32, [_vp, _vp, _i64, _vp, _i64, _i32, _vp]),
+    "qe_hpsi_gamma_ngw": (_i64, [_vp]),
+    "qe_hpsi_gamma_destroy": (_i32, [_vp]),
 }
 
 _lib = None
@@ -285,6 +291,68 @@ class Hpsi:
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value is not None:
             self._lib.qe_hpsi_destroy(self._h)
+            self._h = _vp(None)
+        self._keep = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def qe_hpsi_gamma_gsphere(at, ecutwfc, nr) -> np.ndarray:
+    """Half sphere of the k = 0 sphere (NEXT-1): int32 [ngw, 3] Miller triples in canonical order, G = 0 first."""
+    lib = load_library()
+    _a, pa = _darr(at, 9)
+    _n, pn = _iarr(nr, 3)
+    n = _c.c_int64(0)
+    _check(lib.qe_hpsi_gamma_gsphere(pa, float(ecutwfc), pn, _c.byref(n), None))
+    mil = np.zeros((max(n.value, 1), 3), dtype=np.int32)
+    _check(lib.qe_hpsi_gamma_gsphere(pa, float(ecutwfc), pn, _c.byref(n), mil.ctypes.data_as(_pi32)))
+    return mil[:n.value]
+
+
+class HpsiGamma:
+    """Gamma-only handle (k = 0, real wavefunctions on the half sphere). See include/qe_hpsi.h, NEXT-1."""
+
+    def __init__(self, at, ecutwfc, nr, vr: torch.Tensor, beta: torch.Tensor | None = None, blk_off=None, dblocks=None,
+                 max_batch: int = 128, flags: int = 0, stream=None):
+        lib = load_library()
+        self._lib = lib
+        self._h = _vp(None)
+        assert vr.is_cuda and vr.dtype == torch.float64 and vr.is_contiguous()
+        _a, pa = _darr(at, 9)
+        _n, pn = _iarr(nr, 3)
+        nproj = 0 if beta is None else int(beta.shape[0])
+        if nproj:
+            assert beta.is_cuda and beta.dtype == torch.complex128 and beta.stride(1) == 1
+            ldbeta = int(beta.stride(0)) if beta.shape[0] > 1 else int(beta.shape[1])
+            blk = np.ascontiguousarray(np.asarray(blk_off, dtype=np.int32))
+            dpk = np.ascontiguousarray(np.concatenate([np.asarray(d, dtype=np.float64).reshape(-1) for d in dblocks]))
+            pb, nblocks, pdk, bptr = blk.ctypes.data_as(_pi32), blk.size - 1, dpk.ctypes.data_as(_pd), _vp(beta.data_ptr())
+        else:
+            ldbeta, pb, nblocks, pdk, bptr = 0, None, 0, None, _vp(None)
+        self._keep = (vr, beta) if (flags & QE_HPSI_BORROW_BETA) else None
+        _check(lib.qe_hpsi_gamma_create(_c.byref(self._h), pa, float(ecutwfc), pn, _vp(vr.data_ptr()), nproj, bptr, ldbeta,
+                                        nblocks, pb, pdk, int(max_batch), int(flags), _stream_ptr(stream)))
+        self.ngw = int(lib.qe_hpsi_gamma_ngw(self._h))
+        self.nproj = nproj
+
+    def apply(self, psi, hpsi=None, stream=None):
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.dim() == 2 and psi.stride(1) == 1
+        nb = int(psi.shape[0])
+        if hpsi is None:
+            hpsi = torch.zeros_like(psi)
+        ldp = int(psi.stride(0)) if nb > 1 else int(psi.shape[1])
+        ldh = int(hpsi.stride(0)) if nb > 1 else int(hpsi.shape[1])
+        _check(self._lib.qe_hpsi_gamma_apply(self._h, _vp(psi.data_ptr()), ldp, _vp(hpsi.data_ptr()), ldh, nb,
+                                             _stream_ptr(stream)))
+        return hpsi
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value is not None:
+            self._lib.qe_hpsi_gamma_destroy(self._h)
             self._h = _vp(None)
         self._keep = None
 

@@ -141,3 +141,69 @@ def test_density_full_size_properties_and_sampled_points(cfg):
         val = float((occ.cpu().numpy() * np.abs(ph @ phase) ** 2).sum())
         assert abs(rho[i[0], i[1], i[2]].item() - val) <= 1e-11 * max(val, tot)
     h.destroy()
+
+
+# ---- Gamma-only path (NEXT-1) ---------------------------------------------------------------------------------------
+def _gamma_inputs(cfg, nb):
+    """Half-sphere inputs of a real-wavefunction problem at k = 0 from the workload generators: psi and beta restricted
+    to the half sphere with real G = 0 components (the -G half is implied by Hermitian completion)."""
+    wl = inputs.get_workload(cfg)
+    assert all(x == 0.0 for x in wl.xk)
+    sp = _gpu.oracle_sphere(wl)
+    ip, im = orc.gamma_half(sp["miller"])
+    mil_h = qe_hpsi.qe_hpsi_gamma_gsphere(wl.at, wl.ecutwfc, wl.nr)
+    assert np.array_equal(mil_h, sp["miller"][ip])  # half-sphere map bit-exact
+    vr = inputs.gen_vloc(wl)
+    psi = inputs.gen_psi(wl, sp["miller"], 0, nb).numpy()[:, ip].copy()
+    psi[:, 0] = psi[:, 0].real
+    beta = db = None
+    if wl.nproj:
+        beta = inputs.gen_beta(wl, sp["miller"], inputs.gen_atoms(wl)).numpy()[:, ip].copy()
+        beta[:, 0] = beta[:, 0].real
+        db = inputs.gen_dblocks(wl)
+    return wl, sp, vr, psi, beta, db
+
+
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT])
+@pytest.mark.parametrize("cfg,nb", [("T2_radix5", 4), ("T2b_radix5_20", 3), ("T3_aliased", 4), ("T4_noproj", 3), (0, 7), (0, 16)])
+def test_gamma_apply_against_oracle(cfg, nb, flags):
+    wl, sp, vr, psi, beta, db = _gamma_inputs(cfg, nb)
+    ngw = psi.shape[1]
+    ld = inputs.pad8(ngw)
+    blk = np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh if wl.nproj else None
+    bdev = None
+    if wl.nproj:
+        bdev = torch.zeros((wl.nproj, ld), dtype=torch.complex128, device="cuda")
+        bdev[:, :ngw] = torch.from_numpy(beta).cuda()
+    g = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), bdev, blk, db, max_batch=5, flags=flags)
+    assert g.ngw == ngw
+    pdev = torch.zeros((nb, ld), dtype=torch.complex128, device="cuda")
+    pdev[:, :ngw] = torch.from_numpy(psi).cuda()
+    out = torch.full_like(pdev, 7.0)
+    g.apply(pdev, out)
+    torch.cuda.synchronize()
+    ref = orc.hpsi_gamma(sp["miller"], sp["fft_index"], sp["g2kin"], tuple(wl.nr), vr.numpy(), psi, beta, db)
+    got = out.cpu().numpy()
+    assert _gpu.rel_l2(got[:, :ngw], ref).max() <= TOL
+    assert np.all(got[:, ngw:] == 7.0)
+    g.destroy()
+
+
+def test_gamma_matches_the_full_sphere_path_on_config_1():
+    """Full size (config 1, 64 atoms, 80^3): the Gamma path on the half sphere against the complex full-sphere library path
+    AND the oracle on sampled bands, same real-wavefunction problem."""
+    nb = 12
+    wl, sp, vr, psi, beta, db = _gamma_inputs(1, nb)
+    ip, im = orc.gamma_half(sp["miller"])
+    npw, ngw = sp["miller"].shape[0], psi.shape[1]
+    blk = np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh
+    g = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), torch.from_numpy(beta).cuda(), blk, db, max_batch=8)
+    got = g.apply(torch.from_numpy(psi).cuda()).cpu().numpy()
+    ref = orc.hpsi_gamma(sp["miller"], sp["fft_index"], sp["g2kin"], tuple(wl.nr), vr.numpy(), psi[:3], beta, db)
+    assert _gpu.rel_l2(got[:3], ref).max() <= TOL
+    full = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr.cuda(), torch.from_numpy(orc.gamma_expand(beta, ip, im, npw)).cuda(),
+                        blk, db, max_batch=nb)
+    hf = full.apply(torch.from_numpy(orc.gamma_expand(psi, ip, im, npw)).cuda()).cpu().numpy()
+    assert _gpu.rel_l2(got, hf[:, ip]).max() <= TOL
+    g.destroy()
+    full.destroy()
