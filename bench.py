@@ -206,6 +206,33 @@ def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
     by = nb * 16.0 * (npw + 2 * info["S"] * n3 + 2 * info["P"] * n2 * n3) + 16.0 * n1 * n2 * n3 * -(-nb // info["fft_nb"])
     out["density"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "algorithmic_gbs": by / ms * 1e-6, "bound": "hbm",
                       "frac": by / ms * 1e-6 / hbm_peak}
+    # NEXT-1: the same chunk as a real-wavefunction problem on the half sphere (k = 0 configs only)
+    if all(x == 0.0 for x in wl.xk):
+        from paper_2104_10502_b200 import inputs, qe_hpsi
+        mil_h = qe_hpsi.qe_hpsi_gamma_gsphere(wl.at, wl.ecutwfc, wl.nr)
+        ngw = mil_h.shape[0]
+        ldg = inputs.pad8(ngw)
+        mh = torch.as_tensor(mil_h, device="cuda")
+        bh = None
+        blk = db = None
+        if wl.nproj:
+            bh = torch.zeros((wl.nproj, ldg), dtype=torch.complex128, device="cuda")
+            for a0 in range(0, wl.natoms, 16):
+                na = min(16, wl.natoms - a0)
+                inputs.gen_beta(wl, mh, inp["atoms"], a0, na, ld=ldg, device="cuda", out=bh[a0 * wl.nh:(a0 + na) * wl.nh])
+            bh[:, 0] = bh[:, 0].real.to(torch.complex128)
+            blk = np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh
+            db = inp["dblocks"]
+        g = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, inp["vr"], bh, blk, db, max_batch=nb, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
+        pg = inputs.gen_psi(wl, mh, 0, nb, ld=ldg, device="cuda")
+        pg[:, 0] = pg[:, 0].real.to(torch.complex128)
+        hg = torch.empty_like(pg)
+        ms = ev_time(lambda: g.apply(pg, hg))
+        flg = 2 * 2 * 2.0 * wl.nproj * (2 * ngw) * nb / 2  # two real GEMMs over 2*ngw real components: 2*M*N*K each
+        out["gamma_apply"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "ngw": ngw, "real_proj_tflops": flg / ms * 1e-9,
+                              "speedup_vs_complex_path": None}
+        g.destroy()
+        del bh, pg, hg
     return out
 
 
@@ -386,6 +413,8 @@ def main():
             "stages": stages, "cpu_baseline": cpu, "setup_s": t_setup}
     if args.next:
         line["next_rows"] = time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak)
+        if "gamma_apply" in line["next_rows"]:
+            line["next_rows"]["gamma_apply"]["speedup_vs_complex_path"] = line["next_rows"]["gamma_apply"]["bands_per_s"] / (value / world)
     print(json.dumps(line), flush=True)
 
     if args.detail:
