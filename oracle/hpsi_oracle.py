@@ -341,3 +341,48 @@ def hpsi_gamma(miller, fft_index, g2kin, nr, vr, psi_half, beta_half=None, dbloc
     psi = gamma_expand(psi_half, ip, im, npw)
     beta = gamma_expand(beta_half, ip, im, npw) if beta_half is not None and beta_half.shape[0] else None
     return hpsi_dual(fft_index, g2kin, nr, vr, psi, beta, dblocks)[:, ip]
+
+
+# ----------------------------------------------------------------------------------------------------------
+# NEXT-3, the rest of the Davidson step around H|psi> ("iterative diagonalization", L168 "RCI"):
+# diagonal of H and S for the preconditioner, the preconditioner itself, and the basis rotation.
+# ----------------------------------------------------------------------------------------------------------
+
+
+def hdiag_of(g2kin, vbar, beta=None, dblocks=None):
+    """diag(H)(G) = |k+G|^2 + vbar + sum_a sum_i D^a_ii |beta_ai(G)|^2 with vbar = mean of V(r) (= Vt[0], the diagonal
+    of the local term)."""
+    out = np.asarray(g2kin, dtype=np.float64) + float(vbar)
+    if beta is not None and beta.shape[0]:
+        nat, nh, _ = dblocks.shape
+        dii = np.stack([np.diag(dblocks[a]) for a in range(nat)]).reshape(-1)  # [nproj]
+        out = out + dii @ (beta.real**2 + beta.imag**2)
+    return out
+
+
+def sdiag_of(npw, beta=None, qblocks=None):
+    """diag(S)(G) = 1 + sum_a sum_i q^a_ii |beta_ai(G)|^2."""
+    return hdiag_of(np.ones(npw), 0.0, beta, qblocks)
+
+
+def precond_of(r, e, hdiag, sdiag):
+    """Davidson preconditioner (the smooth form used by plane-wave codes): x = hdiag(G) - e_b sdiag(G),
+    r_b(G) / ( (1 + x + sqrt(1 + (x-1)^2)) / 2 ).  r [nb,npw], e [nb]."""
+    x = hdiag[None, :] - np.asarray(e)[:, None] * sdiag[None, :]
+    return r / (0.5 * (1.0 + x + np.sqrt(1.0 + (x - 1.0) ** 2)))
+
+
+def rotate_of(x, coef):
+    """Basis rotation y[k][G] = sum_j coef[k][j] x[j][G].  x [nx,npw], coef [ny,nx] -> [ny,npw]."""
+    return coef @ x
+
+
+def dense_s(beta, qblocks, npw):
+    """S[G,G'] = delta + sum_a beta_a(G) q^a beta_a(G')^H (tiny cases)."""
+    s = np.eye(npw, dtype=np.complex128)
+    if beta is not None and beta.shape[0]:
+        nat, nh, _ = qblocks.shape
+        for a in range(nat):
+            ba = beta[a * nh:(a + 1) * nh]
+            s += ba.T @ (qblocks[a] @ np.conj(ba))
+    return s

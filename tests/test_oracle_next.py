@@ -209,3 +209,40 @@ def test_gamma_single_plane_wave_pair_in_constant_potential():
     ref = np.zeros_like(psi_h)
     ref[0, g] = (pr["g2kin"][ip[g]] + v0) * psi_h[0, g]
     np.testing.assert_allclose(got, ref, atol=1e-13)
+
+
+# ---- Davidson pieces (NEXT-3) -----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5"])
+def test_hdiag_and_sdiag_are_the_diagonals_of_the_dense_operators(cfg):
+    pr = problem(cfg)
+    npw = pr["miller"].shape[0]
+    hd = orc.dense_h(pr["miller"], pr["g2kin"], pr["nr"], pr["vr"], pr["beta"], pr["dblocks"])
+    got = orc.hdiag_of(pr["g2kin"], pr["vr"].mean(), pr["beta"], pr["dblocks"])
+    np.testing.assert_allclose(got, np.diag(hd).real, atol=1e-12 * np.abs(got).max())
+    rng = np.random.default_rng(4)
+    q = rng.uniform(-0.2, 0.2, pr["dblocks"].shape)
+    q = 0.5 * (q + q.transpose(0, 2, 1))
+    sd = orc.dense_s(pr["beta"], q, npw)
+    np.testing.assert_allclose(orc.sdiag_of(npw, pr["beta"], q), np.diag(sd).real, atol=1e-13)
+    # dense S applied to psi is spsi_of
+    np.testing.assert_allclose((sd @ pr["psi"].T).T, orc.spsi_of(pr["beta"], q, pr["psi"]), atol=1e-12)
+
+
+def test_precond_and_rotate_against_python_loops():
+    rng = np.random.default_rng(9)
+    r = rng.standard_normal((2, 11)) + 1j * rng.standard_normal((2, 11))
+    hd, sd, e = rng.uniform(0, 30, 11), rng.uniform(0.8, 1.3, 11), np.array([-0.4, 2.5])
+    got = orc.precond_of(r, e, hd, sd)
+    for b in range(2):
+        for g in range(11):
+            x = hd[g] - e[b] * sd[g]
+            assert abs(got[b, g] - r[b, g] / (0.5 * (1 + x + math.sqrt(1 + (x - 1) ** 2)))) < 1e-14
+    # limits: x = 1 -> 3/2; x >> 1 -> x
+    assert abs(orc.precond_of(np.ones((1, 1)), [0.0], np.array([1.0]), np.array([1.0]))[0, 0] - 1 / 1.5) < 1e-15
+    assert abs(orc.precond_of(np.ones((1, 1)), [0.0], np.array([1e8]), np.array([1.0]))[0, 0] * 1e8 - 1) < 1e-7
+    x = rng.standard_normal((3, 7)) + 1j * rng.standard_normal((3, 7))
+    c = rng.standard_normal((2, 3)) + 1j * rng.standard_normal((2, 3))
+    y = orc.rotate_of(x, c)
+    for k in range(2):
+        for g in range(7):
+            assert abs(y[k, g] - sum(c[k, j] * x[j, g] for j in range(3))) < 1e-14
