@@ -350,8 +350,9 @@ def hpsi_gamma(miller, fft_index, g2kin, nr, vr, psi_half, beta_half=None, dbloc
 
 
 def hdiag_of(g2kin, vbar, beta=None, dblocks=None):
-    """diag(H)(G) = |k+G|^2 + vbar + sum_a sum_i D^a_ii |beta_ai(G)|^2 with vbar = mean of V(r) (= Vt[0], the diagonal
-    of the local term)."""
+    """Preconditioner diagonal h_diag(G) = |k+G|^2 + vbar + sum_a sum_i D^a_ii |beta_ai(G)|^2 with vbar = mean of V(r)
+    (= Vt[0], the diagonal of the local term).  Only the i = j terms of D enter (the usual plane-wave-code choice):
+    it is the exact diagonal of H when every D^a is diagonal, and of H with D replaced by diag(D) otherwise."""
     out = np.asarray(g2kin, dtype=np.float64) + float(vbar)
     if beta is not None and beta.shape[0]:
         nat, nh, _ = dblocks.shape
@@ -361,7 +362,7 @@ def hdiag_of(g2kin, vbar, beta=None, dblocks=None):
 
 
 def sdiag_of(npw, beta=None, qblocks=None):
-    """diag(S)(G) = 1 + sum_a sum_i q^a_ii |beta_ai(G)|^2."""
+    """s_diag(G) = 1 + sum_a sum_i q^a_ii |beta_ai(G)|^2 (same convention as hdiag_of)."""
     return hdiag_of(np.ones(npw), 0.0, beta, qblocks)
 
 

@@ -216,14 +216,16 @@ def test_gamma_single_plane_wave_pair_in_constant_potential():
 def test_hdiag_and_sdiag_are_the_diagonals_of_the_dense_operators(cfg):
     pr = problem(cfg)
     npw = pr["miller"].shape[0]
-    hd = orc.dense_h(pr["miller"], pr["g2kin"], pr["nr"], pr["vr"], pr["beta"], pr["dblocks"])
+    ddiag = np.stack([np.diag(np.diag(d)) for d in pr["dblocks"]])  # D with its off-diagonal entries dropped
+    hd = orc.dense_h(pr["miller"], pr["g2kin"], pr["nr"], pr["vr"], pr["beta"], ddiag)
     got = orc.hdiag_of(pr["g2kin"], pr["vr"].mean(), pr["beta"], pr["dblocks"])
     np.testing.assert_allclose(got, np.diag(hd).real, atol=1e-12 * np.abs(got).max())
     rng = np.random.default_rng(4)
     q = rng.uniform(-0.2, 0.2, pr["dblocks"].shape)
     q = 0.5 * (q + q.transpose(0, 2, 1))
     sd = orc.dense_s(pr["beta"], q, npw)
-    np.testing.assert_allclose(orc.sdiag_of(npw, pr["beta"], q), np.diag(sd).real, atol=1e-13)
+    qdiag = np.stack([np.diag(np.diag(x)) for x in q])
+    np.testing.assert_allclose(orc.sdiag_of(npw, pr["beta"], q), np.diag(orc.dense_s(pr["beta"], qdiag, npw)).real, atol=1e-13)
     # dense S applied to psi is spsi_of
     np.testing.assert_allclose((sd @ pr["psi"].T).T, orc.spsi_of(pr["beta"], q, pr["psi"]), atol=1e-12)
 
