@@ -159,6 +159,21 @@ int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi
 int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb,
                     void* out_dev, int64_t ldo, void* cuda_stream);
 
+/* NEXT-3, the rest of the Davidson step:
+ * qe_hpsi_hdiag:   hdiag[G] = |k+G|^2 + vbar + sum_p D_pp |beta_p(G)|^2  (vbar = mean of V(r), supplied by the caller)
+ *                  sdiag[G] = 1 + sum_p q_pp |beta_p(G)|^2              (needs qe_hpsi_set_s when there are projectors)
+ *                  either output may be NULL; DEVICE arrays of npw doubles.
+ * qe_hpsi_precond: r[b][G] /= (1 + x + sqrt(1 + (x-1)^2)) / 2, x = hdiag[G] - e[b] sdiag[G]; e_dev [nb] on the device,
+ *                  sdiag_dev NULL means 1.
+ * qe_hpsi_rotate:  y[k][G] (+)= sum_j coef[k][j] x[j][G], k < ny, j < nx, over the npw sphere entries; coef_dev complex128
+ *                  [ny][ldcoef], ldcoef >= nx; accumulate = 0 overwrites y[k][0..npw).  Runs the DMMA kernel of step a8.
+ * All asynchronous on cuda_stream. */
+int qe_hpsi_hdiag(qe_hpsi_t h, double vbar, double* hdiag_dev, double* sdiag_dev, void* cuda_stream);
+int qe_hpsi_precond(qe_hpsi_t h, void* r_dev, int64_t ldr, int nb, const double* e_dev, const double* hdiag_dev,
+                    const double* sdiag_dev, void* cuda_stream);
+int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int nx, const void* coef_dev, int64_t ldcoef, void* y_dev,
+                   int64_t ldy, int ny, int accumulate, void* cuda_stream);
+
 /* NEXT-4, charge density ("charge density generation"):
  *   rho[i1][i2][i3] += scale * sum_b occ[b] |psi_b(r_i)|^2,  psi_b(r_i) = sum_G psi[b][G] exp(+2 pi i n.i/N)
  * using steps a1-a2 of the hot path and the inverse half of a3.  rho_dev is a dense [N1][N2][N3] FP64 DEVICE array

@@ -1243,6 +1243,60 @@ extern "C" int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int 
   return QE_HPSI_OK;
 }
 
+// NEXT-3, rest of the Davidson step: preconditioner diagonals, preconditioner, basis rotation (a8's kernel)
+extern "C" int qe_hpsi_hdiag(qe_hpsi_t h, double vbar, double* hdiag_dev, double* sdiag_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!hdiag_dev && !sdiag_dev) return QE_HPSI_EINVAL;
+  if (h->npw == 0) return QE_HPSI_OK;
+  if (sdiag_dev && h->nproj > 0 && !h->qpk) return QE_HPSI_ESTATE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const unsigned nblk = (unsigned)((h->npw + 127) / 128);
+  if (hdiag_dev)
+    k_proj_diag<<<nblk, 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->proj_doff, h->proj_blk0, h->proj_nh, h->dpk,
+                                      h->g2kin, vbar, hdiag_dev);
+  if (sdiag_dev)
+    k_proj_diag<<<nblk, 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->proj_doff, h->proj_blk0, h->proj_nh, h->qpk,
+                                      nullptr, 0.0, sdiag_dev);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_precond(qe_hpsi_t h, void* r_dev, int64_t ldr, int nb, const double* e_dev, const double* hdiag_dev,
+                               const double* sdiag_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nb < 0) return QE_HPSI_EINVAL;
+  if (nb == 0 || h->npw == 0) return QE_HPSI_OK;
+  if (!r_dev || !e_dev || !hdiag_dev || ldr < h->npw) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  k_precond<<<dim3((h->npw + 255) / 256, nb), 256, 0, st>>>(static_cast<double2*>(r_dev), ldr, nb, h->npw, e_dev, hdiag_dev,
+                                                            sdiag_dev);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int nx, const void* coef_dev, int64_t ldcoef,
+                              void* y_dev, int64_t ldy, int ny, int accumulate, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nx < 0 || ny < 0) return QE_HPSI_EINVAL;
+  if (ny == 0 || h->npw == 0) return QE_HPSI_OK;
+  if (!y_dev || ldy < h->npw) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double2* y = static_cast<double2*>(y_dev);
+  if (!accumulate)
+    CU_TRY(h, cudaMemset2DAsync(y, sizeof(double2) * (size_t)ldy, 0, sizeof(double2) * (size_t)h->npw, (size_t)ny, st));
+  if (nx == 0) return QE_HPSI_OK;
+  if (!x_dev || !coef_dev || ldx < h->npw || ldcoef < nx) return QE_HPSI_EINVAL;
+  CU_TRY(h, set_kernel_attrs());
+  using Cfg = ZgV0;
+  const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (ny + Cfg::BN - 1) / Cfg::BN;
+  // y[k][g] += sum_j x[j][g] coef[k][j]: the a8 kernel with A = x (M-contiguous) and B = coef (K-contiguous)
+  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(static_cast<const double2*>(x_dev), ldx, nx, h->npw,
+                                                                    static_cast<const double2*>(coef_dev), (int)ldcoef, ny, y,
+                                                                    ldy);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // NEXT-4: charge density rho += scale * sum_b occ[b] |psi_b(r)|^2 from steps a1, a2 and the inverse half of a3
 // ---------------------------------------------------------------------------------------------------------

@@ -248,6 +248,33 @@ __global__ void k_becp_reduce_gamma(const double2* __restrict__ partial, int nsp
   const double2 b0 = beta[(size_t)p * ldb], c0 = psi[(size_t)b * ldpsi];
   becp[(size_t)p * ldc + b] = make_double2(2.0 * re - (b0.x * c0.x + b0.y * c0.y), 0.0);
 }
+// NEXT-3 (Davidson step): preconditioner diagonals and the preconditioner itself.
+// diag[g] = base[g] (or 1) + shift + sum_p w[p] |beta[p][g]|^2, w[p] = diagonal entry of projector p's D (or q) block
+__global__ void k_proj_diag(const double2* __restrict__ beta, long long ldb, int nproj, int npw,
+                            const long long* __restrict__ proj_doff, const int* __restrict__ proj_blk0,
+                            const int* __restrict__ proj_nh, const double* __restrict__ dpk,
+                            const double* __restrict__ base, double shift, double* __restrict__ out) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= npw) return;
+  double acc = 0.0;
+  for (int p = 0; p < nproj; ++p) {
+    const double w = __ldg(&dpk[proj_doff[p] + (p - proj_blk0[p])]);  // row (p - q0), column (p - q0) of the block
+    const double2 b = beta[(size_t)p * ldb + g];
+    acc += w * (b.x * b.x + b.y * b.y);
+  }
+  out[g] = (base ? base[g] : 1.0) + shift + acc;
+}
+// r[b][g] /= (1 + x + sqrt(1 + (x-1)^2)) / 2,  x = hdiag[g] - e[b] * sdiag[g]  (sdiag == nullptr: 1)
+__global__ void k_precond(double2* __restrict__ r, long long ldr, int nb, int npw, const double* __restrict__ e,
+                          const double* __restrict__ hdiag, const double* __restrict__ sdiag) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (g >= npw) return;
+  const double x = hdiag[g] - e[b] * (sdiag ? sdiag[g] : 1.0);
+  const double den = 0.5 * (1.0 + x + sqrt(1.0 + (x - 1.0) * (x - 1.0)));
+  double2 v = r[(size_t)b * ldr + g];
+  r[(size_t)b * ldr + g] = make_double2(v.x / den, v.y / den);
+}
 // NEXT-3 (reduced matrices <a_i|b_j>): out[i][j] = sum_ks partial[ks][i][j], ks ascending, with its own row stride
 __global__ void k_ovl_reduce(const double2* __restrict__ partial, int nsplit, int na, int ldc, int nb,
                              double2* __restrict__ out, long long ldo) {

@@ -51,6 +51,9 @@ SIGNATURES = {
     "qe_hpsi_apply_hs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i64, _i32, _vp]),
     "qe_hpsi_overlap": (_i32, [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _vp, _i64, _vp]),
     "qe_hpsi_density": (_i32, [_vp, _vp, _i64, _i32, _vp, _dbl, _vp, _vp]),
+    "qe_hpsi_hdiag": (_i32, [_vp, _dbl, _vp, _vp, _vp]),
+    "qe_hpsi_precond": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp, _vp, _vp]),
+    "qe_hpsi_rotate": (_i32, [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _i32, _vp]),
     "qe_hpsi_gamma_gsphere": (_i32, [_pd, _dbl, _pi32, _pi64, _pi32]),
     "qe_hpsi_gamma_create": (_i32, [_c.POINTER(_vp), _pd, _dbl, _pi32, _vp, _i32, _vp, _i64, _i32, _pi32, _pd, _i32,
                                     _c.c_uint, _vp]),
@@ -233,6 +236,39 @@ class Hpsi:
         _check(self._lib.qe_hpsi_overlap(self._h, _vp(a.data_ptr()), lda, na, _vp(b.data_ptr()), ldb, nb,
                                          _vp(out.data_ptr()), ldo, _stream_ptr(stream)), self._h)
         return out
+
+    def hdiag(self, vbar, want_s=False, stream=None):
+        """qe_hpsi_hdiag: (hdiag, sdiag or None) as CUDA float64 [npw] tensors."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        hd = torch.empty(self.npw, dtype=torch.float64, device=dev)
+        sd = torch.empty(self.npw, dtype=torch.float64, device=dev) if want_s else None
+        _check(self._lib.qe_hpsi_hdiag(self._h, float(vbar), _vp(hd.data_ptr()), _vp(sd.data_ptr()) if want_s else _vp(None),
+                                       _stream_ptr(stream)), self._h)
+        return hd, sd
+
+    def precond(self, r, e, hdiag, sdiag=None, stream=None):
+        """qe_hpsi_precond: in place on r [nb, ld]; e CUDA float64 [nb]."""
+        assert r.is_cuda and r.dtype == torch.complex128 and r.stride(1) == 1 and e.is_cuda and e.dtype == torch.float64
+        nb = int(r.shape[0])
+        ldr = int(r.stride(0)) if nb > 1 else int(r.shape[1])
+        _check(self._lib.qe_hpsi_precond(self._h, _vp(r.data_ptr()), ldr, nb, _vp(e.data_ptr()), _vp(hdiag.data_ptr()),
+                                         _vp(sdiag.data_ptr()) if sdiag is not None else _vp(None), _stream_ptr(stream)),
+               self._h)
+        return r
+
+    def rotate(self, x, coef, y=None, accumulate=False, stream=None):
+        """qe_hpsi_rotate: y[k] (+)= sum_j coef[k][j] x[j]; x [nx, ld], coef [ny, nx] complex128 (CUDA)."""
+        assert x.is_cuda and x.dtype == torch.complex128 and x.stride(1) == 1
+        assert coef.is_cuda and coef.dtype == torch.complex128 and coef.stride(1) == 1 and coef.shape[1] == x.shape[0]
+        nx, ny = int(x.shape[0]), int(coef.shape[0])
+        if y is None:
+            y = torch.zeros((ny, x.shape[1]), dtype=torch.complex128, device=x.device)
+        ldx = int(x.stride(0)) if nx > 1 else int(x.shape[1])
+        ldc = int(coef.stride(0)) if ny > 1 else int(coef.shape[1])
+        ldy = int(y.stride(0)) if ny > 1 else int(y.shape[1])
+        _check(self._lib.qe_hpsi_rotate(self._h, _vp(x.data_ptr()), ldx, nx, _vp(coef.data_ptr()), ldc, _vp(y.data_ptr()),
+                                        ldy, ny, 1 if accumulate else 0, _stream_ptr(stream)), self._h)
+        return y
 
     def density(self, psi, occ, scale, rho, stream=None):
         """qe_hpsi_density: rho[N1,N2,N3] += scale * sum_b occ[b] |psi_b(r)|^2 (rho, occ: CUDA float64 tensors)."""

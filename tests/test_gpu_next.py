@@ -207,3 +207,75 @@ def test_gamma_matches_the_full_sphere_path_on_config_1():
     assert _gpu.rel_l2(got, hf[:, ip]).max() <= TOL
     g.destroy()
     full.destroy()
+
+
+# ---- Davidson pieces (NEXT-3) -----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", ["T1_general_k", 0])
+def test_hdiag_precond_rotate_against_oracle(cfg):
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    q = _qblocks(wl, 23)
+    h.set_s(q)
+    vbar = float(inp["vr"].mean().item())
+    hd, sd = h.hdiag(vbar, want_s=True)
+    torch.cuda.synchronize()
+    href = orc.hdiag_of(sp["g2kin"], vbar, beta, inp["dblocks"])
+    sref = orc.sdiag_of(npw, beta, q)
+    assert np.abs(hd.cpu().numpy() - href).max() <= 1e-13 * np.abs(href).max()
+    assert np.abs(sd.cpu().numpy() - sref).max() <= 1e-13 * np.abs(sref).max()
+    nb = 5
+    r = _gpu.gen_psi_dev(inp, 40, nb)
+    rh = r[:, :npw].cpu().numpy()
+    e = torch.linspace(-0.7, 3.1, nb, dtype=torch.float64, device="cuda")
+    h.precond(r, e, hd, sd)
+    torch.cuda.synchronize()
+    pref = orc.precond_of(rh, e.cpu().numpy(), href, sref)
+    assert _gpu.rel_l2(r.cpu().numpy()[:, :npw], pref).max() <= 1e-13
+    # rotation: 3 output vectors from 5 inputs, overwrite then accumulate
+    x = _gpu.gen_psi_dev(inp, 0, 5)
+    gen = torch.Generator().manual_seed(5)
+    coef = torch.randn((3, 5), dtype=torch.complex128, generator=gen).cuda()
+    y = torch.full((3, x.shape[1]), 2.0, dtype=torch.complex128, device="cuda")
+    h.rotate(x, coef, y)
+    torch.cuda.synchronize()
+    yref = orc.rotate_of(x[:, :npw].cpu().numpy(), coef.cpu().numpy())
+    assert _gpu.rel_l2(y.cpu().numpy()[:, :npw], yref).max() <= 1e-13
+    assert np.all(y.cpu().numpy()[:, npw:] == 2.0)
+    h.rotate(x, coef, y, accumulate=True)
+    torch.cuda.synchronize()
+    assert _gpu.rel_l2(y.cpu().numpy()[:, :npw], 2 * yref).max() <= 1e-13
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg,nev,use_s", [("T1_general_k", 4, False), ("T1_general_k", 4, True), (0, 8, True)])
+def test_davidson_finds_the_lowest_eigenpairs_of_the_dense_problem(cfg, nev, use_s):
+    """The driver (paper_2104_10502_b200/davidson.py) around the library calls against a dense generalized
+    eigensolve of the oracle's H and S (scipy.linalg.eigh)."""
+    import scipy.linalg
+
+    from paper_2104_10502_b200.davidson import davidson
+
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h.npw
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    q = 0.2 * _qblocks(wl, 31)  # keeps S positive definite
+    if use_s:
+        h.set_s(q)
+    hd = orc.dense_h(sp["miller"], sp["g2kin"], tuple(wl.nr), inp["vr"].cpu().numpy(), beta, inp["dblocks"])
+    sd = orc.dense_s(beta, q, npw) if use_s else np.eye(npw)
+    eref = scipy.linalg.eigh(hd, sd, eigvals_only=True, subset_by_index=[0, nev - 1])
+    psi0 = _gpu.gen_psi_dev(inp, 0, nev)
+    e, psi, info = davidson(h, psi0, float(inp["vr"].mean().item()), use_s=use_s, tol=1e-9, max_iter=200)
+    torch.cuda.synchronize()
+    assert info["converged"], info
+    assert np.abs(e.cpu().numpy() - eref).max() <= 1e-8 * max(1.0, np.abs(eref).max()), (e.cpu().numpy(), eref)
+    # residual of the returned pairs, evaluated by the oracle
+    ph = psi[:, :npw].cpu().numpy()
+    res = (hd @ ph.T).T - e.cpu().numpy()[:, None] * (sd @ ph.T).T
+    assert np.linalg.norm(res, axis=1).max() <= 1e-7
+    h.destroy()
