@@ -206,6 +206,20 @@ def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
     by = nb * 16.0 * (npw + 2 * info["S"] * n3 + 2 * info["P"] * n2 * n3) + 16.0 * n1 * n2 * n3 * -(-nb // info["fft_nb"])
     out["density"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "algorithmic_gbs": by / ms * 1e-6, "bound": "hbm",
                       "frac": by / ms * 1e-6 / hbm_peak}
+    # NEXT-3, rest of the Davidson step: preconditioner diagonals (beta streamed once), preconditioner, rotation
+    if wl.nproj:
+        ms = ev_time(lambda: h.hdiag(0.0, want_s=True))
+        by = 2 * 16.0 * wl.nproj * npw  # beta read once for hdiag and once for sdiag
+        out["hdiag_sdiag"] = {"ms": ms, "gbs": by / ms * 1e-6, "bound": "hbm", "frac": by / ms * 1e-6 / hbm_peak}
+    hd, _ = h.hdiag(0.0)
+    ev = torch.zeros(nb, dtype=torch.float64, device="cuda")
+    ms = ev_time(lambda: h.precond(sp, ev, hd))
+    by = 2 * 16.0 * nb * npw
+    out["precond"] = {"ms": ms, "gbs": by / ms * 1e-6, "bound": "hbm", "frac": by / ms * 1e-6 / hbm_peak}
+    coef = torch.eye(nb, dtype=torch.complex128, device="cuda")
+    ms = ev_time(lambda: h.rotate(p, coef, sp))
+    fl = 8.0 * nb * nb * npw
+    out["rotate"] = {"ms": ms, "shape": [npw, nb, nb], "tflops": fl / ms * 1e-9, "bound": "tensor", "frac": fl / ms * 1e-9 / dmma}
     # NEXT-1: the same chunk as a real-wavefunction problem on the half sphere (k = 0 configs only)
     if all(x == 0.0 for x in wl.xk):
         from paper_2104_10502_b200 import inputs, qe_hpsi
@@ -412,7 +426,9 @@ def main():
                                   "proj_flops_per_band": m["f_proj"], "note": "max(bytes/HBM, projector flops/FP64 tensor) per band"},
             "stages": stages, "cpu_baseline": cpu, "setup_s": t_setup}
     if args.next:
+        torch.cuda.profiler.start()  # the next-rows pass is visible to `ncu --profile-from-start off` too
         line["next_rows"] = time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak)
+        torch.cuda.profiler.stop()
         if "gamma_apply" in line["next_rows"]:
             line["next_rows"]["gamma_apply"]["speedup_vs_complex_path"] = line["next_rows"]["gamma_apply"]["bands_per_s"] / (value / world)
     print(json.dumps(line), flush=True)

@@ -896,9 +896,26 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     h->workspace_bytes += (size_t)h->fft_nb * per_band;
     // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
     // gridDim.y only as far as needed to give every SM a few CTAs
+    // (fewer splits = V(r) reused over more bands), choosing the split that fills whole waves of resident CTAs
     const long long xt = (long long)nr[1] * g.ntz;
-    int split = (int)std::min<long long>(h->fft_nb, std::max<long long>(1, (4LL * h->num_sms + xt - 1) / xt));
-    h->x_split = std::max(1, split);
+    int occ = 0;
+    if (h->f2p[0])
+      CR_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->f2p[0]->x, h->f2p[0]->nthreads, h->smem_x2p));
+    else
+      CR_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_x_vmul, FFT_NT, h->smem_x));
+    const long long slots = (long long)std::max(occ, 1) * h->num_sms;
+    int best = 1;
+    double best_score = -1.0;
+    for (int sp = 1; sp <= std::min(h->fft_nb, 8); ++sp) {
+      const long long ctas = xt * sp, waves = (ctas + slots - 1) / slots;
+      const double score = (double)ctas / (double)(waves * slots) - 0.01 * (sp - 1);
+      if (score > best_score) {
+        best_score = score;
+        best = sp;
+      }
+    }
+    h->x_split = env_int("QE_HPSI_X_SPLIT", best);
+    h->x_split = std::max(1, std::min(h->x_split, h->fft_nb));
   }
 
   h->overlap = env_int("QE_HPSI_OVERLAP", 0);
