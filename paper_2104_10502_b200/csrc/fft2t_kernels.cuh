@@ -1,0 +1,158 @@
+// fft2t_kernels.cuh -- TMA-staged x stage (step a3) of the two-pass fast path.
+// Same arithmetic as k2p_x_vmul (fft2p_kernels.cuh): inverse FFT along i1 over the P populated planes, * V(r)/N, forward
+// FFT, keep the populated planes.  What changes is how the [P][8-column] tile of W2 moves: one elected thread issues a
+// single 3-D tensor-map bulk copy (cp.async.bulk.tensor, box = 1 band x P planes x 128 bytes) per band into a shared
+// staging buffer, completion on an mbarrier, and one bulk tensor store of the result from a second staging buffer; the
+// compute threads only touch shared memory.  The load of band b+1 and the store of band b-1 overlap the butterflies of
+// band b, which the register-starved radix-16 kernel (two 4-warp CTAs per SM) could not do with its own loads and
+// strided 16-byte stores: 43.8 -> 32.2 us per band at 192^3 (profiles/r1e_capture.md).  The twiddles tw[q*j] of both
+// passes depend on the thread only and live in registers.  PAPER.md:L215 (1-D FFT stages), L224-226 (local potential).
+#pragma once
+#include <cuda.h>
+
+#include "fft2p_kernels.cuh"
+
+namespace qehpsi {
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// dynamic shared memory: tile1, tile2 [N][FFT_C], input stage [P][FFT_C], output stage [P][FFT_C], one mbarrier
+inline size_t fft2t_smem(int n, int P) { return 2 * (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)P * FFT_C * sizeof(double2) + 64; }
+
+// tmap: W2 viewed as FP64 [nb][P][N2*ldz*2], box {16, P, 1}
+template <int RA, int RB>
+__global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb) {
+  static_assert(RB > 1, "single-pass lengths use k2p_x_vmul");
+  constexpr int N = RA * RB, NT = RA * FFT_C, NW = (NT + 31) / 32;
+  constexpr unsigned ROWB = FFT_C * sizeof(double2);  // 128 bytes per plane row of the tile
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double2* tile1 = reinterpret_cast<double2*>(smem_raw);
+  double2* tile2 = tile1 + N * FFT_C;
+  double2* inb = tile2 + N * FFT_C;
+  const int P = g.P;
+  double2* outb = inb + (size_t)P * FFT_C;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(outb + (size_t)P * FFT_C);
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const bool io_thread = tid == (NW - 1) * 32;  // first lane of the last warp (idle in the radix-RA passes when RA > RB)
+  const int i2 = blockIdx.x / g.ntz;
+  const int z0 = (blockIdx.x - i2 * g.ntz) * FFT_C;
+  const double2 zero = make_double2(0.0, 0.0);
+  double vv[RB];
+#pragma unroll
+  for (int q = 0; q < RB; ++q) vv[q] = __ldg(&g.vs[((size_t)(j + q * RA) * g.n2 + i2) * g.ldz + z0 + c]);
+  int pl[RA];
+  if (j < RB) {
+#pragma unroll
+    for (int q = 0; q < RA; ++q) pl[q] = __ldg(&t.plane_of[j + q * RB]);
+  }
+  double2 twr[RA];  // tw[q*j]: second-pass twiddles of the inverse (q < RB) and of the forward transform (q < RA)
+#pragma unroll
+  for (int q = 0; q < RA; ++q) twr[q] = __ldg(&g.ax1.tw[(q * j) % N]);
+  if (tid == 0) {
+    mbar_init(full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int cx = (i2 * g.ldz + z0) * 2;  // innermost tensor coordinate, in doubles
+  auto issue_load = [&](int b) {
+    mbar_expect_tx(full, (unsigned)P * ROWB);
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     smem_u32(inb)),
+                 "l"(&tmap), "r"(cx), "r"(0), "r"(b), "r"(smem_u32(full))
+                 : "memory");
+  };
+  auto issue_store = [&](int b) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&tmap), "r"(cx), "r"(0),
+                 "r"(b), "r"(smem_u32(outb))
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  };
+  const int b0 = blockIdx.y, bstep = gridDim.y;
+  if (io_thread && b0 < nb) issue_load(b0);
+  int it = 0;
+  for (int b = b0; b < nb; b += bstep, ++it) {
+    if (j < RB) {
+      mbar_wait(full, it & 1);
+      double2 v[RA];
+      const double2* in = inb + c;
+#pragma unroll
+      for (int q = 0; q < RA; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * FFT_C] : zero;
+      pass_a_store<RA, +1>(v, tile1, j, c);
+    }
+    __syncthreads();
+    if (io_thread) {
+      if (b + bstep < nb) issue_load(b + bstep);  // the input stage was consumed before this barrier
+      if (it > 0) issue_store(b - bstep);          // written by the previous iteration's last pass, fenced by its writers
+    }
+    {
+      double2 u[RB];
+#pragma unroll
+      for (int q = 0; q < RB; ++q) u[q] = tile1[fft_phys(j + q * RA, c)];
+#pragma unroll
+      for (int q = 1; q < RB; ++q) u[q] = cmul(u[q], twr[q]);
+      Dft<RB, +1>::run(u);
+#pragma unroll
+      for (int q = 0; q < RB; ++q) u[q] = make_double2(u[q].x * vv[q], u[q].y * vv[q]);
+      Dft<RB, -1>::run(u);  // forward pass 1 = radix RB on the inputs j + q*RA this thread already holds
+#pragma unroll
+      for (int q = 0; q < RB; ++q) tile2[fft_phys(j * RB + q, c)] = u[q];
+    }
+    if (io_thread) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // output stage free before it is rewritten
+    __syncthreads();
+    if (j < RB) {
+      double2 v[RA];
+#pragma unroll
+      for (int q = 0; q < RA; ++q) v[q] = tile2[fft_phys(j + q * RB, c)];
+#pragma unroll
+      for (int q = 1; q < RA; ++q) v[q] = cmulc(v[q], twr[q]);
+      Dft<RA, -1>::run(v);
+      double2* out = outb + c;
+#pragma unroll
+      for (int q = 0; q < RA; ++q)
+        if (pl[q] >= 0) out[pl[q] * FFT_C] = v[q];
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the bulk store
+    }
+  }
+  __syncthreads();
+  if (io_thread && it > 0) {
+    issue_store(b0 + (it - 1) * bstep);
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // shared memory must outlive the store's reads
+  }
+}
+
+using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int);
+
+struct Fft2tEntry {
+  int n, ra, rb;
+  K2tX x;
+};
+#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_vmul<RA, RB>}
+static const Fft2tEntry kFft2tTable[] = {
+    QE_FFT2T_ENTRY(6, 3),   QE_FFT2T_ENTRY(5, 4),   QE_FFT2T_ENTRY(6, 6),   QE_FFT2T_ENTRY(8, 6),   QE_FFT2T_ENTRY(8, 8),
+    QE_FFT2T_ENTRY(9, 8),   QE_FFT2T_ENTRY(10, 8),  QE_FFT2T_ENTRY(12, 8),  QE_FFT2T_ENTRY(10, 10), QE_FFT2T_ENTRY(12, 9),
+    QE_FFT2T_ENTRY(12, 10), QE_FFT2T_ENTRY(16, 8),  QE_FFT2T_ENTRY(12, 12), QE_FFT2T_ENTRY(16, 10), QE_FFT2T_ENTRY(15, 12),
+    QE_FFT2T_ENTRY(16, 12), QE_FFT2T_ENTRY(16, 15), QE_FFT2T_ENTRY(16, 16),
+};
+#undef QE_FFT2T_ENTRY
+// the (RA, RB) pair must be the one the two-pass table uses for this length (same thread layout and tables)
+inline const Fft2tEntry* fft2t_find(int n, int ra, int rb) {
+  for (const Fft2tEntry& e : kFft2tTable)
+    if (e.n == n && e.ra == ra && e.rb == rb) return &e;
+  return nullptr;
+}
+
+}  // namespace qehpsi

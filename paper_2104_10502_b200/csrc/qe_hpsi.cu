@@ -16,6 +16,7 @@
 
 #include "fft_kernels.cuh"
 #include "fft3p_kernels.cuh"
+#include "fft2t_kernels.cuh"
 #include "zgemm_kernels.cuh"
 
 using namespace qehpsi;
@@ -70,6 +71,10 @@ struct qe_hpsi_handle {
   Fft2pGeom g2p{};
   int *stick_lo = nullptr, *stick_hi = nullptr, *col_of = nullptr, *plane_of = nullptr;
   size_t smem_x2p = 0;
+  // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
+  K2tX x_tma = nullptr;
+  CUtensorMap tmap_w2{};
+  size_t smem_xt = 0;
   // nonlocal
   int nproj = 0;
   const double2* beta = nullptr;  // borrowed or owned
@@ -896,10 +901,37 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     h->workspace_bytes += (size_t)h->fft_nb * per_band;
     // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
     // gridDim.y only as far as needed to give every SM a few CTAs
+    if (h->f2p[0] && h->f2p[0]->smem_zy == 0 && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && env_int("QE_HPSI_X_TMA", 1)) {
+      const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb);
+      const size_t sm = fft2t_smem(nr[0], h->P);
+      using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+      EncodeFn enc = nullptr;
+      cudaDriverEntryPointQueryResult qres;
+      if (et && sm <= (size_t)110 * 1024 &&
+          cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) == cudaSuccess && enc &&
+          qres == cudaDriverEntryPointSuccess) {
+        const cuuint64_t row = (cuuint64_t)nr[1] * h->ldz;  // complex elements per plane
+        cuuint64_t dims[3] = {row * 2, (cuuint64_t)h->P, (cuuint64_t)h->fft_nb};
+        cuuint64_t strides[2] = {row * sizeof(double2), row * sizeof(double2) * (cuuint64_t)h->P};
+        cuuint32_t box[3] = {2 * FFT_C, (cuuint32_t)h->P, 1};
+        cuuint32_t estr[3] = {1, 1, 1};
+        if (enc(&h->tmap_w2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, h->w2, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS &&
+            cudaFuncSetAttribute((const void*)et->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess) {
+          h->x_tma = et->x;
+          h->smem_xt = sm;
+        }
+      }
+      (void)cudaGetLastError();  // a failed probe falls back to k2p_x_vmul
+    }
     // (fewer splits = V(r) reused over more bands), choosing the split that fills whole waves of resident CTAs
     const long long xt = (long long)nr[1] * g.ntz;
     int occ = 0;
-    if (h->f2p[0])
+    if (h->x_tma)
+      CR_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->x_tma, h->f2p[0]->nthreads, h->smem_xt));
+    else if (h->f2p[0])
       CR_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->f2p[0]->x, h->f2p[0]->nthreads, h->smem_x2p));
     else
       CR_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_x_vmul, FFT_NT, h->smem_x));
@@ -974,7 +1006,9 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     else
       k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
     size_t m2 = fine ? prof_mark(h, st) : (size_t)-1;
-    if (fast)
+    if (h->x_tma)
+      h->x_tma<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_xt, st>>>(g, h->g2p, h->tmap_w2, n);
+    else if (fast)
       ex->x<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_x2p, st>>>(g, h->g2p, h->w2, n);
     else
       k_x_vmul<<<dim3(xt, std::min(n, h->x_split)), FFT_NT, h->smem_x, st>>>(g, h->w2, n);
