@@ -10,7 +10,7 @@
 #pragma once
 #include <cuda.h>
 
-#include "fft2p_kernels.cuh"
+#include "fft3p_kernels.cuh"
 
 namespace qehpsi {
 
@@ -134,6 +134,102 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, 
   }
 }
 
+
+// three-pass variant (lengths of fft3p_kernels.cuh): same staging, arithmetic of k3p_x_vmul
+template <int R1, int R2, int R3>
+__global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap,
+                                                                int nb) {
+  using PP = P3<R1, R2, R3>;
+  constexpr int N = PP::N, NT = PP::NT, NW = (NT + 31) / 32;
+  constexpr unsigned ROWB = FFT_C * sizeof(double2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double2* tA = reinterpret_cast<double2*>(smem_raw);
+  double2* tB = tA + N * FFT_C;
+  double2* inb = tB + N * FFT_C;
+  const int P = g.P;
+  double2* outb = inb + (size_t)P * FFT_C;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(outb + (size_t)P * FFT_C);
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const bool io_thread = tid == (NW - 1) * 32;
+  const int i2 = blockIdx.x / g.ntz;
+  const int z0 = (blockIdx.x - i2 * g.ntz) * FFT_C;
+  const double2 zero = make_double2(0.0, 0.0);
+  double vv[R3];
+  if (j < PP::T3) {
+#pragma unroll
+    for (int q = 0; q < R3; ++q) vv[q] = __ldg(&g.vs[((size_t)(j + q * PP::T3) * g.n2 + i2) * g.ldz + z0 + c]);
+  }
+  int pl[R1];
+  if (j < PP::T1) {
+#pragma unroll
+    for (int q = 0; q < R1; ++q) pl[q] = __ldg(&t.plane_of[j + q * PP::T1]);
+  }
+  if (tid == 0) {
+    mbar_init(full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int cx = (i2 * g.ldz + z0) * 2;
+  auto issue_load = [&](int b) {
+    mbar_expect_tx(full, (unsigned)P * ROWB);
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     smem_u32(inb)),
+                 "l"(&tmap), "r"(cx), "r"(0), "r"(b), "r"(smem_u32(full))
+                 : "memory");
+  };
+  auto issue_store = [&](int b) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&tmap), "r"(cx), "r"(0),
+                 "r"(b), "r"(smem_u32(outb))
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  };
+  const int b0 = blockIdx.y, bstep = gridDim.y;
+  if (io_thread && b0 < nb) issue_load(b0);
+  int it = 0;
+  for (int b = b0; b < nb; b += bstep, ++it) {
+    if (j < PP::T1) {
+      mbar_wait(full, it & 1);
+      double2 v[R1];
+      const double2* in = inb + c;
+#pragma unroll
+      for (int q = 0; q < R1; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * FFT_C] : zero;
+      pass_a_store<R1, +1>(v, tA, j, c);
+    }
+    __syncthreads();
+    if (io_thread) {
+      if (b + bstep < nb) issue_load(b + bstep);
+      if (it > 0) issue_store(b - bstep);
+    }
+    if (j < PP::T2) pass_mid<R2, +1>(tA, tB, g.ax1.tw, N, R1, j, c);
+    __syncthreads();
+    if (j < PP::T3) {
+      double2 u[R3];
+      pass_b_load<PP::T3, R3, +1>(tB, g.ax1.tw, j, c, u);
+#pragma unroll
+      for (int q = 0; q < R3; ++q) u[q] = make_double2(u[q].x * vv[q], u[q].y * vv[q]);
+      pass_a_store<R3, -1>(u, tA, j, c);
+    }
+    __syncthreads();
+    if (j < PP::T2) pass_mid<R2, -1>(tA, tB, g.ax1.tw, N, R3, j, c);
+    if (io_thread) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    __syncthreads();
+    if (j < PP::T1) {
+      double2 v[R1];
+      pass_b_load<PP::T1, R1, -1>(tB, g.ax1.tw, j, c, v);
+      double2* out = outb + c;
+#pragma unroll
+      for (int q = 0; q < R1; ++q)
+        if (pl[q] >= 0) out[pl[q] * FFT_C] = v[q];
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+  }
+  __syncthreads();
+  if (io_thread && it > 0) {
+    issue_store(b0 + (it - 1) * bstep);
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  }
+}
+
 using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int);
 
 struct Fft2tEntry {
@@ -148,8 +244,20 @@ static const Fft2tEntry kFft2tTable[] = {
     QE_FFT2T_ENTRY(16, 12), QE_FFT2T_ENTRY(16, 15), QE_FFT2T_ENTRY(16, 16),
 };
 #undef QE_FFT2T_ENTRY
+// three-pass lengths: ra = R1, rb = R2*R3 as in kFft3pTable
+#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), k3t_x_vmul<R1, R2, R3>}
+static const Fft2tEntry kFft3tTable[] = {
+    QE_FFT3T_ENTRY(5, 5, 5),  QE_FFT3T_ENTRY(6, 5, 5),  QE_FFT3T_ENTRY(8, 5, 5),  QE_FFT3T_ENTRY(6, 6, 6), QE_FFT3T_ENTRY(10, 5, 5),
+    QE_FFT3T_ENTRY(8, 6, 6),  QE_FFT3T_ENTRY(10, 6, 5), QE_FFT3T_ENTRY(8, 8, 5),  QE_FFT3T_ENTRY(10, 6, 6), QE_FFT3T_ENTRY(8, 8, 6),
+};
+#undef QE_FFT3T_ENTRY
 // the (RA, RB) pair must be the one the two-pass table uses for this length (same thread layout and tables)
-inline const Fft2tEntry* fft2t_find(int n, int ra, int rb) {
+inline const Fft2tEntry* fft2t_find(int n, int ra, int rb, bool three_pass) {
+  if (three_pass) {
+    for (const Fft2tEntry& e : kFft3tTable)
+      if (e.n == n && e.ra == ra && e.rb == rb) return &e;
+    return nullptr;
+  }
   for (const Fft2tEntry& e : kFft2tTable)
     if (e.n == n && e.ra == ra && e.rb == rb) return &e;
   return nullptr;

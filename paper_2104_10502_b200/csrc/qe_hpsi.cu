@@ -901,8 +901,8 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     h->workspace_bytes += (size_t)h->fft_nb * per_band;
     // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
     // gridDim.y only as far as needed to give every SM a few CTAs
-    if (h->f2p[0] && h->f2p[0]->smem_zy == 0 && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && env_int("QE_HPSI_X_TMA", 1)) {
-      const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb);
+    if (h->f2p[0] && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && env_int("QE_HPSI_X_TMA", 1)) {
+      const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb, h->f2p[0]->smem_zy != 0);
       const size_t sm = fft2t_smem(nr[0], h->P);
       using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
