@@ -230,13 +230,135 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3t_x_vmul(FftGeom g, Fft2
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// z stages (a1, a5) with bulk-copy staging of the W1 side: the 8 sticks of a tile are 8 contiguous rows of W1, so the tile
+// moves as eight 1-D bulk copies of N*16 bytes instead of 16-byte accesses at a row stride (lanes run across sticks).
+// Stage layout [stick c][N + 1] complex (odd pitch: the 8 lanes of a quarter warp hit 8 different 16-byte bank groups).
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, unsigned bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* sdst, const void* gsrc, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(sdst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+inline size_t fft2t_smem_z(int n) { return ((size_t)n * FFT_C + (size_t)FFT_C * (n + 1)) * sizeof(double2) + 64; }
+
+// a1: psi(G) -> z sticks, inverse FFT along i3 -> W1 (bulk stores)
+template <int RA, int RB>
+__global__ void __launch_bounds__(RA* FFT_C) k2t_scatter_zinv(FftGeom g, Fft2pGeom t, const double2* __restrict__ psi,
+                                                              long long ldpsi, double2* __restrict__ w1) {
+  static_assert(RB > 1, "single-pass lengths use k2p_scatter_zinv");
+  constexpr int N = RA * RB, PITCH = N + 1;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double2* tile = reinterpret_cast<double2*>(smem_raw);
+  double2* stage = tile + N * FFT_C;  // [FFT_C][PITCH]
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const int b = blockIdx.y;
+  const int s0 = blockIdx.x * FFT_C, s = s0 + c;
+  const bool sok = s < g.S;
+  const double2 zero = make_double2(0.0, 0.0);
+  if (j < RB) {
+    double2 v[RA];
+    if (sok) {
+      const int start = g.stick_start[s], lo = t.stick_lo[s], hi = t.stick_hi[s];
+      const double2* pb = psi + (size_t)b * ldpsi;
+#pragma unroll
+      for (int q = 0; q < RA; ++q) {
+        const int pos = stick_pos(start, lo, hi, j + q * RB, N);
+        v[q] = pos >= 0 ? pb[pos] : zero;
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < RA; ++q) v[q] = zero;
+    }
+    pass_a_store<RA, +1>(v, tile, j, c);
+  }
+  __syncthreads();
+  {
+    double2 u[RB];
+    pass_b_load<RA, RB, +1>(tile, g.ax3.tw, j, c, u);
+    double2* out = stage + c * PITCH + j;
+#pragma unroll
+    for (int q = 0; q < RB; ++q) out[q * RA] = u[q];
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid < FFT_C && s0 + tid < g.S) {
+    bulk_s2g(w1 + ((size_t)b * g.S + s0 + tid) * g.ldz, stage + tid * PITCH, (unsigned)(N * sizeof(double2)));
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // shared memory must outlive the store's reads
+  }
+}
+
+// a5: W1 (bulk loads) -> forward FFT along i3, gather the sphere, add g2kin*psi -> hpsi
+template <int RA, int RB>
+__global__ void __launch_bounds__(RA* FFT_C) k2t_zfwd_gather(FftGeom g, Fft2pGeom t, const double2* __restrict__ w1,
+                                                             const double2* __restrict__ psi, long long ldpsi,
+                                                             double2* __restrict__ hpsi, long long ldh) {
+  static_assert(RB > 1, "single-pass lengths use k2p_zfwd_gather");
+  constexpr int N = RA * RB, PITCH = N + 1;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double2* tile = reinterpret_cast<double2*>(smem_raw);
+  double2* stage = tile + N * FFT_C;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(stage + FFT_C * PITCH);
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const int b = blockIdx.y;
+  const int s0 = blockIdx.x * FFT_C, s = s0 + c;
+  const int nst = min(FFT_C, g.S - s0);
+  const bool sok = s < g.S;
+  const double2 zero = make_double2(0.0, 0.0);
+  if (tid == 0) {
+    mbar_init(full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) mbar_expect_tx(full, (unsigned)(nst * N * sizeof(double2)));
+  __syncthreads();
+  if (tid < nst) bulk_g2s(stage + tid * PITCH, w1 + ((size_t)b * g.S + s0 + tid) * g.ldz, (unsigned)(N * sizeof(double2)), full);
+  int start = 0, lo = 1, hi = 0;
+  if (sok) {
+    start = g.stick_start[s];
+    lo = t.stick_lo[s];
+    hi = t.stick_hi[s];
+  }
+  const double2* pb = psi + (size_t)b * ldpsi;
+  double2* hb = hpsi + (size_t)b * ldh;
+  if (j < RB) {
+    mbar_wait(full, 0);
+    double2 v[RA];
+    const double2* in = stage + c * PITCH;
+#pragma unroll
+    for (int q = 0; q < RA; ++q) v[q] = sok ? in[j + q * RB] : zero;
+    pass_a_store<RA, -1>(v, tile, j, c);
+  }
+  __syncthreads();
+  {
+    double2 u[RB];
+    pass_b_load<RA, RB, -1>(tile, g.ax3.tw, j, c, u);
+#pragma unroll
+    for (int q = 0; q < RB; ++q) {
+      const int pos = stick_pos(start, lo, hi, j + q * RA, N);
+      if (pos >= 0) {
+        const double2 cpsi = pb[pos];
+        const double k2 = __ldg(&g.g2kin[pos]);
+        hb[pos] = make_double2(u[q].x + k2 * cpsi.x, u[q].y + k2 * cpsi.y);
+      }
+    }
+  }
+}
+
 using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int);
 
 struct Fft2tEntry {
   int n, ra, rb;
   K2tX x;
+  K2pZinv zinv;  // bulk-staged z stages (two-pass lengths only; null for the three-pass table)
+  K2pZfwd zfwd;
 };
-#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_vmul<RA, RB>}
+#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
 static const Fft2tEntry kFft2tTable[] = {
     QE_FFT2T_ENTRY(6, 3),   QE_FFT2T_ENTRY(5, 4),   QE_FFT2T_ENTRY(6, 6),   QE_FFT2T_ENTRY(8, 6),   QE_FFT2T_ENTRY(8, 8),
     QE_FFT2T_ENTRY(9, 8),   QE_FFT2T_ENTRY(10, 8),  QE_FFT2T_ENTRY(12, 8),  QE_FFT2T_ENTRY(10, 10), QE_FFT2T_ENTRY(12, 9),
@@ -245,7 +367,7 @@ static const Fft2tEntry kFft2tTable[] = {
 };
 #undef QE_FFT2T_ENTRY
 // three-pass lengths: ra = R1, rb = R2*R3 as in kFft3pTable
-#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), k3t_x_vmul<R1, R2, R3>}
+#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
 static const Fft2tEntry kFft3tTable[] = {
     QE_FFT3T_ENTRY(5, 5, 5),  QE_FFT3T_ENTRY(6, 5, 5),  QE_FFT3T_ENTRY(8, 5, 5),  QE_FFT3T_ENTRY(6, 6, 6), QE_FFT3T_ENTRY(10, 5, 5),
     QE_FFT3T_ENTRY(8, 6, 6),  QE_FFT3T_ENTRY(10, 6, 5), QE_FFT3T_ENTRY(8, 8, 5),  QE_FFT3T_ENTRY(10, 6, 6), QE_FFT3T_ENTRY(8, 8, 6),

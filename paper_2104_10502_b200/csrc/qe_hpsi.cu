@@ -73,6 +73,9 @@ struct qe_hpsi_handle {
   size_t smem_x2p = 0;
   // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
   K2tX x_tma = nullptr;
+  K2pZinv z_tma_inv = nullptr;  // bulk-staged a1 / a5 (fft2t_kernels.cuh)
+  K2pZfwd z_tma_fwd = nullptr;
+  size_t smem_zt = 0;
   CUtensorMap tmap_w2{};
   size_t smem_xt = 0;
   // nonlocal
@@ -926,6 +929,19 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
       }
       (void)cudaGetLastError();  // a failed probe falls back to k2p_x_vmul
     }
+    if (h->f2p[2] && h->f2p[2]->smem_zy == 0 && h->f2p[2]->rb > 1 && env_int("QE_HPSI_Z_TMA", 1)) {
+      const Fft2tEntry* et = fft2t_find(nr[2], h->f2p[2]->ra, h->f2p[2]->rb, false);
+      const size_t sm = fft2t_smem_z(nr[2]);
+      if (et && et->zinv && sm <= (size_t)100 * 1024 &&
+          cudaFuncSetAttribute((const void*)et->zinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess &&
+          cudaFuncSetAttribute((const void*)et->zfwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess) {
+        const int m = env_int("QE_HPSI_Z_TMA", 1);  // bit 0: a1, bit 1: a5 (default 1 -> both via the mask below)
+        h->z_tma_inv = (m == 1 || (m & 2)) ? et->zinv : nullptr;
+        h->z_tma_fwd = (m == 1 || (m & 4)) ? et->zfwd : nullptr;
+        h->smem_zt = sm;
+      }
+      (void)cudaGetLastError();
+    }
     // (fewer splits = V(r) reused over more bands), choosing the split that fills whole waves of resident CTAs
     const long long xt = (long long)nr[1] * g.ntz;
     int occ = 0;
@@ -996,7 +1012,9 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     const bool fast = h->f2p[0] != nullptr;
     const Fft2pEntry *ex = h->f2p[0], *ey = h->f2p[1], *ez = h->f2p[2];
     size_t m0 = fine ? prof_mark(h, st) : (size_t)-1;
-    if (fast)
+    if (h->z_tma_inv)
+      h->z_tma_inv<<<dim3(zt, n), ez->nthreads, h->smem_zt, st>>>(g, h->g2p, p, ldpsi, h->w1);
+    else if (fast)
       ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
     else
       k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
@@ -1018,7 +1036,9 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
     else
       k_yfwd<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w2, h->w1);
     size_t m4 = fine ? prof_mark(h, st) : (size_t)-1;
-    if (fast)
+    if (h->z_tma_fwd)
+      h->z_tma_fwd<<<dim3(zt, n), ez->nthreads, h->smem_zt, st>>>(g, h->g2p, h->w1, p, ldpsi, o, ldh);
+    else if (fast)
       ez->zfwd<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, h->w1, p, ldpsi, o, ldh);
     else
       k_zfwd_gather<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, h->w1, p, ldpsi, o, ldh);
