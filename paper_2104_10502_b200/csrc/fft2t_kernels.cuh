@@ -255,20 +255,32 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_scatter_zinv(FftGeom g, Fft2pGe
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tile = reinterpret_cast<double2*>(smem_raw);
   double2* stage = tile + N * FFT_C;  // [FFT_C][PITCH]
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(stage + FFT_C * PITCH);
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
   const int b = blockIdx.y;
   const int s0 = blockIdx.x * FFT_C, s = s0 + c;
   const bool sok = s < g.S;
   const double2 zero = make_double2(0.0, 0.0);
+  // the sphere entries of the tile's sticks are one contiguous chunk of psi (canonical order): one bulk load
+  const int base = g.stick_start[s0], cnt = g.stick_start[min(s0 + FFT_C, g.S)] - base;
+  if (tid == 0) {
+    mbar_init(full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (cnt > 0) {
+      mbar_expect_tx(full, (unsigned)(cnt * sizeof(double2)));
+      bulk_g2s(stage, psi + (size_t)b * ldpsi + base, (unsigned)(cnt * sizeof(double2)), full);
+    }
+  }
+  __syncthreads();
   if (j < RB) {
     double2 v[RA];
     if (sok) {
-      const int start = g.stick_start[s], lo = t.stick_lo[s], hi = t.stick_hi[s];
-      const double2* pb = psi + (size_t)b * ldpsi;
+      const int start = g.stick_start[s] - base, lo = t.stick_lo[s], hi = t.stick_hi[s];
+      if (cnt > 0) mbar_wait(full, 0);
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
         const int pos = stick_pos(start, lo, hi, j + q * RB, N);
-        v[q] = pos >= 0 ? pb[pos] : zero;
+        v[q] = pos >= 0 ? stage[pos] : zero;
       }
     } else {
 #pragma unroll
