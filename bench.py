@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--detail", action="store_true", help="extra pass with per-FFT-kernel events (stderr table)")
+    ap.add_argument("--graph", type=int, default=-1, help="replay the step from a CUDA graph: 1 on, 0 off, -1 (default) only "
+                    "for launch-latency-bound workloads (a step under 0.5 ms); stage timers are taken in a separate eager pass")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows (apply_hs, overlap, density): "
                     "adds a next_rows object to the JSON line")
     return ap.parse_args()
@@ -326,7 +328,35 @@ def main():
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    h.profile(1)
+    # launch-latency-bound workloads: capture the step (apply enqueues kernels only) and replay it
+    use_graph = args.graph == 1
+    if args.graph == -1:
+        t0 = time.perf_counter()
+        step()
+        torch.cuda.synchronize()
+        use_graph = (time.perf_counter() - t0) < 0.5e-3
+    prof_eager = None
+    if use_graph:
+        h.profile(1)
+        step()
+        torch.cuda.synchronize()
+        prof_eager = h.profile_read()  # stage timers cannot record inside a capture: one eager pass
+        h.profile(0)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            cap = torch.cuda.current_stream()
+            for b0, n in calls:
+                h.apply(psi[b0:b0 + n], hpsi[b0:b0 + n], cap)
+        eager_step = step
+
+        def step():  # noqa: F811
+            graph.replay()
+
+        for _ in range(3):
+            step()
+        barrier()
+    else:
+        h.profile(1)
     sampler = ClockSampler(torch.cuda.current_device())
     sampler.start()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -343,7 +373,7 @@ def main():
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = float(sum(step_ms))
-    prof = h.profile_read()
+    prof = prof_eager if use_graph else h.profile_read()
     h.profile(0)
     total_ms = sharding.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
@@ -415,7 +445,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": wl.name, "nbands": nb, "batch": batch, "grid": list(wl.nr), "npw": npw, "nproj": wl.nproj,
-                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["nsplit"],
+                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["nsplit"], "cuda_graph": bool(use_graph),
                        "l2": "inputs per step exceed L2" if flush is None else "L2 flushed (256 MB write) between steps",
                        "sharding": "bands / k-point pools per rank, no collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": h.launch_count(batch) * chunks_per_step * args.steps if nb % batch == 0
@@ -435,7 +465,7 @@ def main():
 
     if args.detail:
         h.profile(2)
-        step()
+        (eager_step if use_graph else step)()
         torch.cuda.synchronize()
         d = h.profile_read()
         h.profile(0)

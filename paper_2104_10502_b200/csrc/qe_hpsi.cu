@@ -615,7 +615,9 @@ int env_int(const char* name, int dflt) {
 void choose_split(qe_hpsi_handle* h) {
   const int ZG_BM = ZG_BM_TAB[h->zg_variant], ZG_BN = ZG_BN_TAB[h->zg_variant], ZG_BK = ZG_BK_TAB[h->zg_variant];
   const int ntile = ((h->nproj + ZG_BM - 1) / ZG_BM) * ((h->max_batch + ZG_BN - 1) / ZG_BN);
-  const int ksmax = std::max(1, h->npw / 512);
+  // slices of at least 512 plane waves, unless that cannot even fill two waves (few projectors, small sphere): then 128
+  int ksmax = std::max(1, h->npw / 512);
+  if ((long long)ntile * ksmax < 2LL * h->num_sms) ksmax = std::max(1, h->npw / 128);
   int best = 1;
   double best_score = -1.0;
   for (int ks = 1; ks <= std::min(ksmax, 1024); ++ks) {

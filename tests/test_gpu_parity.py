@@ -232,3 +232,36 @@ def test_local_term_for_every_fft_length(n):
         err = _gpu.rel_l2(out.cpu().numpy()[:, :npw], ref)
         assert err.max() <= TOL, (n, axis, nr, err)
         h.destroy()
+
+
+def test_apply_can_be_captured_in_a_cuda_graph():
+    """qe_hpsi_apply enqueues kernels only (no allocation, no host sync): it can be stream-captured and replayed, which
+    is how a launch-latency-bound caller (config 0: 9 launches for 16 bands) should drive it. Replays must reproduce the
+    eager result bit for bit, also after psi is overwritten in place."""
+    h, inp = _gpu.make(0)
+    wl = inp["wl"]
+    npw = h.npw
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    ref1 = h.apply(psi).clone()
+    psi2 = _gpu.gen_psi_dev(inp, 50, wl.nbands)
+    ref2 = h.apply(psi2).clone()
+    torch.cuda.synchronize()
+    buf = psi.clone()
+    out = torch.zeros_like(buf)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        h.apply(buf, out, side)  # warm-up on the capture stream
+    torch.cuda.current_stream().wait_stream(side)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        h.apply(buf, out, torch.cuda.current_stream())
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out[:, :npw].view(torch.float64), ref1[:, :npw].view(torch.float64))
+    buf.copy_(psi2)
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out[:, :npw].view(torch.float64), ref2[:, :npw].view(torch.float64))
+    del g
+    h.destroy()
