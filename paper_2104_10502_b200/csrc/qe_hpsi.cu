@@ -1658,9 +1658,16 @@ extern "C" int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldp
   const double2* psi = static_cast<const double2*>(psi_host);
   double2* hpsi = static_cast<double2*>(hpsi_host);
   const size_t width = sizeof(double2) * (size_t)h->npw;
+  // chunks of max_batch bands, except that the first and the last chunk are halved (down to a 64-band ZGEMM tile) when
+  // there are several: the H2D copy of the first chunk and the D2H copy of the last one are the only transfers that do
+  // not overlap compute
+  const int half = (h->max_batch >= 128 && nbands > h->max_batch) ? (h->max_batch / 2 + 63) / 64 * 64 : h->max_batch;
   int ci = 0;
-  for (int b0 = 0; b0 < nbands; b0 += h->max_batch, ++ci) {
-    const int nb = std::min(h->max_batch, nbands - b0);
+  for (int b0 = 0, nb = 0; b0 < nbands; b0 += nb, ++ci) {
+    const int left = nbands - b0;
+    nb = std::min(h->max_batch, left);
+    if (ci == 0) nb = std::min(half, left);
+    else if (left > h->max_batch && left < h->max_batch + half) nb = left - half;  // leave exactly `half` for the last chunk
     const int u = ci & 1;
     if (ci >= 2) CU_TRY(h, cudaStreamWaitEvent(h->st_in, h->ev_comp[u], 0));  // compute of chunk ci-2 read psi buf u
     if (width)
