@@ -1,0 +1,308 @@
+// Projector contractions a6 / a8 on the 5th-generation tensor cores (tcgen05, kind::i8, s32 accumulators in TMEM) through an
+// error-free split of the FP64 operands into signed 7-bit slices (the "Ozaki scheme"): SURVEY.md section 8(a) rows a6 and a8,
+// DESIGN.md section 5.6.  tcgen05 has no f64 kind; int8 x int8 -> int32 products are exact, so
+//
+//   x = 2^e * sum_{i<S} x_i 2^-(6+7i) + O(2^(e-7S)),  x_i in [-64, 64]        (e = exponent of the row maximum)
+//   sum_k a_k b_k = 2^(ea+eb-12) * sum_{L<S} 2^-7L * sum_{i+j=L} sum_k a_ik b_jk   + O((S+1) 2^-7S |a|max |b|max K)
+//
+// Both contractions are brought to the one form D[m][n] = sum_k A[m][k] B[n][k] over REAL k (a complex number is two
+// consecutive reals), A and B stored as S planes of int8, K contiguous:
+//   a6  becp[p][b]   : A row p  = (beta_r, beta_i)[p][g]      k = 2g+c        B row 2b = (psi_r, psi_i), row 2b+1 = (psi_i, -psi_r)
+//   a8  hpsi[b][g] += : A row g  = (beta_r, beta_i)[p][g]      k = 2p+c        B row 2b = (d_r, -d_i),    row 2b+1 = (d_i, d_r)
+// One CTA owns a 128 x 64 tile of D for one K range: S level accumulators of 64 TMEM columns each (level L = i+j), operands
+// staged by TMA (SWIZZLE_64B, 64 bytes of K per stage) on a full/empty mbarrier ring, one thread issuing the MMAs, four
+// warps converting the S int32 levels to FP64 in the epilogue.  Integer sums are exact, so results are bit-reproducible and do
+// not depend on the batch composition (each band carries its own exponent).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace qehpsi {
+namespace oz {
+
+constexpr int BM = 128, BN = 64, KB = 64, NT = 192;
+constexpr int A_BYTES = BM * KB, B_BYTES = BN * KB;
+constexpr int MAX_STAGES = 4;
+// (L+1) * Kc * 64 * 64 < 2^31 for every level L < S: Kc <= 2^19 / S reals per CTA
+__host__ __device__ constexpr long long max_k_per_cta(int S) { return ((1LL << 19) / S) / KB * KB - KB; }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t n) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t sdst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(sdst),
+               "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+               : "memory");
+}
+// K-major operand tile, rows of 64 bytes, SWIZZLE_64B: 8-row groups 512 bytes apart
+__device__ __forceinline__ uint64_t desc_sw64(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)1 << 16) | ((uint64_t)(512 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)4 << 61);
+}
+__device__ __forceinline__ void mma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(acc)
+      : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// s8 x s8 -> s32, both operands K-major, M = 128, N = 64
+constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+
+// MODE 0 (a6): out = partial[split][m][ldo] complex, written; MODE 1 (a8): out = hpsi[b][ldo] complex at column m, accumulated
+template <int S, int MODE>
+__global__ void __launch_bounds__(NT, 1)
+k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nstages, int nkb, int kchunk,
+          const int* __restrict__ ea, const int* __restrict__ eb, long long mvalid, int nb, double2* __restrict__ out,
+          long long ldo, long long split_stride) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ uint64_t full[MAX_STAGES], empty[MAX_STAGES], done;
+  __shared__ uint32_t tmem_base;
+  constexpr uint32_t STAGE = S * (A_BYTES + B_BYTES);
+  constexpr uint32_t TCOLS = S * BN <= 256 ? 256 : 512;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int q = blockIdx.x, mt = blockIdx.y, ks = blockIdx.z;
+  const int kb0 = ks * kchunk;
+  const int nit = max(0, min(nkb, kb0 + kchunk) - kb0);
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base)), "r"(TCOLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (threadIdx.x == 32) {
+    for (int i = 0; i < MAX_STAGES; ++i) {
+      mbar_init(&full[i], 1);
+      mbar_init(&empty[i], 1);
+    }
+    mbar_init(&done, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tm = tmem_base;
+  const uint32_t sbase0 = smem_u32(smem);
+
+  if (warp == 0 && lane == 0) {
+    // ---- TMA producer ----
+    for (int it = 0; it < nit; ++it) {
+      const int st = it % nstages;
+      const uint32_t ph = (uint32_t)(it / nstages) & 1u;
+      mbar_wait(&empty[st], ph ^ 1u);
+      mbar_expect_tx(&full[st], STAGE);
+      const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
+      const int kx = (kb0 + it) * KB;
+#pragma unroll
+      for (int i = 0; i < S; ++i) tma_load_3d(sb + i * A_BYTES, &tmA, kx, mt * BM, i, &full[st]);
+#pragma unroll
+      for (int j = 0; j < S; ++j) tma_load_3d(sb + S * A_BYTES + j * B_BYTES, &tmB, kx, q * BN, j, &full[st]);
+    }
+  } else if (warp == 1 && lane == 0) {
+    // ---- MMA issuer: level L = i + j accumulates into TMEM columns [L*64, L*64+64) ----
+    for (int it = 0; it < nit; ++it) {
+      const int st = it % nstages;
+      const uint32_t ph = (uint32_t)(it / nstages) & 1u;
+      mbar_wait(&full[st], ph);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
+#pragma unroll
+      for (int kk = 0; kk < KB / 32; ++kk) {
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+          const uint64_t da = desc_sw64(sb + i * A_BYTES) + 2 * kk;
+#pragma unroll
+          for (int j = 0; j < S - i; ++j) {
+            const uint64_t db = desc_sw64(sb + S * A_BYTES + j * B_BYTES) + 2 * kk;
+            mma_i8(tm + (uint32_t)(i + j) * BN, da, db, IDESC, (it | kk | i) ? 1u : 0u);
+          }
+        }
+      }
+      mma_commit(&empty[st]);
+    }
+    mma_commit(&done);
+  } else if (warp >= 2) {
+    // ---- epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31; thread = row of the tile ----
+    mbar_wait(&done, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const int wq = warp & 3;
+    const long long m = (long long)mt * BM + wq * 32 + lane;
+    const int em = (m < mvalid) ? ea[m] : 0;
+#pragma unroll 1
+    for (int n0 = 0; n0 < BN; n0 += 8) {
+      double d[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) d[j] = 0.0;
+      if (nit > 0) {
+        uint32_t v[S][8];
+#pragma unroll
+        for (int L = 0; L < S; ++L) {
+          const uint32_t ta = tm + ((uint32_t)(wq * 32) << 16) + (uint32_t)(L * BN + n0);
+          asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                       : "=r"(v[L][0]), "=r"(v[L][1]), "=r"(v[L][2]), "=r"(v[L][3]), "=r"(v[L][4]), "=r"(v[L][5]), "=r"(v[L][6]),
+                         "=r"(v[L][7])
+                       : "r"(ta));
+        }
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int L = S - 1; L >= 0; --L) {  // smallest contributions first
+          const double w = 1.0 / (double)(1ULL << (7 * L));
+#pragma unroll
+          for (int j = 0; j < 8; ++j) d[j] = fma((double)(int)v[L][j], w, d[j]);
+        }
+      }
+      if (m < mvalid) {
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const int b = (q * BN + n0) / 2 + jj;
+          if (b < nb) {
+            const int ex = em + eb[b] - 12;
+            const double re = scalbn(d[2 * jj], ex), im = scalbn(d[2 * jj + 1], ex);
+            if (MODE == 0) {
+              out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(re, im);
+            } else {
+              double2* o = out + (size_t)b * ldo + m;
+              double2 t = *o;
+              t.x += re;
+              t.y += im;
+              *o = t;
+            }
+          }
+        }
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) {
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "r"(TCOLS) : "memory");
+  }
+}
+
+// ---- exponents: e = ilogb(max |component|) + 1 (0 for an all-zero row), so that |x| 2^-e < 1 ----
+__device__ __forceinline__ int exp_of(double mx) { return mx > 0.0 ? ilogb(mx) + 1 : 0; }
+
+// one CTA per row of a complex matrix X[rows][ldx], n entries per row
+__global__ void __launch_bounds__(256) k_oz_rowexp(const double2* __restrict__ X, long long ldx, long long n, int* __restrict__ e) {
+  __shared__ double red[256];
+  const double2* x = X + (size_t)blockIdx.x * ldx;
+  double mx = 0.0;
+  for (long long i = threadIdx.x; i < n; i += 256) {
+    const double2 v = x[i];
+    mx = fmax(mx, fmax(fabs(v.x), fabs(v.y)));
+  }
+  red[threadIdx.x] = mx;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) red[threadIdx.x] = fmax(red[threadIdx.x], red[threadIdx.x + s]);
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) e[blockIdx.x] = exp_of(red[0]);
+}
+// one thread per column g of X[rows][ldx]
+__global__ void __launch_bounds__(128) k_oz_colexp(const double2* __restrict__ X, long long ldx, int rows, long long n, int* __restrict__ e) {
+  const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (g >= n) return;
+  double mx = 0.0;
+  for (int p = 0; p < rows; ++p) {
+    const double2 v = X[(size_t)p * ldx + g];
+    mx = fmax(mx, fmax(fabs(v.x), fabs(v.y)));
+  }
+  e[g] = exp_of(mx);
+}
+
+// 16 reals -> S x 16 int8 (one 16-byte store per slice); r[] already scaled to (-1, 1)
+template <int S>
+__device__ __forceinline__ void slice16(double (&r)[16], uint4 (&o)[S]) {
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) {
+    const double mult = sl == 0 ? 64.0 : 128.0;
+    uint32_t w[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+      const double y = r[t] * mult;
+      const double qv = rint(y);
+      r[t] = y - qv;
+      w[t >> 2] |= ((uint32_t)(int)qv & 0xFFu) << (8 * (t & 3));
+    }
+    o[sl] = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+}
+
+// rows of X (complex, n per row) -> int8 planes out[sl][orow][kpad], k = 2g + c.
+// mode 0: orow = r: (re, im).  mode 1: orow = 2r: (re, im), 2r+1: (im, -re).  mode 2: orow = 2r: (re, -im), 2r+1: (im, re).
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice(const double2* __restrict__ X, long long ldx, long long n, const int* __restrict__ e, int8_t* __restrict__ out,
+           long long kpad, long long slice_stride, int mode) {
+  const long long g0 = ((long long)blockIdx.x * 128 + threadIdx.x) * 8;
+  if (g0 * 2 >= kpad) return;
+  const int r = blockIdx.y;
+  const int ex = -e[r];
+  double a[16], b2[16];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    double2 v = make_double2(0.0, 0.0);
+    if (g0 + t < n) v = X[(size_t)r * ldx + g0 + t];
+    const double re = scalbn(v.x, ex), im = scalbn(v.y, ex);
+    if (mode == 2) {
+      a[2 * t] = re, a[2 * t + 1] = -im;
+      b2[2 * t] = im, b2[2 * t + 1] = re;
+    } else {
+      a[2 * t] = re, a[2 * t + 1] = im;
+      b2[2 * t] = im, b2[2 * t + 1] = -re;
+    }
+  }
+  uint4 o[S];
+  slice16<S>(a, o);
+  const long long orow = mode == 0 ? r : 2LL * r;
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)orow * kpad + 2 * g0) = o[sl];
+  if (mode != 0) {
+    slice16<S>(b2, o);
+#pragma unroll
+    for (int sl = 0; sl < S; ++sl)
+      *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)(orow + 1) * kpad + 2 * g0) = o[sl];
+  }
+}
+
+// transpose-and-slice: X[rows = p][ldx] -> out[sl][g][kpad], k = 2p + c, row g scaled by 2^-e[g]; 8 rows p per thread
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice_t(const double2* __restrict__ X, long long ldx, int rows, long long n, const int* __restrict__ e,
+             int8_t* __restrict__ out, long long kpad, long long slice_stride) {
+  const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (g >= n) return;
+  const int p0 = blockIdx.y * 8;
+  const int ex = -e[g];
+  double a[16];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    double2 v = make_double2(0.0, 0.0);
+    if (p0 + t < rows) v = X[(size_t)(p0 + t) * ldx + g];
+    a[2 * t] = scalbn(v.x, ex);
+    a[2 * t + 1] = scalbn(v.y, ex);
+  }
+  uint4 o[S];
+  slice16<S>(a, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)g * kpad + 2 * p0) = o[sl];
+}
+
+}  // namespace oz
+}  // namespace qehpsi
