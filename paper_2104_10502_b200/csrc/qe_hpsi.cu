@@ -18,6 +18,7 @@
 #include "fft3p_kernels.cuh"
 #include "fft2t_kernels.cuh"
 #include "zgemm_kernels.cuh"
+#include "ozaki_kernels.cuh"
 
 using namespace qehpsi;
 
@@ -91,6 +92,14 @@ struct qe_hpsi_handle {
   int nsplit = 1, kchunk = 0;
   int zg_variant = 0;
   double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
+  // projector contractions on tcgen05 int8 slices (ozaki_kernels.cuh): oz_s = slices per FP64 operand, 0 = FP64 DMMA path
+  int oz_s = 0, oz_stages = 0, oz_nsplit = 1, oz_kchunk = 0;
+  size_t oz_smem = 0;
+  long long oz_k1 = 0, oz_k2 = 0;  // padded real K of a6 (2 npw) and a8 (2 nproj), bytes per int8 row
+  int8_t *oz_a1 = nullptr, *oz_a2 = nullptr, *oz_b = nullptr;  // [S][nproj][k1], [S][npw][k2], [S][2 max_batch][max(k1,k2)]
+  int *oz_ep = nullptr, *oz_eg = nullptr, *oz_eb = nullptr;     // exponents: per projector, per plane wave, per band
+  double2* oz_partial = nullptr;
+  CUtensorMap oz_tm_a1{}, oz_tm_a2{}, oz_tm_b1{}, oz_tm_b2{};
   // NEXT-2: overlap operator S (q blocks packed like D; qbecp/qbT mirror dbecp/dbT)
   long long d_total = 0;
   double* qpk = nullptr;
@@ -585,6 +594,13 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->qbecp);
   cudaFree(h->qbT);
   cudaFree(h->ovl_partial);
+  cudaFree(h->oz_a1);
+  cudaFree(h->oz_a2);
+  cudaFree(h->oz_b);
+  cudaFree(h->oz_ep);
+  cudaFree(h->oz_eg);
+  cudaFree(h->oz_eb);
+  cudaFree(h->oz_partial);
   for (int i = 0; i < 2; ++i) {
     cudaFree(h->hbuf_psi[i]);
     cudaFree(h->hbuf_h[i]);
@@ -637,6 +653,124 @@ void choose_split(qe_hpsi_handle* h) {
   if (kchunk < ZG_BK) kchunk = ZG_BK;
   h->kchunk = kchunk;
   h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+}
+
+// ---- projector contractions on tcgen05 int8 slices (ozaki_kernels.cuh) --------------------------
+long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+
+// int8 planes [S][rows][kpad] as a 3-D tensor map (K bytes, rows, slice), SWIZZLE_64B boxes of box_rows x 64 bytes
+bool oz_make_map(CUtensorMap* tm, void* base, long long kpad, long long rows, int S, long long slice_stride, int box_rows) {
+  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn enc = nullptr;
+  if (!enc) {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      enc = nullptr;
+  }
+  if (!enc) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)kpad, (cuuint64_t)rows, (cuuint64_t)S};
+  cuuint64_t strides[2] = {(cuuint64_t)kpad, (cuuint64_t)slice_stride};
+  cuuint32_t box[3] = {(cuuint32_t)oz::KB, (cuuint32_t)box_rows, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int S>
+cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(oz::k_oz_gemm<S, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(oz::k_oz_gemm<S, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem);
+  if (e != cudaSuccess) return e;
+  const long long k1 = h->oz_k1, k2 = h->oz_k2;
+  // a6 operand: rows p scaled by 2^-ep[p]; a8 operand: rows g scaled by 2^-eg[g] (transposed beta)
+  oz::k_oz_rowexp<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep);
+  oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
+                                                                                    k1, (long long)h->nproj * k1, 0);
+  oz::k_oz_colexp<<<(unsigned)((h->npw + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg);
+  oz::k_oz_slice_t<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
+      h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, (long long)h->npw * k2);
+  return cudaGetLastError();
+}
+
+// a6 on int8 slices: exponents + slices of psi, then the level GEMM into oz_partial[split][nproj][ldc]
+template <int S>
+void oz_becp_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
+  const long long k1 = h->oz_k1;
+  oz::k_oz_rowexp<<<nb, 256, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb);
+  oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), nb), 128, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb, h->oz_b, k1,
+                                                                             2LL * h->max_batch * k1, 1);
+  oz::k_oz_gemm<S, 0><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit), oz::NT, h->oz_smem, st>>>(
+      h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(k1 / oz::KB), h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb, h->oz_partial,
+      h->ldc, (long long)h->nproj * h->ldc);
+}
+// a8 on int8 slices: hpsi[b][g] += sum_p beta[p][g] bT[b][p]
+template <int S>
+void oz_vnl_t(qe_hpsi_handle* h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const long long k2 = h->oz_k2;
+  oz::k_oz_rowexp<<<nb, 256, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb);
+  oz::k_oz_slice<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
+                                                                             2LL * h->max_batch * k2, 2);
+  oz::k_oz_gemm<S, 1><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
+      h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, (int)(k2 / oz::KB), (int)(k2 / oz::KB), h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0);
+}
+#define OZ_DISPATCH(S_, CALL)            \
+  switch (S_) {                          \
+    case 5: CALL(5); break;              \
+    case 6: CALL(6); break;              \
+    case 8: CALL(8); break;              \
+    default: CALL(7); break;             \
+  }
+
+// plan + operand slices for the int8 path; leaves h->oz_s = 0 (FP64 DMMA path) when the device or a resource says no
+cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
+  int S = env_int("QE_HPSI_OZAKI", 7);
+  if (S <= 0 || h->gamma || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
+  S = std::min(std::max(S, 5), 8);
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDeviceProperties(&prop, h->device);
+  if (e != cudaSuccess) return e;
+  if (prop.major != 10) return cudaSuccess;  // tcgen05 kind::i8 is an sm_100 feature
+  const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up(2LL * h->nproj, 128);
+  if ((long long)k2 > oz::max_k_per_cta(S)) return cudaSuccess;  // a8 runs unsplit: int32 level sums must not overflow
+  h->oz_k1 = k1;
+  h->oz_k2 = k2;
+  const int stage = S * (oz::A_BYTES + oz::B_BYTES);
+  h->oz_stages = std::min(oz::MAX_STAGES, (200 * 1024) / stage);
+  h->oz_smem = (size_t)h->oz_stages * stage;
+  // split-K of a6: K ranges short enough for exact int32 sums, and enough CTAs for two waves
+  const int nkb = (int)(k1 / oz::KB);
+  const long long tiles = (long long)((2 * max_batch + oz::BN - 1) / oz::BN) * ((h->nproj + oz::BM - 1) / oz::BM);
+  long long ns = (k1 + oz::max_k_per_cta(S) - 1) / oz::max_k_per_cta(S);
+  ns = std::max(ns, (2LL * h->num_sms + tiles - 1) / tiles);
+  ns = std::min<long long>(ns, std::max(1, nkb / 8));
+  ns = std::max<long long>(ns, (k1 + oz::max_k_per_cta(S) - 1) / oz::max_k_per_cta(S));
+  h->oz_kchunk = (int)((nkb + ns - 1) / ns);
+  h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
+  const size_t a1 = (size_t)S * h->nproj * k1, a2 = (size_t)S * h->npw * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
+  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit;
+  if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
+      (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
+      (e = cudaMalloc(&h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
+      (e = cudaMalloc(&h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
+      (e = cudaMalloc(&h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess)
+    return e;
+  if ((e = cudaMemsetAsync(h->oz_b, 0, bb, st)) != cudaSuccess) return e;
+  if (!oz_make_map(&h->oz_tm_a1, h->oz_a1, k1, h->nproj, S, (long long)h->nproj * k1, oz::BM) ||
+      !oz_make_map(&h->oz_tm_a2, h->oz_a2, k2, h->npw, S, (long long)h->npw * k2, oz::BM) ||
+      !oz_make_map(&h->oz_tm_b1, h->oz_b, k1, 2LL * max_batch, S, 2LL * max_batch * k1, oz::BN) ||
+      !oz_make_map(&h->oz_tm_b2, h->oz_b, k2, 2LL * max_batch, S, 2LL * max_batch * k2, oz::BN))
+    return cudaErrorNotSupported;
+#define OZ_CALL(S_) e = oz_prepare_t<S_>(h, st)
+  OZ_DISPATCH(S, OZ_CALL)
+#undef OZ_CALL
+  if (e != cudaSuccess) return e;
+  h->oz_s = S;
+  h->workspace_bytes += a1 + a2 + bb + pc;
+  return cudaSuccess;
 }
 
 // nonlocal state of a handle whose npw is already set (K dimension of a6 / M dimension of a8): beta (copied or
@@ -698,6 +832,7 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
     CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
     CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
     h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
+    if (!(flags & QE_HPSI_FP64_DMMA)) CR_TRY(setup_ozaki(h, max_batch, st));
   #undef CR_TRY
   return cudaSuccess;
 }
@@ -1078,7 +1213,11 @@ void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, in
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const size_t t0 = prof_mark(h, st);
-  if (h->gamma) {
+  if (h->oz_s) {
+#define OZ_CALL(S_) oz_becp_t<S_>(h, psi, ldpsi, nb, st)
+    OZ_DISPATCH(h->oz_s, OZ_CALL)
+#undef OZ_CALL
+  } else if (h->gamma) {
     using Cfg = ZgV0;
     const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
     k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
@@ -1099,7 +1238,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->beta, h->ldbeta, psi, ldpsi,
                                             h->becp);
   else
-    k_becp_reduce<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->becp);
+    k_becp_reduce<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
+                                      h->becp);
   k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
                             h->dbT, h->ldp);
   prof_span(h, t1, prof_mark(h, st), SLOT_DMUL);
@@ -1110,7 +1250,11 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 
 // a8
 int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
-  if (h->gamma) {
+  if (h->oz_s) {
+#define OZ_CALL(S_) oz_vnl_t<S_>(h, bT, hpsi, ldh, nb, st)
+    OZ_DISPATCH(h->oz_s, OZ_CALL)
+#undef OZ_CALL
+  } else if (h->gamma) {
     using Cfg = ZgV0;
     const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
     if (mt > 0)
@@ -1728,7 +1872,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += 4;
+    if (h->nproj > 0) total += h->oz_s ? 8 : 4;
   }
   return total;
 }
@@ -1750,6 +1894,8 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[10] = h->x_split;
   info[11] = h->num_sms;
   info[12] = h->f2p[0] ? 1 : 0;
+  info[13] = h->oz_s;
+  info[14] = h->oz_nsplit;
   return QE_HPSI_OK;
 }
 

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_PKG, "libqe_hpsi.so")
 QE_HPSI_OK, QE_HPSI_EINVAL, QE_HPSI_EGRID, QE_HPSI_ENOMEM, QE_HPSI_ECUDA, QE_HPSI_ESTATE = 0, -1, -2, -3, -4, -5
 QE_HPSI_BORROW_BETA = 1
 QE_HPSI_GENERIC_FFT = 2
+QE_HPSI_FP64_DMMA = 4
 QE_HPSI_MAX_N = 720
 
 _c = ctypes
@@ -304,7 +305,7 @@ class Hpsi:
         buf = (_c.c_int64 * 16)()
         _check(self._lib.qe_hpsi_info(self._h, buf), self._h)
         keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
-                "x_split", "num_sms"]
+                "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit"]
         return {k: int(buf[i]) for i, k in enumerate(keys)}
 
     PROFILE_SLOTS = ["a6_becp", "a7_reduce_dmul", "a1_a5_fft_chain", "a8_vnl_add", "a1_scatter_zinv", "a2_yinv",

@@ -1,0 +1,113 @@
+"""GPU parity of the int8-slice projector path (csrc/ozaki_kernels.cuh): a6 / a8 computed exactly on
+the int8 tensor cores from S 7-bit slices of the FP64 operands.  The oracle is oracle/hpsi_oracle.py (becp_of, vnl_psi); the
+FP64 DMMA path (flag QE_HPSI_FP64_DMMA) is a second, independent implementation of the same rows."""
+from __future__ import annotations
+
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import hpsi_oracle as orc
+from paper_2104_10502_b200 import qe_hpsi
+from tests import _gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _nonlocal(h, inp, nb):
+    psi = _gpu.gen_psi_dev(inp, 0, nb)
+    out = h.nonlocal_add(psi, torch.zeros_like(psi))
+    becp, _ = h.becp(nb)
+    torch.cuda.synchronize()
+    return psi, out, becp
+
+
+def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
+    h, _ = _gpu.make(0)
+    assert h.info()["ozaki_slices"] == 7 and h.info()["ozaki_nsplit"] >= 1
+    h.destroy()
+    h, _ = _gpu.make(0, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
+    assert h.info()["ozaki_slices"] == 0
+    h.destroy()
+
+
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
+def test_becp_and_vnl_against_oracle(cfg):
+    h, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    npw = h.npw
+    psi, out, becp = _nonlocal(h, inp, wl.nbands)
+    ph = psi[:, :npw].cpu().numpy()
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    bref = orc.becp_of(beta, ph)
+    # error law of the split: (S+1) 2^-7S K max|beta_p| max|psi_b| per entry, S = 7 -> ~1e-14 K-independent in practice
+    assert np.abs(becp.cpu().numpy() - bref).max() <= 1e-13 * max(1.0, np.abs(bref).max())
+    vref = orc.vnl_psi(beta, inp["dblocks"], ph)
+    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], vref).max() <= 1e-12
+    h.destroy()
+
+
+def test_int8_path_agrees_with_the_fp64_tensor_path_on_config_1():
+    h, inp = _gpu.make(1)
+    _, out, becp = _nonlocal(h, inp, 128)
+    h.destroy()
+    h2, inp2 = _gpu.make(1, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
+    _, out2, becp2 = _nonlocal(h2, inp2, 128)
+    h2.destroy()
+    assert float((becp - becp2).abs().max()) <= 2e-12 * float(becp2.abs().max())
+    num = torch.linalg.vector_norm(out - out2, dim=1)
+    den = torch.linalg.vector_norm(out2, dim=1)
+    assert float((num / den).max()) <= 1e-12
+
+
+@pytest.mark.parametrize("slices,tol", [(5, 1e-7), (6, 1e-9), (7, 1e-11), (8, 1e-13)])
+def test_error_falls_by_2_to_the_7_per_slice(slices, tol):
+    """Each extra slice adds 7 bits: the measured error must respect the law (and S = 5 must be visibly worse than S = 8,
+    i.e. the slices are really what is being multiplied)."""
+    os.environ["QE_HPSI_OZAKI"] = str(slices)
+    try:
+        h, inp = _gpu.make(0)
+    finally:
+        del os.environ["QE_HPSI_OZAKI"]
+    assert h.info()["ozaki_slices"] == slices
+    wl = inp["wl"]
+    npw = h.npw
+    psi, out, _ = _nonlocal(h, inp, wl.nbands)
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
+    err = _gpu.rel_l2(out.cpu().numpy()[:, :npw], vref).max()
+    assert err <= tol, err
+    if slices == 5:
+        assert err >= 1e-12, err
+    h.destroy()
+
+
+def test_bits_do_not_depend_on_batch_composition_or_run():
+    h, inp = _gpu.make(1, max_batch=48)
+    psi = _gpu.gen_psi_dev(inp, 0, 100)  # chunks 48, 48, 4
+    a = h.apply(psi).clone()
+    b = h.apply(psi).clone()
+    one = h.apply(psi[77:78].contiguous()).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(a.view(torch.float64), b.view(torch.float64))
+    assert torch.equal(a[77].view(torch.float64), one[0].view(torch.float64))
+    h.destroy()
+
+
+def test_zero_band_and_huge_dynamic_range():
+    h, inp = _gpu.make("T1_general_k")
+    wl = inp["wl"]
+    npw = h.npw
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    psi[0] = 0  # all-zero band: exponent 0, slices 0
+    psi[1, :npw] *= torch.logspace(0, -30, npw, dtype=torch.float64, device="cuda")  # entries far below 2^-49 of the row maximum
+    out = h.nonlocal_add(psi, torch.zeros_like(psi))
+    torch.cuda.synchronize()
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
+    got = out.cpu().numpy()[:, :npw]
+    assert np.all(got[0] == 0)
+    assert _gpu.rel_l2(got[1:], vref[1:]).max() <= 1e-12
+    h.destroy()

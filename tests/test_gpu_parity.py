@@ -33,7 +33,7 @@ def test_maps_bit_exact(cfg):
     h.destroy()
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT])
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA])
 @pytest.mark.parametrize("cfg", TINY + [0])
 def test_small_cases_against_dense_h(cfg, flags):
     """Level A (dense H from the definition) on every tiny case and config 0; both radix plans."""
@@ -110,8 +110,9 @@ def test_batch_composition_and_chunking_do_not_change_bits():
     h.destroy()
 
 
-def test_config1_all_bands():
-    h, inp = _gpu.make(1)
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_FP64_DMMA])
+def test_config1_all_bands(flags):
+    h, inp = _gpu.make(1, flags=flags)
     wl = inp["wl"]
     sp = _gpu.oracle_sphere(wl)
     psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
@@ -132,12 +133,12 @@ def test_config1_all_bands():
     h.destroy()
 
 
-@pytest.mark.parametrize("cfg", [2, 3, 4])
-def test_full_size_sampled_bands(cfg):
+@pytest.mark.parametrize("cfg,flags", [(2, 0), (3, 0), (4, 0), (4, qe_hpsi.QE_HPSI_FP64_DMMA)])
+def test_full_size_sampled_bands(cfg, flags):
     """BASELINE.json's full sizes in the launch configuration bench.py times (batch = wl.batch, beta borrowed):
     Level B oracle on sampled bands + a Hermitian probe <phi|H psi_b> = <H phi|psi_b> covering every band of the
     batch at the cost of one extra oracle application."""
-    h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
+    h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA | flags)
     wl = inp["wl"]
     sp = _gpu.oracle_sphere(wl)
     npw = h.npw
