@@ -42,6 +42,8 @@ def parse():
     ap.add_argument("--detail", action="store_true", help="extra pass with per-FFT-kernel events (stderr table)")
     ap.add_argument("--graph", type=int, default=-1, help="replay the step from a CUDA graph: 1 on, 0 off, -1 (default) only "
                     "for launch-latency-bound workloads (a step under 0.5 ms); stage timers are taken in a separate eager pass")
+    ap.add_argument("--dmma", action="store_true", help="projector contractions on the FP64 tensor pipe (create flag "
+                    "QE_HPSI_FP64_DMMA) instead of the default int8 digit path")
     ap.add_argument("--next", action="store_true", help="also time the SURVEY 8(f) rows (apply_hs, overlap, density): "
                     "adds a next_rows object to the JSON line")
     return ap.parse_args()
@@ -297,7 +299,7 @@ def main():
 
     # ---- inputs, resident in HBM ---------------------------------------------------------------------
     t_setup = time.perf_counter()
-    h, inp = qe_hpsi.from_workload(wl, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
+    h, inp = qe_hpsi.from_workload(wl, flags=qe_hpsi.QE_HPSI_BORROW_BETA | (qe_hpsi.QE_HPSI_FP64_DMMA if args.dmma else 0))
     info = h.info()
     npw, ld = h.npw, inp["ld"]
     nb, batch = wl.nbands, wl.batch
@@ -414,7 +416,33 @@ def main():
     t_becp, t_vnl, t_fft = stage["a6_becp"][0], stage["a8_vnl_add"][0], stage["a1_a5_fft_chain"][0]
     flops_launch = 8.0 * wl.nproj * npw * min(batch, nb)  # per ZGEMM launch (one chunk)
     roof_t = max((m["b_fft"] + m["b_beta"]) / (hbm_peak * 1e9), m["f_proj"] / (dmma * 1e12))  # s per band
-    if wl.nproj and t_vnl + t_becp > t_fft:
+    oz_s = info.get("ozaki_slices", 0)
+    int8 = None
+    if wl.nproj and oz_s and t_vnl + t_becp > t_fft:
+        # projector contractions on the int8 tensor cores: S (S+1) / 2 digit-pair products per real product, each exact
+        pairs = oz_s * (oz_s + 1) // 2
+        kname, t_k = ("k_oz_gemm<S,1> (a8)", t_vnl) if t_vnl >= t_becp else ("k_oz_gemm<S,0> (a6)", t_becp)
+        ops_launch = pairs * flops_launch  # 4 real MACs per complex MAC x 2 ops x pairs
+        ach = ops_launch / (t_k * 1e-3) * 1e-12
+        bf16_sus = float(mp.get("bf16_tflops_sustained", 0.0)) or 1414.0
+        peak = 2.0 * bf16_sus
+        t_slice = stage["a6_a8_int8_digits"][0]
+        roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
+                    "traffic": committed_traffic(args.config, "k_oz_gemm"),
+                    "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; "
+                    "the kernel runs inside a long step); a register-free UTCIMMA loop on the same chip measured 4540 TOP/s "
+                    "(profiles/r1g_int8.md)", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
+                    "digit_pairs": pairs, "fp64_equivalent_tflops": flops_launch / (t_k * 1e-3) * 1e-12,
+                    "vs_fp64_dmma_peak": flops_launch / (t_k * 1e-3) * 1e-12 / dmma,
+                    "digit_kernels_ms_per_launch": t_slice,
+                    "note": "achieved = executed int8 ops of the S-digit split (every one of them is needed for the FP64 result); "
+                            "fp64_equivalent_tflops = 8 flops per complex MAC / time, comparable with the FP64 DMMA peak"}
+        t_int8 = pairs * m["f_proj"] / (peak * 1e12)
+        b_beta8 = 2.0 * oz_s * 2 * wl.nproj * npw / wl.batch  # int8 digit planes of beta, streamed once by a6 and once by a8
+        roof8 = max((m["b_fft"] + b_beta8) / (hbm_peak * 1e9), t_int8)
+        int8 = {"bands_per_s": 1.0 / roof8, "frac": value / world * roof8, "int8_tops": peak, "bytes_per_band": m["b_fft"] + b_beta8,
+                "int8_ops_per_band": pairs * m["f_proj"], "note": "max(bytes/HBM, digit-pair int8 ops/int8 tensor peak) per band"}
+    elif wl.nproj and t_vnl + t_becp > t_fft:
         kname, t_k = ("k_vnl_add", t_vnl) if t_vnl >= t_becp else ("k_becp", t_becp)
         ach = flops_launch / (t_k * 1e-3) * 1e-12
         roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
@@ -434,7 +462,8 @@ def main():
               "per": f"chunk of {min(batch, nb)} bands", "chunks_per_step": chunks_per_step,
               "becp_tflops": flops_launch / (t_becp * 1e-3) * 1e-12 if t_becp else None,
               "vnl_tflops": flops_launch / (t_vnl * 1e-3) * 1e-12 if t_vnl else None,
-              "fft_algorithmic_gbs": m["b_fft"] * min(batch, nb) / (t_fft * 1e-3) * 1e-9 if t_fft else None}
+              "fft_algorithmic_gbs": m["b_fft"] * min(batch, nb) / (t_fft * 1e-3) * 1e-9 if t_fft else None,
+              "int8_digit_kernels_ms": stage["a6_a8_int8_digits"][0] * 2 if oz_s else None}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -445,7 +474,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": wl.name, "nbands": nb, "batch": batch, "grid": list(wl.nr), "npw": npw, "nproj": wl.nproj,
-                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["nsplit"], "cuda_graph": bool(use_graph),
+                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["ozaki_nsplit"] if info.get("ozaki_slices") else info["nsplit"], "projector_path": f"int8 digits x{info['ozaki_slices']} (tcgen05)" if info.get("ozaki_slices") else "fp64 dmma (3M)", "cuda_graph": bool(use_graph),
                        "l2": "inputs per step exceed L2" if flush is None else "L2 flushed (256 MB write) between steps",
                        "sharding": "bands / k-point pools per rank, no collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": h.launch_count(batch) * chunks_per_step * args.steps if nb % batch == 0
@@ -455,6 +484,9 @@ def main():
                                   "fp64_tensor_tflops": dmma, "fp64_dfma_tflops": dfma, "bytes_per_band": m["b_fft"] + m["b_beta"],
                                   "proj_flops_per_band": m["f_proj"], "note": "max(bytes/HBM, projector flops/FP64 tensor) per band"},
             "stages": stages, "cpu_baseline": cpu, "setup_s": t_setup}
+    if int8 is not None:
+        line["combined_roofline_int8"] = int8
+        line["dtype"] = f"f64 (projector contractions: exact int8 digit products, {oz_s} digits per operand)"
     if args.next:
         torch.cuda.profiler.start()  # the next-rows pass is visible to `ncu --profile-from-start off` too
         line["next_rows"] = time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak)

@@ -52,11 +52,13 @@ typedef enum {
 #define QE_HPSI_BORROW_BETA 1u   /* use beta_dev in place (caller keeps it alive and unchanged) instead of copying */
 #define QE_HPSI_GENERIC_FFT 2u   /* (testing) use only radices 2,3,4,5 in the FFT passes                           */
 #define QE_HPSI_FP64_DMMA   4u   /* projector contractions a6 / a8 on the FP64 tensor pipe (mma.sync DMMA, 3M product) */
-                                 /* instead of the default: error-free 7-bit slices of the FP64 operands multiplied  */
-                                 /* exactly on the int8 tensor cores (tcgen05, int32 sums in TMEM), S = 7 slices:    */
-                                 /* |error| <= ~(S+1) 2^(-7S) K max|a| max|b| per contraction, 2^(-49) = 1.8e-15;    */
-                                 /* costs S/8 of the bytes of beta twice over (a K-major and a transposed copy).     */
-                                 /* Env QE_HPSI_OZAKI = 0 | 5..8 overrides the slice count (0 = same as this flag).  */
+                                 /* instead of the default: the FP64 operands are split error-free into S = 6 signed */
+                                 /* 8-bit digits (per-row exponent) whose products are summed exactly on the int8    */
+                                 /* tensor cores (tcgen05, int32 level sums in TMEM) and recombined in FP64:         */
+                                 /* |error| <= ~(S+1) 2^(-8S+1) K max|a| max|b| per contraction (2^-47 = 7e-15);     */
+                                 /* costs 2 S bytes per complex entry of beta, twice (K-major and transposed planes).*/
+                                 /* Env QE_HPSI_OZAKI = 0 | 4..7 overrides the digit count (0 = same as this flag).  */
+                                 /* Non-finite operands are not propagated by the int8 path (use this flag for them). */
 
 #define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */
 

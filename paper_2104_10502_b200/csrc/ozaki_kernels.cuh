@@ -1,9 +1,10 @@
 // Projector contractions a6 / a8 on the 5th-generation tensor cores (tcgen05, kind::i8, s32 accumulators in TMEM) through an
-// error-free split of the FP64 operands into signed 7-bit slices (the "Ozaki scheme"): SURVEY.md section 8(a) rows a6 and a8,
-// DESIGN.md section 5.6.  tcgen05 has no f64 kind; int8 x int8 -> int32 products are exact, so
+// error-free split of the FP64 operands into signed 8-bit digits (the "Ozaki scheme"): SURVEY.md section 8(a) rows a6 and a8,
+// DESIGN.md section 5.6.  tcgen05 has no f64 kind; int8 x int8 -> int32 products are exact, so with the balanced radix-256
+// digits x_i in [-128, 127] of X = rint(x 2^(8S-1-e)) (e = exponent of the row maximum, |x| 2^-e <= 0.99, so |x_0| <= 127)
 //
-//   x = 2^e * sum_{i<S} x_i 2^-(6+7i) + O(2^(e-7S)),  x_i in [-64, 64]        (e = exponent of the row maximum)
-//   sum_k a_k b_k = 2^(ea+eb-12) * sum_{L<S} 2^-7L * sum_{i+j=L} sum_k a_ik b_jk   + O((S+1) 2^-7S |a|max |b|max K)
+//   x = 2^e * sum_{i<S} x_i 2^-(7+8i) + O(2^(e-8S)),
+//   sum_k a_k b_k = 2^(ea+eb-14) * sum_{L<S} 2^-8L * sum_{i+j=L} sum_k a_ik b_jk   + O((S+1) 2^(-8S+1) |a|max |b|max K)
 //
 // Both contractions are brought to the one form D[m][n] = sum_k A[m][k] B[n][k] over REAL k (a complex number is two
 // consecutive reals), A and B stored as S planes of int8, K contiguous:
@@ -24,8 +25,8 @@ namespace oz {
 constexpr int BM = 128, BN = 64, KB = 64, NT = 192;
 constexpr int A_BYTES = BM * KB, B_BYTES = BN * KB;
 constexpr int MAX_STAGES = 4;
-// (L+1) * Kc * 64 * 64 < 2^31 for every level L < S: Kc <= 2^19 / S reals per CTA
-__host__ __device__ constexpr long long max_k_per_cta(int S) { return ((1LL << 19) / S) / KB * KB - KB; }
+// (L+1) * Kc * 128 * 128 < 2^31 for every level L < S: Kc <= 2^17 / S reals per CTA
+__host__ __device__ constexpr long long max_k_per_cta(int S) { return ((1LL << 17) / S) / KB * KB - KB; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t n) {
@@ -160,7 +161,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
         for (int L = S - 1; L >= 0; --L) {  // smallest contributions first
-          const double w = 1.0 / (double)(1ULL << (7 * L));
+          const double w = 1.0 / (double)(1ULL << (8 * L));
 #pragma unroll
           for (int j = 0; j < 8; ++j) d[j] = fma((double)(int)v[L][j], w, d[j]);
         }
@@ -170,7 +171,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         for (int jj = 0; jj < 4; ++jj) {
           const int b = (q * BN + n0) / 2 + jj;
           if (b < nb) {
-            const int ex = em + eb[b] - 12;
+            const int ex = em + eb[b] - 14;
             const double re = scalbn(d[2 * jj], ex), im = scalbn(d[2 * jj + 1], ex);
             if (MODE == 0) {
               out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(re, im);
@@ -194,8 +195,13 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   }
 }
 
-// ---- exponents: e = ilogb(max |component|) + 1 (0 for an all-zero row), so that |x| 2^-e < 1 ----
-__device__ __forceinline__ int exp_of(double mx) { return mx > 0.0 ? ilogb(mx) + 1 : 0; }
+// ---- exponents: smallest e with max |component| 2^-e <= 0.99 (0 for an all-zero row): the leading digit then fits an int8 ----
+__device__ __forceinline__ int exp_of(double mx) {
+  if (!(mx > 0.0)) return 0;
+  int e = ilogb(mx) + 1;
+  if (scalbn(mx, -e) > 0.99) ++e;
+  return e;
+}
 
 // one CTA per row of a complex matrix X[rows][ldx], n entries per row
 __global__ void __launch_bounds__(256) k_oz_rowexp(const double2* __restrict__ X, long long ldx, long long n, int* __restrict__ e) {
@@ -226,22 +232,26 @@ __global__ void __launch_bounds__(128) k_oz_colexp(const double2* __restrict__ X
   e[g] = exp_of(mx);
 }
 
-// 16 reals -> S x 16 int8 (one 16-byte store per slice); r[] already scaled to (-1, 1)
+// 16 reals -> S x 16 int8 (one 16-byte store per slice); r[] already scaled to [-0.99, 0.99].  Balanced radix-256 digits of the
+// integer X = rint(r 2^(8S-1)), least significant first: d = ((X + 128) mod 256) - 128, X <- (X - d) / 256.  Exact for S <= 7.
 template <int S>
 __device__ __forceinline__ void slice16(double (&r)[16], uint4 (&o)[S]) {
+  static_assert(S >= 2 && S <= 7, "8S-1 bits must fit an int64");
+  uint32_t w[S][4];
 #pragma unroll
-  for (int sl = 0; sl < S; ++sl) {
-    const double mult = sl == 0 ? 64.0 : 128.0;
-    uint32_t w[4] = {0, 0, 0, 0};
+  for (int sl = 0; sl < S; ++sl) w[sl][0] = w[sl][1] = w[sl][2] = w[sl][3] = 0u;
 #pragma unroll
-    for (int t = 0; t < 16; ++t) {
-      const double y = r[t] * mult;
-      const double qv = rint(y);
-      r[t] = y - qv;
-      w[t >> 2] |= ((uint32_t)(int)qv & 0xFFu) << (8 * (t & 3));
+  for (int t = 0; t < 16; ++t) {
+    long long X = __double2ll_rn(r[t] * (double)(1ULL << (8 * S - 1)));
+#pragma unroll
+    for (int sl = S - 1; sl >= 0; --sl) {
+      const long long d = ((X + 128) & 255) - 128;
+      X = (X - d) >> 8;
+      w[sl][t >> 2] |= ((uint32_t)d & 0xFFu) << (8 * (t & 3));
     }
-    o[sl] = make_uint4(w[0], w[1], w[2], w[3]);
   }
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) o[sl] = make_uint4(w[sl][0], w[sl][1], w[sl][2], w[sl][3]);
 }
 
 // rows of X (complex, n per row) -> int8 planes out[sl][orow][kpad], k = 2g + c.

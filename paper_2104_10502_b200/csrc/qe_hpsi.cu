@@ -150,7 +150,8 @@ namespace {
 int g_last_cuda = 0;
 
 // ---- stage timing helpers ---------------------------------------------------------------------------------
-enum { SLOT_BECP = 0, SLOT_DMUL = 1, SLOT_FFT = 2, SLOT_VNL = 3, SLOT_A1 = 4, SLOT_A2 = 5, SLOT_A3 = 6, SLOT_A4 = 7, SLOT_A5 = 8 };
+enum { SLOT_BECP = 0, SLOT_DMUL = 1, SLOT_FFT = 2, SLOT_VNL = 3, SLOT_A1 = 4, SLOT_A2 = 5, SLOT_A3 = 6, SLOT_A4 = 7, SLOT_A5 = 8,
+       SLOT_OZ_SLICE = 9 };
 
 void prof_drain(qe_hpsi_handle* h) {
   if (h->prof_spans.empty()) {
@@ -696,40 +697,47 @@ cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-// a6 on int8 slices: exponents + slices of psi, then the level GEMM into oz_partial[split][nproj][ldc]
+// a6 on int8 slices: exponents + digits of psi (oz_becp_slice_t), then the level GEMM into oz_partial[split][nproj][ldc]
 template <int S>
-void oz_becp_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
+void oz_becp_slice_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const long long k1 = h->oz_k1;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb);
   oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), nb), 128, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb, h->oz_b, k1,
                                                                              2LL * h->max_batch * k1, 1);
+}
+template <int S>
+void oz_becp_gemm_t(qe_hpsi_handle* h, int nb, cudaStream_t st) {
   oz::k_oz_gemm<S, 0><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit), oz::NT, h->oz_smem, st>>>(
-      h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(k1 / oz::KB), h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb, h->oz_partial,
-      h->ldc, (long long)h->nproj * h->ldc);
+      h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb,
+      h->oz_partial, h->ldc, (long long)h->nproj * h->ldc);
 }
 // a8 on int8 slices: hpsi[b][g] += sum_p beta[p][g] bT[b][p]
 template <int S>
-void oz_vnl_t(qe_hpsi_handle* h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+void oz_vnl_slice_t(qe_hpsi_handle* h, const double2* bT, int nb, cudaStream_t st) {
   const long long k2 = h->oz_k2;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb);
   oz::k_oz_slice<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
                                                                              2LL * h->max_batch * k2, 2);
+}
+template <int S>
+void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const int nkb = (int)(h->oz_k2 / oz::KB);
   oz::k_oz_gemm<S, 1><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
-      h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, (int)(k2 / oz::KB), (int)(k2 / oz::KB), h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0);
+      h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, nkb, h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0);
 }
 #define OZ_DISPATCH(S_, CALL)            \
   switch (S_) {                          \
+    case 4: CALL(4); break;              \
     case 5: CALL(5); break;              \
-    case 6: CALL(6); break;              \
-    case 8: CALL(8); break;              \
-    default: CALL(7); break;             \
+    case 7: CALL(7); break;              \
+    default: CALL(6); break;             \
   }
 
 // plan + operand slices for the int8 path; leaves h->oz_s = 0 (FP64 DMMA path) when the device or a resource says no
 cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
-  int S = env_int("QE_HPSI_OZAKI", 7);
+  int S = env_int("QE_HPSI_OZAKI", 6);
   if (S <= 0 || h->gamma || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
-  S = std::min(std::max(S, 5), 8);
+  S = std::min(std::max(S, 4), 7);
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, h->device);
   if (e != cudaSuccess) return e;
@@ -739,7 +747,7 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   h->oz_k1 = k1;
   h->oz_k2 = k2;
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
-  h->oz_stages = std::min(oz::MAX_STAGES, (200 * 1024) / stage);
+  h->oz_stages = std::min(oz::MAX_STAGES, (222 * 1024) / stage);
   h->oz_smem = (size_t)h->oz_stages * stage;
   // split-K of a6: K ranges short enough for exact int32 sums, and enough CTAs for two waves
   const int nkb = (int)(k1 / oz::KB);
@@ -1213,8 +1221,14 @@ void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, in
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const size_t t0 = prof_mark(h, st);
+  size_t ts = t0;
   if (h->oz_s) {
-#define OZ_CALL(S_) oz_becp_t<S_>(h, psi, ldpsi, nb, st)
+#define OZ_CALL(S_) oz_becp_slice_t<S_>(h, psi, ldpsi, nb, st)
+    OZ_DISPATCH(h->oz_s, OZ_CALL)
+#undef OZ_CALL
+    ts = prof_mark(h, st);
+    prof_span(h, t0, ts, SLOT_OZ_SLICE);
+#define OZ_CALL(S_) oz_becp_gemm_t<S_>(h, nb, st)
     OZ_DISPATCH(h->oz_s, OZ_CALL)
 #undef OZ_CALL
   } else if (h->gamma) {
@@ -1232,7 +1246,7 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st); break;
   }
   const size_t t1 = prof_mark(h, st);
-  prof_span(h, t0, t1, SLOT_BECP);
+  prof_span(h, ts, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
   if (h->gamma)
     k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->beta, h->ldbeta, psi, ldpsi,
@@ -1251,9 +1265,16 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 // a8
 int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   if (h->oz_s) {
-#define OZ_CALL(S_) oz_vnl_t<S_>(h, bT, hpsi, ldh, nb, st)
+    const size_t t0 = prof_mark(h, st);
+#define OZ_CALL(S_) oz_vnl_slice_t<S_>(h, bT, nb, st)
     OZ_DISPATCH(h->oz_s, OZ_CALL)
 #undef OZ_CALL
+    const size_t ts = prof_mark(h, st);
+    prof_span(h, t0, ts, SLOT_OZ_SLICE);
+#define OZ_CALL(S_) oz_vnl_gemm_t<S_>(h, hpsi, ldh, nb, st)
+    OZ_DISPATCH(h->oz_s, OZ_CALL)
+#undef OZ_CALL
+    prof_span(h, ts, prof_mark(h, st), SLOT_VNL);
   } else if (h->gamma) {
     using Cfg = ZgV0;
     const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
@@ -1301,9 +1322,9 @@ int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi,
     if (h->prof_mode == 1) prof_span(h, t0, prof_mark(h, st), SLOT_FFT);
   }
   if (nl) {
-    const size_t t0 = prof_mark(h, st);
+    const size_t t0 = h->oz_s ? (size_t)-1 : prof_mark(h, st);  // the int8 path records its own spans (slices | GEMM)
     rc = launch_vnl_add(h, h->dbT, hpsi, ldh, nb, st);
-    prof_span(h, t0, prof_mark(h, st), SLOT_VNL);
+    if (!h->oz_s) prof_span(h, t0, prof_mark(h, st), SLOT_VNL);
   }
   return rc;
 }

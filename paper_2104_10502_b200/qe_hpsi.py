@@ -309,7 +309,7 @@ class Hpsi:
         return {k: int(buf[i]) for i, k in enumerate(keys)}
 
     PROFILE_SLOTS = ["a6_becp", "a7_reduce_dmul", "a1_a5_fft_chain", "a8_vnl_add", "a1_scatter_zinv", "a2_yinv",
-                     "a3_x_vmul", "a4_yfwd", "a5_zfwd_gather"]
+                     "a3_x_vmul", "a4_yfwd", "a5_zfwd_gather", "a6_a8_int8_digits"]
 
     def profile(self, mode: int):
         """qe_hpsi_profile: 0 off, 1 stage events, 2 per-FFT-kernel events. Resets the accumulators."""

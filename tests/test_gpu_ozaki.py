@@ -1,5 +1,5 @@
 """GPU parity of the int8-slice projector path (csrc/ozaki_kernels.cuh): a6 / a8 computed exactly on
-the int8 tensor cores from S 7-bit slices of the FP64 operands.  The oracle is oracle/hpsi_oracle.py (becp_of, vnl_psi); the
+the int8 tensor cores from S balanced 8-bit digits of the FP64 operands.  The oracle is oracle/hpsi_oracle.py (becp_of, vnl_psi); the
 FP64 DMMA path (flag QE_HPSI_FP64_DMMA) is a second, independent implementation of the same rows."""
 from __future__ import annotations
 
@@ -26,7 +26,7 @@ def _nonlocal(h, inp, nb):
 
 def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
     h, _ = _gpu.make(0)
-    assert h.info()["ozaki_slices"] == 7 and h.info()["ozaki_nsplit"] >= 1
+    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_nsplit"] >= 1
     h.destroy()
     h, _ = _gpu.make(0, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
     assert h.info()["ozaki_slices"] == 0
@@ -42,10 +42,11 @@ def test_becp_and_vnl_against_oracle(cfg):
     ph = psi[:, :npw].cpu().numpy()
     beta = inp["beta"][:, :npw].cpu().numpy()
     bref = orc.becp_of(beta, ph)
-    # error law of the split: (S+1) 2^-7S K max|beta_p| max|psi_b| per entry, S = 7 -> ~1e-14 K-independent in practice
-    assert np.abs(becp.cpu().numpy() - bref).max() <= 1e-13 * max(1.0, np.abs(bref).max())
+    # error law of the split: (S+1) 2^(-8S+2) K max|beta_p| max|psi_b| per entry, S = 6 -> ~1e-14 in practice
+    assert np.abs(becp.cpu().numpy() - bref).max() <= 5e-12 * np.abs(bref).max()
     vref = orc.vnl_psi(beta, inp["dblocks"], ph)
-    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], vref).max() <= 1e-12
+    # north_star's 1e-11 per band, demanded of the nonlocal part ALONE (it is ~1e-5 of |H psi| on these workloads)
+    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], vref).max() <= 1e-11
     h.destroy()
 
 
@@ -56,16 +57,16 @@ def test_int8_path_agrees_with_the_fp64_tensor_path_on_config_1():
     h2, inp2 = _gpu.make(1, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
     _, out2, becp2 = _nonlocal(h2, inp2, 128)
     h2.destroy()
-    assert float((becp - becp2).abs().max()) <= 2e-12 * float(becp2.abs().max())
+    assert float((becp - becp2).abs().max()) <= 5e-12 * float(becp2.abs().max())
     num = torch.linalg.vector_norm(out - out2, dim=1)
     den = torch.linalg.vector_norm(out2, dim=1)
-    assert float((num / den).max()) <= 1e-12
+    assert float((num / den).max()) <= 1e-11
 
 
-@pytest.mark.parametrize("slices,tol", [(5, 1e-7), (6, 1e-9), (7, 1e-11), (8, 1e-13)])
-def test_error_falls_by_2_to_the_7_per_slice(slices, tol):
-    """Each extra slice adds 7 bits: the measured error must respect the law (and S = 5 must be visibly worse than S = 8,
-    i.e. the slices are really what is being multiplied)."""
+@pytest.mark.parametrize("slices,tol", [(4, 2e-7), (5, 1e-9), (6, 1e-11), (7, 1e-13)])
+def test_error_falls_by_2_to_the_8_per_digit(slices, tol):
+    """Each extra digit adds 8 bits: the measured error must respect the law (and S = 4 must be visibly worse than S = 7,
+    i.e. the digits are really what is being multiplied)."""
     os.environ["QE_HPSI_OZAKI"] = str(slices)
     try:
         h, inp = _gpu.make(0)
@@ -79,7 +80,7 @@ def test_error_falls_by_2_to_the_7_per_slice(slices, tol):
     vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
     err = _gpu.rel_l2(out.cpu().numpy()[:, :npw], vref).max()
     assert err <= tol, err
-    if slices == 5:
+    if slices == 4:
         assert err >= 1e-12, err
     h.destroy()
 
@@ -102,12 +103,12 @@ def test_zero_band_and_huge_dynamic_range():
     npw = h.npw
     psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
     psi[0] = 0  # all-zero band: exponent 0, slices 0
-    psi[1, :npw] *= torch.logspace(0, -30, npw, dtype=torch.float64, device="cuda")  # entries far below 2^-49 of the row maximum
+    psi[1, :npw] *= torch.logspace(0, -30, npw, dtype=torch.float64, device="cuda")  # entries far below 2^-46 of the row maximum
     out = h.nonlocal_add(psi, torch.zeros_like(psi))
     torch.cuda.synchronize()
     beta = inp["beta"][:, :npw].cpu().numpy()
     vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
     got = out.cpu().numpy()[:, :npw]
     assert np.all(got[0] == 0)
-    assert _gpu.rel_l2(got[1:], vref[1:]).max() <= 1e-12
+    assert _gpu.rel_l2(got[1:], vref[1:]).max() <= 1e-11
     h.destroy()
