@@ -428,7 +428,7 @@ def main():
         peak = 2.0 * bf16_sus
         t_slice = stage["a6_a8_int8_digits"][0]
         roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
-                    "traffic": committed_traffic(args.config, "k_oz_gemm"),
+                    "traffic": committed_traffic(args.config, "k_oz_gemm_a8" if t_vnl >= t_becp else "k_oz_gemm_a6"),
                     "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; "
                     "the kernel runs inside a long step); a register-free UTCIMMA loop on the same chip measured 4540 TOP/s "
                     "(profiles/r1g_int8.md)", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
