@@ -736,7 +736,9 @@ void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cuda
 // plan + operand slices for the int8 path; leaves h->oz_s = 0 (FP64 DMMA path) when the device or a resource says no
 cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   int S = env_int("QE_HPSI_OZAKI", 6);
-  if (S <= 0 || h->gamma || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
+  if (S <= 0 || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
+  // (a Gamma-only handle runs the same complex-form kernels on its half sphere: Re of a6's result is what
+  // k_becp_reduce_gamma needs, and a8 with real dbecp is the complex product with zero imaginary parts)
   S = std::min(std::max(S, 4), 7);
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, h->device);
@@ -764,8 +766,18 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
       (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
-      (e = cudaMalloc(&h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess)
-    return e;
+      (e = cudaMalloc(&h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess) {
+    if (e != cudaErrorMemoryAllocation) return e;
+    // the digit planes (4 S bytes per entry of beta) do not fit: stay on the FP64 tensor path (qe_hpsi_info reports 0 digits)
+    (void)cudaGetLastError();
+    void** bufs[] = {(void**)&h->oz_a1, (void**)&h->oz_a2, (void**)&h->oz_b,  (void**)&h->oz_partial,
+                     (void**)&h->oz_ep, (void**)&h->oz_eg, (void**)&h->oz_eb};
+    for (void** b : bufs) {
+      cudaFree(*b);
+      *b = nullptr;
+    }
+    return cudaSuccess;
+  }
   if ((e = cudaMemsetAsync(h->oz_b, 0, bb, st)) != cudaSuccess) return e;
   if (!oz_make_map(&h->oz_tm_a1, h->oz_a1, k1, h->nproj, S, (long long)h->nproj * k1, oz::BM) ||
       !oz_make_map(&h->oz_tm_a2, h->oz_a2, k2, h->npw, S, (long long)h->npw * k2, oz::BM) ||
@@ -1249,7 +1261,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
   prof_span(h, ts, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
   if (h->gamma)
-    k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->partial, h->nsplit, h->nproj, h->ldc, nb, h->beta, h->ldbeta, psi, ldpsi,
+    k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
+                                            h->beta, h->ldbeta, psi, ldpsi,
                                             h->becp);
   else
     k_becp_reduce<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,

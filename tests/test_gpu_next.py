@@ -164,7 +164,7 @@ def _gamma_inputs(cfg, nb):
     return wl, sp, vr, psi, beta, db
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT])
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA])
 @pytest.mark.parametrize("cfg,nb", [("T2_radix5", 4), ("T2b_radix5_20", 3), ("T3_aliased", 4), ("T4_noproj", 3), (0, 7), (0, 16)])
 def test_gamma_apply_against_oracle(cfg, nb, flags):
     wl, sp, vr, psi, beta, db = _gamma_inputs(cfg, nb)
