@@ -171,6 +171,7 @@ def oracle_sample_time(wl, nbands_sample=2, atoms_sample=16):
 def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
     """CUDA-event timings of the rows SURVEY.md 8(f) marks next, on one chunk of `batch` bands of the workload:
     qe_hpsi_apply_hs (H psi and S psi), qe_hpsi_overlap (<psi|H psi>, batch x batch), qe_hpsi_density."""
+    from paper_2104_10502_b200 import inputs, qe_hpsi
     nb = min(batch, psi.shape[0])
     p, hp = psi[:nb], hpsi[:nb]
     sp = torch.empty_like(p)
@@ -191,6 +192,19 @@ def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
         rng = np.random.default_rng(7)
         q = rng.uniform(-1, 1, (wl.natoms, wl.nh, wl.nh))
         h.set_s(0.5 * (q + q.transpose(0, 2, 1)))
+    if wl.nproj and h.info().get("ozaki_slices", 0):
+        # the int8 digit path against the FP64 tensor path of the same library, on the nonlocal part alone (a6-a8 only)
+        h2 = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, inp["vr"], inp["beta"], np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh,
+                          inp["dblocks"], max_batch=batch, flags=qe_hpsi.QE_HPSI_BORROW_BETA | qe_hpsi.QE_HPSI_FP64_DMMA)
+        a = h.nonlocal_add(p, torch.zeros_like(p))
+        b = h2.nonlocal_add(p, torch.zeros_like(p))
+        torch.cuda.synchronize()
+        err = torch.linalg.vector_norm(a[:, :npw] - b[:, :npw], dim=1) / torch.linalg.vector_norm(b[:, :npw], dim=1)
+        full = torch.linalg.vector_norm(h.apply(p)[:, :npw] - h2.apply(p)[:, :npw], dim=1) / torch.linalg.vector_norm(h2.apply(p)[:, :npw], dim=1)
+        out["int8_vs_fp64_tensor_path"] = {"digits": h.info()["ozaki_slices"], "bands": nb, "max_rel_l2_nonlocal_part": float(err.max()),
+                                           "max_rel_l2_hpsi": float(full.max())}
+        h2.destroy()
+        del a, b, err, full
     ms = ev_time(lambda: h.apply_hs(p, hp, sp))
     fl = 3 * 8.0 * wl.nproj * npw * nb  # a6 once + a8 twice
     out["apply_hs"] = {"ms": ms, "bands_per_s": nb / ms * 1e3, "proj_tflops": fl / ms * 1e-9 if wl.nproj else None,
@@ -226,7 +240,6 @@ def time_next_rows(h, wl, inp, psi, hpsi, batch, npw, dmma, hbm_peak):
     out["rotate"] = {"ms": ms, "shape": [npw, nb, nb], "tflops": fl / ms * 1e-9, "bound": "tensor", "frac": fl / ms * 1e-9 / dmma}
     # NEXT-1: the same chunk as a real-wavefunction problem on the half sphere (k = 0 configs only)
     if all(x == 0.0 for x in wl.xk):
-        from paper_2104_10502_b200 import inputs, qe_hpsi
         mil_h = qe_hpsi.qe_hpsi_gamma_gsphere(wl.at, wl.ecutwfc, wl.nr)
         ngw = mil_h.shape[0]
         ldg = inputs.pad8(ngw)

@@ -57,7 +57,8 @@ typedef enum {
                                  /* tensor cores (tcgen05, int32 level sums in TMEM) and recombined in FP64:         */
                                  /* |error| <= ~(S+1) 2^(-8S+1) K max|a| max|b| per contraction (2^-47 = 7e-15);     */
                                  /* costs 2 S bytes per complex entry of beta, twice (K-major and transposed planes).*/
-                                 /* Env QE_HPSI_OZAKI = 0 | 4..7 overrides the digit count (0 = same as this flag).  */
+                                 /* Default only when nproj * npw >= 2^20 (smaller steps are launch-latency bound).  */
+                                 /* Env QE_HPSI_OZAKI = 0 | 4..7 forces the digit count (0 = same as this flag).     */
                                  /* Non-finite operands are not propagated by the int8 path (use this flag for them). */
 
 #define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */

@@ -735,7 +735,9 @@ void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cuda
 
 // plan + operand slices for the int8 path; leaves h->oz_s = 0 (FP64 DMMA path) when the device or a resource says no
 cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
-  int S = env_int("QE_HPSI_OZAKI", 6);
+  // default: 6 digits when the contraction is big enough to pay for the four extra launches per chunk (digit kernels) --
+  // below ~1e6 entries of beta the step is launch-latency bound and the FP64 tensor path is the shorter sequence
+  int S = env_int("QE_HPSI_OZAKI", (long long)h->nproj * h->npw >= (1LL << 20) ? 6 : 0);
   if (S <= 0 || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
   // (a Gamma-only handle runs the same complex-form kernels on its half sphere: Re of a6's result is what
   // k_becp_reduce_gamma needs, and a8 with real dbecp is the complex product with zero imaginary parts)

@@ -3,6 +3,8 @@ from exactly the inputs the GPU used (device arrays copied to the host; beta str
 config 4's 25 GB never has to sit in host memory)."""
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import torch
 
@@ -10,8 +12,30 @@ from oracle import hpsi_oracle as orc
 from paper_2104_10502_b200 import inputs, qe_hpsi
 
 
+INT8 = 1 << 16  # test-only pseudo flag: force the int8 digit path (QE_HPSI_OZAKI=6) where the library's size rule would not
+
+
+class force_int8:
+    """with force_int8(flags) as f: create handles with flags f; tiny workloads otherwise default to the FP64 tensor path."""
+
+    def __init__(self, flags, digits=6):
+        self.on, self.flags, self.digits = bool(flags & INT8), flags & ~INT8, digits
+
+    def __enter__(self):
+        if self.on:
+            os.environ["QE_HPSI_OZAKI"] = str(self.digits)
+        return self.flags
+
+    def __exit__(self, *exc):
+        if self.on:
+            del os.environ["QE_HPSI_OZAKI"]
+
+
 def make(key, max_batch=None, flags=0):
-    h, inp = qe_hpsi.from_workload(key, max_batch=max_batch, flags=flags)
+    with force_int8(flags) as f:
+        h, inp = qe_hpsi.from_workload(key, max_batch=max_batch, flags=f)
+    if flags & INT8:
+        assert inputs.get_workload(key).nproj == 0 or h.info()["ozaki_slices"] == 6
     return h, inp
 
 

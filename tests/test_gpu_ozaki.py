@@ -16,6 +16,12 @@ from tests import _gpu
 pytestmark = pytest.mark.gpu
 
 
+def _make_int8(key, digits=6, **kw):
+    """Handle with the int8 digit path forced (tiny workloads default to the FP64 tensor path: launch-latency bound)."""
+    with _gpu.force_int8(_gpu.INT8, digits):
+        return qe_hpsi.from_workload(key, **kw)
+
+
 def _nonlocal(h, inp, nb):
     psi = _gpu.gen_psi_dev(inp, 0, nb)
     out = h.nonlocal_add(psi, torch.zeros_like(psi))
@@ -25,17 +31,21 @@ def _nonlocal(h, inp, nb):
 
 
 def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
-    h, _ = _gpu.make(0)
+    h, _ = _gpu.make(1)
     assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_nsplit"] >= 1
     h.destroy()
-    h, _ = _gpu.make(0, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
+    h, _ = _gpu.make(1, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
+    assert h.info()["ozaki_slices"] == 0
+    h.destroy()
+    h, _ = _gpu.make(0)  # 8 x 2103 entries of beta: launch-latency bound, stays on the FP64 tensor path unless forced
     assert h.info()["ozaki_slices"] == 0
     h.destroy()
 
 
 @pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
 def test_becp_and_vnl_against_oracle(cfg):
-    h, inp = _gpu.make(cfg)
+    h, inp = _make_int8(cfg)
+    assert h.info()["ozaki_slices"] == 6
     wl = inp["wl"]
     npw = h.npw
     psi, out, becp = _nonlocal(h, inp, wl.nbands)
@@ -67,11 +77,7 @@ def test_int8_path_agrees_with_the_fp64_tensor_path_on_config_1():
 def test_error_falls_by_2_to_the_8_per_digit(slices, tol):
     """Each extra digit adds 8 bits: the measured error must respect the law (and S = 4 must be visibly worse than S = 7,
     i.e. the digits are really what is being multiplied)."""
-    os.environ["QE_HPSI_OZAKI"] = str(slices)
-    try:
-        h, inp = _gpu.make(0)
-    finally:
-        del os.environ["QE_HPSI_OZAKI"]
+    h, inp = _make_int8(0, digits=slices)
     assert h.info()["ozaki_slices"] == slices
     wl = inp["wl"]
     npw = h.npw
@@ -98,7 +104,7 @@ def test_bits_do_not_depend_on_batch_composition_or_run():
 
 
 def test_zero_band_and_huge_dynamic_range():
-    h, inp = _gpu.make("T1_general_k")
+    h, inp = _make_int8("T1_general_k")
     wl = inp["wl"]
     npw = h.npw
     psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)

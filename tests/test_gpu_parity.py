@@ -33,7 +33,7 @@ def test_maps_bit_exact(cfg):
     h.destroy()
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA])
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA, _gpu.INT8])
 @pytest.mark.parametrize("cfg", TINY + [0])
 def test_small_cases_against_dense_h(cfg, flags):
     """Level A (dense H from the definition) on every tiny case and config 0; both radix plans."""
