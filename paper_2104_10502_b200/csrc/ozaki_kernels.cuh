@@ -71,14 +71,14 @@ template <int S, int MODE>
 __global__ void __launch_bounds__(NT, 1)
 k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nstages, int nkb, int kchunk,
           const int* __restrict__ ea, const int* __restrict__ eb, long long mvalid, int nb, double2* __restrict__ out,
-          long long ldo, long long split_stride) {
+          long long ldo, long long split_stride, int ks_base) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint64_t full[MAX_STAGES], empty[MAX_STAGES], done;
   __shared__ uint32_t tmem_base;
   constexpr uint32_t STAGE = S * (A_BYTES + B_BYTES);
   constexpr uint32_t TCOLS = S * BN <= 256 ? 256 : 512;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int q = blockIdx.x, mt = blockIdx.y, ks = blockIdx.z;
+  const int q = blockIdx.x, mt = blockIdx.y, ks = ks_base + blockIdx.z;  // ks_base: a8 walks its K ranges launch by launch
   const int kb0 = ks * kchunk;
   const int nit = max(0, min(nkb, kb0 + kchunk) - kb0);
   if (warp == 0) {

@@ -93,7 +93,7 @@ struct qe_hpsi_handle {
   int zg_variant = 0;
   double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
   // projector contractions on tcgen05 int8 slices (ozaki_kernels.cuh): oz_s = slices per FP64 operand, 0 = FP64 DMMA path
-  int oz_s = 0, oz_stages = 0, oz_nsplit = 1, oz_kchunk = 0;
+  int oz_s = 0, oz_stages = 0, oz_nsplit = 1, oz_kchunk = 0, oz_kchunk2 = 0;  // K blocks per CTA of a6 / per launch of a8
   size_t oz_smem = 0;
   long long oz_k1 = 0, oz_k2 = 0;  // padded real K of a6 (2 npw) and a8 (2 nproj), bytes per int8 row
   int8_t *oz_a1 = nullptr, *oz_a2 = nullptr, *oz_b = nullptr;  // [S][nproj][k1], [S][npw][k2], [S][2 max_batch][max(k1,k2)]
@@ -709,7 +709,7 @@ template <int S>
 void oz_becp_gemm_t(qe_hpsi_handle* h, int nb, cudaStream_t st) {
   oz::k_oz_gemm<S, 0><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit), oz::NT, h->oz_smem, st>>>(
       h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb,
-      h->oz_partial, h->ldc, (long long)h->nproj * h->ldc);
+      h->oz_partial, h->ldc, (long long)h->nproj * h->ldc, 0);
 }
 // a8 on int8 slices: hpsi[b][g] += sum_p beta[p][g] bT[b][p]
 template <int S>
@@ -722,8 +722,10 @@ void oz_vnl_slice_t(qe_hpsi_handle* h, const double2* bT, int nb, cudaStream_t s
 template <int S>
 void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   const int nkb = (int)(h->oz_k2 / oz::KB);
-  oz::k_oz_gemm<S, 1><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
-      h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, nkb, h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0);
+  // the K ranges (int32 level sums must stay exact) accumulate into the same hpsi entries: one launch after the other
+  for (int ks = 0; ks * h->oz_kchunk2 < nkb; ++ks)
+    oz::k_oz_gemm<S, 1><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
+        h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, h->oz_kchunk2, h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0, ks);
 }
 #define OZ_DISPATCH(S_, CALL)            \
   switch (S_) {                          \
@@ -747,7 +749,9 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   if (e != cudaSuccess) return e;
   if (prop.major != 10) return cudaSuccess;  // tcgen05 kind::i8 is an sm_100 feature
   const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up(2LL * h->nproj, 128);
-  if ((long long)k2 > oz::max_k_per_cta(S)) return cudaSuccess;  // a8 runs unsplit: int32 level sums must not overflow
+  // K range per CTA: int32 level sums must not overflow (QE_HPSI_OZ_KMAX lowers it: testing the multi-range paths on small cases)
+  const long long kmax_env = env_int("QE_HPSI_OZ_KMAX", 0);
+  const long long kmax = kmax_env >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_env / oz::KB * oz::KB) : oz::max_k_per_cta(S);
   h->oz_k1 = k1;
   h->oz_k2 = k2;
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
@@ -756,12 +760,13 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   // split-K of a6: K ranges short enough for exact int32 sums, and enough CTAs for two waves
   const int nkb = (int)(k1 / oz::KB);
   const long long tiles = (long long)((2 * max_batch + oz::BN - 1) / oz::BN) * ((h->nproj + oz::BM - 1) / oz::BM);
-  long long ns = (k1 + oz::max_k_per_cta(S) - 1) / oz::max_k_per_cta(S);
+  long long ns = (k1 + kmax - 1) / kmax;
   ns = std::max(ns, (2LL * h->num_sms + tiles - 1) / tiles);
   ns = std::min<long long>(ns, std::max(1, nkb / 8));
-  ns = std::max<long long>(ns, (k1 + oz::max_k_per_cta(S) - 1) / oz::max_k_per_cta(S));
+  ns = std::max<long long>(ns, (k1 + kmax - 1) / kmax);
   h->oz_kchunk = (int)((nkb + ns - 1) / ns);
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
+  h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
   const size_t a1 = (size_t)S * h->nproj * k1, a2 = (size_t)S * h->npw * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
   const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit;
   if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
@@ -1908,7 +1913,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 8 : 4;
+    if (h->nproj > 0) total += h->oz_s ? 7 + (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2) : 4;
   }
   return total;
 }

@@ -118,3 +118,23 @@ def test_zero_band_and_huge_dynamic_range():
     assert np.all(got[0] == 0)
     assert _gpu.rel_l2(got[1:], vref[1:]).max() <= 1e-11
     h.destroy()
+
+
+def test_k_ranges_of_a8_and_forced_splits_of_a6_give_the_same_result():
+    """2 nproj beyond the exact-int32 K range makes a8 walk its K ranges launch by launch (and a6 split finer); forced here on
+    config 1 by lowering the range (QE_HPSI_OZ_KMAX), checked against the default plan and the FP64 tensor path."""
+    h, inp = _gpu.make(1)
+    psi, ref, _ = _nonlocal(h, inp, 64)
+    h.destroy()
+    os.environ["QE_HPSI_OZ_KMAX"] = "384"
+    try:
+        h2, inp2 = _gpu.make(1)
+    finally:
+        del os.environ["QE_HPSI_OZ_KMAX"]
+    assert h2.info()["ozaki_slices"] == 6
+    assert h2.launch_count(64) == 5 + 7 + 3  # a1-a5, digit/reduce/a6 kernels, a8 in ceil(1024 / 384) = 3 launches
+    _, out, _ = _nonlocal(h2, inp2, 64)
+    h2.destroy()
+    num = torch.linalg.vector_norm(out - ref, dim=1)
+    den = torch.linalg.vector_norm(ref, dim=1)
+    assert float((num / den).max()) <= 1e-13  # same digits, same exact integer sums; only the FP64 order of the K ranges differs
