@@ -66,7 +66,9 @@ __device__ __forceinline__ void mma_commit(uint64_t* bar) {
 // s8 x s8 -> s32, both operands K-major, M = 128, N = 64
 constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 
-// MODE 0 (a6): out = partial[split][m][ldo] complex, written; MODE 1 (a8): out = hpsi[b][ldo] complex at column m, accumulated
+// MODE 0 (a6): out = partial[split][m][ldo] complex, written; MODE 1 (a8): out = hpsi[b][ldo] complex at column m, accumulated.
+// Gamma-only (real) forms, one column per band: MODE 2 (a6): partial[split][m][b] = (value, 0); MODE 3 (a8): row m = 2g + c
+// of the transposed planar digits of beta, component c of hpsi[b][g] accumulated.
 template <int S, int MODE>
 __global__ void __launch_bounds__(NT, 1)
 k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nstages, int nkb, int kchunk,
@@ -142,7 +144,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int wq = warp & 3;
     const long long m = (long long)mt * BM + wq * 32 + lane;
-    const int em = (m < mvalid) ? ea[m] : 0;
+    const int em = (m < mvalid) ? ea[MODE == 3 ? (m >> 1) : m] : 0;  // MODE 3: rows 2g, 2g+1 share the exponent of plane wave g
 #pragma unroll 1
     for (int n0 = 0; n0 < BN; n0 += 8) {
       double d[8];
@@ -166,7 +168,21 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           for (int j = 0; j < 8; ++j) d[j] = fma((double)(int)v[L][j], w, d[j]);
         }
       }
-      if (m < mvalid) {
+      if (MODE >= 2) {  // real forms of the Gamma-only handle: one column per band
+        if (m < mvalid) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int b = q * BN + n0 + j;
+            if (b < nb) {
+              const double val = scalbn(d[j], em + eb[b] - 14);
+              if (MODE == 2)
+                out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(val, 0.0);
+              else
+                reinterpret_cast<double*>(out + (size_t)b * ldo)[m] += val;  // m = 2g + c: component c of hpsi[b][g]
+            }
+          }
+        }
+      } else if (m < mvalid) {
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
           const int b = (q * BN + n0) / 2 + jj;
@@ -256,6 +272,7 @@ __device__ __forceinline__ void slice16(double (&r)[16], uint4 (&o)[S]) {
 
 // rows of X (complex, n per row) -> int8 planes out[sl][orow][kpad], k = 2g + c.
 // mode 0: orow = r: (re, im).  mode 1: orow = 2r: (re, im), 2r+1: (im, -re).  mode 2: orow = 2r: (re, -im), 2r+1: (im, re).
+// (real parts only, k = g: k_oz_slice_re below)
 template <int S>
 __global__ void __launch_bounds__(128)
 k_oz_slice(const double2* __restrict__ X, long long ldx, long long n, const int* __restrict__ e, int8_t* __restrict__ out,
@@ -312,6 +329,49 @@ k_oz_slice_t(const double2* __restrict__ X, long long ldx, int rows, long long n
   slice16<S>(a, o);
 #pragma unroll
   for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)g * kpad + 2 * p0) = o[sl];
+}
+
+// Gamma-only a8, B operand: rows of X (complex with zero imaginary part, n per row) -> out[sl][r][kpad], k = g, value Re x
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice_re(const double2* __restrict__ X, long long ldx, long long n, const int* __restrict__ e, int8_t* __restrict__ out,
+              long long kpad, long long slice_stride) {
+  const long long g0 = ((long long)blockIdx.x * 128 + threadIdx.x) * 16;
+  if (g0 >= kpad) return;
+  const int r = blockIdx.y;
+  const int ex = -e[r];
+  double a[16];
+#pragma unroll
+  for (int t = 0; t < 16; ++t) a[t] = g0 + t < n ? scalbn(X[(size_t)r * ldx + g0 + t].x, ex) : 0.0;
+  uint4 o[S];
+  slice16<S>(a, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)r * kpad + g0) = o[sl];
+}
+// Gamma-only a8, A operand: X[rows = p][ldx] -> out[sl][2g + c][kpad], k = p, rows 2g and 2g+1 scaled by 2^-e[g]; 16 rows p per thread
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice_tp(const double2* __restrict__ X, long long ldx, int rows, long long n, const int* __restrict__ e,
+              int8_t* __restrict__ out, long long kpad, long long slice_stride) {
+  const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (g >= n) return;
+  const int p0 = blockIdx.y * 16;
+  const int ex = -e[g];
+  double re[16], im[16];
+#pragma unroll
+  for (int t = 0; t < 16; ++t) {
+    double2 v = make_double2(0.0, 0.0);
+    if (p0 + t < rows) v = X[(size_t)(p0 + t) * ldx + g];
+    re[t] = scalbn(v.x, ex);
+    im[t] = scalbn(v.y, ex);
+  }
+  uint4 o[S];
+  slice16<S>(re, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)(2 * g) * kpad + p0) = o[sl];
+  slice16<S>(im, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)(2 * g + 1) * kpad + p0) = o[sl];
 }
 
 }  // namespace oz

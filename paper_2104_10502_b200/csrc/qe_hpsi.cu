@@ -682,18 +682,23 @@ bool oz_make_map(CUtensorMap* tm, void* base, long long kpad, long long rows, in
 
 template <int S>
 cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(oz::k_oz_gemm<S, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(oz::k_oz_gemm<S, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem);
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
+  const void* kern[4] = {(const void*)oz::k_oz_gemm<S, 0>, (const void*)oz::k_oz_gemm<S, 1>, (const void*)oz::k_oz_gemm<S, 2>,
+                         (const void*)oz::k_oz_gemm<S, 3>};
+  for (const void* k : kern)
+    if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem)) != cudaSuccess) return e;
   const long long k1 = h->oz_k1, k2 = h->oz_k2;
   // a6 operand: rows p scaled by 2^-ep[p]; a8 operand: rows g scaled by 2^-eg[g] (transposed beta)
   oz::k_oz_rowexp<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep);
   oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
                                                                                     k1, (long long)h->nproj * k1, 0);
   oz::k_oz_colexp<<<(unsigned)((h->npw + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg);
-  oz::k_oz_slice_t<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
-      h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, (long long)h->npw * k2);
+  if (h->gamma)  // real form: rows 2g + c, K = p
+    oz::k_oz_slice_tp<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
+        h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, 2LL * h->npw * k2);
+  else
+    oz::k_oz_slice_t<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
+        h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, (long long)h->npw * k2);
   return cudaGetLastError();
 }
 
@@ -702,30 +707,39 @@ template <int S>
 void oz_becp_slice_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const long long k1 = h->oz_k1;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb);
+  // Gamma-only: becp is real, one B row (psi_r, psi_i) per band; otherwise the (Re, Im) row pair
   oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), nb), 128, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb, h->oz_b, k1,
-                                                                             2LL * h->max_batch * k1, 1);
+                                                                             2LL * h->max_batch * k1, h->gamma ? 0 : 1);
 }
 template <int S>
 void oz_becp_gemm_t(qe_hpsi_handle* h, int nb, cudaStream_t st) {
-  oz::k_oz_gemm<S, 0><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit), oz::NT, h->oz_smem, st>>>(
-      h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb,
-      h->oz_partial, h->ldc, (long long)h->nproj * h->ldc, 0);
+  const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit);
+  auto kern = h->gamma ? oz::k_oz_gemm<S, 2> : oz::k_oz_gemm<S, 0>;
+  kern<<<grid, oz::NT, h->oz_smem, st>>>(h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep,
+                                        h->oz_eb, h->nproj, nb, h->oz_partial, h->ldc, (long long)h->nproj * h->ldc, 0);
 }
 // a8 on int8 slices: hpsi[b][g] += sum_p beta[p][g] bT[b][p]
 template <int S>
 void oz_vnl_slice_t(qe_hpsi_handle* h, const double2* bT, int nb, cudaStream_t st) {
   const long long k2 = h->oz_k2;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb);
-  oz::k_oz_slice<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
-                                                                             2LL * h->max_batch * k2, 2);
+  if (h->gamma)  // dbecp is real: K = p
+    oz::k_oz_slice_re<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
+                                                                                  2LL * h->max_batch * k2);
+  else
+    oz::k_oz_slice<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
+                                                                               2LL * h->max_batch * k2, 2);
 }
 template <int S>
 void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   const int nkb = (int)(h->oz_k2 / oz::KB);
   // the K ranges (int32 level sums must stay exact) accumulate into the same hpsi entries: one launch after the other
+  const long long mrows = (h->gamma ? 2LL : 1LL) * h->npw;  // Gamma-only: rows 2g + c of the planar transposed digits
+  const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (unsigned)((mrows + oz::BM - 1) / oz::BM), 1);
+  auto kern = h->gamma ? oz::k_oz_gemm<S, 3> : oz::k_oz_gemm<S, 1>;
   for (int ks = 0; ks * h->oz_kchunk2 < nkb; ++ks)
-    oz::k_oz_gemm<S, 1><<<dim3((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
-        h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, h->oz_kchunk2, h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh, 0, ks);
+    kern<<<grid, oz::NT, h->oz_smem, st>>>(h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, h->oz_kchunk2, h->oz_eg, h->oz_eb, mrows, nb, hpsi,
+                                          ldh, 0, ks);
 }
 #define OZ_DISPATCH(S_, CALL)            \
   switch (S_) {                          \
@@ -741,14 +755,13 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   // below ~1e6 entries of beta the step is launch-latency bound and the FP64 tensor path is the shorter sequence
   int S = env_int("QE_HPSI_OZAKI", (long long)h->nproj * h->npw >= (1LL << 20) ? 6 : 0);
   if (S <= 0 || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
-  // (a Gamma-only handle runs the same complex-form kernels on its half sphere: Re of a6's result is what
-  // k_becp_reduce_gamma needs, and a8 with real dbecp is the complex product with zero imaginary parts)
+  // (a Gamma-only handle runs the real forms: one B row per band in a6, planar transposed digits of beta in a8)
   S = std::min(std::max(S, 4), 7);
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, h->device);
   if (e != cudaSuccess) return e;
   if (prop.major != 10) return cudaSuccess;  // tcgen05 kind::i8 is an sm_100 feature
-  const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up(2LL * h->nproj, 128);
+  const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up((h->gamma ? 1LL : 2LL) * h->nproj, 128);
   // K range per CTA: int32 level sums must not overflow (QE_HPSI_OZ_KMAX lowers it: testing the multi-range paths on small cases)
   const long long kmax_env = env_int("QE_HPSI_OZ_KMAX", 0);
   const long long kmax = kmax_env >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_env / oz::KB * oz::KB) : oz::max_k_per_cta(S);
@@ -767,7 +780,8 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   h->oz_kchunk = (int)((nkb + ns - 1) / ns);
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
   h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
-  const size_t a1 = (size_t)S * h->nproj * k1, a2 = (size_t)S * h->npw * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
+  const long long a2rows = (h->gamma ? 2LL : 1LL) * h->npw;
+  const size_t a1 = (size_t)S * h->nproj * k1, a2 = (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
   const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit;
   if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
@@ -787,7 +801,7 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   }
   if ((e = cudaMemsetAsync(h->oz_b, 0, bb, st)) != cudaSuccess) return e;
   if (!oz_make_map(&h->oz_tm_a1, h->oz_a1, k1, h->nproj, S, (long long)h->nproj * k1, oz::BM) ||
-      !oz_make_map(&h->oz_tm_a2, h->oz_a2, k2, h->npw, S, (long long)h->npw * k2, oz::BM) ||
+      !oz_make_map(&h->oz_tm_a2, h->oz_a2, k2, a2rows, S, a2rows * k2, oz::BM) ||
       !oz_make_map(&h->oz_tm_b1, h->oz_b, k1, 2LL * max_batch, S, 2LL * max_batch * k1, oz::BN) ||
       !oz_make_map(&h->oz_tm_b2, h->oz_b, k2, 2LL * max_batch, S, 2LL * max_batch * k2, oz::BN))
     return cudaErrorNotSupported;
