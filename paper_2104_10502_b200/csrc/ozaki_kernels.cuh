@@ -140,10 +140,22 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     mma_commit(&done);
   } else if (warp >= 2) {
     // ---- epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31; thread = row of the tile ----
-    mbar_wait(&done, 0);
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int wq = warp & 3;
     const long long m = (long long)mt * BM + wq * 32 + lane;
+    if ((MODE == 1 || MODE == 3) && m < mvalid) {
+      // these warps idle while the MMAs run: pull the hpsi entries of the tile towards L2 for the read-modify-write below
+      const int ncol = MODE == 1 ? BN / 2 : BN;
+      for (int j = 0; j < ncol; ++j) {
+        const int b = q * ncol + j;
+        if (b < nb) {
+          const void* a = MODE == 1 ? (const void*)(out + (size_t)b * ldo + m)
+                                    : (const void*)(reinterpret_cast<const double*>(out + (size_t)b * ldo) + m);
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+        }
+      }
+    }
+    mbar_wait(&done, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int em = (m < mvalid) ? ea[MODE == 3 ? (m >> 1) : m] : 0;  // MODE 3: rows 2g, 2g+1 share the exponent of plane wave g
 #pragma unroll 1
     for (int n0 = 0; n0 < BN; n0 += 8) {

@@ -777,6 +777,14 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   ns = std::max(ns, (2LL * h->num_sms + tiles - 1) / tiles);
   ns = std::min<long long>(ns, std::max(1, nkb / 8));
   ns = std::max<long long>(ns, (k1 + kmax - 1) / kmax);
+  {  // a few more splits if that fills the last wave: cost = rounds of CTAs x K blocks per CTA (one CTA per SM)
+    long long best = ns, best_cost = -1;
+    for (long long c = ns; c <= ns + 40 && c <= std::max<long long>(ns, nkb / 8); ++c) {
+      const long long cost = ((tiles * c + h->num_sms - 1) / h->num_sms) * ((nkb + c - 1) / c + 4);  // + 4: prologue / epilogue
+      if (best_cost < 0 || cost < best_cost) best = c, best_cost = cost;
+    }
+    ns = best;
+  }
   h->oz_kchunk = (int)((nkb + ns - 1) / ns);
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
   h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
