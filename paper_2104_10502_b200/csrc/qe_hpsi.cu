@@ -1071,12 +1071,17 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
     g.vs = h->vs;
   }
 
-  // FFT workspace: sub-chunks of fft_nb bands (workspace budget QE_HPSI_FFT_WS_MB, default 2.5 GB)
+  // FFT workspace: sub-chunks of fft_nb bands (workspace budget QE_HPSI_FFT_WS_MB, default up to 12 GB)
   {
     const size_t per_band = ((size_t)h->S + (size_t)h->P * nr[1]) * h->ldz * sizeof(double2);
     // Measured on B200 (profiles/r1b): the chain gets faster with more bands per launch up to ~32 (fewer partial
     // waves, V(r) reused across the bands of a sub-chunk in a3); L2 residency of one band's workspace is worth less.
-    const size_t budget = (size_t)env_int("QE_HPSI_FFT_WS_MB", 2560) << 20;
+    // Capture G: one sub-chunk per call is best on every config (cfg 2: 15.7 -> 14.6 ms per 512 bands, cfg 4: 10.6 -> 10.4 ms per
+    // 128), so the default budget is 12 GB, but never more than a quarter of what is free on the device right now.
+    size_t mem_free = 0, mem_total = 0;
+    if (cudaMemGetInfo(&mem_free, &mem_total) != cudaSuccess) mem_free = (size_t)10 << 30;
+    const size_t dflt_mb = std::max<size_t>(256, std::min<size_t>(12288, (mem_free / 4) >> 20));
+    const size_t budget = (size_t)env_int("QE_HPSI_FFT_WS_MB", (int)dflt_mb) << 20;
     long long nbf = per_band ? (long long)(budget / per_band) : max_batch;
     nbf = std::max<long long>(1, std::min<long long>(nbf, max_batch));
     const int forced = env_int("QE_HPSI_FFT_NB", 0);
