@@ -99,7 +99,8 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tm = tmem_base;
-  const uint32_t sbase0 = smem_u32(smem);
+  // the swizzle pattern is a function of the address: align the ring explicitly (the launch asks for 1 KB more than it uses)
+  const uint32_t sbase0 = (smem_u32(smem) + 1023u) & ~1023u;
 
   if (warp == 0 && lane == 0) {
     // ---- TMA producer ----

@@ -769,7 +769,7 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   h->oz_k2 = k2;
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
   h->oz_stages = std::min(oz::MAX_STAGES, (222 * 1024) / stage);
-  h->oz_smem = (size_t)h->oz_stages * stage;
+  h->oz_smem = (size_t)h->oz_stages * stage + 1024;  // + 1 KB: the kernel aligns its ring to 1024 bytes itself
   // split-K of a6: K ranges short enough for exact int32 sums, and enough CTAs for two waves
   const int nkb = (int)(k1 / oz::KB);
   const long long tiles = (long long)((2 * max_batch + oz::BN - 1) / oz::BN) * ((h->nproj + oz::BM - 1) / oz::BM);
