@@ -10,6 +10,8 @@
 // consecutive reals), A and B stored as S planes of int8, K contiguous:
 //   a6  becp[p][b]   : A row p  = (beta_r, beta_i)[p][g]      k = 2g+c        B row 2b = (psi_r, psi_i), row 2b+1 = (psi_i, -psi_r)
 //   a8  hpsi[b][g] += : A row g  = (beta_r, beta_i)[p][g]      k = 2p+c        B row 2b = (d_r, -d_i),    row 2b+1 = (d_i, d_r)
+// (Gamma-only handles: real forms, one B row / D column per band: a6 with B row b = (psi_r, psi_i); a8 with A row 2g+c =
+//  component c of beta[.][g], k = p, and B row b = Re dbecp.)
 // One CTA owns a 128 x 64 tile of D for one K range: S level accumulators of 64 TMEM columns each (level L = i+j), operands
 // staged by TMA (SWIZZLE_64B, 64 bytes of K per stage) on a full/empty mbarrier ring, one thread issuing the MMAs, four
 // warps converting the S int32 levels to FP64 in the epilogue.  Integer sums are exact, so results are bit-reproducible and do
