@@ -389,5 +389,53 @@ k_oz_slice_tp(const double2* __restrict__ X, long long ldx, int rows, long long 
   for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(out + (size_t)sl * slice_stride + (size_t)(2 * g + 1) * kpad + p0) = o[sl];
 }
 
+// ---- integer 3M form of a6 (complex handles): conj(beta) psi from three real products over the complex index g --------------
+// planes 0, 1, 2 of a row x: Re x, Im x, (Re x + sgn Im x) / 2   (sgn = -1 for beta: the conjugate; +1 for psi), so that with
+// Q1 = sum beta_r psi_r, Q2 = sum beta_i psi_i, Q3 = sum plane2(beta) plane2(psi):  becp = (Q1 + Q2) + i (4 Q3 - Q1 + Q2).
+// out[sl][plane][row][kpad], k = g; 16 complex entries per thread.
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice3(const double2* __restrict__ X, long long ldx, long long n, const int* __restrict__ e, int8_t* __restrict__ out,
+            long long kpad, long long plane_stride, long long slice_stride, double sgn) {
+  const long long g0 = ((long long)blockIdx.x * 128 + threadIdx.x) * 16;
+  if (g0 >= kpad) return;
+  const int r = blockIdx.y;
+  const int ex = -e[r];
+  double re[16], im[16], sm[16];
+#pragma unroll
+  for (int t = 0; t < 16; ++t) {
+    double2 v = make_double2(0.0, 0.0);
+    if (g0 + t < n) v = X[(size_t)r * ldx + g0 + t];
+    re[t] = scalbn(v.x, ex);
+    im[t] = scalbn(v.y, ex);
+    sm[t] = 0.5 * (re[t] + sgn * im[t]);
+  }
+  uint4 o[S];
+  int8_t* base = out + (size_t)r * kpad + g0;
+  slice16<S>(re, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride) = o[sl];
+  slice16<S>(im, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride + plane_stride) = o[sl];
+  slice16<S>(sm, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride + 2 * plane_stride) = o[sl];
+}
+// a7 front end of the 3M form: partial[plane][split][p][ldc].x summed over the splits in ascending order, then combined
+__global__ void k_oz_reduce3(const double2* __restrict__ partial, int nsplit, int nproj, int ldc, int nb, double2* __restrict__ becp) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (b >= nb) return;
+  double q[3];
+#pragma unroll
+  for (int pl = 0; pl < 3; ++pl) {
+    double acc = 0.0;
+    for (int ks = 0; ks < nsplit; ++ks) acc += partial[(((size_t)pl * nsplit + ks) * nproj + p) * ldc + b].x;
+    q[pl] = acc;
+  }
+  becp[(size_t)p * ldc + b] = make_double2(q[0] + q[1], (4.0 * q[2] - q[0]) + q[1]);
+}
+
 }  // namespace oz
 }  // namespace qehpsi

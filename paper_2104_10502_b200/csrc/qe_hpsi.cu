@@ -100,6 +100,10 @@ struct qe_hpsi_handle {
   int *oz_ep = nullptr, *oz_eg = nullptr, *oz_eb = nullptr;     // exponents: per projector, per plane wave, per band
   double2* oz_partial = nullptr;
   CUtensorMap oz_tm_a1{}, oz_tm_a2{}, oz_tm_b1{}, oz_tm_b2{};
+  // integer 3M form of a6 (complex handles): planar digit planes (Re, Im, (Re -/+ Im)/2), three real GEMMs over the complex index
+  bool oz_3m = false;
+  long long oz_k1c = 0;
+  CUtensorMap oz_tm_a3[3] = {}, oz_tm_b3[3] = {};
   // NEXT-2: overlap operator S (q blocks packed like D; qbecp/qbT mirror dbecp/dbT)
   long long d_total = 0;
   double* qpk = nullptr;
@@ -690,8 +694,12 @@ cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
   const long long k1 = h->oz_k1, k2 = h->oz_k2;
   // a6 operand: rows p scaled by 2^-ep[p]; a8 operand: rows g scaled by 2^-eg[g] (transposed beta)
   oz::k_oz_rowexp<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep);
-  oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
-                                                                                    k1, (long long)h->nproj * k1, 0);
+  if (h->oz_3m)
+    oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k1c / 16 + 127) / 128), h->nproj), 128, 0, st>>>(
+        h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1, h->oz_k1c, (long long)h->nproj * h->oz_k1c, 3LL * h->nproj * h->oz_k1c, -1.0);
+  else
+    oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
+                                                                                      k1, (long long)h->nproj * k1, 0);
   oz::k_oz_colexp<<<(unsigned)((h->npw + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg);
   if (h->gamma)  // real form: rows 2g + c, K = p
     oz::k_oz_slice_tp<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
@@ -707,12 +715,26 @@ template <int S>
 void oz_becp_slice_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const long long k1 = h->oz_k1;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb);
+  if (h->oz_3m) {  // planes Re, Im, (Re + Im) / 2 of every band
+    oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k1c / 16 + 127) / 128), nb), 128, 0, st>>>(
+        psi, ldpsi, h->npw, h->oz_eb, h->oz_b, h->oz_k1c, (long long)h->max_batch * h->oz_k1c, 3LL * h->max_batch * h->oz_k1c, 1.0);
+    return;
+  }
   // Gamma-only: becp is real, one B row (psi_r, psi_i) per band; otherwise the (Re, Im) row pair
   oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), nb), 128, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb, h->oz_b, k1,
                                                                              2LL * h->max_batch * k1, h->gamma ? 0 : 1);
 }
 template <int S>
 void oz_becp_gemm_t(qe_hpsi_handle* h, int nb, cudaStream_t st) {
+  if (h->oz_3m) {
+    const dim3 g3((nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit);
+    const size_t slab = (size_t)h->nproj * h->ldc;
+    for (int pl = 0; pl < 3; ++pl)
+      oz::k_oz_gemm<S, 2><<<g3, oz::NT, h->oz_smem, st>>>(h->oz_tm_a3[pl], h->oz_tm_b3[pl], h->oz_stages, (int)(h->oz_k1c / oz::KB),
+                                                         h->oz_kchunk, h->oz_ep, h->oz_eb, h->nproj, nb,
+                                                         h->oz_partial + (size_t)pl * h->oz_nsplit * slab, h->ldc, (long long)slab, 0);
+    return;
+  }
   const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit);
   auto kern = h->gamma ? oz::k_oz_gemm<S, 2> : oz::k_oz_gemm<S, 0>;
   kern<<<grid, oz::NT, h->oz_smem, st>>>(h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep,
@@ -767,16 +789,20 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   const long long kmax = kmax_env >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_env / oz::KB * oz::KB) : oz::max_k_per_cta(S);
   h->oz_k1 = k1;
   h->oz_k2 = k2;
+  // 3M form of a6 (three real GEMMs instead of a real-form complex one: -25 % MMAs, three launches): pays from ~2^26 entries of beta
+  h->oz_3m = !h->gamma && env_int("QE_HPSI_OZ_3M", (long long)h->nproj * h->npw >= (1LL << 26) ? 1 : 0) != 0;
+  h->oz_k1c = round_up(h->npw, 128);
+  const long long ka6 = h->oz_3m ? h->oz_k1c : k1;  // contraction length of one a6 GEMM (reals)
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
   h->oz_stages = std::min(oz::MAX_STAGES, (222 * 1024) / stage);
   h->oz_smem = (size_t)h->oz_stages * stage + 1024;  // + 1 KB: the kernel aligns its ring to 1024 bytes itself
   // split-K of a6: K ranges short enough for exact int32 sums, and enough CTAs for two waves
-  const int nkb = (int)(k1 / oz::KB);
-  const long long tiles = (long long)((2 * max_batch + oz::BN - 1) / oz::BN) * ((h->nproj + oz::BM - 1) / oz::BM);
-  long long ns = (k1 + kmax - 1) / kmax;
+  const int nkb = (int)(ka6 / oz::KB);
+  const long long tiles = (long long)(((h->oz_3m || h->gamma ? 1 : 2) * max_batch + oz::BN - 1) / oz::BN) * ((h->nproj + oz::BM - 1) / oz::BM);
+  long long ns = (ka6 + kmax - 1) / kmax;
   ns = std::max(ns, (2LL * h->num_sms + tiles - 1) / tiles);
   ns = std::min<long long>(ns, std::max(1, nkb / 8));
-  ns = std::max<long long>(ns, (k1 + kmax - 1) / kmax);
+  ns = std::max<long long>(ns, (ka6 + kmax - 1) / kmax);
   {  // a few more splits if that fills the last wave: cost = rounds of CTAs x K blocks per CTA (one CTA per SM)
     long long best = ns, best_cost = -1;
     for (long long c = ns; c <= ns + 40 && c <= std::max<long long>(ns, nkb / 8); ++c) {
@@ -789,8 +815,8 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
   h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
   const long long a2rows = (h->gamma ? 2LL : 1LL) * h->npw;
-  const size_t a1 = (size_t)S * h->nproj * k1, a2 = (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
-  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit;
+  const size_t a1 = h->oz_3m ? (size_t)S * 3 * h->nproj * h->oz_k1c : (size_t)S * h->nproj * k1, a2 = (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
+  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit * (h->oz_3m ? 3 : 1);
   if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
@@ -813,6 +839,13 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
       !oz_make_map(&h->oz_tm_b1, h->oz_b, k1, 2LL * max_batch, S, 2LL * max_batch * k1, oz::BN) ||
       !oz_make_map(&h->oz_tm_b2, h->oz_b, k2, 2LL * max_batch, S, 2LL * max_batch * k2, oz::BN))
     return cudaErrorNotSupported;
+  if (h->oz_3m)
+    for (int pl = 0; pl < 3; ++pl)
+      if (!oz_make_map(&h->oz_tm_a3[pl], h->oz_a1 + (size_t)pl * h->nproj * h->oz_k1c, h->oz_k1c, h->nproj, S, 3LL * h->nproj * h->oz_k1c,
+                       oz::BM) ||
+          !oz_make_map(&h->oz_tm_b3[pl], h->oz_b + (size_t)pl * max_batch * h->oz_k1c, h->oz_k1c, max_batch, S,
+                       3LL * max_batch * h->oz_k1c, oz::BN))
+        return cudaErrorNotSupported;
 #define OZ_CALL(S_) e = oz_prepare_t<S_>(h, st)
   OZ_DISPATCH(S, OZ_CALL)
 #undef OZ_CALL
@@ -1298,6 +1331,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
                                             h->beta, h->ldbeta, psi, ldpsi,
                                             h->becp);
+  else if (h->oz_s && h->oz_3m)
+    oz::k_oz_reduce3<<<rg, 128, 0, st>>>(h->oz_partial, h->oz_nsplit, h->nproj, h->ldc, nb, h->becp);
   else
     k_becp_reduce<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
                                       h->becp);
@@ -1940,7 +1975,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 7 + (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2) : 4;
+    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2) : 4;
   }
   return total;
 }
