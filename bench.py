@@ -487,7 +487,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": wl.name, "nbands": nb, "batch": batch, "grid": list(wl.nr), "npw": npw, "nproj": wl.nproj,
-                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["ozaki_nsplit"] if info.get("ozaki_slices") else info["nsplit"], "projector_path": f"int8 digits x{info['ozaki_slices']} (tcgen05)" if info.get("ozaki_slices") else "fp64 dmma (3M)", "cuda_graph": bool(use_graph),
+                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["ozaki_nsplit"] if info.get("ozaki_slices") else info["nsplit"], "projector_path": (f"int8 digits x{info['ozaki_slices']} (tcgen05)" + (", a6 in the integer 3M form" if info.get("ozaki_3m") else "")) if info.get("ozaki_slices") else "fp64 dmma (3M)", "cuda_graph": bool(use_graph),
                        "l2": "inputs per step exceed L2" if flush is None else "L2 flushed (256 MB write) between steps",
                        "sharding": "bands / k-point pools per rank, no collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": h.launch_count(batch) * chunks_per_step * args.steps if nb % batch == 0

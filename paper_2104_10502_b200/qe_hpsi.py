@@ -305,7 +305,7 @@ class Hpsi:
         buf = (_c.c_int64 * 16)()
         _check(self._lib.qe_hpsi_info(self._h, buf), self._h)
         keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
-                "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit"]
+                "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit", "ozaki_3m"]
         return {k: int(buf[i]) for i, k in enumerate(keys)}
 
     PROFILE_SLOTS = ["a6_becp", "a7_reduce_dmul", "a1_a5_fft_chain", "a8_vnl_add", "a1_scatter_zinv", "a2_yinv",

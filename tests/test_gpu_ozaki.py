@@ -32,7 +32,7 @@ def _nonlocal(h, inp, nb):
 
 def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
     h, _ = _gpu.make(1)
-    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_nsplit"] >= 1
+    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_nsplit"] >= 1 and h.info()["ozaki_3m"] == 0  # 12 M entries of beta < 2^26
     h.destroy()
     h, _ = _gpu.make(1, flags=qe_hpsi.QE_HPSI_FP64_DMMA)
     assert h.info()["ozaki_slices"] == 0
@@ -42,10 +42,16 @@ def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
     h.destroy()
 
 
+@pytest.mark.parametrize("three_m", [0, 1])
 @pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
-def test_becp_and_vnl_against_oracle(cfg):
-    h, inp = _make_int8(cfg)
-    assert h.info()["ozaki_slices"] == 6
+def test_becp_and_vnl_against_oracle(cfg, three_m):
+    """Both forms of a6: the real-form complex GEMM and the integer 3M form (three real GEMMs on planar digit planes)."""
+    os.environ["QE_HPSI_OZ_3M"] = str(three_m)
+    try:
+        h, inp = _make_int8(cfg)
+    finally:
+        del os.environ["QE_HPSI_OZ_3M"]
+    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_3m"] == three_m
     wl = inp["wl"]
     npw = h.npw
     psi, out, becp = _nonlocal(h, inp, wl.nbands)
