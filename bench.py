@@ -434,8 +434,10 @@ def main():
     if wl.nproj and oz_s and t_vnl + t_becp > t_fft:
         # projector contractions on the int8 tensor cores: S (S+1) / 2 digit-pair products per real product, each exact
         pairs = oz_s * (oz_s + 1) // 2
-        kname, t_k = ("k_oz_gemm<S,1> (a8)", t_vnl) if t_vnl >= t_becp else ("k_oz_gemm<S,0> (a6)", t_becp)
+        kname, t_k = ("k_oz_gemm<S,1> (a8)", t_vnl) if t_vnl >= t_becp else ("k_oz_gemm<S,0|2> (a6)", t_becp)
         ops_launch = pairs * flops_launch  # 4 real MACs per complex MAC x 2 ops x pairs
+        if t_vnl < t_becp and info.get("ozaki_3m"):
+            ops_launch *= 0.75  # a6 in the integer 3M form executes 3 real products per complex one
         ach = ops_launch / (t_k * 1e-3) * 1e-12
         bf16_sus = float(mp.get("bf16_tflops_sustained", 0.0)) or 1414.0
         peak = 2.0 * bf16_sus
@@ -450,11 +452,12 @@ def main():
                     "digit_kernels_ms_per_launch": t_slice,
                     "note": "achieved = executed int8 ops of the S-digit split (every one of them is needed for the FP64 result); "
                             "fp64_equivalent_tflops = 8 flops per complex MAC / time, comparable with the FP64 DMMA peak"}
-        t_int8 = pairs * m["f_proj"] / (peak * 1e12)
+        a6_units = 0.75 if info.get("ozaki_3m") else 1.0  # integer 3M form of a6: 6 of the 8 tile-GEMM units
+        t_int8 = pairs * m["f_proj"] * 0.5 * (1.0 + a6_units) / (peak * 1e12)
         b_beta8 = 2.0 * oz_s * 2 * wl.nproj * npw / wl.batch  # int8 digit planes of beta, streamed once by a6 and once by a8
         roof8 = max((m["b_fft"] + b_beta8) / (hbm_peak * 1e9), t_int8)
         int8 = {"bands_per_s": 1.0 / roof8, "frac": value / world * roof8, "int8_tops": peak, "bytes_per_band": m["b_fft"] + b_beta8,
-                "int8_ops_per_band": pairs * m["f_proj"], "note": "max(bytes/HBM, digit-pair int8 ops/int8 tensor peak) per band"}
+                "int8_ops_per_band": pairs * m["f_proj"] * 0.5 * (1.0 + a6_units), "note": "max(bytes/HBM, digit-pair int8 ops/int8 tensor peak) per band"}
     elif wl.nproj and t_vnl + t_becp > t_fft:
         kname, t_k = ("k_vnl_add", t_vnl) if t_vnl >= t_becp else ("k_becp", t_becp)
         ach = flops_launch / (t_k * 1e-3) * 1e-12
