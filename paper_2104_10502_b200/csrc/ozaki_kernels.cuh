@@ -437,5 +437,182 @@ __global__ void k_oz_reduce3(const double2* __restrict__ partial, int nsplit, in
   becp[(size_t)p * ldc + b] = make_double2(q[0] + q[1], (4.0 * q[2] - q[0]) + q[1]);
 }
 
+// ---- integer 3M form of a8 (complex handles): hpsi[b][g] += sum_p beta[p][g] d[p][b] from three real products over p ---------
+// A planes (k_oz_slice_t3): rows g, k = p: beta_r, beta_i, (beta_r + beta_i) / 2;  B planes (k_oz_slice3, sgn = +1): d_r, d_i, half sum.
+// Q1 = sum beta_r d_r, Q2 = sum beta_i d_i, Q3 = sum of the half-sum planes:  Re = Q1 - Q2,  Im = 4 Q3 - Q1 - Q2.
+// One CTA runs the three planes back to back for its 128 x 64 (rows g x bands) tile: the TMA ring and the MMA issue never stop;
+// after each plane the epilogue warps pull the S levels out of TMEM into 64 FP64 registers per thread, hand TMEM back, and add
+// (cr, ci) * Q to hpsi while the next plane is being multiplied.  K = nproj is not split (needs 128-padded nproj <= max_k_per_cta).
+template <int S>
+__global__ void __launch_bounds__(NT, 1)
+k_oz_vnl3(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmA2,
+          const __grid_constant__ CUtensorMap tmB0, const __grid_constant__ CUtensorMap tmB1, const __grid_constant__ CUtensorMap tmB2,
+          int nstages, int nkb, const int* __restrict__ ea, const int* __restrict__ eb, long long mvalid, int nb,
+          double2* __restrict__ out, long long ldo) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ uint64_t full[MAX_STAGES], empty[MAX_STAGES], done, tfree;
+  __shared__ uint32_t tmem_base;
+  constexpr uint32_t STAGE = S * (A_BYTES + B_BYTES);
+  constexpr uint32_t TCOLS = S * BN <= 256 ? 256 : 512;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int q = blockIdx.x, mt = blockIdx.y;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base)), "r"(TCOLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (threadIdx.x == 32) {
+    for (int i = 0; i < MAX_STAGES; ++i) {
+      mbar_init(&full[i], 1);
+      mbar_init(&empty[i], 1);
+    }
+    mbar_init(&done, 1);
+    mbar_init(&tfree, 128);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tm = tmem_base;
+  const uint32_t sbase0 = (smem_u32(smem) + 1023u) & ~1023u;
+
+  if (warp == 0 && lane == 0) {
+    // ---- TMA producer: planes 0, 1, 2 back to back through one ring ----
+    int n = 0;
+    for (int pl = 0; pl < 3; ++pl) {
+      const CUtensorMap* ta = pl == 0 ? &tmA0 : pl == 1 ? &tmA1 : &tmA2;
+      const CUtensorMap* tb = pl == 0 ? &tmB0 : pl == 1 ? &tmB1 : &tmB2;
+      for (int it = 0; it < nkb; ++it, ++n) {
+        const int st = n % nstages;
+        const uint32_t ph = (uint32_t)(n / nstages) & 1u;
+        mbar_wait(&empty[st], ph ^ 1u);
+        mbar_expect_tx(&full[st], STAGE);
+        const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
+#pragma unroll
+        for (int i = 0; i < S; ++i) tma_load_3d(sb + i * A_BYTES, ta, it * KB, mt * BM, i, &full[st]);
+#pragma unroll
+        for (int j = 0; j < S; ++j) tma_load_3d(sb + S * A_BYTES + j * B_BYTES, tb, it * KB, q * BN, j, &full[st]);
+      }
+    }
+  } else if (warp == 1 && lane == 0) {
+    // ---- MMA issuer ----
+    int n = 0;
+    for (int pl = 0; pl < 3; ++pl) {
+      if (pl > 0) {  // the epilogue warps have read plane pl-1 out of TMEM
+        mbar_wait(&tfree, (uint32_t)(pl - 1) & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      }
+      for (int it = 0; it < nkb; ++it, ++n) {
+        const int st = n % nstages;
+        const uint32_t ph = (uint32_t)(n / nstages) & 1u;
+        mbar_wait(&full[st], ph);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
+#pragma unroll
+        for (int kk = 0; kk < KB / 32; ++kk) {
+#pragma unroll
+          for (int i = 0; i < S; ++i) {
+            const uint64_t da = desc_sw64(sb + i * A_BYTES) + 2 * kk;
+#pragma unroll
+            for (int j = 0; j < S - i; ++j) {
+              const uint64_t db = desc_sw64(sb + S * A_BYTES + j * B_BYTES) + 2 * kk;
+              mma_i8(tm + (uint32_t)(i + j) * BN, da, db, IDESC, (it | kk | i) ? 1u : 0u);
+            }
+          }
+        }
+        mma_commit(&empty[st]);
+      }
+      mma_commit(&done);
+    }
+  } else if (warp >= 2) {
+    // ---- epilogue warps: thread = row g of the tile ----
+    const int wq = warp & 3;
+    const long long m = (long long)mt * BM + wq * 32 + lane;
+    const bool row_ok = m < mvalid;
+    const int em = row_ok ? ea[m] : 0;
+    if (row_ok)
+      for (int j = 0; j < BN; ++j)
+        if (q * BN + j < nb) asm volatile("prefetch.global.L2 [%0];" ::"l"(out + (size_t)(q * BN + j) * ldo + m));
+    for (int pl = 0; pl < 3; ++pl) {
+      mbar_wait(&done, (uint32_t)pl & 1u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      double val[BN];
+#pragma unroll
+      for (int n0 = 0; n0 < BN; n0 += 8) {
+        uint32_t v[S][8];
+#pragma unroll
+        for (int L = 0; L < S; ++L) {
+          const uint32_t ta = tm + ((uint32_t)(wq * 32) << 16) + (uint32_t)(L * BN + n0);
+          asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                       : "=r"(v[L][0]), "=r"(v[L][1]), "=r"(v[L][2]), "=r"(v[L][3]), "=r"(v[L][4]), "=r"(v[L][5]), "=r"(v[L][6]),
+                         "=r"(v[L][7])
+                       : "r"(ta));
+        }
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int j = 0; j < 8; ++j) val[n0 + j] = 0.0;
+#pragma unroll
+        for (int L = S - 1; L >= 0; --L) {
+          const double w = 1.0 / (double)(1ULL << (8 * L));
+#pragma unroll
+          for (int j = 0; j < 8; ++j) val[n0 + j] = fma((double)(int)v[L][j], w, val[n0 + j]);
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&tfree)) : "memory");
+      const double cr = pl == 0 ? 1.0 : pl == 1 ? -1.0 : 0.0, ci = pl == 2 ? 4.0 : -1.0;
+      if (row_ok) {
+#pragma unroll
+        for (int j = 0; j < BN; ++j) {
+          const int b = q * BN + j;
+          if (b < nb) {
+            const double x = scalbn(val[j], em + eb[b] - 14);
+            double2* o = out + (size_t)b * ldo + m;
+            double2 t = *o;
+            t.x = fma(cr, x, t.x);
+            t.y = fma(ci, x, t.y);
+            *o = t;
+          }
+        }
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) {
+    __syncwarp();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "r"(TCOLS) : "memory");
+  }
+}
+// A operand of k_oz_vnl3: X[rows = p][ldx] -> out[sl][plane][g][kpad], k = p, row g scaled by 2^-e[g]; 16 rows p per thread
+template <int S>
+__global__ void __launch_bounds__(128)
+k_oz_slice_t3(const double2* __restrict__ X, long long ldx, int rows, long long n, const int* __restrict__ e,
+              int8_t* __restrict__ out, long long kpad, long long plane_stride, long long slice_stride) {
+  const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (g >= n) return;
+  const int p0 = blockIdx.y * 16;
+  const int ex = -e[g];
+  double re[16], im[16], sm[16];
+#pragma unroll
+  for (int t = 0; t < 16; ++t) {
+    double2 v = make_double2(0.0, 0.0);
+    if (p0 + t < rows) v = X[(size_t)(p0 + t) * ldx + g];
+    re[t] = scalbn(v.x, ex);
+    im[t] = scalbn(v.y, ex);
+    sm[t] = 0.5 * (re[t] + im[t]);
+  }
+  uint4 o[S];
+  int8_t* base = out + (size_t)g * kpad + p0;
+  slice16<S>(re, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride) = o[sl];
+  slice16<S>(im, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride + plane_stride) = o[sl];
+  slice16<S>(sm, o);
+#pragma unroll
+  for (int sl = 0; sl < S; ++sl) *reinterpret_cast<uint4*>(base + (size_t)sl * slice_stride + 2 * plane_stride) = o[sl];
+}
+
 }  // namespace oz
 }  // namespace qehpsi

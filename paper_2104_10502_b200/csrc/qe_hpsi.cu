@@ -104,6 +104,9 @@ struct qe_hpsi_handle {
   bool oz_3m = false;
   long long oz_k1c = 0;
   CUtensorMap oz_tm_a3[3] = {}, oz_tm_b3[3] = {};
+  bool oz_3m8 = false;  // a8 in the 3M form too (k_oz_vnl3): needs the padded nproj within one exact-int32 K range
+  long long oz_k2c = 0;
+  CUtensorMap oz_tm_a4[3] = {}, oz_tm_b4[3] = {};
   // NEXT-2: overlap operator S (q blocks packed like D; qbecp/qbT mirror dbecp/dbT)
   long long d_total = 0;
   double* qpk = nullptr;
@@ -701,7 +704,11 @@ cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
     oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
                                                                                       k1, (long long)h->nproj * k1, 0);
   oz::k_oz_colexp<<<(unsigned)((h->npw + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg);
-  if (h->gamma)  // real form: rows 2g + c, K = p
+  if (h->oz_3m8) {
+    if ((e = cudaFuncSetAttribute(oz::k_oz_vnl3<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem)) != cudaSuccess) return e;
+    oz::k_oz_slice_t3<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(h->oz_k2c / 16)), 128, 0, st>>>(
+        h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, h->oz_k2c, (long long)h->npw * h->oz_k2c, 3LL * h->npw * h->oz_k2c);
+  } else if (h->gamma)  // real form: rows 2g + c, K = p
     oz::k_oz_slice_tp<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
         h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, 2LL * h->npw * k2);
   else
@@ -745,7 +752,10 @@ template <int S>
 void oz_vnl_slice_t(qe_hpsi_handle* h, const double2* bT, int nb, cudaStream_t st) {
   const long long k2 = h->oz_k2;
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb);
-  if (h->gamma)  // dbecp is real: K = p
+  if (h->oz_3m8)  // planes Re, Im, (Re + Im) / 2 of dbecp^T, K = p
+    oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k2c / 16 + 127) / 128), nb), 128, 0, st>>>(
+        bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, h->oz_k2c, (long long)h->max_batch * h->oz_k2c, 3LL * h->max_batch * h->oz_k2c, 1.0);
+  else if (h->gamma)  // dbecp is real: K = p
     oz::k_oz_slice_re<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), nb), 128, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
                                                                                   2LL * h->max_batch * k2);
   else
@@ -756,6 +766,12 @@ template <int S>
 void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   const int nkb = (int)(h->oz_k2 / oz::KB);
   // the K ranges (int32 level sums must stay exact) accumulate into the same hpsi entries: one launch after the other
+  if (h->oz_3m8) {
+    oz::k_oz_vnl3<S><<<dim3((nb + oz::BN - 1) / oz::BN, (unsigned)((h->npw + oz::BM - 1) / oz::BM), 1), oz::NT, h->oz_smem, st>>>(
+        h->oz_tm_a4[0], h->oz_tm_a4[1], h->oz_tm_a4[2], h->oz_tm_b4[0], h->oz_tm_b4[1], h->oz_tm_b4[2], h->oz_stages,
+        (int)(h->oz_k2c / oz::KB), h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh);
+    return;
+  }
   const long long mrows = (h->gamma ? 2LL : 1LL) * h->npw;  // Gamma-only: rows 2g + c of the planar transposed digits
   const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (unsigned)((mrows + oz::BM - 1) / oz::BM), 1);
   auto kern = h->gamma ? oz::k_oz_gemm<S, 3> : oz::k_oz_gemm<S, 1>;
@@ -792,6 +808,11 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   // 3M form of a6 (three real GEMMs instead of a real-form complex one: -25 % MMAs, three launches): pays from ~2^26 entries of beta
   h->oz_3m = !h->gamma && env_int("QE_HPSI_OZ_3M", (long long)h->nproj * h->npw >= (1LL << 26) ? 1 : 0) != 0;
   h->oz_k1c = round_up(h->npw, 128);
+  h->oz_k2c = round_up(h->nproj, 128);
+  // a8 in the 3M form: one exact-int32 K range, and enough K blocks per plane to amortise the three epilogues (measured: pays at
+  // nproj = 1728, not at 1024); QE_HPSI_OZ_3M=2: 3M form for a6 only, 3: for a8 whatever nproj is (testing)
+  const int m3 = env_int("QE_HPSI_OZ_3M", 1);
+  h->oz_3m8 = h->oz_3m && h->oz_k2c <= kmax && m3 != 2 && (h->oz_k2c >= 1536 || m3 == 3);
   const long long ka6 = h->oz_3m ? h->oz_k1c : k1;  // contraction length of one a6 GEMM (reals)
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
   h->oz_stages = std::min(oz::MAX_STAGES, (222 * 1024) / stage);
@@ -815,7 +836,7 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
   h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
   const long long a2rows = (h->gamma ? 2LL : 1LL) * h->npw;
-  const size_t a1 = h->oz_3m ? (size_t)S * 3 * h->nproj * h->oz_k1c : (size_t)S * h->nproj * k1, a2 = (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
+  const size_t a1 = h->oz_3m ? (size_t)S * 3 * h->nproj * h->oz_k1c : (size_t)S * h->nproj * k1, a2 = h->oz_3m8 ? (size_t)S * 3 * h->npw * h->oz_k2c : (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
   const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit * (h->oz_3m ? 3 : 1);
   if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
@@ -845,6 +866,13 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
                        oz::BM) ||
           !oz_make_map(&h->oz_tm_b3[pl], h->oz_b + (size_t)pl * max_batch * h->oz_k1c, h->oz_k1c, max_batch, S,
                        3LL * max_batch * h->oz_k1c, oz::BN))
+        return cudaErrorNotSupported;
+  if (h->oz_3m8)
+    for (int pl = 0; pl < 3; ++pl)
+      if (!oz_make_map(&h->oz_tm_a4[pl], h->oz_a2 + (size_t)pl * h->npw * h->oz_k2c, h->oz_k2c, h->npw, S, 3LL * h->npw * h->oz_k2c,
+                       oz::BM) ||
+          !oz_make_map(&h->oz_tm_b4[pl], h->oz_b + (size_t)pl * max_batch * h->oz_k2c, h->oz_k2c, max_batch, S,
+                       3LL * max_batch * h->oz_k2c, oz::BN))
         return cudaErrorNotSupported;
 #define OZ_CALL(S_) e = oz_prepare_t<S_>(h, st)
   OZ_DISPATCH(S, OZ_CALL)
@@ -1975,7 +2003,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2) : 4;
+    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : 4;
   }
   return total;
 }

@@ -42,16 +42,17 @@ def test_default_handle_runs_the_int8_path_and_the_flag_turns_it_off():
     h.destroy()
 
 
-@pytest.mark.parametrize("three_m", [0, 1])
+@pytest.mark.parametrize("three_m", [0, 1, 3])
 @pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
 def test_becp_and_vnl_against_oracle(cfg, three_m):
-    """Both forms of a6: the real-form complex GEMM and the integer 3M form (three real GEMMs on planar digit planes)."""
+    """Both forms of a6 and a8: the real-form complex GEMMs and the integer 3M forms (three real GEMMs on planar digit planes;
+    QE_HPSI_OZ_3M = 1: a6, and a8 from nproj 1536; 3: both whatever the size)."""
     os.environ["QE_HPSI_OZ_3M"] = str(three_m)
     try:
         h, inp = _make_int8(cfg)
     finally:
         del os.environ["QE_HPSI_OZ_3M"]
-    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_3m"] == three_m
+    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_3m"] == (1 if three_m else 0)
     wl = inp["wl"]
     npw = h.npw
     psi, out, becp = _nonlocal(h, inp, wl.nbands)
