@@ -434,16 +434,20 @@ def main():
     if wl.nproj and oz_s and t_vnl + t_becp > t_fft:
         # projector contractions on the int8 tensor cores: S (S+1) / 2 digit-pair products per real product, each exact
         pairs = oz_s * (oz_s + 1) // 2
-        kname, t_k = ("k_oz_gemm<S,1> (a8)", t_vnl) if t_vnl >= t_becp else ("k_oz_gemm<S,0|2> (a6)", t_becp)
+        m3 = info.get("ozaki_3m", 0)  # 1: a6 in the integer 3M form (3 real products per complex one), 2: a8 too
+        a8_is_top = t_vnl >= t_becp
+        kname, t_k = (("k_oz_vnl3<S> (a8, 3M form)" if m3 == 2 else "k_oz_gemm<S,1> (a8)"), t_vnl) if a8_is_top else \
+            (("k_oz_gemm<S,2> x 3 (a6, 3M form)" if m3 else "k_oz_gemm<S,0> (a6)"), t_becp)
         ops_launch = pairs * flops_launch  # 4 real MACs per complex MAC x 2 ops x pairs
-        if t_vnl < t_becp and info.get("ozaki_3m"):
-            ops_launch *= 0.75  # a6 in the integer 3M form executes 3 real products per complex one
+        if (a8_is_top and m3 == 2) or (not a8_is_top and m3 >= 1):
+            ops_launch *= 0.75
         ach = ops_launch / (t_k * 1e-3) * 1e-12
         bf16_sus = float(mp.get("bf16_tflops_sustained", 0.0)) or 1414.0
         peak = 2.0 * bf16_sus
         t_slice = stage["a6_a8_int8_digits"][0]
         roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
-                    "traffic": committed_traffic(args.config, "k_oz_gemm_a8" if t_vnl >= t_becp else "k_oz_gemm_a6"),
+                    "traffic": committed_traffic(args.config, ("k_oz_vnl3" if m3 == 2 else "k_oz_gemm_a8") if a8_is_top else
+                                                  ("k_oz_gemm_a6_3m" if m3 else "k_oz_gemm_a6")),
                     "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; "
                     "the kernel runs inside a long step); a register-free UTCIMMA loop on the same chip measured 4540 TOP/s "
                     "(profiles/r1g_int8.md)", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
@@ -452,12 +456,12 @@ def main():
                     "digit_kernels_ms_per_launch": t_slice,
                     "note": "achieved = executed int8 ops of the S-digit split (every one of them is needed for the FP64 result); "
                             "fp64_equivalent_tflops = 8 flops per complex MAC / time, comparable with the FP64 DMMA peak"}
-        a6_units = 0.75 if info.get("ozaki_3m") else 1.0  # integer 3M form of a6: 6 of the 8 tile-GEMM units
-        t_int8 = pairs * m["f_proj"] * 0.5 * (1.0 + a6_units) / (peak * 1e12)
+        a6_units = (0.75 if m3 >= 1 else 1.0) + (0.75 if m3 == 2 else 1.0)  # integer 3M forms: 6 of the 8 tile-GEMM units each
+        t_int8 = pairs * m["f_proj"] * 0.5 * a6_units / (peak * 1e12)
         b_beta8 = 2.0 * oz_s * 2 * wl.nproj * npw / wl.batch  # int8 digit planes of beta, streamed once by a6 and once by a8
         roof8 = max((m["b_fft"] + b_beta8) / (hbm_peak * 1e9), t_int8)
         int8 = {"bands_per_s": 1.0 / roof8, "frac": value / world * roof8, "int8_tops": peak, "bytes_per_band": m["b_fft"] + b_beta8,
-                "int8_ops_per_band": pairs * m["f_proj"] * 0.5 * (1.0 + a6_units), "note": "max(bytes/HBM, digit-pair int8 ops/int8 tensor peak) per band"}
+                "int8_ops_per_band": pairs * m["f_proj"] * 0.5 * a6_units, "note": "max(bytes/HBM, digit-pair int8 ops/int8 tensor peak) per band"}
     elif wl.nproj and t_vnl + t_becp > t_fft:
         kname, t_k = ("k_vnl_add", t_vnl) if t_vnl >= t_becp else ("k_becp", t_becp)
         ach = flops_launch / (t_k * 1e-3) * 1e-12
@@ -490,7 +494,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": wl.name, "nbands": nb, "batch": batch, "grid": list(wl.nr), "npw": npw, "nproj": wl.nproj,
-                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["ozaki_nsplit"] if info.get("ozaki_slices") else info["nsplit"], "projector_path": (f"int8 digits x{info['ozaki_slices']} (tcgen05)" + (", a6 in the integer 3M form" if info.get("ozaki_3m") else "")) if info.get("ozaki_slices") else "fp64 dmma (3M)", "cuda_graph": bool(use_graph),
+                       "sticks": info["S"], "planes": info["P"], "fft_band_chunk": info["fft_nb"], "split_k": info["ozaki_nsplit"] if info.get("ozaki_slices") else info["nsplit"], "projector_path": (f"int8 digits x{info['ozaki_slices']} (tcgen05)" + ({0: "", 1: ", a6 in the integer 3M form", 2: ", a6 and a8 in the integer 3M form"}[info.get("ozaki_3m", 0)])) if info.get("ozaki_slices") else "fp64 dmma (3M)", "cuda_graph": bool(use_graph),
                        "l2": "inputs per step exceed L2" if flush is None else "L2 flushed (256 MB write) between steps",
                        "sharding": "bands / k-point pools per rank, no collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": h.launch_count(batch) * chunks_per_step * args.steps if nb % batch == 0

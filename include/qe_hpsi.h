@@ -125,7 +125,7 @@ int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands);
 /* info[0..15]: npw, S, P, fft band chunk, split-K count (FP64 path), workspace bytes, per axis j=0..2 the number of
  * generic FFT passes, K chunk, x split, SM count, two-pass FFT plan in use, then the projector path: [13] digits per
  * FP64 operand of the int8 path (0 = FP64 tensor path), [14] its split-K count of a6, [15] 1 if a6 runs in the
- * integer 3M form.  For the roofline report and the tests. */
+ * integer 3M form, 2 if a8 does too.  For the roofline report and the tests. */
 int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);
 const char* qe_hpsi_strerror(int status);
 int qe_hpsi_last_cuda_error(qe_hpsi_t h);    /* cudaError_t of the last QE_HPSI_ECUDA (0 if none)               */

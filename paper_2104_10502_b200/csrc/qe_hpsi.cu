@@ -2027,7 +2027,7 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[12] = h->f2p[0] ? 1 : 0;
   info[13] = h->oz_s;
   info[14] = h->oz_nsplit;
-  info[15] = h->oz_3m ? 1 : 0;
+  info[15] = h->oz_3m ? (h->oz_3m8 ? 2 : 1) : 0;
   return QE_HPSI_OK;
 }
 
