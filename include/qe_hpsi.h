@@ -56,8 +56,8 @@ typedef enum {
                                  /* 8-bit digits (per-row exponent) whose products are summed exactly on the int8    */
                                  /* tensor cores (tcgen05, int32 level sums in TMEM) and recombined in FP64:         */
                                  /* |error| <= ~(S+1) 2^(-8S+1) K max|a| max|b| per contraction (2^-47 = 7e-15);     */
-                                 /* costs 2 S bytes per complex entry of beta for a8 (transposed planes) and 3 S for */
-                                 /* a6 (planes Re, Im, half sum of its integer 3M form; 2 S below 2^26 entries).     */
+                                 /* costs 3 S bytes per complex entry of beta for a6 and 3 S for a8 (planes Re, Im,  */
+                                 /* half sum of the integer 3M forms; 2 S each for small problems).                  */
                                  /* Default only when nproj * npw >= 2^20 (smaller steps are launch-latency bound).  */
                                  /* Env QE_HPSI_OZAKI = 0 | 4..7 forces the digit count (0 = same as this flag).     */
                                  /* Non-finite operands are not propagated by the int8 path (use this flag for them). */
