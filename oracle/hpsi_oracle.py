@@ -35,8 +35,10 @@ potential shift; rank-1 projector), FFT round trip / Parseval / naive O(n^2) DFT
 covariance, time reversal at k=0, linearity, A == A' == B on tiny cases, independently enumerated npw counts
 (tests/golden/npw_counts.txt from SURVEY.md 8 table). The functions of the "next" rows at the end of the file
 (`spsi_of`, `overlap_of`, `psi_r`, `density_of`) are pinned in tests/test_oracle_next.py (rank-1 closed form, brute-force
-loops, Hermiticity, single / two plane-wave closed forms, Parseval, explicit DFT matrices). Nothing here is "parity
-unpinned".
+loops, Hermiticity, single / two plane-wave closed forms, Parseval, explicit DFT matrices). The error metric `rel_l2`
+(the gate of every parity assertion) is pinned by hand-built vectors with known per-band errors
+(test_rel_l2_is_per_band_relative_to_the_reference); the `becp=` branch of `hpsi_rows` by
+test_sampled_rows_with_becp_accumulated_over_atom_chunks. Nothing here is "parity unpinned".
 """
 from __future__ import annotations
 

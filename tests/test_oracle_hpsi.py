@@ -262,8 +262,66 @@ def test_config1_sampled_rows_match_dual_space():
     assert np.abs(ap - b[:, rows]).max() < 1e-13 * np.abs(b).max()
 
 
+def test_sampled_rows_with_becp_accumulated_over_atom_chunks():
+    """The `becp=` branch of hpsi_rows (what the full-size GPU tests use: beta streamed in atom chunks, only its columns at
+    the sampled rows kept) against the dense definition on a tiny case and against the in-memory branch on config 1."""
+    p = problem("T1_general_k")
+    wl, npw = p["wl"], p["miller"].shape[0]
+    rows = np.array([0, 3, npw // 2, npw - 1])
+    vt = orc.vloc_coeffs(p["vr"])
+    nh = wl.nh
+    becp = np.zeros((wl.nproj, p["psi"].shape[0]), complex)
+    for a in range(wl.natoms):  # one atom per chunk
+        becp[a * nh:(a + 1) * nh] = orc.becp_of(p["beta"][a * nh:(a + 1) * nh], p["psi"])
+    got = orc.hpsi_rows(rows, p["miller"], p["g2kin"], p["nr"], vt, p["psi"], p["beta"][:, rows], p["dblocks"], becp=becp)
+    hd = orc.dense_h(p["miller"], p["g2kin"], p["nr"], p["vr"], p["beta"], p["dblocks"])
+    ref = orc.hpsi_dense(hd, p["psi"])[:, rows]
+    assert np.abs(got - ref).max() < 1e-13 * np.abs(ref).max()
+    # full beta passed together with becp: the columns are picked inside
+    got2 = orc.hpsi_rows(rows, p["miller"], p["g2kin"], p["nr"], vt, p["psi"], p["beta"], p["dblocks"], becp=becp)
+    assert np.array_equal(got, got2)
+    # a wrong becp must show (the branch really uses what it is given)
+    bad = orc.hpsi_rows(rows, p["miller"], p["g2kin"], p["nr"], vt, p["psi"], p["beta"][:, rows], p["dblocks"], becp=2 * becp)
+    assert np.abs(bad - ref).max() > 1e-6 * np.abs(ref).max()
+
+
 # ---------------------------------------------------------------------------------------------------------
-# generators (inputs.py holds no method arithmetic; these check the recipe of SURVEY 8(c) items 6-10)
+# the error metric every parity assertion goes through (SURVEY.md 8(c) item 12)
+# ---------------------------------------------------------------------------------------------------------
+
+
+def test_rel_l2_is_per_band_relative_to_the_reference():
+    """rel_l2(x, ref)[b] = ||x_b - ref_b||_2 / ||ref_b||_2 over the entries of band b, hand-built so that a wrong axis,
+    a wrong normaliser, a dropped square root or an average over bands each gives a different number."""
+    ref = np.array([[3.0, 4.0j, 0.0], [3.0, 4.0j, 0.0], [0.0, 0.0, 10.0], [6.0, 8.0j, 0.0]])  # norms 5, 5, 10, 10
+    x = ref.copy()
+    x[1, 1] += 5e-3            # off by a known vector of norm 5e-3 -> 1e-3 exactly
+    x[2] += np.array([3e-6j, 0.0, 4e-6])  # norm 5e-6 against 10 -> 5e-7
+    x[3, 2] += 1e-2j           # purely imaginary error in an entry where ref is 0 -> 1e-3 of norm 10
+    err = orc.rel_l2(x, ref)
+    assert err.shape == (4,) and err.dtype == np.float64
+    assert err[0] == 0.0
+    np.testing.assert_allclose(err[1:], [1e-3, 5e-7, 1e-3], rtol=1e-9)  # x = ref + e is rounded: (10 + 4e-6) - 10 is exact to 1e-10
+    # one bad band among many good ones is not averaged away, and the good ones stay exact
+    big = np.tile(ref[:1], (1000, 1))
+    y = big.copy()
+    y[417, 0] += 0.05
+    e = orc.rel_l2(y, big)
+    assert e[417] == pytest.approx(1e-2, rel=1e-12) and np.count_nonzero(e) == 1
+    # relative to ||ref||, not to ||x||: scaling x's error direction changes the numerator only
+    r1 = np.array([[1.0, 0.0]])
+    assert orc.rel_l2(np.array([[3.0, 0.0]]), r1)[0] == pytest.approx(2.0, rel=1e-15)   # ||x-ref|| / ||ref|| = 2, / ||x|| would be 2/3
+    # invariant under a common scale, linear in the error
+    np.testing.assert_allclose(orc.rel_l2(8.0 * x, 8.0 * ref), err, rtol=1e-13)  # power of two: exact scaling
+    np.testing.assert_allclose(orc.rel_l2(ref + 3.0 * (x - ref), ref), 3.0 * err, rtol=1e-9)
+    # long-double accumulation: tiny errors on a large reference do not vanish in the subtraction of squares
+    ref2 = np.full((1, 4096), 1.0 + 0j)
+    x2 = ref2 * (1.0 + 2.0 ** -50)
+    assert orc.rel_l2(x2, ref2)[0] == pytest.approx(2.0 ** -50, rel=1e-6)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# generators(inputs.py holds no method arithmetic; these check the recipe of SURVEY 8(c) items 6-10)
 # ---------------------------------------------------------------------------------------------------------
 
 
