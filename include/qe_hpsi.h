@@ -14,6 +14,9 @@
  * H builder of an iterative eigensolver; the caller owns streams and synchronisation
  * (PAPER.md:L134-136).
  *
+ * This header is the PRODUCT boundary.  Measurement and test helpers (stage entry points, stage timers, the FP64
+ * peak probe, launch counts) are exported by the same library but declared in qe_hpsi_test.h.
+ *
  * Conventions shared by all calls
  *   - `at[9]`: lattice vectors a_1,a_2,a_3 as rows (row-major 3x3), bohr.  Reciprocal rows b_j, a_i.b_j = 2 pi d_ij.
  *   - `xk[3]`: Cartesian k in bohr^-1.  `nr[3]`: FFT grid N1,N2,N3; every N_j must factor into 2,3,5.
@@ -26,6 +29,8 @@
  *   - "dev" pointers are CUDA device pointers on the current device, "host" pointers ordinary host memory.
  *   - Every function returns 0 (QE_HPSI_OK) or a negative qe_hpsi_status; none throws, aborts or exits.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns QE_HPSI_ECUDA.
+ *   - Arithmetic: FP64 throughout by default.  The only other accuracy class (int8 digit products for the projector
+ *     contractions) is an explicit create flag, never chosen by problem size, device or environment.
  */
 #ifndef QE_HPSI_H
 #define QE_HPSI_H
@@ -40,27 +45,40 @@ typedef struct qe_hpsi_handle* qe_hpsi_t;
 
 typedef enum {
   QE_HPSI_OK = 0,
-  QE_HPSI_EINVAL = -1, /* null pointer, negative size, ld < npw, psi aliases hpsi, bad block table        */
+  QE_HPSI_EINVAL = -1, /* null pointer, negative size, ld < npw, psi aliases hpsi, bad block table, bad flags */
   QE_HPSI_EGRID = -2,  /* N_j has a prime factor other than 2,3,5, exceeds QE_HPSI_MAX_N, or is smaller  */
                        /* than the sphere's index extent along j (the sphere itself would wrap)          */
-  QE_HPSI_ENOMEM = -3, /* host or device allocation failed                                               */
-  QE_HPSI_ECUDA = -4,  /* CUDA runtime error; the cudaError_t is returned by qe_hpsi_last_cuda_error     */
-  QE_HPSI_ESTATE = -5  /* handle is NULL / destroyed                                                     */
+  QE_HPSI_ENOMEM = -3, /* host or device allocation failed (including the digit planes of QE_HPSI_PROJ_INT8) */
+  QE_HPSI_ECUDA = -4,  /* CUDA runtime error; the cudaError_t is returned by qe_hpsi_last_error          */
+  QE_HPSI_ESTATE = -5  /* handle is NULL / destroyed / not prepared for the call                         */
 } qe_hpsi_status;
 
 /* flags for qe_hpsi_create */
 #define QE_HPSI_BORROW_BETA 1u   /* use beta_dev in place (caller keeps it alive and unchanged) instead of copying */
 #define QE_HPSI_GENERIC_FFT 2u   /* (testing) use only radices 2,3,4,5 in the FFT passes                           */
-#define QE_HPSI_FP64_DMMA   4u   /* projector contractions a6 / a8 on the FP64 tensor pipe (mma.sync DMMA, 3M product) */
-                                 /* instead of the default: the FP64 operands are split error-free into S = 6 signed */
-                                 /* 8-bit digits (per-row exponent) whose products are summed exactly on the int8    */
-                                 /* tensor cores (tcgen05, int32 level sums in TMEM) and recombined in FP64:         */
-                                 /* |error| <= ~(S+1) 2^(-8S+1) K max|a| max|b| per contraction (2^-47 = 7e-15);     */
-                                 /* costs 3 S bytes per complex entry of beta for a6 and 3 S for a8 (planes Re, Im,  */
-                                 /* half sum of the integer 3M forms; 2 S each for small problems).                  */
-                                 /* Default only when nproj * npw >= 2^20 (smaller steps are launch-latency bound).  */
-                                 /* Env QE_HPSI_OZAKI = 0 | 4..7 forces the digit count (0 = same as this flag).     */
-                                 /* Non-finite operands are not propagated by the int8 path (use this flag for them). */
+#define QE_HPSI_FP64_DMMA   4u   /* projector contractions a6 / a8 on the FP64 tensor pipe (mma.sync DMMA, 3M       */
+                                 /* product).  THIS IS THE DEFAULT (the flag only names it): every product and sum   */
+                                 /* of the path is IEEE FP64, as in the paper's port (cuBLAS FP64 GEMM) */
+/* Opt-in accuracy class for a6 / a8: the FP64 operands are split into S signed 8-bit digits under one exponent per
+ * row (projector, plane wave or band), the digit products are summed EXACTLY on the int8 tensor cores (tcgen05
+ * kind::i8, int32 level sums in TMEM) and recombined in FP64.  This is block fixed point, not FP64: per contraction
+ *     |error| <= ~(S+1) 2^(-8S+1) K max|a| max|b|     (K = contraction length; relative to the ROW MAXIMA, not the entry)
+ * i.e. 8S-1 bits under the row exponent: S = 7 -> 55 bits, S = 6 -> 47 bits.  Digits: QE_HPSI_PROJ_DIGITS(4..7);
+ * 0 = 7.  Costs 3 S bytes per complex entry of beta for a6 and 3 S for a8 of device memory (2 S each for small
+ * problems) NEXT TO the FP64 beta: at S = 6 that is 2.25 x the size of beta (56 GB for the 25 GB beta of the
+ * largest benchmark workload), 2.6 x at S = 7.  If those planes cannot be allocated qe_hpsi_create FAILS with
+ * QE_HPSI_ENOMEM; it never changes the arithmetic silently.  Non-finite operands give NaN for the affected
+ * projector / band.  Needs an sm_100 device (tcgen05).
+ * QE_HPSI_PROJ_CERTIFY (with QE_HPSI_PROJ_INT8) adds an a-posteriori check of every int8 result and the automatic
+ * FP64 re-computation of the bands that fail it: see qe_hpsi_set_proj_tolerance. */
+#define QE_HPSI_PROJ_INT8    8u
+#define QE_HPSI_PROJ_CERTIFY 16u
+#define QE_HPSI_PROJ_DIGITS(s) (((unsigned)(s) & 15u) << 8)
+/* integer 3M forms of the int8 contractions (three real digit GEMMs per complex product instead of four).  Default:
+ * chosen by size (a6 from 2^26 entries of beta, a8 from 1536 projectors).  The forms differ in rounding only. */
+#define QE_HPSI_PROJ_3M_OFF (1u << 12)
+#define QE_HPSI_PROJ_3M_A6  (2u << 12)
+#define QE_HPSI_PROJ_3M_ALL (3u << 12)
 
 #define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */
 
@@ -82,6 +100,8 @@ int qe_hpsi_gsphere(const double at[9], const double xk[3], double ecutwfc, cons
  *   d_host     the real symmetric D^a blocks packed one after another, block a row-major nh_a x nh_a
  *              (nh_a = blk_off[a+1]-blk_off[a]), Ry.  COPIED.
  *   max_batch  largest number of bands processed as one internal chunk (workspace is sized for it), >= 1.
+ *   flags      OR of the QE_HPSI_* flags above; unknown bits, QE_HPSI_FP64_DMMA together with QE_HPSI_PROJ_INT8, a digit
+ *              count outside 4..7, or QE_HPSI_PROJ_CERTIFY / DIGITS / 3M without QE_HPSI_PROJ_INT8 give QE_HPSI_EINVAL.
  *   cuda_stream  cudaStream_t (NULL = default stream) on which create's device work is enqueued; create
  *              synchronises that stream before returning.
  * On failure *out = NULL. */
@@ -95,8 +115,9 @@ int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc, const dou
  *   accumulated; entries ig >= npw of each row untouched).  ldpsi, ldhpsi >= npw.  The two arrays must not
  *   overlap.  Any nbands >= 0; internally processed in chunks of at most max_batch bands; the result for a
  *   band does not depend on which other bands are in the call.
- * Asynchronous: all work is enqueued on cuda_stream, no host synchronisation, no device->host traffic.  Only
- * argument errors are reported synchronously.  One in-flight apply per handle (the workspace is shared). */
+ * Asynchronous: all work is enqueued on cuda_stream, no host synchronisation, no device->host traffic (also with
+ * QE_HPSI_PROJ_CERTIFY: the check and the re-computation are decided on the device).  Only argument errors are
+ * reported synchronously.  One in-flight apply per handle (the workspace is shared). */
 int qe_hpsi_apply(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
                   void* cuda_stream);
 
@@ -110,46 +131,38 @@ int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldpsi, void* h
  * used the handle. */
 int qe_hpsi_destroy(qe_hpsi_t h);
 
-/* ---- accessors (needed for the bit-exact map check, the roofline report and diagnostics) ---- */
+/* ---- accessors -------------------------------------------------------------------------------------------- */
 int64_t qe_hpsi_npw(qe_hpsi_t h);            /* sphere size, or a negative status                               */
 int64_t qe_hpsi_nsticks(qe_hpsi_t h);        /* S: (i1,i2) columns holding >= 1 sphere point                    */
 int64_t qe_hpsi_nplanes(qe_hpsi_t h);        /* P: i1 planes holding >= 1 sphere point                          */
 /* Copies the device-built maps into caller DEVICE arrays (any may be NULL): miller [npw][3] int32,
  * fft_index [npw] int32, g2kin [npw] float64.  Enqueued on cuda_stream. */
 int qe_hpsi_get_maps(qe_hpsi_t h, int32_t* miller_dev, int32_t* fftidx_dev, double* g2kin_dev, void* cuda_stream);
-/* Stage access for tests: becp = beta^H psi (a6) and dbecp = D becp (a7) of the LAST chunk applied, as
- * complex128 [nproj][nb_last] band-contiguous, into caller DEVICE arrays (either may be NULL). */
-int qe_hpsi_get_becp(qe_hpsi_t h, void* becp_dev, void* dbecp_dev, void* cuda_stream);
-/* Number of kernel launches qe_hpsi_apply enqueues for nbands bands (for the benchmark's gpu_launches). */
-int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands);
 /* info[0..15]: npw, S, P, fft band chunk, split-K count (FP64 path), workspace bytes, per axis j=0..2 the number of
  * generic FFT passes, K chunk, x split, SM count, two-pass FFT plan in use, then the projector path: [13] digits per
  * FP64 operand of the int8 path (0 = FP64 tensor path), [14] its split-K count of a6, [15] 1 if a6 runs in the
- * integer 3M form, 2 if a8 does too.  For the roofline report and the tests. */
+ * integer 3M form, 2 if a8 does too, +4 if QE_HPSI_PROJ_CERTIFY is on. */
 int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);
 const char* qe_hpsi_strerror(int status);
-int qe_hpsi_last_cuda_error(qe_hpsi_t h);    /* cudaError_t of the last QE_HPSI_ECUDA (0 if none)               */
+int qe_hpsi_last_error(qe_hpsi_t h);         /* cudaError_t of the last QE_HPSI_ECUDA (0 if none); h may be NULL */
 
-/* Stage timing for the roofline report.  mode 0 = off (default; apply records no events), 1 = CUDA events around
- * a6 (slot 0), a7 (slot 1), the whole a1-a5 chain (slot 2) and a8 (slot 3) of every chunk, 2 = additionally
- * around each of the five FFT kernels a1..a5 (slots 4..8; slot 2 is then not recorded).  Events are recorded
- * on the stream passed to apply.  qe_hpsi_profile resets the accumulators; qe_hpsi_profile_read synchronises
- * the pending events and returns, per slot, the summed milliseconds and the number of spans. */
-int qe_hpsi_profile(qe_hpsi_t h, int mode);
-int qe_hpsi_profile_read(qe_hpsi_t h, double ms[16], int64_t count[16]);
-
-/* Measurement helper (not on the hot path): runs register-resident FP64 DMMA (mma.sync m8n8k4.f64) and DFMA
- * loops on every SM for about `millis` ms each and returns the achieved TFLOP/s.  bench.py uses the DMMA
- * figure as the measured FP64 tensor peak of the box.  Synchronises the device. */
-int qe_hpsi_probe_fp64(double millis, double* dmma_tflops, double* dfma_tflops);
-
-/* Stand-alone stage entry points for tests and micro-benchmarks (same kernels the hot path launches):
- *   qe_hpsi_fft_local: hpsi = g2kin*psi + local term only (a1-a5), ignoring projectors.
- *   qe_hpsi_nonlocal:  hpsi += beta D beta^H psi (a6-a8) on top of the caller's hpsi contents. */
-int qe_hpsi_fft_local(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
-                      void* cuda_stream);
-int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, int nbands,
-                     void* cuda_stream);
+/* ---- certified int8 projector path (QE_HPSI_PROJ_INT8 | QE_HPSI_PROJ_CERTIFY) ------------------------------
+ * The agreement the paper reports between its CPU and GPU runs is an FP64 statement; the int8
+ * digit path is block fixed point and its worst-case bound (above) is far looser than what it delivers on smooth
+ * operands.  With QE_HPSI_PROJ_CERTIFY every chunk is checked a posteriori: the nonlocal
+ * part v_b = V_NL psi_b computed on the int8 path is kept apart, and for QE_HPSI_NPROBE random sign vectors s_t the
+ * identity  sum_G s_t(G) v_b(G) = <y_t|psi_b>,  y_t = V_NL^H s_t  (computed once, in FP64, at create) is tested;
+ *     est_b = sqrt( mean_t |sum_G s_t v_b - <y_t|psi_b>|^2 )      estimates ||v_b - V_NL psi_b||_2  (Freivalds / Hutchinson)
+ * to within a factor 2 with probability > 0.998 down to the FP64 rounding of the check itself (~1e-15 ||v_b||).
+ * Bands with est_b > tol * ||v_b||_2 (or a non-finite value) are re-computed on the FP64 tensor path -- selected, compacted and
+ * launched on the device, no host synchronisation -- and the FP64 result is what is added to hpsi.
+ * qe_hpsi_set_proj_tolerance: tol >= 0, default 1e-11 (north_star's parity tolerance, demanded of the nonlocal part alone).
+ * qe_hpsi_get_proj_check: for the LAST chunk applied, est_b / ||v_b|| per band into rel_dev [nb_last] (FP64, device) and
+ *   1 / 0 = re-computed in FP64 / int8 result kept into redo_dev [nb_last] (int32, device); either may be NULL; enqueued
+ *   on cuda_stream.  QE_HPSI_ESTATE if the handle was not created with QE_HPSI_PROJ_CERTIFY. */
+#define QE_HPSI_NPROBE 8
+int qe_hpsi_set_proj_tolerance(qe_hpsi_t h, double tol);
+int qe_hpsi_get_proj_check(qe_hpsi_t h, double* rel_dev, int32_t* redo_dev, void* cuda_stream);
 
 /* ---- rows SURVEY.md 8(f) marks "next": same kernels and tables as the hot path ---------------------------- */
 
@@ -159,7 +172,8 @@ int qe_hpsi_nonlocal(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi
  * synchronises).  qe_hpsi_apply_hs computes hpsi = H psi and spsi = S psi in one call: becp = beta^H psi (a6) is
  * computed once and shared; spsi[b][0..npw) is overwritten, entries >= npw untouched; spsi must not overlap psi or
  * hpsi.  hpsi_dev may be NULL (S psi only).  Without projectors S = 1.  QE_HPSI_ESTATE if set_s was never called
- * on a handle that has projectors.  Asynchronous on cuda_stream like qe_hpsi_apply. */
+ * on a handle that has projectors.  Asynchronous on cuda_stream like qe_hpsi_apply.  (Not certified: with
+ * QE_HPSI_PROJ_CERTIFY this call returns QE_HPSI_ESTATE.) */
 int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host);
 int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, void* spsi_dev,
                      int64_t ldspsi, int nbands, void* cuda_stream);
@@ -167,7 +181,8 @@ int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi
 /* NEXT-3, reduced matrices of the iterative diagonaliser: out[i][j] = <a_i|b_j> =
  * sum_G conj(a[i][G]) b[j][G] over the npw sphere entries, i < na, j < nb.  a_dev [na][lda], b_dev [nb][ldb]
  * complex128 (may be the same array), out_dev [na][ldo] complex128, ldo >= nb (entries j >= nb untouched).  Runs the
- * split-K DMMA kernel of step a6 with a fixed-order reduction (bit-reproducible).  Asynchronous on cuda_stream. */
+ * split-K DMMA kernel of step a6 with a fixed-order reduction (bit-reproducible).  Asynchronous on cuda_stream: no
+ * allocation, no synchronisation (the split-K workspace is part of the handle). */
 int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb,
                     void* out_dev, int64_t ldo, void* cuda_stream);
 
@@ -179,12 +194,19 @@ int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const v
  *                  sdiag_dev NULL means 1.
  * qe_hpsi_rotate:  y[k][G] (+)= sum_j coef[k][j] x[j][G], k < ny, j < nx, over the npw sphere entries; coef_dev complex128
  *                  [ny][ldcoef], ldcoef >= nx; accumulate = 0 overwrites y[k][0..npw).  Runs the DMMA kernel of step a8.
+ *                  All arguments are validated before anything is written.
+ * qe_hpsi_residual: r[b][G] = hx[b][G] - e[b] sx[b][G] for G < npw (r may be hx or sx), and rnorm2[b] = sum_G |r[b][G]|^2
+ *                  (rnorm2_dev [nb] FP64 on the device, may be NULL; fixed summation order, bit-reproducible).
+ * qe_hpsi_scale:   x[b][G] *= fac[b] (fac_dev [nb] FP64 on the device), e.g. normalisation of correction vectors.
  * All asynchronous on cuda_stream. */
 int qe_hpsi_hdiag(qe_hpsi_t h, double vbar, double* hdiag_dev, double* sdiag_dev, void* cuda_stream);
 int qe_hpsi_precond(qe_hpsi_t h, void* r_dev, int64_t ldr, int nb, const double* e_dev, const double* hdiag_dev,
                     const double* sdiag_dev, void* cuda_stream);
 int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int nx, const void* coef_dev, int64_t ldcoef, void* y_dev,
                    int64_t ldy, int ny, int accumulate, void* cuda_stream);
+int qe_hpsi_residual(qe_hpsi_t h, const void* hx_dev, int64_t ldh, const void* sx_dev, int64_t lds, const double* e_dev,
+                     void* r_dev, int64_t ldr, int nb, double* rnorm2_dev, void* cuda_stream);
+int qe_hpsi_scale(qe_hpsi_t h, void* x_dev, int64_t ldx, int nb, const double* fac_dev, void* cuda_stream);
 
 /* NEXT-4, charge density ("charge density generation"):
  *   rho[i1][i2][i3] += scale * sum_b occ[b] |psi_b(r_i)|^2,  psi_b(r_i) = sum_G psi[b][G] exp(+2 pi i n.i/N)
@@ -199,7 +221,8 @@ int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, int nbands,
  * n2 > 0, or n1 == n2 == 0 and n3 >= 0; order = the order those G have in the canonical full sphere (G = 0 first).
  * psi, hpsi and beta are complex128 arrays over the ngw half-sphere entries with Im(x[G=0]) = 0; beta(-G) = conj(beta(G))
  * is implied (projector functions real in real space).  The library transforms two bands per complex FFT and contracts
- * the projectors as real matrices over the 2*ngw real components.  Arguments as qe_hpsi_create / qe_hpsi_apply (no k). */
+ * the projectors as real matrices over the 2*ngw real components.  Arguments as qe_hpsi_create / qe_hpsi_apply (no k);
+ * flags as for qe_hpsi_create except QE_HPSI_PROJ_CERTIFY (QE_HPSI_EINVAL). */
 typedef struct qe_hpsi_gamma_handle* qe_hpsi_gamma_t;
 int qe_hpsi_gamma_gsphere(const double at[9], double ecutwfc, const int nr[3], int64_t* ngw, int32_t* miller_host);
 int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], double ecutwfc, const int nr[3], const double* vr_dev,

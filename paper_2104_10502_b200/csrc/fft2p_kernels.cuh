@@ -245,7 +245,7 @@ template <int RA, int RB>
 __global__ void __launch_bounds__(RA* FFT_C) k2p_x_vmul(FftGeom g, Fft2pGeom t, double2* __restrict__ w2, int nb) {
   constexpr int N = RA * RB;
   constexpr int NV = RB > 1 ? RB : RA;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tile1 = reinterpret_cast<double2*>(smem_raw);
   double2* tile2 = tile1 + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(RA* FFT_C) k2p_x_rho(FftGeom g, Fft2pGeom t, c
                                                        double* __restrict__ rho) {
   constexpr int N = RA * RB;
   constexpr int NV = RB > 1 ? RB : RA;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tile1 = reinterpret_cast<double2*>(smem_raw);
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
   const int i2 = blockIdx.x / g.ntz;

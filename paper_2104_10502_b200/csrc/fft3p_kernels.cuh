@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_scatter_zinv(FftGeom g
                                                                       long long ldpsi, double2* __restrict__ w1) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_zfwd_gather(FftGeom g,
                                                                      double2* __restrict__ hpsi, long long ldh) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_yinv(FftGeom g, Fft2pG
                                                               double2* __restrict__ w2) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_yfwd(FftGeom g, Fft2pG
                                                               double2* __restrict__ w1) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -211,7 +211,7 @@ template <int R1, int R2, int R3>
 __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_x_vmul(FftGeom g, Fft2pGeom t, double2* __restrict__ w2, int nb) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3p_x_rho(FftGeom g, Fft2p
                                                                double* __restrict__ rho) {
   using P = P3<R1, R2, R3>;
   constexpr int N = P::N;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tA = reinterpret_cast<double2*>(smem_raw);
   double2* tB = tA + N * FFT_C;
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;

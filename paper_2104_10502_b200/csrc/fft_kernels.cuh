@@ -35,7 +35,7 @@ __device__ __forceinline__ void tile_zero(double2* buf, int count, int tid) {
 // a1 ------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(FFT_NT) k_scatter_zinv(FftGeom g, const double2* __restrict__ psi, long long ldpsi,
                                                          double2* __restrict__ w1) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n3 * FFT_C;
   const int tid = threadIdx.x;
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(FFT_NT) k_scatter_zinv(FftGeom g, const double
 
 // a2 ------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(FFT_NT) k_yinv(FftGeom g, const double2* __restrict__ w1, double2* __restrict__ w2) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n2 * FFT_C;
   const int tid = threadIdx.x;
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(FFT_NT) k_yinv(FftGeom g, const double2* __res
 // One CTA owns the (i2, i3-tile) pencil group, keeps its V(r)/N tile in shared memory and loops over bands
 // b = blockIdx.y, blockIdx.y + gridDim.y, ... so that V is read once per CTA, not once per band.
 __global__ void __launch_bounds__(FFT_NT) k_x_vmul(FftGeom g, double2* __restrict__ w2, int nb) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n1 * FFT_C;
   double* vt = reinterpret_cast<double*>(bufB + g.n1 * FFT_C);
@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(FFT_NT) k_x_vmul(FftGeom g, double2* __restric
 // Dynamic shared memory: two [N1][FFT_C] tiles.  gridDim.y must be 1 (one CTA owns its pencils: no atomics).
 __global__ void __launch_bounds__(FFT_NT) k_x_rho(FftGeom g, const double2* __restrict__ w2, int nb,
                                                   const double* __restrict__ occ, double scale, double* __restrict__ rho) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n1 * FFT_C;
   const int tid = threadIdx.x;
@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(FFT_NT) k_x_rho(FftGeom g, const double2* __re
 
 // a4 ------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(FFT_NT) k_yfwd(FftGeom g, const double2* __restrict__ w2, double2* __restrict__ w1) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n2 * FFT_C;
   const int tid = threadIdx.x;
@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(FFT_NT) k_yfwd(FftGeom g, const double2* __res
 __global__ void __launch_bounds__(FFT_NT) k_zfwd_gather(FftGeom g, const double2* __restrict__ w1,
                                                         const double2* __restrict__ psi, long long ldpsi,
                                                         double2* __restrict__ hpsi, long long ldh) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* bufA = reinterpret_cast<double2*>(smem_raw);
   double2* bufB = bufA + g.n3 * FFT_C;
   const int tid = threadIdx.x;

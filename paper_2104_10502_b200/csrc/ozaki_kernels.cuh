@@ -29,6 +29,13 @@ constexpr int A_BYTES = BM * KB, B_BYTES = BN * KB;
 constexpr int MAX_STAGES = 4;
 // (L+1) * Kc * 128 * 128 < 2^31 for every level L < S: Kc <= 2^17 / S reals per CTA
 __host__ __device__ constexpr long long max_k_per_cta(int S) { return ((1LL << 17) / S) / KB * KB - KB; }
+constexpr int E_BAD = -(1 << 28);  // exponent sentinel of a row with a non-finite entry
+// 2^(ea+eb-14) d, or NaN when either operand row was non-finite
+__device__ __forceinline__ double oz_scale(double d, int ea, int eb) {
+  if (ea == E_BAD || eb == E_BAD) return __longlong_as_double(0x7ff8000000000000LL);
+  return scalbn(d, ea + eb - 14);
+}
+__device__ __forceinline__ bool not_finite(double2 v) { return !(fabs(v.x) <= 1.7976931348623157e308) || !(fabs(v.y) <= 1.7976931348623157e308); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t n) {
@@ -189,7 +196,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           for (int j = 0; j < 8; ++j) {
             const int b = q * BN + n0 + j;
             if (b < nb) {
-              const double val = scalbn(d[j], em + eb[b] - 14);
+              const double val = oz_scale(d[j], em, eb[b]);
               if (MODE == 2)
                 out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(val, 0.0);
               else
@@ -202,8 +209,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         for (int jj = 0; jj < 4; ++jj) {
           const int b = (q * BN + n0) / 2 + jj;
           if (b < nb) {
-            const int ex = em + eb[b] - 14;
-            const double re = scalbn(d[2 * jj], ex), im = scalbn(d[2 * jj + 1], ex);
+            const double re = oz_scale(d[2 * jj], em, eb[b]), im = oz_scale(d[2 * jj + 1], em, eb[b]);
             if (MODE == 0) {
               out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(re, im);
             } else {
@@ -227,7 +233,10 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // ---- exponents: smallest e with max |component| 2^-e <= 0.99 (0 for an all-zero row): the leading digit then fits an int8 ----
-__device__ __forceinline__ int exp_of(double mx) {
+// A row holding a NaN or an infinity gets the sentinel E_BAD: its digits are meaningless, and every epilogue writes NaN for
+// the outputs that depend on it (oz_scale), which is what the FP64 contraction would give.
+__device__ __forceinline__ int exp_of(double mx, bool bad) {
+  if (bad) return E_BAD;
   if (!(mx > 0.0)) return 0;
   int e = ilogb(mx) + 1;
   if (scalbn(mx, -e) > 0.99) ++e;
@@ -237,30 +246,37 @@ __device__ __forceinline__ int exp_of(double mx) {
 // one CTA per row of a complex matrix X[rows][ldx], n entries per row
 __global__ void __launch_bounds__(256) k_oz_rowexp(const double2* __restrict__ X, long long ldx, long long n, int* __restrict__ e) {
   __shared__ double red[256];
+  __shared__ int anybad;
+  if (threadIdx.x == 0) anybad = 0;
   const double2* x = X + (size_t)blockIdx.x * ldx;
   double mx = 0.0;
+  bool bad = false;
   for (long long i = threadIdx.x; i < n; i += 256) {
     const double2 v = x[i];
+    bad |= not_finite(v);
     mx = fmax(mx, fmax(fabs(v.x), fabs(v.y)));
   }
   red[threadIdx.x] = mx;
   __syncthreads();
+  if (bad) anybad = 1;
   for (int s = 128; s > 0; s >>= 1) {
     if (threadIdx.x < s) red[threadIdx.x] = fmax(red[threadIdx.x], red[threadIdx.x + s]);
     __syncthreads();
   }
-  if (threadIdx.x == 0) e[blockIdx.x] = exp_of(red[0]);
+  if (threadIdx.x == 0) e[blockIdx.x] = exp_of(red[0], anybad != 0);
 }
 // one thread per column g of X[rows][ldx]
 __global__ void __launch_bounds__(128) k_oz_colexp(const double2* __restrict__ X, long long ldx, int rows, long long n, int* __restrict__ e) {
   const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
   if (g >= n) return;
   double mx = 0.0;
+  bool bad = false;
   for (int p = 0; p < rows; ++p) {
     const double2 v = X[(size_t)p * ldx + g];
+    bad |= not_finite(v);
     mx = fmax(mx, fmax(fabs(v.x), fabs(v.y)));
   }
-  e[g] = exp_of(mx);
+  e[g] = exp_of(mx, bad);
 }
 
 // 16 reals -> S x 16 int8 (one 16-byte store per slice); r[] already scaled to [-0.99, 0.99].  Balanced radix-256 digits of the
@@ -565,7 +581,7 @@ k_oz_vnl3(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUte
         for (int j = 0; j < BN; ++j) {
           const int b = q * BN + j;
           if (b < nb) {
-            const double x = scalbn(val[j], em + eb[b] - 14);
+            const double x = oz_scale(val[j], em, eb[b]);
             double2* o = out + (size_t)b * ldo + m;
             double2 t = *o;
             t.x = fma(cr, x, t.x);

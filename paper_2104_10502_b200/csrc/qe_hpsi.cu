@@ -2,15 +2,17 @@
 // sequence of the hot path (a1-a8).  No torch types, no cuFFT / cuBLAS: every step runs in this library's kernels.
 // PAPER.md:L105 (the operation), L224-226 (the three terms), L176 (vi) (sphere + FFT mapping); formulas and
 // readings: DESIGN.md sections 2-3.
-#include "../../include/qe_hpsi.h"
+#include "../../include/qe_hpsi_test.h"
 
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -19,6 +21,7 @@
 #include "fft2t_kernels.cuh"
 #include "zgemm_kernels.cuh"
 #include "ozaki_kernels.cuh"
+#include "cert_kernels.cuh"
 
 using namespace qehpsi;
 
@@ -111,9 +114,20 @@ struct qe_hpsi_handle {
   long long d_total = 0;
   double* qpk = nullptr;
   double2 *qbecp = nullptr, *qbT = nullptr;
-  // NEXT-3: split-K workspace of qe_hpsi_overlap (grown on demand)
+  // NEXT-3: split-K workspace of qe_hpsi_overlap (allocated at create: its size depends on npw only)
   double2* ovl_partial = nullptr;
-  size_t ovl_cap = 0;
+  int ovl_ns = 1, ovl_kchunk = 0;
+  // QE_HPSI_PROJ_CERTIFY: a-posteriori check of the int8 nonlocal part + FP64 re-computation
+  bool certify = false;
+  double cert_tol = 1e-11;
+  long long cert_ld = 0;                      // row stride of the scratch arrays below
+  double2* cert_y = nullptr;                  // [QE_HPSI_NPROBE][cert_ld]  y_t = V_NL s_t (FP64 tensor path, at create)
+  double2 *cert_v8 = nullptr, *cert_psif = nullptr, *cert_vf = nullptr;  // [max_batch][cert_ld]: int8 v, compacted psi, FP64 v
+  double* cert_part = nullptr;                // [max_batch][cert_nch][2 NPROBE + 1] partial sums of the check
+  int cert_nch = 0;
+  double* cert_rel = nullptr;                 // [max_batch] est_b / ||v_b||
+  int *cert_redo = nullptr, *cert_slot = nullptr, *cert_list = nullptr, *cert_count = nullptr;
+  double2 *partial_f = nullptr, *becp_f = nullptr, *dbecp_f = nullptr, *dbT_f = nullptr;  // a6-a7 buffers of the re-computation
   bool rho_attr_done = false;
   // NEXT-1: this handle is the half-sphere nonlocal part of a Gamma-only handle (real becp, two real DMMAs per block)
   bool gamma = false;
@@ -154,11 +168,11 @@ namespace {
     }                                                     \
   } while (0)
 
-int g_last_cuda = 0;
+std::atomic<int> g_last_cuda{0};  // last CUDA error of calls that have no handle (diagnostic only)
 
 // ---- stage timing helpers ---------------------------------------------------------------------------------
 enum { SLOT_BECP = 0, SLOT_DMUL = 1, SLOT_FFT = 2, SLOT_VNL = 3, SLOT_A1 = 4, SLOT_A2 = 5, SLOT_A3 = 6, SLOT_A4 = 7, SLOT_A5 = 8,
-       SLOT_OZ_SLICE = 9 };
+       SLOT_OZ_SLICE = 9, SLOT_CERT = 10 };
 
 void prof_drain(qe_hpsi_handle* h) {
   if (h->prof_spans.empty()) {
@@ -185,7 +199,12 @@ size_t prof_mark(qe_hpsi_handle* h, cudaStream_t st) {
     } else {
       cudaEvent_t e;
       if (cudaEventCreate(&e) != cudaSuccess) return (size_t)-1;
-      h->prof_pool.push_back(e);
+      try {
+        h->prof_pool.push_back(e);
+      } catch (...) {  // out of host memory: this span is simply not timed
+        cudaEventDestroy(e);
+        return (size_t)-1;
+      }
     }
   }
   const size_t i = h->prof_used++;
@@ -194,7 +213,10 @@ size_t prof_mark(qe_hpsi_handle* h, cudaStream_t st) {
 }
 void prof_span(qe_hpsi_handle* h, size_t e0, size_t e1, int slot) {
   if (e0 == (size_t)-1 || e1 == (size_t)-1 || e1 < e0) return;
-  h->prof_spans.push_back({e0, e1, slot});
+  try {
+    h->prof_spans.push_back({e0, e1, slot});
+  } catch (...) {
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -447,10 +469,10 @@ int build_sphere(const SphereGeom& sg, cudaStream_t st, SphereOut* out) {
   qe_hpsi_handle* h = nullptr;
   const long long ntot = (long long)sg.n1 * sg.n2 * sg.n3;
   const int nblk = (int)((ntot + SPH_NT * SPH_PER - 1) / (SPH_NT * SPH_PER));
+  std::vector<int> counts(nblk);  // (may throw: before any device allocation; the C entry points catch it)
   int* d_counts = nullptr;
   CU_TRY(h, cudaMalloc(&d_counts, sizeof(int) * (size_t)nblk));
   k_sphere_count<<<nblk, SPH_NT, 0, st>>>(sg, ntot, d_counts);
-  std::vector<int> counts(nblk);
   cudaError_t e = cudaMemcpyAsync(counts.data(), d_counts, sizeof(int) * (size_t)nblk, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) {
@@ -491,12 +513,18 @@ cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t st) {
   return e;
 }
 
-bool g_attr_done = false;
+// cudaFuncSetAttribute is per device: keep the "done" state per device id, under a mutex (handles may be created from
+// several host threads and on several devices of one process)
+constexpr int MAX_DEVICES = 64;
+bool g_attr_done[MAX_DEVICES] = {};
+std::mutex g_attr_mutex;
+long long g_int8_kmax = 0;  // qe_hpsi_test_set_int8_kmax
 cudaError_t set_kernel_attrs() {
-  if (g_attr_done) return cudaSuccess;
   int dev = 0, optin = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  if (dev >= 0 && dev < MAX_DEVICES && g_attr_done[dev]) return cudaSuccess;
   e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return e;
 #define SET_SMEM(k)                                                                     \
@@ -525,7 +553,7 @@ cudaError_t set_kernel_attrs() {
   e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
   if (e != cudaSuccess) return e;
 #undef SET_SMEM
-  g_attr_done = true;
+  if (dev >= 0 && dev < MAX_DEVICES) g_attr_done[dev] = true;
   return cudaSuccess;
 }
 
@@ -541,13 +569,18 @@ extern "C" const char* qe_hpsi_strerror(int status) {
     case QE_HPSI_EINVAL: return "invalid argument";
     case QE_HPSI_EGRID: return "unsupported FFT grid (factors other than 2,3,5, too large, or smaller than the sphere)";
     case QE_HPSI_ENOMEM: return "out of memory";
-    case QE_HPSI_ECUDA: return "CUDA error (see qe_hpsi_last_cuda_error)";
+    case QE_HPSI_ECUDA: return "CUDA error (see qe_hpsi_last_error)";
     case QE_HPSI_ESTATE: return "invalid handle";
     default: return "unknown status";
   }
 }
 
-extern "C" int qe_hpsi_last_cuda_error(qe_hpsi_t h) { return h ? h->last_cuda : g_last_cuda; }
+extern "C" int qe_hpsi_last_error(qe_hpsi_t h) { return h ? h->last_cuda : g_last_cuda.load(); }
+extern "C" int qe_hpsi_test_set_int8_kmax(int64_t kmax) {
+  if (kmax < 0) return QE_HPSI_EINVAL;
+  g_int8_kmax = kmax;
+  return QE_HPSI_OK;
+}
 
 extern "C" int qe_hpsi_gsphere(const double at[9], const double xk[3], double ecutwfc, const int nr[3], int64_t* npw,
                                int32_t* miller_host) {
@@ -556,7 +589,11 @@ extern "C" int qe_hpsi_gsphere(const double at[9], const double xk[3], double ec
   int rc = validate_grid(at, xk, ecutwfc, nr, &sg);
   if (rc) return rc;
   SphereOut so;
-  rc = build_sphere(sg, nullptr, &so);
+  try {
+    rc = build_sphere(sg, nullptr, &so);
+  } catch (const std::bad_alloc&) {
+    rc = QE_HPSI_ENOMEM;
+  }
   if (rc) return rc;
   *npw = so.npw;
   if (miller_host && so.npw > 0) {
@@ -609,6 +646,20 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->oz_eg);
   cudaFree(h->oz_eb);
   cudaFree(h->oz_partial);
+  cudaFree(h->cert_y);
+  cudaFree(h->cert_v8);
+  cudaFree(h->cert_psif);
+  cudaFree(h->cert_vf);
+  cudaFree(h->cert_part);
+  cudaFree(h->cert_rel);
+  cudaFree(h->cert_redo);
+  cudaFree(h->cert_slot);
+  cudaFree(h->cert_list);
+  cudaFree(h->cert_count);
+  cudaFree(h->partial_f);
+  cudaFree(h->becp_f);
+  cudaFree(h->dbecp_f);
+  cudaFree(h->dbT_f);
   for (int i = 0; i < 2; ++i) {
     cudaFree(h->hbuf_psi[i]);
     cudaFree(h->hbuf_h[i]);
@@ -661,6 +712,58 @@ void choose_split(qe_hpsi_handle* h) {
   if (kchunk < ZG_BK) kchunk = ZG_BK;
   h->kchunk = kchunk;
   h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+}
+
+// buffers of one a6-a7 pass on the FP64 tensor path: split-K partials, becp, dbecp, dbecp transposed
+struct NlBufs {
+  double2 *partial, *becp, *dbecp, *dbT;
+};
+
+template <class Cfg>
+void becp_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st, double2* partial, const int* nb_dev) {
+  const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  k_becp<Cfg><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
+                                                                         h->npw, h->kchunk, partial, h->ldc, nb_dev);
+}
+template <class Cfg>
+void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
+  const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  if (mt == 0) return;
+  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT, h->ldp,
+                                                                    nb, hpsi, ldh, nb_dev);
+}
+
+// a6 on the FP64 tensor path (complex handles): split-K partials of conj(beta) psi.  nb_dev != nullptr: the band count is
+// min(nb, *nb_dev), read on the device (re-computation pass of QE_HPSI_PROJ_CERTIFY)
+void becp_fp64(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st, double2* partial, const int* nb_dev) {
+  switch (h->zg_variant) {
+    case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+    case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+    case 3: becp_launch<ZgV3>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+    case 4: becp_launch<ZgV4>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+    case 5: becp_launch<ZgV5>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+    default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
+  }
+}
+void vnl_fp64(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
+  switch (h->zg_variant) {
+    case 1: vnl_launch<ZgV1>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+    case 2: vnl_launch<ZgV2>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+    case 3: vnl_launch<ZgV3>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+    case 4: vnl_launch<ZgV4>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+    case 5: vnl_launch<ZgV5>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+    default: vnl_launch<ZgV0>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
+  }
+}
+// a6-a8 entirely on the FP64 tensor path of a complex handle: out[b] += V_NL psi[b] (used by the certified path's
+// re-computation and, at create, for its probe images)
+void nonlocal_fp64(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* out, long long ldo, int nb, cudaStream_t st,
+                   const NlBufs& B, const int* nb_dev) {
+  becp_fp64(h, psi, ldpsi, nb, st, B.partial, nb_dev);
+  const dim3 rg((nb + 127) / 128, h->nproj);
+  k_becp_reduce<<<rg, 128, 0, st>>>(B.partial, h->nsplit, h->nproj, h->ldc, nb, B.becp, nb_dev);
+  k_dmul<<<rg, 128, 0, st>>>(B.becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, B.dbecp, B.dbT, h->ldp, nb_dev);
+  vnl_fp64(h, B.dbT, out, ldo, nb, st, nb_dev);
 }
 
 // ---- projector contractions on tcgen05 int8 slices (ozaki_kernels.cuh) --------------------------
@@ -787,31 +890,26 @@ void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cuda
     default: CALL(6); break;             \
   }
 
-// plan + operand slices for the int8 path; leaves h->oz_s = 0 (FP64 DMMA path) when the device or a resource says no
-cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
-  // default: 6 digits when the contraction is big enough to pay for the four extra launches per chunk (digit kernels) --
-  // below ~1e6 entries of beta the step is launch-latency bound and the FP64 tensor path is the shorter sequence
-  int S = env_int("QE_HPSI_OZAKI", (long long)h->nproj * h->npw >= (1LL << 20) ? 6 : 0);
-  if (S <= 0 || h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
-  // (a Gamma-only handle runs the real forms: one B row per band in a6, planar transposed digits of beta in a8)
-  S = std::min(std::max(S, 4), 7);
-  cudaDeviceProp prop;
-  cudaError_t e = cudaGetDeviceProperties(&prop, h->device);
-  if (e != cudaSuccess) return e;
-  if (prop.major != 10) return cudaSuccess;  // tcgen05 kind::i8 is an sm_100 feature
+// plan + operand digit planes of the int8 path (flag QE_HPSI_PROJ_INT8; digits and 3M forms from the flag fields).  Any
+// failure is returned: a handle never changes its accuracy class on its own.
+cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, unsigned flags, cudaStream_t st) {
+  if (h->nproj <= 0 || h->npw <= 0) return cudaSuccess;
+  int S = (int)((flags >> 8) & 15u);
+  if (S == 0) S = 7;
+  cudaError_t e = cudaSuccess;
   const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up((h->gamma ? 1LL : 2LL) * h->nproj, 128);
-  // K range per CTA: int32 level sums must not overflow (QE_HPSI_OZ_KMAX lowers it: testing the multi-range paths on small cases)
-  const long long kmax_env = env_int("QE_HPSI_OZ_KMAX", 0);
-  const long long kmax = kmax_env >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_env / oz::KB * oz::KB) : oz::max_k_per_cta(S);
+  // K range per CTA: int32 level sums must not overflow (qe_hpsi_test_set_int8_kmax lowers it: the multi-range paths on small cases)
+  const long long kmax_t = g_int8_kmax;
+  const long long kmax = kmax_t >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_t / oz::KB * oz::KB) : oz::max_k_per_cta(S);
   h->oz_k1 = k1;
   h->oz_k2 = k2;
   // 3M form of a6 (three real GEMMs instead of a real-form complex one: -25 % MMAs, three launches): pays from ~2^26 entries of beta
-  h->oz_3m = !h->gamma && env_int("QE_HPSI_OZ_3M", (long long)h->nproj * h->npw >= (1LL << 26) ? 1 : 0) != 0;
+  const unsigned m3 = (flags >> 12) & 3u;  // 0 by size, 1 off, 2 a6 only, 3 a6 and a8 whatever the size
+  h->oz_3m = !h->gamma && (m3 == 0 ? (long long)h->nproj * h->npw >= (1LL << 26) : m3 >= 2);
   h->oz_k1c = round_up(h->npw, 128);
   h->oz_k2c = round_up(h->nproj, 128);
   // a8 in the 3M form: one exact-int32 K range, and enough K blocks per plane to amortise the three epilogues (measured: pays at
-  // nproj = 1728, not at 1024); QE_HPSI_OZ_3M=2: 3M form for a6 only, 3: for a8 whatever nproj is (testing)
-  const int m3 = env_int("QE_HPSI_OZ_3M", 1);
+  // nproj = 1728, not at 1024)
   h->oz_3m8 = h->oz_3m && h->oz_k2c <= kmax && m3 != 2 && (h->oz_k2c >= 1536 || m3 == 3);
   const long long ka6 = h->oz_3m ? h->oz_k1c : k1;  // contraction length of one a6 GEMM (reals)
   const int stage = S * (oz::A_BYTES + oz::B_BYTES);
@@ -843,16 +941,9 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, cudaStream_t st) {
       (e = cudaMalloc(&h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
       (e = cudaMalloc(&h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess) {
-    if (e != cudaErrorMemoryAllocation) return e;
-    // the digit planes (4 S bytes per entry of beta) do not fit: stay on the FP64 tensor path (qe_hpsi_info reports 0 digits)
-    (void)cudaGetLastError();
-    void** bufs[] = {(void**)&h->oz_a1, (void**)&h->oz_a2, (void**)&h->oz_b,  (void**)&h->oz_partial,
-                     (void**)&h->oz_ep, (void**)&h->oz_eg, (void**)&h->oz_eb};
-    for (void** b : bufs) {
-      cudaFree(*b);
-      *b = nullptr;
-    }
-    return cudaSuccess;
+    // the digit planes do not fit (or another CUDA error): qe_hpsi_create fails with QE_HPSI_ENOMEM / QE_HPSI_ECUDA; the buffers
+    // allocated so far are released by qe_hpsi_destroy
+    return e;
   }
   if ((e = cudaMemsetAsync(h->oz_b, 0, bb, st)) != cudaSuccess) return e;
   if (!oz_make_map(&h->oz_tm_a1, h->oz_a1, k1, h->nproj, S, (long long)h->nproj * k1, oz::BM) ||
@@ -942,22 +1033,116 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
     CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
     CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
     h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
-    if (!(flags & QE_HPSI_FP64_DMMA)) CR_TRY(setup_ozaki(h, max_batch, st));
+    if (flags & QE_HPSI_PROJ_INT8) CR_TRY(setup_ozaki(h, max_batch, flags, st));
   #undef CR_TRY
   return cudaSuccess;
 }
 
+// QE_HPSI_PROJ_CERTIFY: scratch arrays, the second set of a6-a7 buffers, and the probe images y_t = V_NL s_t computed on the
+// FP64 tensor path.  Runs after setup_nonlocal; synchronises the stream.
+cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
+#define CR_TRY(expr)                     \
+  do {                                   \
+    cudaError_t e__ = (expr);            \
+    if (e__ != cudaSuccess) return e__;  \
+  } while (0)
+  const long long ld = round_up(h->npw, 8);
+  h->cert_ld = ld;
+  const size_t row = sizeof(double2) * (size_t)ld, mb = (size_t)h->max_batch;
+  h->cert_nch = (int)std::max<long long>(1, std::min<long long>(64, (h->npw + 32767) / 32768));
+  CR_TRY(cudaMalloc(&h->cert_y, row * cert::NPROBE));
+  CR_TRY(cudaMalloc(&h->cert_v8, row * mb));
+  CR_TRY(cudaMalloc(&h->cert_psif, row * mb));
+  CR_TRY(cudaMalloc(&h->cert_vf, row * mb));
+  CR_TRY(cudaMalloc(&h->cert_part, sizeof(double) * mb * h->cert_nch * cert::NVAL));
+  CR_TRY(cudaMalloc(&h->cert_rel, sizeof(double) * mb));
+  CR_TRY(cudaMalloc(&h->cert_redo, sizeof(int) * mb));
+  CR_TRY(cudaMalloc(&h->cert_slot, sizeof(int) * mb));
+  CR_TRY(cudaMalloc(&h->cert_list, sizeof(int) * mb));
+  CR_TRY(cudaMalloc(&h->cert_count, sizeof(int)));
+  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2);
+  CR_TRY(cudaMalloc(&h->partial_f, pc * h->nsplit));
+  CR_TRY(cudaMalloc(&h->becp_f, pc));
+  CR_TRY(cudaMalloc(&h->dbecp_f, pc));
+  CR_TRY(cudaMalloc(&h->dbT_f, mb * h->ldp * sizeof(double2)));
+  CR_TRY(cudaMemsetAsync(h->dbT_f, 0, mb * h->ldp * sizeof(double2), st));
+  CR_TRY(cudaMemsetAsync(h->cert_y, 0, row * cert::NPROBE, st));
+  CR_TRY(cudaMemsetAsync(h->cert_rel, 0, sizeof(double) * mb, st));
+  CR_TRY(cudaMemsetAsync(h->cert_redo, 0, sizeof(int) * mb, st));
+  CR_TRY(cudaMemsetAsync(h->cert_count, 0, sizeof(int), st));
+  h->workspace_bytes += row * (cert::NPROBE + 3 * mb) + pc * (h->nsplit + 2) + mb * h->ldp * sizeof(double2);
+  double2* sgn = nullptr;
+  CR_TRY(cudaMalloc(&sgn, row * cert::NPROBE));
+  cudaError_t e = cudaMemsetAsync(sgn, 0, row * cert::NPROBE, st);
+  if (e == cudaSuccess) {
+    cert::k_cert_signs<<<(unsigned)((h->npw + 255) / 256), 256, 0, st>>>(sgn, ld, h->npw);
+    const NlBufs B{h->partial_f, h->becp_f, h->dbecp_f, h->dbT_f};
+    for (int t0 = 0; t0 < cert::NPROBE; t0 += h->max_batch)
+      nonlocal_fp64(h, sgn + (size_t)t0 * ld, ld, h->cert_y + (size_t)t0 * ld, ld, std::min(h->max_batch, cert::NPROBE - t0), st, B,
+                    nullptr);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  cudaFree(sgn);
+  CR_TRY(e);
+  h->certify = true;
+#undef CR_TRY
+  return cudaSuccess;
+}
+
+// create flags: known bits only, one accuracy class, int8 sub-fields only with QE_HPSI_PROJ_INT8, 4..7 digits
+int validate_flags(unsigned flags, bool gamma) {
+  const unsigned known = QE_HPSI_BORROW_BETA | QE_HPSI_GENERIC_FFT | QE_HPSI_FP64_DMMA | QE_HPSI_PROJ_INT8 | QE_HPSI_PROJ_CERTIFY |
+                         (15u << 8) | (3u << 12);
+  if (flags & ~known) return QE_HPSI_EINVAL;
+  if ((flags & QE_HPSI_FP64_DMMA) && (flags & QE_HPSI_PROJ_INT8)) return QE_HPSI_EINVAL;
+  if (!(flags & QE_HPSI_PROJ_INT8) && (flags & (QE_HPSI_PROJ_CERTIFY | (15u << 8) | (3u << 12)))) return QE_HPSI_EINVAL;
+  const unsigned dig = (flags >> 8) & 15u;
+  if (dig != 0 && (dig < 4 || dig > 7)) return QE_HPSI_EINVAL;
+  if (gamma && (flags & QE_HPSI_PROJ_CERTIFY)) return QE_HPSI_EINVAL;
+  return QE_HPSI_OK;
+}
+
+int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], double ecutwfc, const double xk[3], const int nr[3],
+                const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags, void* cuda_stream);
+
 }  // namespace
 
+// The C entry point never lets a C++ exception (std::bad_alloc of the host-side tables) cross the boundary
 extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc, const double xk[3], const int nr[3],
                               const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
                               const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
                               void* cuda_stream) {
   if (!out) return QE_HPSI_EINVAL;
   *out = nullptr;
+  qe_hpsi_handle* live = nullptr;
+  int rc;
+  try {
+    rc = create_impl(out, &live, at, ecutwfc, xk, nr, vr_dev, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, max_batch,
+                     flags, cuda_stream);
+  } catch (const std::bad_alloc&) {
+    rc = QE_HPSI_ENOMEM;
+  } catch (...) {
+    rc = QE_HPSI_ESTATE;
+  }
+  if (rc != QE_HPSI_OK) {
+    if (live) qe_hpsi_destroy(live);
+    *out = nullptr;
+  }
+  return rc;
+}
+
+namespace {
+
+int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], double ecutwfc, const double xk[3], const int nr[3],
+                const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags, void* cuda_stream) {
   if (!vr_dev || nproj < 0 || max_batch < 1) return QE_HPSI_EINVAL;
+  int rc = validate_flags(flags, false);
+  if (rc) return rc;
   SphereGeom sg;
-  int rc = validate_grid(at, xk, ecutwfc, nr, &sg);
+  rc = validate_grid(at, xk, ecutwfc, nr, &sg);
   if (rc) return rc;
   long long d_total = 0;
   if (nproj > 0) {
@@ -972,12 +1157,13 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   qe_hpsi_handle* h = new (std::nothrow) qe_hpsi_handle();
   if (!h) return QE_HPSI_ENOMEM;
+  *live = h;  // on any failure below the caller (qe_hpsi_create) destroys it
 #define CR_TRY(expr)                                                             \
   do {                                                                           \
     cudaError_t e__ = (expr);                                                    \
     if (e__ != cudaSuccess) {                                                    \
       g_last_cuda = (int)e__;                                                    \
-      qe_hpsi_destroy(h);                                                        \
+      (void)cudaGetLastError();                                                  \
       return e__ == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA;  \
     }                                                                            \
   } while (0)
@@ -992,18 +1178,12 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   // ---- a0: sphere maps --------------------------------------------------------------------------------
   SphereOut so;
   rc = build_sphere(sg, st, &so);
-  if (rc) {
-    qe_hpsi_destroy(h);
-    return rc;
-  }
+  if (rc) return rc;
   h->npw = so.npw;
   h->miller = so.miller;
   h->fftidx = so.fftidx;
   h->g2kin = so.g2kin;
-  if (nproj > 0 && ldbeta < h->npw) {
-    qe_hpsi_destroy(h);
-    return QE_HPSI_EINVAL;
-  }
+  if (nproj > 0 && ldbeta < h->npw) return QE_HPSI_EINVAL;
   std::vector<int> idx((size_t)h->npw);
   if (h->npw) CR_TRY(cudaMemcpy(idx.data(), h->fftidx, sizeof(int) * (size_t)h->npw, cudaMemcpyDeviceToHost));
   // sticks ((i1,i2) columns) and populated planes, in canonical order
@@ -1088,10 +1268,7 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   for (int j = 0; j < 3; ++j) {
     std::vector<int> rad;
     plan_radices(nr[j], (flags & QE_HPSI_GENERIC_FFT) != 0, &rad);
-    if ((int)rad.size() > FFT_MAX_PASS) {
-      qe_hpsi_destroy(h);
-      return QE_HPSI_EGRID;
-    }
+    if ((int)rad.size() > FFT_MAX_PASS) return QE_HPSI_EGRID;
     axes[j]->n = nr[j];
     axes[j]->npass = (int)rad.size();
     for (size_t p = 0; p < rad.size(); ++p) axes[j]->radix[p] = rad[p];
@@ -1228,11 +1405,26 @@ extern "C" int qe_hpsi_create(qe_hpsi_t* out, const double at[9], double ecutwfc
   // ---- nonlocal ---------------------------------------------------------------------------------------
   if (nproj > 0)
     CR_TRY(setup_nonlocal(h, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
+  if ((flags & QE_HPSI_PROJ_CERTIFY) && h->oz_s) CR_TRY(setup_certify(h, st));
+  // NEXT-3: split-K workspace of qe_hpsi_overlap; K slices depend on npw only, so an element's bits do not depend on how many
+  // rows / columns a call has (chunks of 512 x 128)
+  if (h->npw > 0) {
+    const int ns0 = std::max(1, std::min(32, h->npw / 2048));
+    int kchunk = (h->npw + ns0 - 1) / ns0;
+    kchunk = std::max(ZgV0::BK, (kchunk + ZgV0::BK - 1) / ZgV0::BK * ZgV0::BK);
+    h->ovl_kchunk = kchunk;
+    h->ovl_ns = std::max(1, (h->npw + kchunk - 1) / kchunk);
+    CR_TRY(cudaMalloc(&h->ovl_partial, sizeof(double2) * (size_t)h->ovl_ns * 512 * 128));
+    h->workspace_bytes += sizeof(double2) * (size_t)h->ovl_ns * 512 * 128;
+  }
   CR_TRY(cudaStreamSynchronize(st));
 #undef CR_TRY
+  *live = nullptr;
   *out = h;
   return QE_HPSI_OK;
 }
+
+}  // namespace
 
 namespace {
 
@@ -1311,20 +1503,6 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
   return QE_HPSI_OK;
 }
 
-template <class Cfg>
-void becp_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
-  const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
-  k_becp<Cfg><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
-                                                                         h->npw, h->kchunk, h->partial, h->ldc);
-}
-template <class Cfg>
-void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
-  const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
-  if (mt == 0) return;
-  k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT, h->ldp,
-                                                                    nb, hpsi, ldh);
-}
-
 // a6-a7 for nb bands: becp, dbecp, dbT
 int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const size_t t0 = prof_mark(h, st);
@@ -1344,14 +1522,7 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
                                                                                  h->npw, h->kchunk, h->partial, h->ldc);
   } else
-  switch (h->zg_variant) {
-    case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st); break;
-    case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st); break;
-    case 3: becp_launch<ZgV3>(h, psi, ldpsi, nb, st); break;
-    case 4: becp_launch<ZgV4>(h, psi, ldpsi, nb, st); break;
-    case 5: becp_launch<ZgV5>(h, psi, ldpsi, nb, st); break;
-    default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st); break;
-  }
+    becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);
   const size_t t1 = prof_mark(h, st);
   prof_span(h, ts, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
@@ -1392,14 +1563,30 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
       k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
                                                                                 h->ldp, nb, hpsi, ldh);
   } else
-  switch (h->zg_variant) {
-    case 1: vnl_launch<ZgV1>(h, bT, hpsi, ldh, nb, st); break;
-    case 2: vnl_launch<ZgV2>(h, bT, hpsi, ldh, nb, st); break;
-    case 3: vnl_launch<ZgV3>(h, bT, hpsi, ldh, nb, st); break;
-    case 4: vnl_launch<ZgV4>(h, bT, hpsi, ldh, nb, st); break;
-    case 5: vnl_launch<ZgV5>(h, bT, hpsi, ldh, nb, st); break;
-    default: vnl_launch<ZgV0>(h, bT, hpsi, ldh, nb, st); break;
-  }
+    vnl_fp64(h, bT, hpsi, ldh, nb, st, nullptr);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// QE_HPSI_PROJ_CERTIFY, after a6-a7 of the int8 path: a8 into the scratch v8, the check, the FP64 re-computation of the bands
+// that fail it, and hpsi[b] += (FP64 result or int8 result).  DESIGN.md section 5.7; kernels in cert_kernels.cuh.
+int launch_vnl_certified(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  const long long ld = h->cert_ld;
+  CU_TRY(h, cudaMemsetAsync(h->cert_v8, 0, sizeof(double2) * (size_t)nb * ld, st));
+  int rc = launch_vnl_add(h, h->dbT, h->cert_v8, ld, nb, st);
+  if (rc) return rc;
+  const size_t t0 = prof_mark(h, st);
+  const int gchunk = (int)((h->npw + h->cert_nch - 1) / h->cert_nch);
+  cert::k_cert_probe<<<dim3(h->cert_nch, nb), cert::NT, 0, st>>>(h->cert_v8, ld, psi, ldpsi, h->cert_y, ld, h->npw, gchunk, h->cert_part,
+                                                               h->cert_nch);
+  cert::k_cert_decide<<<1, cert::NT, 0, st>>>(h->cert_part, h->cert_nch, nb, h->cert_tol, h->cert_rel, h->cert_redo, h->cert_slot,
+                                            h->cert_list, h->cert_count);
+  const unsigned gx = (unsigned)std::min<long long>((h->npw + 255) / 256, 64);
+  cert::k_cert_gather<<<dim3(gx, nb), 256, 0, st>>>(psi, ldpsi, h->npw, h->cert_list, h->cert_count, h->cert_psif, h->cert_vf, ld);
+  const NlBufs B{h->partial_f, h->becp_f, h->dbecp_f, h->dbT_f};
+  nonlocal_fp64(h, h->cert_psif, ld, h->cert_vf, ld, nb, st, B, h->cert_count);
+  cert::k_cert_commit<<<dim3(gx, nb), 256, 0, st>>>(h->cert_v8, h->cert_vf, ld, h->cert_redo, h->cert_slot, h->npw, hpsi, ldh);
+  prof_span(h, t0, prof_mark(h, st), SLOT_CERT);
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
 }
@@ -1408,7 +1595,7 @@ int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi,
                 bool local, bool nonlocal) {
   int rc = QE_HPSI_OK;
   const bool nl = nonlocal && h->nproj > 0 && h->npw > 0;
-  if (h->prof_mode && h->prof_used + 16 > 16384) prof_drain(h);
+  if (h->prof_mode && h->prof_used + 24 > 16384) prof_drain(h);
   // a6-a7 and a1-a5 are independent (both only read psi): with QE_HPSI_OVERLAP=1 the FFT chain runs on an internal
   // stream forked from the caller's stream while the projector ZGEMM runs on the caller's stream; joined before a8.
   const bool fork = nl && local && h->overlap && h->st_fft && !h->prof_mode;
@@ -1432,6 +1619,7 @@ int apply_chunk(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi,
     if (h->prof_mode == 1) prof_span(h, t0, prof_mark(h, st), SLOT_FFT);
   }
   if (nl) {
+    if (h->certify) return launch_vnl_certified(h, psi, ldpsi, hpsi, ldh, nb, st);
     const size_t t0 = h->oz_s ? (size_t)-1 : prof_mark(h, st);  // the int8 path records its own spans (slices | GEMM)
     rc = launch_vnl_add(h, h->dbT, hpsi, ldh, nb, st);
     if (!h->oz_s) prof_span(h, t0, prof_mark(h, st), SLOT_VNL);
@@ -1492,6 +1680,7 @@ extern "C" int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host) {
 extern "C" int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi,
                                 void* spsi_dev, int64_t ldspsi, int nbands, void* cuda_stream) {
   if (!h) return QE_HPSI_ESTATE;
+  if (h->certify) return QE_HPSI_ESTATE;  // the a-posteriori check covers qe_hpsi_apply / qe_hpsi_apply_host only
   if (!spsi_dev) return QE_HPSI_EINVAL;
   int rc = check_apply_args(h, psi_dev, ldpsi, spsi_dev, ldspsi, nbands);
   if (rc) return rc;
@@ -1557,27 +1746,10 @@ extern "C" int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int 
     CU_TRY(h, cudaMemset2DAsync(out, sizeof(double2) * (size_t)ldo, 0, sizeof(double2) * (size_t)nb, (size_t)na, st));
     return QE_HPSI_OK;
   }
-  CU_TRY(h, set_kernel_attrs());
-  // K slices depend on npw only, so an element's bits do not depend on how many rows/columns the call has
+  // K slices depend on npw only (plan and workspace made at create), so an element's bits do not depend on how many
+  // rows / columns the call has, and the call allocates and synchronises nothing
   constexpr int MA = 512, NB = 128, LDC = 128;
-  const int ns0 = std::max(1, std::min(32, h->npw / 2048));
-  int kchunk = (h->npw + ns0 - 1) / ns0;
-  kchunk = std::max(ZgV0::BK, (kchunk + ZgV0::BK - 1) / ZgV0::BK * ZgV0::BK);
-  const int ns = std::max(1, (h->npw + kchunk - 1) / kchunk);
-  const size_t need = sizeof(double2) * (size_t)ns * (size_t)std::min(na, MA) * LDC;
-  if (need > h->ovl_cap) {
-    CU_TRY(h, cudaStreamSynchronize(st));  // an earlier call on this stream may still read the old buffer
-    cudaFree(h->ovl_partial);
-    h->ovl_partial = nullptr;
-    h->ovl_cap = 0;
-    const size_t cap = sizeof(double2) * (size_t)ns * MA * LDC;
-    cudaError_t e = cudaMalloc(&h->ovl_partial, cap);
-    if (e != cudaSuccess) {
-      h->last_cuda = (int)e;
-      return e == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA;
-    }
-    h->ovl_cap = cap;
-  }
+  const int ns = h->ovl_ns, kchunk = h->ovl_kchunk;
   for (int a0 = 0; a0 < na; a0 += MA) {
     const int ma = std::min(MA, na - a0);
     for (int b0 = 0; b0 < nb; b0 += NB) {
@@ -1630,13 +1802,12 @@ extern "C" int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int n
   if (nx < 0 || ny < 0) return QE_HPSI_EINVAL;
   if (ny == 0 || h->npw == 0) return QE_HPSI_OK;
   if (!y_dev || ldy < h->npw) return QE_HPSI_EINVAL;
+  if (nx > 0 && (!x_dev || !coef_dev || ldx < h->npw || ldcoef < nx)) return QE_HPSI_EINVAL;  // before anything is written
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* y = static_cast<double2*>(y_dev);
   if (!accumulate)
     CU_TRY(h, cudaMemset2DAsync(y, sizeof(double2) * (size_t)ldy, 0, sizeof(double2) * (size_t)h->npw, (size_t)ny, st));
   if (nx == 0) return QE_HPSI_OK;
-  if (!x_dev || !coef_dev || ldx < h->npw || ldcoef < nx) return QE_HPSI_EINVAL;
-  CU_TRY(h, set_kernel_attrs());
   using Cfg = ZgV0;
   const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (ny + Cfg::BN - 1) / Cfg::BN;
   // y[k][g] += sum_j x[j][g] coef[k][j]: the a8 kernel with A = x (M-contiguous) and B = coef (K-contiguous)
@@ -1644,6 +1815,48 @@ extern "C" int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int n
                                                                     static_cast<const double2*>(coef_dev), (int)ldcoef, ny, y,
                                                                     ldy);
   CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_residual(qe_hpsi_t h, const void* hx_dev, int64_t ldh, const void* sx_dev, int64_t lds,
+                                const double* e_dev, void* r_dev, int64_t ldr, int nb, double* rnorm2_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nb < 0) return QE_HPSI_EINVAL;
+  if (nb == 0) return QE_HPSI_OK;
+  if (!hx_dev || !sx_dev || !e_dev || !r_dev || ldh < h->npw || lds < h->npw || ldr < h->npw) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  k_residual<<<nb, 1024, 0, st>>>(static_cast<const double2*>(hx_dev), ldh, static_cast<const double2*>(sx_dev), lds, e_dev,
+                                  static_cast<double2*>(r_dev), ldr, h->npw, rnorm2_dev);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+extern "C" int qe_hpsi_scale(qe_hpsi_t h, void* x_dev, int64_t ldx, int nb, const double* fac_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (nb < 0) return QE_HPSI_EINVAL;
+  if (nb == 0 || h->npw == 0) return QE_HPSI_OK;
+  if (!x_dev || !fac_dev || ldx < h->npw) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  k_scale_rows<<<dim3((unsigned)((h->npw + 255) / 256), nb), 256, 0, st>>>(static_cast<double2*>(x_dev), ldx, h->npw, fac_dev);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
+// certified int8 projector path: tolerance and the check results of the last chunk (include/qe_hpsi.h)
+extern "C" int qe_hpsi_set_proj_tolerance(qe_hpsi_t h, double tol) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!(tol >= 0.0)) return QE_HPSI_EINVAL;
+  if (!h->certify) return QE_HPSI_ESTATE;
+  h->cert_tol = tol;
+  return QE_HPSI_OK;
+}
+extern "C" int qe_hpsi_get_proj_check(qe_hpsi_t h, double* rel_dev, int32_t* redo_dev, void* cuda_stream) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (!h->certify) return QE_HPSI_ESTATE;
+  if (h->nb_last == 0) return QE_HPSI_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (rel_dev) CU_TRY(h, cudaMemcpyAsync(rel_dev, h->cert_rel, sizeof(double) * (size_t)h->nb_last, cudaMemcpyDeviceToDevice, st));
+  if (redo_dev) CU_TRY(h, cudaMemcpyAsync(redo_dev, h->cert_redo, sizeof(int) * (size_t)h->nb_last, cudaMemcpyDeviceToDevice, st));
   return QE_HPSI_OK;
 }
 
@@ -1741,7 +1954,12 @@ extern "C" int qe_hpsi_gamma_gsphere(const double at[9], double ecutwfc, const i
   int64_t npw = 0;
   int rc = qe_hpsi_gsphere(at, xk, ecutwfc, nr, &npw, nullptr);
   if (rc) return rc;
-  std::vector<int32_t> mil((size_t)std::max<int64_t>(npw, 1) * 3);
+  std::vector<int32_t> mil;
+  try {
+    mil.resize((size_t)std::max<int64_t>(npw, 1) * 3);
+  } catch (const std::bad_alloc&) {
+    return QE_HPSI_ENOMEM;
+  }
   rc = qe_hpsi_gsphere(at, xk, ecutwfc, nr, &npw, mil.data());
   if (rc) return rc;
   int64_t n = 0;
@@ -1770,13 +1988,15 @@ extern "C" int qe_hpsi_gamma_destroy(qe_hpsi_gamma_t g) {
   return QE_HPSI_OK;
 }
 
-extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], double ecutwfc, const int nr[3],
-                                    const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
-                                    const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
-                                    void* cuda_stream) {
-  if (!out) return QE_HPSI_EINVAL;
-  *out = nullptr;
+namespace {
+int gamma_create_impl(qe_hpsi_gamma_t* out, qe_hpsi_gamma_handle** live, const double at[9], double ecutwfc, const int nr[3],
+                      const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                      const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags, void* cuda_stream) {
   if (!vr_dev || nproj < 0 || max_batch < 1) return QE_HPSI_EINVAL;
+  {
+    const int frc = validate_flags(flags, true);
+    if (frc) return frc;
+  }
   long long d_total = 0;
   if (nproj > 0) {
     if (!beta_dev || !blk_off_host || !d_host || nblocks < 1) return QE_HPSI_EINVAL;
@@ -1790,22 +2010,20 @@ extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], do
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   qe_hpsi_gamma_handle* g = new (std::nothrow) qe_hpsi_gamma_handle();
   if (!g) return QE_HPSI_ENOMEM;
+  *live = g;  // on any failure below the caller (qe_hpsi_gamma_create) destroys it
   g->max_batch = max_batch;
   g->pairs = (max_batch + 1) / 2;
   const double xk[3] = {0.0, 0.0, 0.0};
   int rc = qe_hpsi_create(&g->loc, at, ecutwfc, xk, nr, vr_dev, 0, nullptr, 0, 0, nullptr, nullptr, g->pairs,
                           flags & QE_HPSI_GENERIC_FFT, cuda_stream);
-  if (rc) {
-    delete g;
-    return rc;
-  }
+  if (rc) return rc;
   g->npw = g->loc->npw;
 #define CG_TRY(expr)                                                           \
   do {                                                                         \
     cudaError_t e__ = (expr);                                                  \
     if (e__ != cudaSuccess) {                                                  \
       g_last_cuda = (int)e__;                                                  \
-      qe_hpsi_gamma_destroy(g);                                                \
+      (void)cudaGetLastError();                                                \
       return e__ == cudaErrorMemoryAllocation ? QE_HPSI_ENOMEM : QE_HPSI_ECUDA; \
     }                                                                          \
   } while (0)
@@ -1825,18 +2043,12 @@ extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], do
       lin = lin * nr[j] + ((n % nr[j]) + nr[j]) % nr[j];
     }
     auto it = std::lower_bound(fidx.begin(), fidx.begin() + g->npw, (int)lin);
-    if (it == fidx.begin() + g->npw || *it != (int)lin) {  // cannot happen for a k = 0 sphere
-      qe_hpsi_gamma_destroy(g);
-      return QE_HPSI_ESTATE;
-    }
+    if (it == fidx.begin() + g->npw || *it != (int)lin) return QE_HPSI_ESTATE;  // cannot happen for a k = 0 sphere
     ip.push_back(i);
     im.push_back((int)(it - fidx.begin()));
   }
   g->ngw = (int)ip.size();
-  if (nproj > 0 && ldbeta < g->ngw) {
-    qe_hpsi_gamma_destroy(g);
-    return QE_HPSI_EINVAL;
-  }
+  if (nproj > 0 && ldbeta < g->ngw) return QE_HPSI_EINVAL;
   CG_TRY(upload(&g->idx_plus, ip, st));
   CG_TRY(upload(&g->idx_minus, im, st));
   g->ldf = ((long long)g->npw + 7) / 8 * 8;
@@ -1847,10 +2059,7 @@ extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], do
   CG_TRY(cudaMemsetAsync(g->hphi, 0, fb, st));
   if (nproj > 0 && g->ngw > 0) {
     g->nl = new (std::nothrow) qe_hpsi_handle();
-    if (!g->nl) {
-      qe_hpsi_gamma_destroy(g);
-      return QE_HPSI_ENOMEM;
-    }
+    if (!g->nl) return QE_HPSI_ENOMEM;
     g->nl->device = g->loc->device;
     g->nl->num_sms = g->loc->num_sms;
     g->nl->npw = g->ngw;
@@ -1862,9 +2071,35 @@ extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], do
   }
   CG_TRY(cudaStreamSynchronize(st));
 #undef CG_TRY
+  *live = nullptr;
   *out = g;
   return QE_HPSI_OK;
 }
+}  // namespace
+
+extern "C" int qe_hpsi_gamma_create(qe_hpsi_gamma_t* out, const double at[9], double ecutwfc, const int nr[3],
+                                    const double* vr_dev, int nproj, const void* beta_dev, int64_t ldbeta, int nblocks,
+                                    const int32_t* blk_off_host, const double* d_host, int max_batch, unsigned flags,
+                                    void* cuda_stream) {
+  if (!out) return QE_HPSI_EINVAL;
+  *out = nullptr;
+  qe_hpsi_gamma_handle* live = nullptr;
+  int rc;
+  try {
+    rc = gamma_create_impl(out, &live, at, ecutwfc, nr, vr_dev, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, max_batch,
+                           flags, cuda_stream);
+  } catch (const std::bad_alloc&) {
+    rc = QE_HPSI_ENOMEM;
+  } catch (...) {
+    rc = QE_HPSI_ESTATE;
+  }
+  if (rc != QE_HPSI_OK) {
+    if (live) qe_hpsi_gamma_destroy(live);
+    *out = nullptr;
+  }
+  return rc;
+}
+
 
 extern "C" int64_t qe_hpsi_gamma_ngw(qe_hpsi_gamma_t g) { return g ? g->ngw : (int64_t)QE_HPSI_ESTATE; }
 
@@ -2004,6 +2239,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
     if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : 4;
+    if (h->certify) total += 8;  // probe, decide, gather, the four FP64 kernels (empty grids when nothing failed), commit
   }
   return total;
 }
@@ -2027,7 +2263,7 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[12] = h->f2p[0] ? 1 : 0;
   info[13] = h->oz_s;
   info[14] = h->oz_nsplit;
-  info[15] = h->oz_3m ? (h->oz_3m8 ? 2 : 1) : 0;
+  info[15] = (h->oz_3m ? (h->oz_3m8 ? 2 : 1) : 0) + (h->certify ? 4 : 0);
   return QE_HPSI_OK;
 }
 

@@ -99,17 +99,22 @@ __device__ __forceinline__ void mma2r(double (&P)[TM][TN][2], double (&Q)[TM][TN
 template <class Cfg, bool GAMMA = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_becp(const double2* __restrict__ beta, long long ldb, int nproj, const double2* __restrict__ psi, long long ldpsi,
-           int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc) {
+           int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc, const int* __restrict__ nb_dev = nullptr) {
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS;
   constexpr int STAGE = (BM + BN) * BK;  // complex elements per stage
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* sm = reinterpret_cast<double2*>(smem_raw);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / WN) * (BM / WM), wn0 = (warp % WN) * (BN / WN);
-  const int ntn = (nb + BN - 1) / BN;
+  const int ntn = (nb + BN - 1) / BN;  // the grid was sized for the host-side nb
   const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
+  // nb_dev (QE_HPSI_PROJ_CERTIFY): the number of bands to process is decided on the device; tiles beyond it retire at once
+  if (nb_dev) {
+    nb = min(nb, *nb_dev);
+    if (n0 >= nb) return;
+  }
   const int ks = blockIdx.y;
   const int kb = ks * kchunk, ke = min(npw, kb + kchunk);
   const int nkt = (ke - kb + BK - 1) / BK;
@@ -223,9 +228,10 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 // a7 ------------------------------------------------------------------------------------------------------
 // becp[p][b] = sum_ks partial[ks][p][b], ks ascending (deterministic, independent of the batch composition)
 __global__ void k_becp_reduce(const double2* __restrict__ partial, int nsplit, int nproj, int ldc, int nb,
-                              double2* __restrict__ becp) {
+                              double2* __restrict__ becp, const int* __restrict__ nb_dev = nullptr) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   const int p = blockIdx.y;
+  if (nb_dev) nb = min(nb, *nb_dev);
   if (b >= nb) return;
   double re = 0.0, im = 0.0;
   for (int ks = 0; ks < nsplit; ++ks) {
@@ -292,9 +298,11 @@ __global__ void k_ovl_reduce(const double2* __restrict__ partial, int nsplit, in
 // dbecp[p][b] = sum_j D[p][j] becp[blk_start(p)+j][b]; written both as dbecp[p][b] and transposed dbT[b][p]
 __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int nb, const int* __restrict__ proj_blk0,
                        const int* __restrict__ proj_nh, const long long* __restrict__ proj_doff,
-                       const double* __restrict__ dpk, double2* __restrict__ dbecp, double2* __restrict__ dbT, int ldp) {
+                       const double* __restrict__ dpk, double2* __restrict__ dbecp, double2* __restrict__ dbT, int ldp,
+                       const int* __restrict__ nb_dev = nullptr) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   const int p = blockIdx.y;
+  if (nb_dev) nb = min(nb, *nb_dev);
   if (b >= nb) return;
   const int q0 = proj_blk0[p], nh = proj_nh[p];
   const double* drow = dpk + proj_doff[p];  // row (p - q0) of the block
@@ -314,17 +322,21 @@ __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int
 template <class Cfg, bool GAMMA = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_add(const double2* __restrict__ beta, long long ldb, int nproj, int npw, const double2* __restrict__ dbT,
-              int ldp, int nb, double2* __restrict__ hpsi, long long ldh) {
+              int ldp, int nb, double2* __restrict__ hpsi, long long ldh, const int* __restrict__ nb_dev = nullptr) {
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS, LDA = Cfg::LDA_M;
   constexpr int STAGE = BK * LDA + BN * BK;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* sm = reinterpret_cast<double2*>(smem_raw);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / WN) * (BM / WM), wn0 = (warp % WN) * (BN / WN);
   const int ntn = (nb + BN - 1) / BN;
   const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
+  if (nb_dev) {  // see k_becp
+    nb = min(nb, *nb_dev);
+    if (n0 >= nb) return;
+  }
   const int nkt = (nproj + BK - 1) / BK;
 
   // Per-thread copy plan (see k_becp).  A tile [BK][LDA]: thread owns column gc of rows ra, ra+RPA, ...; B tile

@@ -1,11 +1,12 @@
 """Block Davidson driver around the library's H|psi> / S|psi> (the paper's KS_Solvers call the
 Hamiltonian builder through exactly this kind of loop).
 
-Host orchestration only. Every O(npw) operation runs in libqe_hpsi.so: qe_hpsi_apply(_hs) (H psi, S psi),
-qe_hpsi_overlap (reduced matrices), qe_hpsi_rotate (basis rotation), qe_hpsi_hdiag / qe_hpsi_precond (preconditioner).
-The small dense generalized eigenproblem of the reduced matrices (at most 4 nev x 4 nev) is solved with torch.linalg on
-the device -- the role LAXlib / cuSOLVER play in the paper -- and the residual combination
-h - e s is a pointwise torch expression.
+Host orchestration only. Every arithmetic operation on O(npw) data runs in libqe_hpsi.so: qe_hpsi_apply(_hs) (H psi,
+S psi), qe_hpsi_overlap (reduced matrices), qe_hpsi_rotate (basis rotation), qe_hpsi_residual (h - e s and its squared
+norms), qe_hpsi_hdiag / qe_hpsi_precond (preconditioner), qe_hpsi_scale (normalisation). What torch does here: row
+copies between band arrays, O(nev) scalar work on the norms, and the small dense generalized eigenproblem of the
+reduced matrices (at most 4 nev x 4 nev) via torch.linalg on the device -- the role LAXlib / cuSOLVER play in the
+paper.
 """
 from __future__ import annotations
 
@@ -62,9 +63,8 @@ def davidson(h, psi0, vbar, use_s=False, tol=1e-9, max_iter=60, max_basis=4):
         psi = h.rotate(x[:m], coef)
         hpsi = h.rotate(hx[:m], coef)
         spsi = h.rotate(sx[:m], coef) if use_s else psi
-        r = hpsi - e.to(torch.complex128)[:, None] * spsi
-        r[:, npw:] = 0
-        resn = torch.linalg.vector_norm(r[:, :npw], dim=1)
+        r, rn2 = h.residual(hpsi, spsi, e)  # r = H c - e S c over the sphere entries, |r|^2 per band
+        resn = rn2.sqrt()
         unconv = (resn > tol * torch.clamp(e.abs(), min=1.0)).nonzero().flatten()
         k = int(unconv.numel())
         if k == 0:
@@ -76,7 +76,8 @@ def davidson(h, psi0, vbar, use_s=False, tol=1e-9, max_iter=60, max_basis=4):
             m = nev
         t = r[unconv].contiguous()
         h.precond(t, e[unconv].contiguous(), hd, sd)
-        t = t / torch.linalg.vector_norm(t[:, :npw], dim=1)[:, None]
+        _, tn2 = h.residual(t, t, torch.zeros(k, dtype=torch.float64, device=dev), r=t)  # e = 0: t unchanged, |t|^2
+        h.scale(t, tn2.rsqrt())
         x[m:m + k] = t
         apply(x[m:m + k], hx[m:m + k], sx[m:m + k] if use_s else None)
         napply += k

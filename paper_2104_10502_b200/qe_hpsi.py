@@ -1,6 +1,7 @@
-"""ctypes binding of libqe_hpsi.so (include/qe_hpsi.h). Argument marshalling only: every step of H|psi> runs in
-the library's CUDA kernels. PyTorch supplies device memory and streams. There is NO fallback: if the shared
-library is missing or cannot be loaded, importing callers get a RuntimeError.
+"""ctypes binding of libqe_hpsi.so (include/qe_hpsi.h; the measurement / test helpers of include/qe_hpsi_test.h are
+bound too and marked as such). Argument marshalling only: every step of H|psi> runs in the library's CUDA kernels.
+PyTorch supplies device memory and streams. There is NO fallback: if the shared library is missing or cannot be
+loaded, importing callers get a RuntimeError.
 
 Function names mirror the C ABI (qe_hpsi_gsphere, qe_hpsi_create, qe_hpsi_apply, ...); `Hpsi` is a small RAII
 convenience around a handle.
@@ -19,8 +20,18 @@ LIB_PATH = os.path.join(_PKG, "libqe_hpsi.so")
 QE_HPSI_OK, QE_HPSI_EINVAL, QE_HPSI_EGRID, QE_HPSI_ENOMEM, QE_HPSI_ECUDA, QE_HPSI_ESTATE = 0, -1, -2, -3, -4, -5
 QE_HPSI_BORROW_BETA = 1
 QE_HPSI_GENERIC_FFT = 2
-QE_HPSI_FP64_DMMA = 4
+QE_HPSI_FP64_DMMA = 4      # the default accuracy class (FP64 tensor pipe); the flag only names it
+QE_HPSI_PROJ_INT8 = 8      # opt-in: a6 / a8 as exact int8 digit products (block fixed point, 8S-1 bits under a row exponent)
+QE_HPSI_PROJ_CERTIFY = 16  # with PROJ_INT8: a-posteriori check of every chunk + FP64 re-computation of failing bands
+QE_HPSI_PROJ_3M_OFF, QE_HPSI_PROJ_3M_A6, QE_HPSI_PROJ_3M_ALL = 1 << 12, 2 << 12, 3 << 12
+QE_HPSI_NPROBE = 8
 QE_HPSI_MAX_N = 720
+
+
+def QE_HPSI_PROJ_DIGITS(s: int) -> int:
+    """Digit-count field of the create flags (4..7; 0 = 7)."""
+    return (int(s) & 15) << 8
+
 
 _c = ctypes
 _vp, _i64, _i32, _dbl = _c.c_void_p, _c.c_int64, _c.c_int, _c.c_double
@@ -42,7 +53,13 @@ SIGNATURES = {
     "qe_hpsi_launch_count": (_i64, [_vp, _i32]),
     "qe_hpsi_info": (_i32, [_vp, _pi64]),
     "qe_hpsi_strerror": (_c.c_char_p, [_i32]),
-    "qe_hpsi_last_cuda_error": (_i32, [_vp]),
+    "qe_hpsi_last_error": (_i32, [_vp]),
+    "qe_hpsi_set_proj_tolerance": (_i32, [_vp, _dbl]),
+    "qe_hpsi_get_proj_check": (_i32, [_vp, _vp, _vp, _vp]),
+    "qe_hpsi_residual": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i64, _i32, _vp, _vp]),
+    "qe_hpsi_scale": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp]),
+    # ---- include/qe_hpsi_test.h: measurement and test helpers, not the product boundary ----
+    "qe_hpsi_test_set_int8_kmax": (_i32, [_i64]),
     "qe_hpsi_probe_fp64": (_i32, [_dbl, _pd, _pd]),
     "qe_hpsi_profile": (_i32, [_vp, _i32]),
     "qe_hpsi_profile_read": (_i32, [_vp, _pd, _pi64]),
@@ -93,7 +110,7 @@ class QeHpsiError(RuntimeError):
 
 def _check(rc, handle=None):
     if rc != 0:
-        raise QeHpsiError(rc, load_library().qe_hpsi_last_cuda_error(handle))
+        raise QeHpsiError(rc, load_library().qe_hpsi_last_error(handle))
 
 
 def _darr(x, n):
@@ -128,8 +145,13 @@ def qe_hpsi_gsphere(at, xk, ecutwfc, nr) -> np.ndarray:
     return mil
 
 
+def qe_hpsi_test_set_int8_kmax(kmax: int):
+    """(qe_hpsi_test.h) K range per CTA of the int8 GEMMs for handles created from now on; 0 = natural."""
+    _check(load_library().qe_hpsi_test_set_int8_kmax(int(kmax)))
+
+
 def qe_hpsi_probe_fp64(millis=200.0):
-    """(DMMA TFLOP/s, DFMA TFLOP/s) measured on the current device."""
+    """(qe_hpsi_test.h) (DMMA TFLOP/s, DFMA TFLOP/s) measured on the current device."""
     lib = load_library()
     a, b = _c.c_double(0), _c.c_double(0)
     _check(lib.qe_hpsi_probe_fp64(float(millis), _c.byref(a), _c.byref(b)))
@@ -271,6 +293,42 @@ class Hpsi:
                                         ldy, ny, 1 if accumulate else 0, _stream_ptr(stream)), self._h)
         return y
 
+    def residual(self, hx, sx, e, r=None, want_norm=True, stream=None):
+        """qe_hpsi_residual: r = hx - e[b] sx over the sphere entries and rnorm2[b] = |r_b|^2 (CUDA float64 [nb])."""
+        nb = int(hx.shape[0])
+        for t in (hx, sx):
+            assert t.is_cuda and t.dtype == torch.complex128 and t.stride(1) == 1 and t.shape[0] == nb
+        assert e.is_cuda and e.dtype == torch.float64 and e.numel() == nb
+        if r is None:
+            r = torch.zeros_like(hx)
+        n2 = torch.empty(nb, dtype=torch.float64, device=hx.device) if want_norm else None
+        ld = lambda t: int(t.stride(0)) if nb > 1 else int(t.shape[1])
+        _check(self._lib.qe_hpsi_residual(self._h, _vp(hx.data_ptr()), ld(hx), _vp(sx.data_ptr()), ld(sx), _vp(e.data_ptr()),
+                                          _vp(r.data_ptr()), ld(r), nb, _vp(n2.data_ptr()) if want_norm else _vp(None),
+                                          _stream_ptr(stream)), self._h)
+        return r, n2
+
+    def scale(self, x, fac, stream=None):
+        """qe_hpsi_scale: x[b] *= fac[b] in place (fac CUDA float64 [nb])."""
+        nb = int(x.shape[0])
+        assert x.is_cuda and x.dtype == torch.complex128 and x.stride(1) == 1
+        assert fac.is_cuda and fac.dtype == torch.float64 and fac.numel() == nb
+        ldx = int(x.stride(0)) if nb > 1 else int(x.shape[1])
+        _check(self._lib.qe_hpsi_scale(self._h, _vp(x.data_ptr()), ldx, nb, _vp(fac.data_ptr()), _stream_ptr(stream)), self._h)
+        return x
+
+    def set_proj_tolerance(self, tol: float):
+        """qe_hpsi_set_proj_tolerance (handles created with QE_HPSI_PROJ_INT8 | QE_HPSI_PROJ_CERTIFY)."""
+        _check(self._lib.qe_hpsi_set_proj_tolerance(self._h, float(tol)), self._h)
+
+    def proj_check(self, nb):
+        """qe_hpsi_get_proj_check: (est_b / |v_b| float64 [nb], redo int32 [nb]) of the last chunk applied (CUDA tensors)."""
+        dev = torch.device("cuda", torch.cuda.current_device())
+        rel = torch.empty(nb, dtype=torch.float64, device=dev)
+        redo = torch.empty(nb, dtype=torch.int32, device=dev)
+        _check(self._lib.qe_hpsi_get_proj_check(self._h, _vp(rel.data_ptr()), _vp(redo.data_ptr()), _stream_ptr(None)), self._h)
+        return rel, redo
+
     def density(self, psi, occ, scale, rho, stream=None):
         """qe_hpsi_density: rho[N1,N2,N3] += scale * sum_b occ[b] |psi_b(r)|^2 (rho, occ: CUDA float64 tensors)."""
         assert psi.is_cuda and psi.dtype == torch.complex128 and psi.dim() == 2 and psi.stride(1) == 1
@@ -306,10 +364,13 @@ class Hpsi:
         _check(self._lib.qe_hpsi_info(self._h, buf), self._h)
         keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
                 "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit", "ozaki_3m"]
-        return {k: int(buf[i]) for i, k in enumerate(keys)}
+        d = {k: int(buf[i]) for i, k in enumerate(keys)}
+        d["certify"] = d["ozaki_3m"] >> 2
+        d["ozaki_3m"] &= 3
+        return d
 
     PROFILE_SLOTS = ["a6_becp", "a7_reduce_dmul", "a1_a5_fft_chain", "a8_vnl_add", "a1_scatter_zinv", "a2_yinv",
-                     "a3_x_vmul", "a4_yfwd", "a5_zfwd_gather", "a6_a8_int8_digits"]
+                     "a3_x_vmul", "a4_yfwd", "a5_zfwd_gather", "a6_a8_int8_digits", "certify_check_redo"]
 
     def profile(self, mode: int):
         """qe_hpsi_profile: 0 off, 1 stage events, 2 per-FFT-kernel events. Resets the accumulators."""
@@ -398,31 +459,3 @@ class HpsiGamma:
             self.destroy()
         except Exception:
             pass
-
-
-def from_workload(wl, max_batch=None, flags=0, device="cuda", beta=None):
-    """Build every input of a BASELINE.json workload on the GPU with the seeded generators (inputs.py) and the
-    library's own sphere, and create a handle. Returns (Hpsi, dict of inputs)."""
-    from . import inputs
-
-    wl = inputs.get_workload(wl)
-    mil = qe_hpsi_gsphere(wl.at, wl.xk, wl.ecutwfc, wl.nr)
-    npw = mil.shape[0]
-    ld = inputs.pad8(npw)
-    vr = inputs.gen_vloc(wl, device="cpu").to(device)  # input generation only (CPU FFT); not the product path
-    atoms = inputs.gen_atoms(wl)
-    mil_d = torch.as_tensor(mil, device=device)
-    if wl.nproj:
-        if beta is None:
-            beta = torch.zeros((wl.nproj, ld), dtype=torch.complex128, device=device)
-            step = 16
-            for a0 in range(0, wl.natoms, step):
-                na = min(step, wl.natoms - a0)
-                inputs.gen_beta(wl, mil_d, atoms, a0, na, ld=ld, device=device, out=beta[a0 * wl.nh:(a0 + na) * wl.nh])
-        blk = np.arange(wl.natoms + 1, dtype=np.int32) * wl.nh
-        db = inputs.gen_dblocks(wl)
-    else:
-        beta, blk, db = None, None, None
-    mb = wl.batch if max_batch is None else max_batch
-    h = Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, vr, beta, blk, db, max_batch=mb, flags=flags)
-    return h, dict(wl=wl, miller=mil, miller_dev=mil_d, ld=ld, vr=vr, atoms=atoms, beta=beta, dblocks=db)

@@ -13,11 +13,12 @@ from paper_2104_10502_b200 import qe_hpsi
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "qe_hpsi.h")
+TEST_HEADER = os.path.join(ROOT, "include", "qe_hpsi_test.h")
 
 
-def declared_functions():
-    """Names of every function prototype in include/qe_hpsi.h (comments stripped)."""
-    src = open(HEADER).read()
+def declared_functions(headers=(HEADER, TEST_HEADER)):
+    """Names of every function prototype in include/*.h (comments stripped)."""
+    src = "\n".join(open(h).read() for h in headers)
     src = re.sub(r"/\*.*?\*/", " ", src, flags=re.S)
     src = re.sub(r"//[^\n]*", " ", src)
     src = re.sub(r"^\s*#.*$", " ", src, flags=re.M)
@@ -91,6 +92,47 @@ def test_argument_errors_are_reported_before_any_device_work(lib):
     rc = lib.qe_hpsi_create(ctypes.byref(out), at.ctypes.data_as(pd), 8.0, xk.ctypes.data_as(pd), n.ctypes.data_as(pi),
                             None, 0, None, 0, 0, None, None, 1, 0, None)
     assert rc == qe_hpsi.QE_HPSI_EINVAL and out.value is None  # vr_dev NULL
+
+
+def test_precision_is_an_explicit_flag_and_bad_flag_words_are_rejected(lib):
+    """The accuracy class of the projector contractions is chosen by the caller, never by size or environment; malformed
+    flag words are EINVAL before any device work (include/qe_hpsi.h, qe_hpsi_create)."""
+    import numpy as np
+
+    at = np.diag([7.0, 7.0, 7.0]).reshape(-1)
+    xk = np.zeros(3)
+    n = np.asarray((15, 15, 15), dtype=np.int32)
+    pd, pi = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)
+    fake = ctypes.c_void_p(0x1000)  # never dereferenced: the flag check comes first
+
+    def create(flags):
+        out = ctypes.c_void_p(None)
+        rc = lib.qe_hpsi_create(ctypes.byref(out), at.ctypes.data_as(pd), 8.0, xk.ctypes.data_as(pd), n.ctypes.data_as(pi),
+                                fake, 0, None, 0, 0, None, None, 1, flags, None)
+        assert out.value is None
+        return rc
+
+    q = qe_hpsi
+    assert create(1 << 20) == q.QE_HPSI_EINVAL  # unknown bit
+    assert create(q.QE_HPSI_FP64_DMMA | q.QE_HPSI_PROJ_INT8) == q.QE_HPSI_EINVAL  # two accuracy classes
+    assert create(q.QE_HPSI_PROJ_CERTIFY) == q.QE_HPSI_EINVAL  # certify without the int8 path
+    assert create(q.QE_HPSI_PROJ_DIGITS(6)) == q.QE_HPSI_EINVAL  # digits without the int8 path
+    assert create(q.QE_HPSI_PROJ_3M_ALL) == q.QE_HPSI_EINVAL
+    assert create(q.QE_HPSI_PROJ_INT8 | q.QE_HPSI_PROJ_DIGITS(3)) == q.QE_HPSI_EINVAL  # 4..7 only
+    assert create(q.QE_HPSI_PROJ_INT8 | q.QE_HPSI_PROJ_DIGITS(8)) == q.QE_HPSI_EINVAL
+    assert q.QE_HPSI_PROJ_DIGITS(6) == 6 << 8 and q.QE_HPSI_PROJ_3M_A6 == 2 << 12
+    # the source reads no environment variable that changes the arithmetic
+    src = open(os.path.join(ROOT, "paper_2104_10502_b200", "csrc", "qe_hpsi.cu")).read()
+    for name in ("QE_HPSI_OZAKI", "QE_HPSI_OZ_3M", "QE_HPSI_OZ_KMAX"):
+        assert name not in src
+
+
+def test_product_header_holds_no_measurement_helpers():
+    prod = declared_functions((HEADER,))
+    for n in ("qe_hpsi_probe_fp64", "qe_hpsi_profile", "qe_hpsi_profile_read", "qe_hpsi_launch_count", "qe_hpsi_fft_local",
+              "qe_hpsi_nonlocal", "qe_hpsi_get_becp", "qe_hpsi_test_set_int8_kmax"):
+        assert n not in prod and n in declared_functions((TEST_HEADER,))
+    assert "qe_hpsi_last_error" in prod  # SURVEY.md 8(b) name
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):

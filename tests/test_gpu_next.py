@@ -164,7 +164,7 @@ def _gamma_inputs(cfg, nb):
     return wl, sp, vr, psi, beta, db
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA, _gpu.INT8])
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA, _gpu.INT8, _gpu.INT8_S7])
 @pytest.mark.parametrize("cfg,nb", [("T2_radix5", 4), ("T2b_radix5_20", 3), ("T3_aliased", 4), ("T4_noproj", 3), (0, 7), (0, 16)])
 def test_gamma_apply_against_oracle(cfg, nb, flags):
     wl, sp, vr, psi, beta, db = _gamma_inputs(cfg, nb)
@@ -175,8 +175,7 @@ def test_gamma_apply_against_oracle(cfg, nb, flags):
     if wl.nproj:
         bdev = torch.zeros((wl.nproj, ld), dtype=torch.complex128, device="cuda")
         bdev[:, :ngw] = torch.from_numpy(beta).cuda()
-    with _gpu.force_int8(flags) as f:
-        g = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), bdev, blk, db, max_batch=5, flags=f)
+    g = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), bdev, blk, db, max_batch=5, flags=flags)
     assert g.ngw == ngw
     pdev = torch.zeros((nb, ld), dtype=torch.complex128, device="cuda")
     pdev[:, :ngw] = torch.from_numpy(psi).cuda()

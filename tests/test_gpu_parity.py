@@ -33,7 +33,7 @@ def test_maps_bit_exact(cfg):
     h.destroy()
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA, _gpu.INT8])
+@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_GENERIC_FFT, qe_hpsi.QE_HPSI_FP64_DMMA, _gpu.INT8, _gpu.INT8_S7])
 @pytest.mark.parametrize("cfg", TINY + [0])
 def test_small_cases_against_dense_h(cfg, flags):
     """Level A (dense H from the definition) on every tiny case and config 0; both radix plans."""
@@ -110,17 +110,21 @@ def test_batch_composition_and_chunking_do_not_change_bits():
     h.destroy()
 
 
-@pytest.mark.parametrize("flags", [0, qe_hpsi.QE_HPSI_FP64_DMMA])
-def test_config1_all_bands(flags):
-    h, inp = _gpu.make(1, flags=flags)
+@pytest.mark.parametrize("path", ["fp64", "int8_s7", "int8_s6"])
+def test_config1_all_bands(path):
+    h, inp = _gpu.make(1, flags=_gpu.PATHS[path])
     wl = inp["wl"]
     sp = _gpu.oracle_sphere(wl)
     psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
     out = h.apply(psi)
+    vnl = h.nonlocal_add(psi, torch.zeros_like(psi))
     torch.cuda.synchronize()
-    ref = _gpu.oracle_hpsi(inp, sp, psi[:, :h.npw].cpu().numpy())
+    loc_ref, vnl_ref = _gpu.oracle_hpsi(inp, sp, psi[:, :h.npw].cpu().numpy(), parts=True)
+    ref = loc_ref + vnl_ref
     err = _gpu.rel_l2(out.cpu().numpy()[:, :h.npw], ref)
     assert err.max() <= TOL, err.max()
+    evnl = _gpu.rel_l2(vnl.cpu().numpy()[:, :h.npw], vnl_ref)
+    assert evnl.max() <= _gpu.TOL_VNL[path], f"config 1 {path}: nonlocal part alone {evnl.max():.2e}"
     # Level A' (definition, sampled rows) at full scale, no FFT of psi involved
     rows = inputs.aux_choice(wl.seed, 3, h.npw, 16)
     bands = [0, 63, 127]
@@ -133,33 +137,90 @@ def test_config1_all_bands(flags):
     h.destroy()
 
 
-@pytest.mark.parametrize("cfg,flags", [(2, 0), (3, 0), (4, 0), (4, qe_hpsi.QE_HPSI_FP64_DMMA)])
-def test_full_size_sampled_bands(cfg, flags):
-    """BASELINE.json's full sizes in the launch configuration bench.py times (batch = wl.batch, beta borrowed):
-    Level B oracle on sampled bands + a Hermitian probe <phi|H psi_b> = <H phi|psi_b> covering every band of the
-    batch at the cost of one extra oracle application."""
-    h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA | flags)
-    wl = inp["wl"]
-    sp = _gpu.oracle_sphere(wl)
-    npw = h.npw
-    nb = wl.batch
-    band0 = wl.nbands - nb  # last batch
-    psi = _gpu.gen_psi_dev(inp, band0, nb)
-    out = h.apply(psi)
-    torch.cuda.synchronize()
-    sample = sorted({0, nb - 1, nb // 2 + 1})
-    phi = inputs.aux_normal_complex(wl.seed, 99, npw).numpy()
-    phi /= np.linalg.norm(phi)
-    x = np.concatenate([psi[sample, :npw].cpu().numpy(), phi[None]])
-    ref = _gpu.oracle_hpsi(inp, sp, x)
-    err = _gpu.rel_l2(out[sample, :npw].cpu().numpy(), ref[:-1])
-    assert err.max() <= TOL, err
-    hphi = torch.as_tensor(ref[-1], device="cuda")
-    lhs = (torch.as_tensor(phi, device="cuda").conj()[None] * out[:, :npw]).sum(1)
-    rhs = (hphi.conj()[None] * psi[:, :npw]).sum(1)
-    scale = float(torch.linalg.vector_norm(out[:, :npw], dim=1).max())
-    assert float((lhs - rhs).abs().max()) <= 1e-11 * scale
-    h.destroy()
+def _sample_bands(wl):
+    """First and last band of every `batch`-band call plus 8 seeded random bands (SURVEY.md 8(c) pin table)."""
+    s = set()
+    for b0 in range(0, wl.nbands, wl.batch):
+        s.add(b0)
+        s.add(min(wl.nbands, b0 + wl.batch) - 1)
+    s.update(int(x) for x in inputs.aux_choice(wl.seed, 7, wl.nbands, 8))
+    return sorted(s)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_against_oracle_every_projector_path(cfg):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (calls of `batch` bands, beta borrowed), ALL
+    bands applied, for each projector path (FP64 default, int8 S = 7, int8 S = 6):
+      * sampled bands (first + last of every call, 8 random): H psi against oracle Level B, and the NONLOCAL PART ALONE
+        (qe_hpsi_nonlocal on zeros) against the oracle's nonlocal part -- it is ~1e-5 of |H psi| here, so only this isolates
+        a6 / a8 at their full-size shapes (23-37 K splits, 64 K blocks x 3 planes); becp of the sampled bands against orc.becp_of;
+      * every band: Hermitian probes <phi|H psi_b> = <H phi|psi_b> and <phi|V_NL psi_b> = <V_NL phi|psi_b>;
+      * Level A' (the definition, sampled rows, no FFT of psi) with becp accumulated over atom chunks.
+    The oracle runs once per config (beta streamed device -> host in atom chunks)."""
+    wl = inputs.get_workload(cfg)
+    sample = _sample_bands(wl)
+    shared = {}
+    report = {}
+    for path, pflags in _gpu.PATHS.items():
+        h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA | pflags, beta=shared.get("beta"))
+        npw = h.npw
+        if not shared:
+            shared["beta"] = inp["beta"]
+            sp = _gpu.oracle_sphere(wl)
+            psi_s = torch.cat([_gpu.gen_psi_dev(inp, b, 1) for b in sample])[:, :npw].cpu().numpy()
+            phi = inputs.aux_normal_complex(wl.seed, 99, npw).numpy()
+            phi /= np.linalg.norm(phi)
+            loc_ref, vnl_ref, becp_ref = _gpu.oracle_hpsi(inp, sp, np.concatenate([psi_s, phi[None]]), want_becp=True)
+            shared.update(sp=sp, psi_s=psi_s, phi=phi, loc=loc_ref, vnl=vnl_ref, becp=becp_ref)
+        sp, phi = shared["sp"], shared["phi"]
+        loc_ref, vnl_ref, becp_ref = shared["loc"], shared["vnl"], shared["becp"]
+        phi_d = torch.as_tensor(phi, device="cuda")
+        hphi_d = torch.as_tensor(loc_ref[-1] + vnl_ref[-1], device="cuda")
+        vphi_d = torch.as_tensor(vnl_ref[-1], device="cuda")
+        got_h, got_v, got_b = {}, {}, {}
+        herm = herm_v = 0.0
+        scale_h = scale_v = 0.0
+        for b0 in range(0, wl.nbands, wl.batch):  # exactly bench.py's calls
+            n = min(wl.batch, wl.nbands - b0)
+            psi = _gpu.gen_psi_dev(inp, b0, n)
+            out = h.apply(psi)
+            vnl = h.nonlocal_add(psi, torch.zeros_like(psi))
+            becp, _ = h.becp(n)
+            torch.cuda.synchronize()
+            for b in sample:
+                if b0 <= b < b0 + n:
+                    got_h[b] = out[b - b0, :npw].cpu().numpy()
+                    got_v[b] = vnl[b - b0, :npw].cpu().numpy()
+                    got_b[b] = becp[:, b - b0].cpu().numpy()
+            herm = max(herm, float(((phi_d.conj()[None] * out[:, :npw]).sum(1) - (hphi_d.conj()[None] * psi[:, :npw]).sum(1)).abs().max()))
+            herm_v = max(herm_v, float(((phi_d.conj()[None] * vnl[:, :npw]).sum(1) - (vphi_d.conj()[None] * psi[:, :npw]).sum(1)).abs().max()))
+            scale_h = max(scale_h, float(torch.linalg.vector_norm(out[:, :npw], dim=1).max()))
+            scale_v = max(scale_v, float(torch.linalg.vector_norm(vnl[:, :npw], dim=1).max()))
+            del psi, out, vnl, becp
+        eh = _gpu.rel_l2(np.stack([got_h[b] for b in sample]), loc_ref[:-1] + vnl_ref[:-1])
+        ev = _gpu.rel_l2(np.stack([got_v[b] for b in sample]), vnl_ref[:-1])
+        gb = np.stack([got_b[b] for b in sample], 1)
+        eb = np.abs(gb - becp_ref[:, :-1]).max() / np.abs(becp_ref[:, :-1]).max()
+        report[path] = dict(hpsi=eh.max(), vnl=ev.max(), becp=eb, herm=herm / scale_h, herm_vnl=herm_v / scale_v)
+        msg = f"config {cfg} {path}: " + ", ".join(f"{k} {v:.2e}" for k, v in report[path].items())
+        print(msg)
+        assert eh.max() <= TOL, msg
+        assert ev.max() <= _gpu.TOL_VNL[path], msg
+        assert eb <= _gpu.TOL_BECP[path], msg
+        assert herm <= 1e-11 * scale_h, msg
+        assert herm_v <= _gpu.TOL_VNL[path] * 10 * scale_v, msg  # a dot product with a unit vector: same scale as the L2 error
+        if path == "fp64":  # Level A' on the FP64 result (the other paths are within TOL of it by the assertions above)
+            rows = inputs.aux_choice(wl.seed, 3, npw, 16)
+            vt = orc.vloc_coeffs(inp["vr"].cpu().numpy())
+            bcols = inp["beta"][:, torch.as_tensor(rows, device="cuda")].cpu().numpy()
+            ap = orc.hpsi_rows(rows, sp["miller"], sp["g2kin"], tuple(wl.nr), vt, shared["psi_s"][:3], bcols, inp["dblocks"],
+                               becp=becp_ref[:, :3])
+            got = np.stack([got_h[b] for b in sample[:3]])[:, rows]
+            ea = np.abs(got - ap).max() / np.abs(loc_ref[:3]).max()
+            assert ea <= 1e-12, f"config {cfg}: Level A' rows {ea:.2e}"
+        h.destroy()
+        del h
+        torch.cuda.empty_cache()
 
 
 def test_apply_host_matches_device_path():
