@@ -43,6 +43,11 @@ int qe_hpsi_probe_fp64(double millis, double* dmma_tflops, double* dfma_tflops);
  * finer, a8 walking its K ranges launch by launch).  Process-wide; not for production use. */
 int qe_hpsi_test_set_int8_kmax(int64_t kmax);
 
+/* Guard bands (the pool's GPUs do not run compute-sanitizer): every device buffer a handle owns is allocated with a
+ * pattern-filled tail of 256..511 bytes.  Synchronises the device and returns the number of buffers whose tail was
+ * overwritten (0 = no kernel wrote past the end of a workspace since create), or a negative status. */
+int64_t qe_hpsi_test_check_guards(qe_hpsi_t h);
+
 #ifdef __cplusplus
 }
 #endif

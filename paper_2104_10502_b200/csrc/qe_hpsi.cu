@@ -154,6 +154,12 @@ struct qe_hpsi_handle {
   std::vector<ProfSpan> prof_spans;
   double prof_ms[16] = {0};
   long long prof_cnt[16] = {0};
+  // guard bands: every device buffer the handle owns ends in a pattern-filled tail that qe_hpsi_test_check_guards verifies
+  struct Guard {
+    const unsigned char* p;
+    size_t n;
+  };
+  std::vector<Guard> guards;
 };
 
 namespace {
@@ -169,6 +175,26 @@ namespace {
   } while (0)
 
 std::atomic<int> g_last_cuda{0};  // last CUDA error of calls that have no handle (diagnostic only)
+
+// Device allocation of a buffer the handle owns, with a guard band: the bytes from `bytes` up to the next multiple of 256
+// plus 256 more are filled with 0xA5 and registered; qe_hpsi_test_check_guards (include/qe_hpsi_test.h) verifies them, so
+// any kernel that writes past the end of a workspace is caught by the ordinary GPU tests (compute-sanitizer is not
+// available on the test pool).  Costs <= 511 bytes and one small memset per buffer, at create time only.
+constexpr size_t GUARD_BYTES = 256;
+template <typename T>
+cudaError_t guarded_malloc(qe_hpsi_handle* h, T** p, size_t bytes) {
+  const size_t padded = (bytes + 255) / 256 * 256 + GUARD_BYTES;
+  cudaError_t e = cudaMalloc(p, padded);
+  if (e != cudaSuccess) return e;
+  unsigned char* tail = reinterpret_cast<unsigned char*>(*p) + bytes;
+  e = cudaMemset(tail, 0xA5, padded - bytes);
+  if (e != cudaSuccess) return e;
+  try {
+    h->guards.push_back({tail, padded - bytes});
+  } catch (...) {  // out of host memory: this buffer is simply not watched
+  }
+  return cudaSuccess;
+}
 
 // ---- stage timing helpers ---------------------------------------------------------------------------------
 enum { SLOT_BECP = 0, SLOT_DMUL = 1, SLOT_FFT = 2, SLOT_VNL = 3, SLOT_A1 = 4, SLOT_A2 = 5, SLOT_A3 = 6, SLOT_A4 = 7, SLOT_A5 = 8,
@@ -576,6 +602,21 @@ extern "C" const char* qe_hpsi_strerror(int status) {
 }
 
 extern "C" int qe_hpsi_last_error(qe_hpsi_t h) { return h ? h->last_cuda : g_last_cuda.load(); }
+extern "C" int64_t qe_hpsi_test_check_guards(qe_hpsi_t h) {
+  if (!h) return QE_HPSI_ESTATE;
+  if (cudaDeviceSynchronize() != cudaSuccess) return QE_HPSI_ECUDA;
+  int64_t bad = 0;
+  unsigned char buf[512];
+  for (const auto& g : h->guards) {
+    if (g.n > sizeof(buf) || cudaMemcpy(buf, g.p, g.n, cudaMemcpyDeviceToHost) != cudaSuccess) return QE_HPSI_ECUDA;
+    for (size_t i = 0; i < g.n; ++i)
+      if (buf[i] != 0xA5) {
+        ++bad;
+        break;
+      }
+  }
+  return bad;
+}
 extern "C" int qe_hpsi_test_set_int8_kmax(int64_t kmax) {
   if (kmax < 0) return QE_HPSI_EINVAL;
   g_int8_kmax = kmax;
@@ -936,11 +977,11 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, unsigned flags, cudaSt
   const long long a2rows = (h->gamma ? 2LL : 1LL) * h->npw;
   const size_t a1 = h->oz_3m ? (size_t)S * 3 * h->nproj * h->oz_k1c : (size_t)S * h->nproj * k1, a2 = h->oz_3m8 ? (size_t)S * 3 * h->npw * h->oz_k2c : (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
   const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit * (h->oz_3m ? 3 : 1);
-  if ((e = cudaMalloc(&h->oz_a1, a1)) != cudaSuccess || (e = cudaMalloc(&h->oz_a2, a2)) != cudaSuccess ||
-      (e = cudaMalloc(&h->oz_b, bb)) != cudaSuccess || (e = cudaMalloc(&h->oz_partial, pc)) != cudaSuccess ||
-      (e = cudaMalloc(&h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
-      (e = cudaMalloc(&h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
-      (e = cudaMalloc(&h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess) {
+  if ((e = guarded_malloc(h, &h->oz_a1, a1)) != cudaSuccess || (e = guarded_malloc(h, &h->oz_a2, a2)) != cudaSuccess ||
+      (e = guarded_malloc(h, &h->oz_b, bb)) != cudaSuccess || (e = guarded_malloc(h, &h->oz_partial, pc)) != cudaSuccess ||
+      (e = guarded_malloc(h, &h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
+      (e = guarded_malloc(h, &h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
+      (e = guarded_malloc(h, &h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess) {
     // the digit planes do not fit (or another CUDA error): qe_hpsi_create fails with QE_HPSI_ENOMEM / QE_HPSI_ECUDA; the buffers
     // allocated so far are released by qe_hpsi_destroy
     return e;
@@ -990,7 +1031,7 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
       h->ldbeta = ldbeta;
     } else {
       h->ldbeta = ((long long)h->npw + 7) / 8 * 8;
-      CR_TRY(cudaMalloc(&h->beta_own, sizeof(double2) * (size_t)nproj * h->ldbeta));
+      CR_TRY(guarded_malloc(h, &h->beta_own, sizeof(double2) * (size_t)nproj * h->ldbeta));
       CR_TRY(cudaMemsetAsync(h->beta_own, 0, sizeof(double2) * (size_t)nproj * h->ldbeta, st));
       CR_TRY(cudaMemcpy2DAsync(h->beta_own, sizeof(double2) * h->ldbeta, beta_dev, sizeof(double2) * (size_t)ldbeta,
                                sizeof(double2) * (size_t)h->npw, (size_t)nproj, cudaMemcpyDeviceToDevice, st));
@@ -1027,10 +1068,10 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
       h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
     }
     const size_t pc = (size_t)nproj * h->ldc * sizeof(double2);
-    CR_TRY(cudaMalloc(&h->partial, pc * h->nsplit));
-    CR_TRY(cudaMalloc(&h->becp, pc));
-    CR_TRY(cudaMalloc(&h->dbecp, pc));
-    CR_TRY(cudaMalloc(&h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
+    CR_TRY(guarded_malloc(h, &h->partial, pc * h->nsplit));
+    CR_TRY(guarded_malloc(h, &h->becp, pc));
+    CR_TRY(guarded_malloc(h, &h->dbecp, pc));
+    CR_TRY(guarded_malloc(h, &h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
     CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
     h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
     if (flags & QE_HPSI_PROJ_INT8) CR_TRY(setup_ozaki(h, max_batch, flags, st));
@@ -1050,21 +1091,21 @@ cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
   h->cert_ld = ld;
   const size_t row = sizeof(double2) * (size_t)ld, mb = (size_t)h->max_batch;
   h->cert_nch = (int)std::max<long long>(1, std::min<long long>(64, (h->npw + 32767) / 32768));
-  CR_TRY(cudaMalloc(&h->cert_y, row * cert::NPROBE));
-  CR_TRY(cudaMalloc(&h->cert_v8, row * mb));
-  CR_TRY(cudaMalloc(&h->cert_psif, row * mb));
-  CR_TRY(cudaMalloc(&h->cert_vf, row * mb));
-  CR_TRY(cudaMalloc(&h->cert_part, sizeof(double) * mb * h->cert_nch * cert::NVAL));
-  CR_TRY(cudaMalloc(&h->cert_rel, sizeof(double) * mb));
-  CR_TRY(cudaMalloc(&h->cert_redo, sizeof(int) * mb));
-  CR_TRY(cudaMalloc(&h->cert_slot, sizeof(int) * mb));
-  CR_TRY(cudaMalloc(&h->cert_list, sizeof(int) * mb));
-  CR_TRY(cudaMalloc(&h->cert_count, sizeof(int)));
+  CR_TRY(guarded_malloc(h, &h->cert_y, row * cert::NPROBE));
+  CR_TRY(guarded_malloc(h, &h->cert_v8, row * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_psif, row * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_vf, row * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_part, sizeof(double) * mb * h->cert_nch * cert::NVAL));
+  CR_TRY(guarded_malloc(h, &h->cert_rel, sizeof(double) * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_redo, sizeof(int) * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_slot, sizeof(int) * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_list, sizeof(int) * mb));
+  CR_TRY(guarded_malloc(h, &h->cert_count, sizeof(int)));
   const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2);
-  CR_TRY(cudaMalloc(&h->partial_f, pc * h->nsplit));
-  CR_TRY(cudaMalloc(&h->becp_f, pc));
-  CR_TRY(cudaMalloc(&h->dbecp_f, pc));
-  CR_TRY(cudaMalloc(&h->dbT_f, mb * h->ldp * sizeof(double2)));
+  CR_TRY(guarded_malloc(h, &h->partial_f, pc * h->nsplit));
+  CR_TRY(guarded_malloc(h, &h->becp_f, pc));
+  CR_TRY(guarded_malloc(h, &h->dbecp_f, pc));
+  CR_TRY(guarded_malloc(h, &h->dbT_f, mb * h->ldp * sizeof(double2)));
   CR_TRY(cudaMemsetAsync(h->dbT_f, 0, mb * h->ldp * sizeof(double2), st));
   CR_TRY(cudaMemsetAsync(h->cert_y, 0, row * cert::NPROBE, st));
   CR_TRY(cudaMemsetAsync(h->cert_rel, 0, sizeof(double) * mb, st));
@@ -1301,7 +1342,7 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
   // V(r)/N in the padded layout
   {
     const long long rows = (long long)nr[0] * nr[1];
-    CR_TRY(cudaMalloc(&h->vs, sizeof(double) * (size_t)rows * h->ldz));
+    CR_TRY(guarded_malloc(h, &h->vs, sizeof(double) * (size_t)rows * h->ldz));
     const long long tot = rows * h->ldz;
     const double scale = 1.0 / ((double)nr[0] * (double)nr[1] * (double)nr[2]);
     k_scale_pad_v<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(vr_dev, h->vs, nr[2], h->ldz, rows, scale);
@@ -1325,8 +1366,8 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
     const int forced = env_int("QE_HPSI_FFT_NB", 0);
     if (forced > 0) nbf = std::min(forced, max_batch);
     h->fft_nb = (int)nbf;
-    CR_TRY(cudaMalloc(&h->w1, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2))));
-    CR_TRY(cudaMalloc(&h->w2, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2))));
+    CR_TRY(guarded_malloc(h, &h->w1, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2))));
+    CR_TRY(guarded_malloc(h, &h->w2, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2))));
     // pad columns i3 in [N3, ldz) are carried through the y and x passes of the fast path: keep them finite
     CR_TRY(cudaMemsetAsync(h->w1, 0, std::max<size_t>(16, (size_t)h->fft_nb * h->S * h->ldz * sizeof(double2)), st));
     CR_TRY(cudaMemsetAsync(h->w2, 0, std::max<size_t>(16, (size_t)h->fft_nb * h->P * nr[1] * h->ldz * sizeof(double2)), st));
@@ -1414,7 +1455,7 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
     kchunk = std::max(ZgV0::BK, (kchunk + ZgV0::BK - 1) / ZgV0::BK * ZgV0::BK);
     h->ovl_kchunk = kchunk;
     h->ovl_ns = std::max(1, (h->npw + kchunk - 1) / kchunk);
-    CR_TRY(cudaMalloc(&h->ovl_partial, sizeof(double2) * (size_t)h->ovl_ns * 512 * 128));
+    CR_TRY(guarded_malloc(h, &h->ovl_partial, sizeof(double2) * (size_t)h->ovl_ns * 512 * 128));
     h->workspace_bytes += sizeof(double2) * (size_t)h->ovl_ns * 512 * 128;
   }
   CR_TRY(cudaStreamSynchronize(st));
@@ -1667,9 +1708,9 @@ extern "C" int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host) {
   CU_TRY(h, cudaSetDevice(h->device));
   if (!h->qpk) {
     const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2);
-    CU_TRY(h, cudaMalloc(&h->qpk, sizeof(double) * (size_t)std::max<long long>(h->d_total, 1)));
-    CU_TRY(h, cudaMalloc(&h->qbecp, pc));
-    CU_TRY(h, cudaMalloc(&h->qbT, (size_t)h->max_batch * h->ldp * sizeof(double2)));
+    CU_TRY(h, guarded_malloc(h, &h->qpk, sizeof(double) * (size_t)std::max<long long>(h->d_total, 1)));
+    CU_TRY(h, guarded_malloc(h, &h->qbecp, pc));
+    CU_TRY(h, guarded_malloc(h, &h->qbT, (size_t)h->max_batch * h->ldp * sizeof(double2)));
     CU_TRY(h, cudaMemset(h->qbT, 0, (size_t)h->max_batch * h->ldp * sizeof(double2)));
     h->workspace_bytes += pc + (size_t)h->max_batch * h->ldp * sizeof(double2);
   }
@@ -2157,8 +2198,8 @@ extern "C" int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldp
     h->ldint = ((long long)h->npw + 7) / 8 * 8;
     const size_t bytes = std::max<size_t>(16, (size_t)h->max_batch * h->ldint * sizeof(double2));
     for (int i = 0; i < 2; ++i) {
-      CU_TRY(h, cudaMalloc(&h->hbuf_psi[i], bytes));
-      CU_TRY(h, cudaMalloc(&h->hbuf_h[i], bytes));
+      CU_TRY(h, guarded_malloc(h, &h->hbuf_psi[i], bytes));
+      CU_TRY(h, guarded_malloc(h, &h->hbuf_h[i], bytes));
       CU_TRY(h, cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
       CU_TRY(h, cudaEventCreateWithFlags(&h->ev_comp[i], cudaEventDisableTiming));
       CU_TRY(h, cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming));

@@ -60,6 +60,7 @@ SIGNATURES = {
     "qe_hpsi_scale": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp]),
     # ---- include/qe_hpsi_test.h: measurement and test helpers, not the product boundary ----
     "qe_hpsi_test_set_int8_kmax": (_i32, [_i64]),
+    "qe_hpsi_test_check_guards": (_i64, [_vp]),
     "qe_hpsi_probe_fp64": (_i32, [_dbl, _pd, _pd]),
     "qe_hpsi_profile": (_i32, [_vp, _i32]),
     "qe_hpsi_profile_read": (_i32, [_vp, _pd, _pi64]),
@@ -382,6 +383,13 @@ class Hpsi:
         cnt = (_c.c_int64 * 16)()
         _check(self._lib.qe_hpsi_profile_read(self._h, ms, cnt), self._h)
         return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(self.PROFILE_SLOTS)}
+
+    def check_guards(self) -> int:
+        """(qe_hpsi_test.h) number of handle-owned device buffers whose guard band was overwritten (synchronises)."""
+        n = int(self._lib.qe_hpsi_test_check_guards(self._h))
+        if n < 0:
+            _check(n, self._h)
+        return n
 
     def launch_count(self, nbands) -> int:
         return int(self._lib.qe_hpsi_launch_count(self._h, int(nbands)))

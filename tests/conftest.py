@@ -24,3 +24,24 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(autouse=True)
+def _guard_bands_checked_at_destroy(monkeypatch):
+    """Every handle a GPU test destroys first has its guard bands verified (qe_hpsi_test_check_guards): a kernel that wrote
+    past the end of any workspace of the handle fails the test that used it. Stands in for compute-sanitizer memcheck, which
+    the GPU pool does not run (profiles/r2_sanitizer.md)."""
+    from paper_2104_10502_b200 import qe_hpsi
+
+    orig = qe_hpsi.Hpsi.destroy
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value is not None:
+            bad = self.check_guards()
+            orig(self)
+            assert bad == 0, f"{bad} device buffer(s) of the handle were written past their end"
+        else:
+            orig(self)
+
+    monkeypatch.setattr(qe_hpsi.Hpsi, "destroy", destroy)
+    yield

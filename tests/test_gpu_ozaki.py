@@ -167,3 +167,121 @@ def test_k_ranges_of_a8_and_forced_splits_of_a6_give_the_same_result():
     num = torch.linalg.vector_norm(out - ref, dim=1)
     den = torch.linalg.vector_norm(ref, dim=1)
     assert float((num / den).max()) <= 1e-13  # same digits, same exact integer sums; only the FP64 order of the K ranges differs
+
+
+# ---- QE_HPSI_PROJ_CERTIFY: a-posteriori check + FP64 re-computation -----------------------------------
+def _outer_shell_psi(inp, sp, nb, frac=0.9):
+    """Adversarial bands for a per-row-exponent fixed-point scheme: psi lives only on the outer shell |k+G|^2 > frac ecut,
+    where the Gaussian projectors are 1e-5 .. 1e-10 of their row maxima, so <beta|psi> is carried by digits the 47-bit split
+    has mostly truncated (config 1: e^(-q^2 rc^2 / 2) = 7e-5 at rc 0.8 and 4e-10 at rc 1.2 for q^2 = 30)."""
+    psi = _gpu.gen_psi_dev(inp, 300, nb)
+    wl = inp["wl"]
+    shell = torch.as_tensor(sp["g2kin"] > frac * wl.ecutwfc, device="cuda")
+    psi[:, :shell.numel()] *= shell.to(torch.complex128)[None]
+    psi /= torch.linalg.vector_norm(psi, dim=1)[:, None]
+    return psi
+
+
+def test_certified_path_recomputes_the_bands_the_47_bit_split_gets_wrong():
+    """S = 6 WITHOUT the certificate exceeds north_star's 1e-11 on the nonlocal part of outer-shell bands; the certified handle
+    flags exactly those bands, re-computes them on the FP64 tensor path and meets the tolerance; ordinary bands in the same
+    call keep their int8 result."""
+    h6, inp = _make_int8(1, 6)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h6.npw
+    n_adv, n_ok = 5, 7
+    psi = torch.cat([_gpu.gen_psi_dev(inp, 0, n_ok), _outer_shell_psi(inp, sp, n_adv)])
+    order = torch.as_tensor([0, 7, 1, 8, 2, 9, 3, 10, 4, 11, 5, 6], device="cuda")  # interleave: adversarial bands at 1, 3, 5, 7, 9
+    psi = psi[order].contiguous()
+    adv = np.array([1, 3, 5, 7, 9])
+    ok = np.array([b for b in range(n_adv + n_ok) if b not in adv])
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
+    plain = h6.nonlocal_add(psi, torch.zeros_like(psi)).cpu().numpy()[:, :npw]
+    e_plain = _gpu.rel_l2(plain, vref)
+    assert e_plain[adv].min() > 1e-11, e_plain  # the uncertified 47-bit path really fails here ...
+    assert e_plain[ok].max() <= 1e-11, e_plain  # ... and only here
+    h6.destroy()
+    hc, _ = _gpu.make(1, flags=harness.int8_flags(6, certify=True), beta=inp["beta"])
+    assert hc.info()["certify"] == 1
+    sent = torch.zeros_like(psi)
+    sent[:, npw:] = 3.0  # pad columns must stay untouched
+    out = hc.nonlocal_add(psi, sent)
+    rel, redo = hc.proj_check(psi.shape[0])
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()[:, :npw]
+    e_cert = _gpu.rel_l2(got, vref)
+    redo = redo.cpu().numpy()
+    rel = rel.cpu().numpy()
+    assert np.array_equal(np.nonzero(redo)[0], adv), (redo, rel)
+    assert e_cert.max() <= 1e-11, e_cert
+    assert np.all(out.cpu().numpy()[:, npw:] == 3.0)
+    # qe_hpsi_nonlocal accumulates on top of the caller's array in this mode too
+    base = torch.as_tensor(vref, device="cuda") * (0.5 - 0.25j)
+    acc = torch.zeros_like(psi)
+    acc[:, :npw] = base
+    hc.nonlocal_add(psi, acc)
+    torch.cuda.synchronize()
+    assert _gpu.rel_l2(acc.cpu().numpy()[:, :npw], vref * (1.5 - 0.25j)).max() <= 1e-11
+    # the estimate tracks the true error of the int8 result (within the factor the 8 probes give), flagged or not
+    ratio = rel / np.maximum(e_plain, 1e-300)
+    assert np.all(ratio > 0.3) and np.all(ratio < 3.0), (rel, e_plain)
+    # the whole H psi through qe_hpsi_apply takes the same decision and is the FP64 handle's result for the flagged bands
+    hps = hc.apply(psi)
+    _, redo2 = hc.proj_check(psi.shape[0])
+    assert np.array_equal(redo2.cpu().numpy(), redo)
+    hf, _ = _gpu.make(1, beta=inp["beta"])
+    ref = hf.apply(psi)
+    torch.cuda.synchronize()
+    d = torch.linalg.vector_norm(hps[:, :npw] - ref[:, :npw], dim=1) / torch.linalg.vector_norm(ref[:, :npw], dim=1)
+    assert float(d.max()) <= 1e-13
+    # a looser caller tolerance keeps every int8 result; tolerance 0 re-computes everything
+    hc.set_proj_tolerance(1e-3)
+    hc.nonlocal_add(psi, torch.zeros_like(psi))
+    assert int(hc.proj_check(psi.shape[0])[1].sum()) == 0
+    hc.set_proj_tolerance(0.0)
+    allf = hc.nonlocal_add(psi, torch.zeros_like(psi))
+    assert int(hc.proj_check(psi.shape[0])[1].sum()) == psi.shape[0]
+    fp = hf.nonlocal_add(psi, torch.zeros_like(psi))
+    torch.cuda.synchronize()
+    assert torch.equal(allf[:, :npw].view(torch.float64), fp[:, :npw].view(torch.float64))  # the re-computation IS the FP64 path
+    hc.destroy()
+    hf.destroy()
+
+
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T5_odd_bands", 0])
+def test_certified_path_small_cases_chunking_nan_and_graph(cfg):
+    """max_batch smaller than the probe count and than the band count (several chunks), a NaN band (re-computed: FP64
+    semantics), bit-reproducibility, and CUDA-graph capture (the decision never leaves the device)."""
+    hc, inp = _gpu.make(cfg, flags=harness.int8_flags(6, three_m=3, certify=True), max_batch=3)
+    wl = inp["wl"]
+    npw = hc.npw
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    beta = inp["beta"][:, :npw].cpu().numpy()
+    vref = orc.vnl_psi(beta, inp["dblocks"], psi[:, :npw].cpu().numpy())
+    a = hc.nonlocal_add(psi, torch.zeros_like(psi))
+    b = hc.nonlocal_add(psi, torch.zeros_like(psi))
+    torch.cuda.synchronize()
+    assert torch.equal(a.view(torch.float64), b.view(torch.float64))
+    assert _gpu.rel_l2(a.cpu().numpy()[:, :npw], vref).max() <= 1e-11
+    bad = psi.clone()
+    bad[1, 3] = float("nan")
+    o = hc.nonlocal_add(bad, torch.zeros_like(bad)).cpu().numpy()[:, :npw]
+    assert np.isnan(o[1]).any() and not np.isnan(np.delete(o, 1, 0)).any()
+    # graph capture of the full apply
+    ref = hc.apply(psi).clone()
+    buf, out = psi.clone(), torch.zeros_like(psi)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        hc.apply(buf, out, side)
+    torch.cuda.current_stream().wait_stream(side)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        hc.apply(buf, out, torch.cuda.current_stream())
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out[:, :npw].view(torch.float64), ref[:, :npw].view(torch.float64))
+    del g
+    hc.destroy()

@@ -6,7 +6,7 @@ import pytest
 import torch
 
 from oracle import hpsi_oracle as orc
-from paper_2104_10502_b200 import inputs, qe_hpsi
+from paper_2104_10502_b200 import harness, inputs, qe_hpsi
 from tests import _gpu
 
 pytestmark = pytest.mark.gpu
@@ -221,6 +221,32 @@ def test_full_size_against_oracle_every_projector_path(cfg):
         h.destroy()
         del h
         torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("flags", [0, _gpu.INT8, _gpu.INT8_S7, harness.int8_flags(6, three_m=3, certify=True)])
+@pytest.mark.parametrize("cfg", ["T1_general_k", "T5_odd_bands", 0])
+def test_apply_writes_nothing_outside_its_output_rows(cfg, flags):
+    """Caller-side guard bands: hpsi is a window in the middle of a sentinel-filled allocation (guard rows before and after,
+    pad columns inside); after apply / nonlocal / apply_host-style chunking every byte outside [b][0..npw) is untouched.
+    (The handle's own workspaces carry guard bands too, verified at destroy: tests/conftest.py.)"""
+    h, inp = _gpu.make(cfg, flags=flags, max_batch=5)
+    wl = inp["wl"]
+    npw, nb = h.npw, wl.nbands
+    ld = inp["ld"] + 8  # a row stride larger than the generator's
+    psi = torch.zeros((nb, ld), dtype=torch.complex128, device="cuda")
+    psi[:, :inp["ld"]] = _gpu.gen_psi_dev(inp, 0, nb)
+    guard = 3
+    buf = torch.full((nb + 2 * guard, ld), complex(7.0, -7.0), dtype=torch.complex128, device="cuda")
+    win = buf[guard:guard + nb]
+    h.apply(psi, win)
+    h.nonlocal_add(psi, win)
+    torch.cuda.synchronize()
+    host = buf.cpu().numpy()
+    assert np.all(host[:guard] == complex(7.0, -7.0)) and np.all(host[guard + nb:] == complex(7.0, -7.0))
+    assert np.all(host[guard:guard + nb, npw:] == complex(7.0, -7.0))
+    assert np.isfinite(host[guard:guard + nb, :npw]).all() and not np.any(host[guard:guard + nb, :npw] == complex(7.0, -7.0))
+    assert h.check_guards() == 0
+    h.destroy()
 
 
 def test_apply_host_matches_device_path():
