@@ -18,6 +18,9 @@ struct Fft2pGeom {
   const int* stick_hi;    // [S] highest
   const int* col_of;      // [P][N2] stick index of column (plane p, i2), or -1
   const int* plane_of;    // [N1] populated-plane index of i1, or -1
+  // the populated i1 planes of a convex sphere are the wrapped interval [0..x_hi] u [N1-x_lo..N1-1] (x_hi = -1 / x_lo = 0:
+  // that part is empty) in this order, so plane_of[i1] = i1, resp. i1 - (N1 - P); x_hi = -2 when the pattern does not hold
+  int x_hi, x_lo;
 };
 
 // shared tile [N][FFT_C] with the column XOR swizzle of fft_core.cuh (fft_phys)

@@ -30,22 +30,35 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
       : "memory");
 }
 
-// dynamic shared memory: tile1, tile2 [N][FFT_C], input stage [P][FFT_C], output stage [P][FFT_C], one mbarrier
-inline size_t fft2t_smem(int n, int P) { return 2 * (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)P * FFT_C * sizeof(double2) + 64; }
+// dynamic shared memory: tiles [2][N][FFT_C] (the two-pass kernel uses one), input stage [P][FFT_C], output stage [P][FFT_C],
+// one mbarrier, and (two-pass kernel) the twiddle table tw[q*j] as [RA][RA+1] (RA <= 16)
+// (the mbarrier of the two-pass kernel lives in the unused [0][0] entry of its twiddle table; the three-pass kernel has no table)
+inline size_t fft2t_smem(int n, int P, bool two_pass, bool one_tile) {
+  return (one_tile ? 1 : 2) * (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)P * FFT_C * sizeof(double2) +
+         (two_pass ? 16 * 17 * sizeof(double2) : 64);
+}
 
 // tmap: W2 viewed as FP64 [nb][P][N2*ldz*2], box {16, P, 1}
+// Register diet (round 2): the second-pass twiddles tw[q*j] sit in a padded shared table instead of 64 registers, and the
+// populated-plane index comes from the wrapped-interval rule of Fft2pGeom (x_hi, x_lo) instead of a 16-entry register array:
+// 222 -> under 168 registers, three CTAs per SM instead of two, so the FP64 pipe has 12 warps to pick from across the
+// three barriers of a band (the stage is bound by FP64 issue, not HBM: DESIGN.md section 6).
 template <int RA, int RB>
-__global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb) {
+__global__ void __launch_bounds__(RA* FFT_C, 3)
+k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb, int one_tile) {
   static_assert(RB > 1, "single-pass lengths use k2p_x_vmul");
-  constexpr int N = RA * RB, NT = RA * FFT_C, NW = (NT + 31) / 32;
+  static_assert(RA >= RB && RA <= 16, "twiddle table is [RA][RA+1]");
+  constexpr int N = RA * RB, NT = RA * FFT_C, NW = (NT + 31) / 32, TWP = RA + 1;
   constexpr unsigned ROWB = FFT_C * sizeof(double2);  // 128 bytes per plane row of the tile
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double2* tile1 = reinterpret_cast<double2*>(smem_raw);
-  double2* tile2 = tile1 + N * FFT_C;
+  // one_tile: the tile is reused between the passes (two more barriers per band, 24 KB less per CTA at N = 192)
+  double2* tile2 = one_tile ? tile1 : tile1 + N * FFT_C;
   double2* inb = tile2 + N * FFT_C;
   const int P = g.P;
   double2* outb = inb + (size_t)P * FFT_C;
-  unsigned long long* full = reinterpret_cast<unsigned long long*>(outb + (size_t)P * FFT_C);
+  double2* twt = outb + (size_t)P * FFT_C;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(twt);  // entry [0][0] (tw = 1) is never read: the mbarrier lives there  // [RA][TWP]: tw[(q*j) % N] at j*TWP + q (odd pitch: 4 rows per warp, no conflicts)
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
   const bool io_thread = tid == (NW - 1) * 32;  // first lane of the last warp (idle in the radix-RA passes when RA > RB)
   const int i2 = blockIdx.x / g.ntz;
@@ -54,14 +67,12 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, 
   double vv[RB];
 #pragma unroll
   for (int q = 0; q < RB; ++q) vv[q] = __ldg(&g.vs[((size_t)(j + q * RA) * g.n2 + i2) * g.ldz + z0 + c]);
-  int pl[RA];
-  if (j < RB) {
-#pragma unroll
-    for (int q = 0; q < RA; ++q) pl[q] = __ldg(&t.plane_of[j + q * RB]);
+  for (int idx = tid; idx < RA * RA; idx += NT) {
+    const int jj = idx / RA, q = idx - jj * RA;
+    if (q > 0) twt[jj * TWP + q] = __ldg(&g.ax1.tw[(q * jj) % N]);
   }
-  double2 twr[RA];  // tw[q*j]: second-pass twiddles of the inverse (q < RB) and of the forward transform (q < RA)
-#pragma unroll
-  for (int q = 0; q < RA; ++q) twr[q] = __ldg(&g.ax1.tw[(q * j) % N]);
+  const int xhi = t.x_hi, xlo0 = N - t.x_lo, xsh = N - P;  // plane index of i1: i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : none)
+  const double2* twj = twt + j * TWP;
   if (tid == 0) {
     mbar_init(full, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -90,7 +101,11 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, 
       double2 v[RA];
       const double2* in = inb + c;
 #pragma unroll
-      for (int q = 0; q < RA; ++q) v[q] = pl[q] >= 0 ? in[pl[q] * FFT_C] : zero;
+      for (int q = 0; q < RA; ++q) {
+        const int i1 = j + q * RB;
+        const int p = i1 <= xhi ? i1 : i1 - xsh;
+        v[q] = (i1 <= xhi || i1 >= xlo0) ? in[p * FFT_C] : zero;
+      }
       pass_a_store<RA, +1>(v, tile1, j, c);
     }
     __syncthreads();
@@ -103,27 +118,34 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, 
 #pragma unroll
       for (int q = 0; q < RB; ++q) u[q] = tile1[fft_phys(j + q * RA, c)];
 #pragma unroll
-      for (int q = 1; q < RB; ++q) u[q] = cmul(u[q], twr[q]);
+      for (int q = 1; q < RB; ++q) u[q] = cmul(u[q], twj[q]);
       Dft<RB, +1>::run(u);
 #pragma unroll
       for (int q = 0; q < RB; ++q) u[q] = make_double2(u[q].x * vv[q], u[q].y * vv[q]);
       Dft<RB, -1>::run(u);  // forward pass 1 = radix RB on the inputs j + q*RA this thread already holds
+      if (one_tile) __syncthreads();  // every thread has read its tile1 entries: the tile can take the pass output
 #pragma unroll
       for (int q = 0; q < RB; ++q) tile2[fft_phys(j * RB + q, c)] = u[q];
     }
     if (io_thread) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // output stage free before it is rewritten
     __syncthreads();
+    double2 v[RA];
     if (j < RB) {
-      double2 v[RA];
 #pragma unroll
       for (int q = 0; q < RA; ++q) v[q] = tile2[fft_phys(j + q * RB, c)];
+    }
+    if (one_tile) __syncthreads();  // the tile has been read: the next band's first pass may overwrite it
+    if (j < RB) {
 #pragma unroll
-      for (int q = 1; q < RA; ++q) v[q] = cmulc(v[q], twr[q]);
+      for (int q = 1; q < RA; ++q) v[q] = cmulc(v[q], twj[q]);
       Dft<RA, -1>::run(v);
       double2* out = outb + c;
 #pragma unroll
-      for (int q = 0; q < RA; ++q)
-        if (pl[q] >= 0) out[pl[q] * FFT_C] = v[q];
+      for (int q = 0; q < RA; ++q) {
+        const int i1 = j + q * RB;
+        if (i1 <= xhi) out[i1 * FFT_C] = v[q];
+        else if (i1 >= xlo0) out[(i1 - xsh) * FFT_C] = v[q];
+      }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the bulk store
     }
   }
@@ -138,7 +160,7 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_x_vmul(FftGeom g, Fft2pGeom t, 
 // three-pass variant (lengths of fft3p_kernels.cuh): same staging, arithmetic of k3p_x_vmul
 template <int R1, int R2, int R3>
 __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap,
-                                                                int nb) {
+                                                                int nb, int /*one_tile: two-pass kernel only*/) {
   using PP = P3<R1, R2, R3>;
   constexpr int N = PP::N, NT = PP::NT, NW = (NT + 31) / 32;
   constexpr unsigned ROWB = FFT_C * sizeof(double2);
@@ -362,7 +384,7 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_zfwd_gather(FftGeom g, Fft2pGeo
   }
 }
 
-using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int);
+using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, int);
 
 struct Fft2tEntry {
   int n, ra, rb;

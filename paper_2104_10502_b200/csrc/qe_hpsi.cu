@@ -77,6 +77,7 @@ struct qe_hpsi_handle {
   size_t smem_x2p = 0;
   // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
   K2tX x_tma = nullptr;
+  int x_one_tile = 0;  // two-pass x stage with one shared tile (tuning knob QE_HPSI_X_ONE_TILE)
   K2pZinv z_tma_inv = nullptr;  // bulk-staged a1 / a5 (fft2t_kernels.cuh)
   K2pZfwd z_tma_fwd = nullptr;
   size_t smem_zt = 0;
@@ -1287,6 +1288,21 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
     h->g2p.stick_hi = h->stick_hi;
     h->g2p.col_of = h->col_of;
     h->g2p.plane_of = h->plane_of;
+    // wrapped-interval rule of the populated planes (Fft2pGeom::x_hi / x_lo), verified against the table
+    {
+      int hi = -1, lo = 0;
+      for (int p_ = 0; p_ < h->P; ++p_) {
+        if (plane_i1[p_] < (n1 + 1) / 2) hi = std::max(hi, plane_i1[p_]);
+        else ++lo;
+      }
+      bool ok = (hi + 1) + lo == h->P;
+      for (int i1 = 0; i1 < n1 && ok; ++i1) {
+        const int want = i1 <= hi ? i1 : (i1 >= n1 - lo ? i1 - (n1 - h->P) : -1);
+        ok = plane_of[(size_t)i1] == want;
+      }
+      h->g2p.x_hi = ok ? hi : -2;
+      h->g2p.x_lo = ok ? lo : 0;
+    }
   }
 
   // ---- FFT plan ---------------------------------------------------------------------------------------
@@ -1374,9 +1390,10 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
     h->workspace_bytes += (size_t)h->fft_nb * per_band;
     // x pass: one CTA per (i2, i3 tile) loops over the bands of the sub-chunk; split the band loop over
     // gridDim.y only as far as needed to give every SM a few CTAs
-    if (h->f2p[0] && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && env_int("QE_HPSI_X_TMA", 1)) {
+    if (h->f2p[0] && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && h->g2p.x_hi != -2 && env_int("QE_HPSI_X_TMA", 1)) {
       const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb, h->f2p[0]->smem_zy != 0);
-      const size_t sm = fft2t_smem(nr[0], h->P);
+      h->x_one_tile = h->f2p[0]->smem_zy == 0 ? env_int("QE_HPSI_X_ONE_TILE", 0) : 0;
+      const size_t sm = fft2t_smem(nr[0], h->P, h->f2p[0]->smem_zy == 0, h->x_one_tile != 0);
       using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -1512,7 +1529,7 @@ int launch_local(qe_hpsi_t h, const double2* psi, long long ldpsi, double2* hpsi
       k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);
     size_t m2 = fine ? prof_mark(h, st) : (size_t)-1;
     if (h->x_tma)
-      h->x_tma<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_xt, st>>>(g, h->g2p, h->tmap_w2, n);
+      h->x_tma<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_xt, st>>>(g, h->g2p, h->tmap_w2, n, h->x_one_tile);
     else if (fast)
       ex->x<<<dim3(xt, std::min(n, h->x_split)), ex->nthreads, h->smem_x2p, st>>>(g, h->g2p, h->w2, n);
     else
