@@ -80,6 +80,12 @@ typedef enum {
 #define QE_HPSI_PROJ_3M_A6  (2u << 12)
 #define QE_HPSI_PROJ_3M_ALL (3u << 12)
 
+/* At k = 0 the FP64 path checks at create, bit for bit, whether every projector obeys beta_p(-G) = +-conj(beta_p(G)) (projector
+ * functions real in real space) and D couples equal signs only; if so a6 / a8 contract psi = u + i v as two real-wavefunction
+ * problems over the half sphere: 2/3 of the FP64 tensor work and half of the beta traffic, same FP64 arithmetic, results equal
+ * to the general path up to rounding order.  This flag keeps the general complex contraction. */
+#define QE_HPSI_NO_GAMMA_SYM 32u
+
 #define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */
 
 /* a0, stand-alone (PAPER.md:L176 (vi)).  Canonical sphere for a cell / k / cutoff / grid before any handle
@@ -139,7 +145,8 @@ int64_t qe_hpsi_nplanes(qe_hpsi_t h);        /* P: i1 planes holding >= 1 sphere
  * fft_index [npw] int32, g2kin [npw] float64.  Enqueued on cuda_stream. */
 int qe_hpsi_get_maps(qe_hpsi_t h, int32_t* miller_dev, int32_t* fftidx_dev, double* g2kin_dev, void* cuda_stream);
 /* info[0..15]: npw, S, P, fft band chunk, split-K count (FP64 path), workspace bytes, per axis j=0..2 the number of
- * generic FFT passes, K chunk, x split, SM count, two-pass FFT plan in use, then the projector path: [13] digits per
+ * generic FFT passes, K chunk, x split, SM count, [12] bit 0: two-pass FFT plan in use, bit 1: Gamma-symmetric projector mode of
+ * the FP64 path in use; then the projector path: [13] digits per
  * FP64 operand of the int8 path (0 = FP64 tensor path), [14] its split-K count of a6, [15] 1 if a6 runs in the
  * integer 3M form, 2 if a8 does too, +4 if QE_HPSI_PROJ_CERTIFY is on. */
 int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);

@@ -22,6 +22,7 @@
 #include "zgemm_kernels.cuh"
 #include "ozaki_kernels.cuh"
 #include "cert_kernels.cuh"
+#include "sym_kernels.cuh"
 
 using namespace qehpsi;
 
@@ -38,6 +39,7 @@ using ZgV2 = ZgCfg<128, 32, 4, 2, 16, 4>;
 using ZgV3 = ZgCfg<64, 64, 2, 4, 8, 6>;
 using ZgV4 = ZgCfg<64, 64, 2, 4, 32, 3>;
 using ZgV5 = ZgCfg<64, 64, 2, 4, 16, 6>;
+using ZgS = ZgCfg<64, 128, 2, 4, 16, 4>;  // real forms of the Gamma-symmetric mode: 2 nb columns, 4 x 4 blocks per warp
 constexpr int ZG_NVARIANT = 6;
 constexpr int ZG_BM_TAB[ZG_NVARIANT] = {64, 64, 128, 64, 64, 64};
 constexpr int ZG_BN_TAB[ZG_NVARIANT] = {64, 64, 32, 64, 64, 64};
@@ -118,6 +120,16 @@ struct qe_hpsi_handle {
   // NEXT-3: split-K workspace of qe_hpsi_overlap (allocated at create: its size depends on npw only)
   double2* ovl_partial = nullptr;
   int ovl_ns = 1, ovl_kchunk = 0;
+  // Gamma-symmetric projector mode of the FP64 path (sym_kernels.cuh): detected at create
+  bool sym = false;
+  int sym_m = 0;                      // leading sphere entries with n1 >= 0 (they hold the half sphere)
+  int* sym_minus = nullptr;           // [sym_m] position of -G, -1 skip, -2 G = 0
+  unsigned char* sym_cls = nullptr;   // [nproj] 0: beta(-G) = conj beta(G), 1: = -conj
+  unsigned* sym_cmask = nullptr;      // [ceil(nproj / 16)] bit j: class of projector 16 t + j (K tiles of the symmetric a8)
+  int sym_wide = 1;                   // 128-column tiles (ZgS) instead of ZgV0 (tuning knob QE_HPSI_SYM_WIDE)
+  double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
+  long long sym_ldu = 0;
+  int sym_nsplit = 1, sym_ldc2 = 0;
   // QE_HPSI_PROJ_CERTIFY: a-posteriori check of the int8 nonlocal part + FP64 re-computation
   bool certify = false;
   double cert_tol = 1e-11;
@@ -579,6 +591,12 @@ cudaError_t set_kernel_attrs() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_vnl_add<ZgS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_becp<ZgS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
 #undef SET_SMEM
   if (dev >= 0 && dev < MAX_DEVICES) g_attr_done[dev] = true;
   return cudaSuccess;
@@ -688,6 +706,12 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->oz_eg);
   cudaFree(h->oz_eb);
   cudaFree(h->oz_partial);
+  cudaFree(h->sym_minus);
+  cudaFree(h->sym_cls);
+  cudaFree(h->sym_cmask);
+  cudaFree(h->sym_u);
+  cudaFree(h->sym_e);
+  cudaFree(h->sym_partial);
   cudaFree(h->cert_y);
   cudaFree(h->cert_v8);
   cudaFree(h->cert_psif);
@@ -1132,10 +1156,83 @@ cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
   return cudaSuccess;
 }
 
+// Gamma-symmetric projector mode (sym_kernels.cuh): at k = 0, FP64 path.  Builds the -G map of the leading sphere entries,
+// classifies every projector ON THE DEVICE by exact comparison, checks that D couples equal classes only, and allocates the
+// real-form operands.  Leaves h->sym = false (general complex contraction) whenever any check fails; only CUDA errors are errors.
+cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, const int nr[3], int nblocks,
+                            const int32_t* blk_off_host, const double* d_host, cudaStream_t st) {
+#define CR_TRY(expr)                     \
+  do {                                   \
+    cudaError_t e__ = (expr);            \
+    if (e__ != cudaSuccess) return e__;  \
+  } while (0)
+  const int n1 = nr[0], n2 = nr[1], n3 = nr[2];
+  auto sgn = [](int i, int n) { return i >= (n + 1) / 2 ? i - n : i; };
+  int M = 0;
+  while (M < h->npw && (idx[M] / (n2 * n3)) < (n1 + 1) / 2) ++M;  // canonical order: n1 >= 0 comes first
+  std::vector<int> minus((size_t)std::max(M, 1));
+  for (int g = 0; g < M; ++g) {
+    const int i3 = idx[g] % n3, i2 = (idx[g] / n3) % n2, i1 = idx[g] / (n2 * n3);
+    const int m[3] = {sgn(i1, n1), sgn(i2, n2), sgn(i3, n3)};
+    const bool keep = m[0] > 0 || (m[0] == 0 && (m[1] > 0 || (m[1] == 0 && m[2] >= 0)));
+    if (!keep) {
+      minus[g] = -1;
+      continue;
+    }
+    if (m[0] == 0 && m[1] == 0 && m[2] == 0) {
+      minus[g] = -2;
+      continue;
+    }
+    const long long lin = ((long long)((n1 - m[0]) % n1) * n2 + (n2 - m[1]) % n2) * n3 + (n3 - m[2]) % n3;
+    auto it = std::lower_bound(idx.begin(), idx.end(), (int)lin);
+    if (it == idx.end() || *it != (int)lin) return cudaSuccess;  // sphere not closed under G -> -G: general path
+    minus[g] = (int)(it - idx.begin());
+  }
+  CR_TRY(upload(&h->sym_minus, minus, st));
+  CR_TRY(guarded_malloc(h, &h->sym_cls, (size_t)h->nproj));
+  sym::k_sym_classify<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, M, h->sym_minus, h->sym_cls);
+  std::vector<unsigned char> cls((size_t)h->nproj);
+  CR_TRY(cudaMemcpyAsync(cls.data(), h->sym_cls, (size_t)h->nproj, cudaMemcpyDeviceToHost, st));
+  CR_TRY(cudaStreamSynchronize(st));
+  for (unsigned char c : cls)
+    if (c > 1) return cudaSuccess;  // a projector without the symmetry: general path
+  long long off = 0;
+  for (int a = 0; a < nblocks; ++a) {
+    const int q0 = blk_off_host[a], nh = blk_off_host[a + 1] - q0;
+    for (int i = 0; i < nh; ++i)
+      for (int j = 0; j < nh; ++j)
+        if (d_host[off + (long long)i * nh + j] != 0.0 && cls[q0 + i] != cls[q0 + j]) return cudaSuccess;  // D mixes the classes
+    off += (long long)nh * nh;
+  }
+  {
+    std::vector<unsigned> cm((size_t)(h->nproj + 15) / 16, 0u);
+    for (int p_ = 0; p_ < h->nproj; ++p_)
+      if (cls[(size_t)p_]) cm[(size_t)p_ / 16] |= 1u << (p_ % 16);
+    CR_TRY(upload(&h->sym_cmask, cm, st));
+    CR_TRY(cudaStreamSynchronize(st));  // cm leaves scope
+  }
+  h->sym_wide = env_int("QE_HPSI_SYM_WIDE", 1);
+  h->sym_m = M;
+  h->sym_ldu = round_up(M, 8);
+  h->sym_ldc2 = 2 * h->ldc;
+  h->sym_nsplit = std::max(1, (M + h->kchunk - 1) / h->kchunk);
+  const size_t ub = sizeof(double2) * 2 * (size_t)h->max_batch * h->sym_ldu, eb = sizeof(double2) * 2 * (size_t)h->max_batch * h->ldp;
+  const size_t pb = sizeof(double2) * (size_t)h->sym_nsplit * h->nproj * h->sym_ldc2;
+  CR_TRY(guarded_malloc(h, &h->sym_u, ub));
+  CR_TRY(guarded_malloc(h, &h->sym_e, eb));
+  CR_TRY(guarded_malloc(h, &h->sym_partial, pb));
+  CR_TRY(cudaMemsetAsync(h->sym_u, 0, ub, st));
+  CR_TRY(cudaMemsetAsync(h->sym_e, 0, eb, st));
+  h->workspace_bytes += ub + eb + pb;
+  h->sym = true;
+#undef CR_TRY
+  return cudaSuccess;
+}
+
 // create flags: known bits only, one accuracy class, int8 sub-fields only with QE_HPSI_PROJ_INT8, 4..7 digits
 int validate_flags(unsigned flags, bool gamma) {
   const unsigned known = QE_HPSI_BORROW_BETA | QE_HPSI_GENERIC_FFT | QE_HPSI_FP64_DMMA | QE_HPSI_PROJ_INT8 | QE_HPSI_PROJ_CERTIFY |
-                         (15u << 8) | (3u << 12);
+                         QE_HPSI_NO_GAMMA_SYM | (15u << 8) | (3u << 12);
   if (flags & ~known) return QE_HPSI_EINVAL;
   if ((flags & QE_HPSI_FP64_DMMA) && (flags & QE_HPSI_PROJ_INT8)) return QE_HPSI_EINVAL;
   if (!(flags & QE_HPSI_PROJ_INT8) && (flags & (QE_HPSI_PROJ_CERTIFY | (15u << 8) | (3u << 12)))) return QE_HPSI_EINVAL;
@@ -1463,6 +1560,9 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
   // ---- nonlocal ---------------------------------------------------------------------------------------
   if (nproj > 0)
     CR_TRY(setup_nonlocal(h, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
+  if (nproj > 0 && h->npw > 0 && !h->oz_s && !(flags & QE_HPSI_NO_GAMMA_SYM) && sg.kap[0] == 0.0 && sg.kap[1] == 0.0 &&
+      sg.kap[2] == 0.0)
+    CR_TRY(setup_symmetric(h, idx, nr, nblocks, blk_off_host, d_host, st));
   if ((flags & QE_HPSI_PROJ_CERTIFY) && h->oz_s) CR_TRY(setup_certify(h, st));
   // NEXT-3: split-K workspace of qe_hpsi_overlap; K slices depend on npw only, so an element's bits do not depend on how many
   // rows / columns a call has (chunks of 512 x 128)
@@ -1579,12 +1679,25 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
     k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
                                                                                  h->npw, h->kchunk, h->partial, h->ldc);
+  } else if (h->sym) {
+    // Gamma-symmetric projector mode: psi = u + i v as 2 nb real-wavefunction columns over the leading sym_m sphere entries
+    sym::k_sym_merge<<<dim3((h->sym_m + 255) / 256, nb), 256, 0, st>>>(psi, ldpsi, h->sym_m, h->sym_minus, h->sym_u, h->sym_ldu);
+    auto go = [&](auto cfg) {
+      using Cfg = decltype(cfg);
+      const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (2 * nb + Cfg::BN - 1) / Cfg::BN;
+      k_becp<Cfg, true><<<dim3(mt * nt, h->sym_nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, h->sym_u,
+                                                                                       h->sym_ldu, 2 * nb, h->sym_m, h->kchunk,
+                                                                                       h->sym_partial, h->sym_ldc2, nullptr, h->sym_cls);
+    };
+    if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);
   const size_t t1 = prof_mark(h, st);
   prof_span(h, ts, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
-  if (h->gamma)
+  if (h->sym && !h->oz_s)
+    sym::k_sym_reduce<<<rg, 128, 0, st>>>(h->sym_partial, h->sym_nsplit, h->nproj, h->sym_ldc2, nb, h->sym_cls, h->becp, h->ldc);
+  else if (h->gamma)
     k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
                                             h->beta, h->ldbeta, psi, ldpsi,
                                             h->becp);
@@ -1595,6 +1708,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
                                       h->becp);
   k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
                             h->dbT, h->ldp);
+  if (h->sym && !h->oz_s)  // real coefficient rows (Re e, Im e) of the symmetric a8
+    sym::k_sym_coef<<<rg, 128, 0, st>>>(h->dbecp, h->nproj, h->ldc, nb, h->sym_cls, h->sym_e, h->ldp);
   prof_span(h, t1, prof_mark(h, st), SLOT_DMUL);
   h->nb_last = nb;
   CU_TRY(h, cudaGetLastError());
@@ -1620,6 +1735,17 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
     if (mt > 0)
       k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
                                                                                 h->ldp, nb, hpsi, ldh);
+  } else if (h->sym && bT == h->dbT) {
+    // symmetric a8: X = sum_p b_p Re e_p, Y = sum_p b_p Im e_p over the half sphere; hpsi(G) += X + iY, hpsi(-G) += conj X + i conj Y
+    auto go = [&](auto cfg) {
+      using Cfg = decltype(cfg);
+      const int mt = (h->sym_m + Cfg::BM - 1) / Cfg::BM, nt = (2 * nb + Cfg::BN - 1) / Cfg::BN;
+      if (mt > 0)
+        k_vnl_add<Cfg, true, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->sym_m,
+                                                                                        h->sym_e, h->ldp, 2 * nb, hpsi, ldh, nullptr,
+                                                                                        h->sym_cmask, h->sym_minus);
+    };
+    if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     vnl_fp64(h, bT, hpsi, ldh, nb, st, nullptr);
   CU_TRY(h, cudaGetLastError());
@@ -2296,7 +2422,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : 4;
+    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 : 4);
     if (h->certify) total += 8;  // probe, decide, gather, the four FP64 kernels (empty grids when nothing failed), commit
   }
   return total;
@@ -2318,7 +2444,7 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[9] = h->kchunk;
   info[10] = h->x_split;
   info[11] = h->num_sms;
-  info[12] = h->f2p[0] ? 1 : 0;
+  info[12] = (h->f2p[0] ? 1 : 0) | (h->sym ? 2 : 0);
   info[13] = h->oz_s;
   info[14] = h->oz_nsplit;
   info[15] = (h->oz_3m ? (h->oz_3m8 ? 2 : 1) : 0) + (h->certify ? 4 : 0);

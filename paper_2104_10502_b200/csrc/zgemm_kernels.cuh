@@ -99,7 +99,8 @@ __device__ __forceinline__ void mma2r(double (&P)[TM][TN][2], double (&Q)[TM][TN
 template <class Cfg, bool GAMMA = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_becp(const double2* __restrict__ beta, long long ldb, int nproj, const double2* __restrict__ psi, long long ldpsi,
-           int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc, const int* __restrict__ nb_dev = nullptr) {
+           int nb, int npw, int kchunk, double2* __restrict__ partial, int ldc, const int* __restrict__ nb_dev = nullptr,
+           const unsigned char* __restrict__ cls = nullptr) {
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS;
   constexpr int STAGE = (BM + BN) * BK;  // complex elements per stage
@@ -174,6 +175,15 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     cp_async_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
+  // Gamma-symmetric projector mode (cls != nullptr, GAMMA form): rows of class 1 (beta(-G) = -conj beta(G)) enter as i*beta =
+  // (-a_i, a_r), so that every row is Hermitian and the real form applies; the fragment is only swapped to (a_i, a_r) and the
+  // sign goes into the epilogue (Q - P instead of P + Q): no FP64 instruction is spent on it
+  bool swp[TM];
+#pragma unroll
+  for (int i = 0; i < TM; ++i) {
+    const int p = m0 + wm0 + i * 8 + fr;
+    swp[i] = GAMMA && cls != nullptr && p < nproj && cls[p] != 0;
+  }
   int st_c = 0, st_l = NSTAGE - 1;  // stage being consumed / stage being refilled
   for (int kt = 0; kt < nkt; ++kt) {
     cp_async_wait<NSTAGE - 2>();
@@ -193,9 +203,12 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
-      if constexpr (GAMMA)
+      if constexpr (GAMMA) {
+#pragma unroll
+        for (int i = 0; i < TM; ++i)
+          if (swp[i]) af[kk & 1][i] = make_double2(af[kk & 1][i].y, af[kk & 1][i].x);  // (a_i, a_r): P = sum a_i b_r, Q = sum a_r b_i
         mma2r<TM, TN, true>(P, Q, af[kk & 1], bf[kk & 1]);
-      else
+      } else
         mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
       if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
         if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
@@ -218,7 +231,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
       for (int e = 0; e < 2; ++e) {
         const int b = n0 + wn0 + j * 8 + 2 * fk + e;
         if (b < nb)
-          out[(size_t)p * ldc + b] = GAMMA ? make_double2(P[i][j][e] + Q[i][j][e], 0.0)
+          out[(size_t)p * ldc + b] = GAMMA ? make_double2(swp[i] ? Q[i][j][e] - P[i][j][e] : P[i][j][e] + Q[i][j][e], 0.0)
                                            : make_double2(P[i][j][e] + Q[i][j][e], (R[i][j][e] - P[i][j][e]) + Q[i][j][e]);
       }
     }
@@ -319,10 +332,17 @@ __global__ void k_dmul(const double2* __restrict__ becp, int nproj, int ldc, int
 
 // a8 ------------------------------------------------------------------------------------------------------
 // hpsi[b][g] += sum_p A[p][g] B[b][p];  A = beta ([p][g], g contiguous: "M-major"), B = dbT ([b][p], p contiguous)
-template <class Cfg, bool GAMMA = false>
+// SYM (Gamma-symmetric projector mode of a complex handle; needs GAMMA): rows g run over the leading
+// `npw` = M sphere entries (n1 >= 0), columns come in pairs (2b, 2b+1) = real coefficient vectors (Re e, Im e) of band b, rows p of
+// class 1 enter as i*beta; with X, Y the two complex sums of a pair the epilogue adds X + iY to hpsi[b][g] and conj(X) + i conj(Y)
+// to hpsi[b][minus[g]] (minus[g] = position of -G; -1: g is not in the half sphere, skip; -2: G = 0, no partner).
+template <class Cfg, bool GAMMA = false, bool SYM = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_add(const double2* __restrict__ beta, long long ldb, int nproj, int npw, const double2* __restrict__ dbT,
-              int ldp, int nb, double2* __restrict__ hpsi, long long ldh, const int* __restrict__ nb_dev = nullptr) {
+              int ldp, int nb, double2* __restrict__ hpsi, long long ldh, const int* __restrict__ nb_dev = nullptr,
+              const unsigned* __restrict__ cmask = nullptr, const int* __restrict__ minus = nullptr) {
+  static_assert(!SYM || GAMMA, "the symmetric mode is a real form");
+  static_assert(!SYM || Cfg::BK == 16, "cmask holds one 16-bit class mask per K tile of 16 projectors");
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS, LDA = Cfg::LDA_M;
   constexpr int STAGE = BK * LDA + BN * BK;
@@ -400,6 +420,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     const double2* As = sm + st_c * STAGE;
     const double2* Bs = As + BK * LDA;
     double2 af[2][TM], bf[2][TN];
+    unsigned cm = 0;
+    if constexpr (SYM) cm = __ldg(&cmask[kt]);
 #pragma unroll
     for (int i = 0; i < TM; ++i) af[0][i] = As[fk * LDA + wm0 + i * 8 + fr];
 #pragma unroll
@@ -412,9 +434,25 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
         for (int j = 0; j < TN; ++j) bf[(kk + 1) & 1][j] = Bs[swz_k<BK>(wn0 + j * 8 + fr, (kk + 1) * 4 + fk)];
       }
-      if constexpr (GAMMA)
-        mma2r<TM, TN, false>(P, Q, af[kk & 1], bf[kk & 1]);
-      else
+      if constexpr (GAMMA) {
+        if constexpr (SYM) {  // the k row of this fragment is projector kt*BK + kk*4 + fk: bit kk*4 + fk of the tile's class mask
+          // class 1: i*beta = (-a_i, a_r); the fragment is swapped to (a_i, a_r) and the sign sits in the B operand, whose rows
+          // hold (e, e) for class 0 and (e, -e) for class 1 projectors (k_sym_coef): P += a'.x * b.y, Q += a'.y * b.x
+          if ((cm >> (kk * 4 + fk)) & 1u) {
+#pragma unroll
+            for (int i = 0; i < TM; ++i) af[kk & 1][i] = make_double2(af[kk & 1][i].y, af[kk & 1][i].x);
+          }
+#pragma unroll
+          for (int i = 0; i < TM; ++i)
+#pragma unroll
+            for (int j = 0; j < TN; ++j) dmma884(P[i][j][0], P[i][j][1], af[kk & 1][i].x, bf[kk & 1][j].y);
+#pragma unroll
+          for (int i = 0; i < TM; ++i)
+#pragma unroll
+            for (int j = 0; j < TN; ++j) dmma884(Q[i][j][0], Q[i][j][1], af[kk & 1][i].y, bf[kk & 1][j].x);
+        } else
+          mma2r<TM, TN, false>(P, Q, af[kk & 1], bf[kk & 1]);
+      } else
         mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
       if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
         if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
@@ -425,6 +463,36 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     st_l = (st_l + 1 == NSTAGE) ? 0 : st_l + 1;
   }
   cp_async_wait<0>();
+  if constexpr (SYM) {
+    // columns 2 fk, 2 fk + 1 of an 8-column block are (X, Y) of one band: X = (P, Q)[0], Y = (P, Q)[1]
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+      const int gg = m0 + wm0 + i * 8 + fr;
+      if (gg >= npw) continue;
+      const int mg = minus[gg];
+      if (mg == -1) continue;
+#pragma unroll
+      for (int j = 0; j < TN; ++j) {
+        const int col = n0 + wn0 + j * 8 + 2 * fk;
+        if (col >= nb) continue;  // nb = number of columns = 2 x bands
+        const int b = col >> 1;
+        const double xr = P[i][j][0], xi = Q[i][j][0], yr = P[i][j][1], yi = Q[i][j][1];
+        double2* h = &hpsi[(size_t)b * ldh + gg];
+        double2 v = *h;
+        v.x += xr - yi;
+        v.y += xi + yr;
+        *h = v;
+        if (mg >= 0) {
+          double2* h2 = &hpsi[(size_t)b * ldh + mg];
+          double2 w = *h2;
+          w.x += xr + yi;
+          w.y += yr - xi;
+          *h2 = w;
+        }
+      }
+    }
+    return;
+  }
   // a b = (P - Q) + i (R - P - Q)
 #pragma unroll
   for (int i = 0; i < TM; ++i) {

@@ -24,6 +24,7 @@ QE_HPSI_FP64_DMMA = 4      # the default accuracy class (FP64 tensor pipe); the 
 QE_HPSI_PROJ_INT8 = 8      # opt-in: a6 / a8 as exact int8 digit products (block fixed point, 8S-1 bits under a row exponent)
 QE_HPSI_PROJ_CERTIFY = 16  # with PROJ_INT8: a-posteriori check of every chunk + FP64 re-computation of failing bands
 QE_HPSI_PROJ_3M_OFF, QE_HPSI_PROJ_3M_A6, QE_HPSI_PROJ_3M_ALL = 1 << 12, 2 << 12, 3 << 12
+QE_HPSI_NO_GAMMA_SYM = 32   # keep the general complex contraction at k = 0 (see include/qe_hpsi.h)
 QE_HPSI_NPROBE = 8
 QE_HPSI_MAX_N = 720
 
@@ -366,6 +367,8 @@ class Hpsi:
         keys = ["npw", "S", "P", "fft_nb", "nsplit", "workspace_bytes", "npass1", "npass2", "npass3", "kchunk",
                 "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit", "ozaki_3m"]
         d = {k: int(buf[i]) for i, k in enumerate(keys)}
+        d["gamma_sym"] = (d["fft2p"] >> 1) & 1
+        d["fft2p"] &= 1
         d["certify"] = d["ozaki_3m"] >> 2
         d["ozaki_3m"] &= 3
         return d

@@ -249,6 +249,58 @@ def test_apply_writes_nothing_outside_its_output_rows(cfg, flags):
     h.destroy()
 
 
+def test_gamma_symmetric_projector_mode_is_detected_and_matches_the_general_contraction():
+    """At k = 0 the FP64 path contracts psi = u + i v over the half sphere when EVERY projector passes the bit-exact check
+    beta(-G) = +-conj beta(G) and D couples equal signs only; otherwise it must fall back. Both against the oracle
+    (the other tests) and against the general complex contraction (here, nonlocal part alone)."""
+    for cfg, want in (("T1_general_k", 0), ("T5_odd_bands", 0), ("T2_radix5", 1), ("T2b_radix5_20", 1), ("T3_aliased", 1), (0, 1), (1, 1)):
+        h, inp = _gpu.make(cfg)
+        assert h.info()["gamma_sym"] == want, cfg
+        wl = inp["wl"]
+        if not want:
+            h.destroy()
+            continue
+        hg, _ = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_NO_GAMMA_SYM, beta=inp["beta"])
+        assert hg.info()["gamma_sym"] == 0
+        npw = h.npw
+        psi = _gpu.gen_psi_dev(inp, 0, min(wl.nbands, 37))
+        a = h.nonlocal_add(psi, torch.zeros_like(psi))
+        b = hg.nonlocal_add(psi, torch.zeros_like(psi))
+        ba, _ = h.becp(psi.shape[0]) if psi.shape[0] <= h.max_batch else (None, None)
+        torch.cuda.synchronize()
+        d = torch.linalg.vector_norm(a[:, :npw] - b[:, :npw], dim=1) / torch.linalg.vector_norm(b[:, :npw], dim=1)
+        assert float(d.max()) <= 1e-13, (cfg, float(d.max()))
+        assert torch.equal(a[:, npw:], torch.zeros_like(a[:, npw:]))
+        assert h.launch_count(1) == 5 + 6 and hg.launch_count(1) == 5 + 4
+        h.destroy()
+        hg.destroy()
+    # a projector set WITHOUT the symmetry (one entry nudged by one ulp) and a D that couples s with p: the general path, still right
+    h0, inp = _gpu.make(0)
+    wl = inp["wl"]
+    sp = _gpu.oracle_sphere(wl)
+    npw = h0.npw
+    h0.destroy()
+    beta = inp["beta"].clone()
+    beta[3, 11] = torch.nextafter(beta[3, 11].real, torch.tensor(2.0, dtype=torch.float64, device="cuda")) + 1j * beta[3, 11].imag
+    psi = _gpu.gen_psi_dev(inp, 0, wl.nbands)
+    h1 = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, inp["vr"], beta, inp["blk"], inp["dblocks"], max_batch=wl.batch)
+    assert h1.info()["gamma_sym"] == 0
+    ref = orc.vnl_psi(beta[:, :npw].cpu().numpy(), inp["dblocks"], psi[:, :npw].cpu().numpy())
+    assert _gpu.rel_l2(h1.nonlocal_add(psi, torch.zeros_like(psi)).cpu().numpy()[:, :npw], ref).max() <= 1e-12
+    h1.destroy()
+    dmix = np.array(inp["dblocks"], dtype=np.float64).copy()
+    dmix[:, 0, 1] = dmix[:, 1, 0] = 0.37  # config 0 orders [s; px, py, pz]: couples l = 0 with l = 1 (classes 0 and 1)
+    h2 = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, inp["vr"], inp["beta"], inp["blk"], dmix, max_batch=wl.batch)
+    assert h2.info()["gamma_sym"] == 0
+    ref = orc.vnl_psi(inp["beta"][:, :npw].cpu().numpy(), dmix, psi[:, :npw].cpu().numpy())
+    assert _gpu.rel_l2(h2.nonlocal_add(psi, torch.zeros_like(psi)).cpu().numpy()[:, :npw], ref).max() <= 1e-12
+    h2.destroy()
+    # both classes really occur in the generator's projectors (s: +, p: -), so the i*beta rows are exercised
+    h3, _ = _gpu.make(0)
+    assert h3.info()["gamma_sym"] == 1
+    h3.destroy()
+
+
 def test_apply_host_matches_device_path():
     h, inp = _gpu.make(0, max_batch=6)
     psi = _gpu.gen_psi_dev(inp, 0, 16)
