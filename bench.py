@@ -558,14 +558,21 @@ def main():
         roofline, combined8 = int8_roofline(leg, stage, m, mp, hbm_peak, dmma, args, value, world)
     elif wl.nproj and t_vnl + t_becp > t_fft:
         kname, t_k = ("k_vnl_add", t_vnl) if t_vnl >= t_becp else ("k_becp", t_becp)
+        gsym = bool(info.get("gamma_sym"))
+        ex = 0.5 if gsym else 0.75  # executed / algorithmic flops
         ach = flops_launch / (t_k * 1e-3) * 1e-12
-        roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
-                    "traffic": committed_traffic(args.config, kname), "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-resident "
+        roofline = {"bound": "tensor", "kernel": kname + ("<ZgS, GAMMA, SYM> (Gamma-symmetric real form)" if gsym else " (3M complex form)"),
+                    "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
+                    "traffic": committed_traffic(args.config, kname + ("_sym" if gsym else "")),
+                    "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-resident "
                     "loop measured live by qe_hpsi_probe_fp64; MEASURED_PEAKS.json has no FP64 entry",
-                    "ms_per_launch": t_k, "flops_per_launch": flops_launch,
-                    "executed_dmma_frac": ach / dmma * 0.75,
-                    "note": "achieved counts the algorithmic 8 flops per complex MAC; the 3M product executes 6, so frac can "
-                            "exceed 1 (DESIGN.md section 6); executed_dmma_frac = frac x 0.75 is the pipe utilisation"}
+                    "ms_per_launch": t_k, "flops_per_launch": flops_launch, "executed_flops_per_launch": flops_launch * ex,
+                    "executed_dmma_frac": ach / dmma * ex,
+                    "note": "achieved counts the ALGORITHMIC 8 flops per complex MAC of north_star's F_proj; the kernel executes fewer in "
+                            "the same FP64 arithmetic, so frac can exceed 1: " + ("at k = 0 with projectors that pass the bit-exact "
+                            "beta(-G) = +-conj beta(G) check psi = u + i v is contracted as two real problems over the half sphere, 4 "
+                            "executed flops per complex MAC (DESIGN.md section 5.8)" if gsym else "the 3M complex product executes 6 "
+                            "(DESIGN.md section 6)") + "; executed_dmma_frac is the DMMA pipe utilisation"}
     else:
         bytes_launch = m["b_fft"] * min(batch, nb)
         ach = bytes_launch / (t_fft * 1e-3) * 1e-9
@@ -583,7 +590,7 @@ def main():
               "measured_in": "a separate eager pass right after the timed steps (stage timers are off inside them)",
               "stage_pass_ms_per_step": stage_pass_ms}
 
-    proj_path = "fp64 dmma (3M)" if not oz_s else (f"int8 digits x{oz_s} (tcgen05)" + {0: "", 1: ", a6 in the integer 3M form",
+    proj_path = ("fp64 dmma (Gamma-symmetric real form over the half sphere)" if info.get("gamma_sym") else "fp64 dmma (3M)") if not oz_s else (f"int8 digits x{oz_s} (tcgen05)" + {0: "", 1: ", a6 in the integer 3M form",
                 2: ", a6 and a8 in the integer 3M form"}[info.get("ozaki_3m", 0)] + (", certified" if info.get("certify") else ""))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": PATH_DTYPE[args.path],
