@@ -80,10 +80,11 @@ typedef enum {
 #define QE_HPSI_PROJ_3M_A6  (2u << 12)
 #define QE_HPSI_PROJ_3M_ALL (3u << 12)
 
-/* At k = 0 the FP64 path checks at create, bit for bit, whether every projector obeys beta_p(-G) = +-conj(beta_p(G)) (projector
+/* At k = 0 the library checks at create, bit for bit, whether every projector obeys beta_p(-G) = +-conj(beta_p(G)) (projector
  * functions real in real space) and D couples equal signs only; if so a6 / a8 contract psi = u + i v as two real-wavefunction
  * problems over the half sphere: 2/3 of the FP64 tensor work and half of the beta traffic, same FP64 arithmetic, results equal
- * to the general path up to rounding order.  This flag keeps the general complex contraction. */
+ * to the general path up to rounding order.  The int8 digit path does the same with real-form digit
+ * planes over the half sphere (a third of the plane memory).  This flag keeps the general complex contraction. */
 #define QE_HPSI_NO_GAMMA_SYM 32u
 
 #define QE_HPSI_MAX_N 720        /* largest supported FFT dimension (shared-memory pencil tile)                     */
@@ -180,7 +181,9 @@ int qe_hpsi_get_proj_check(qe_hpsi_t h, double* rel_dev, int32_t* redo_dev, void
  * computed once and shared; spsi[b][0..npw) is overwritten, entries >= npw untouched; spsi must not overlap psi or
  * hpsi.  hpsi_dev may be NULL (S psi only).  Without projectors S = 1.  QE_HPSI_ESTATE if set_s was never called
  * on a handle that has projectors.  Asynchronous on cuda_stream like qe_hpsi_apply.  (Not certified: with
- * QE_HPSI_PROJ_CERTIFY this call returns QE_HPSI_ESTATE.) */
+ * QE_HPSI_PROJ_CERTIFY this call returns QE_HPSI_ESTATE.)  On a QE_HPSI_PROJ_INT8 handle in the Gamma-symmetric mode (k = 0,
+ * see QE_HPSI_NO_GAMMA_SYM) the digit planes hold the real forms only, so q must couple projectors of equal parity only
+ * (as D does); otherwise qe_hpsi_set_s returns QE_HPSI_EINVAL and the handle should be created with QE_HPSI_NO_GAMMA_SYM. */
 int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host);
 int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi_dev, int64_t ldhpsi, void* spsi_dev,
                      int64_t ldspsi, int nbands, void* cuda_stream);

@@ -78,11 +78,14 @@ constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >
 // MODE 0 (a6): out = partial[split][m][ldo] complex, written; MODE 1 (a8): out = hpsi[b][ldo] complex at column m, accumulated.
 // Gamma-only (real) forms, one column per band: MODE 2 (a6): partial[split][m][b] = (value, 0); MODE 3 (a8): row m = 2g + c
 // of the transposed planar digits of beta, component c of hpsi[b][g] accumulated.
+// MODE 4 (a8 of the Gamma-symmetric mode of a complex handle, sym_kernels.cuh): rows m = 2g + c over the leading sphere entries,
+// columns 2b = X, 2b+1 = Y (real coefficient vectors Re e, Im e of band b); hpsi[b][g] += X + iY and hpsi[b][minus[g]] +=
+// conj(X) + i conj(Y): lane pairs (c = 0, 1) exchange their components by shuffle, each lane updates component c of both entries.
 template <int S, int MODE>
 __global__ void __launch_bounds__(NT, 1)
 k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nstages, int nkb, int kchunk,
           const int* __restrict__ ea, const int* __restrict__ eb, long long mvalid, int nb, double2* __restrict__ out,
-          long long ldo, long long split_stride, int ks_base) {
+          long long ldo, long long split_stride, int ks_base, const int* __restrict__ minus = nullptr) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint64_t full[MAX_STAGES], empty[MAX_STAGES], done;
   __shared__ uint32_t tmem_base;
@@ -166,7 +169,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     }
     mbar_wait(&done, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const int em = (m < mvalid) ? ea[MODE == 3 ? (m >> 1) : m] : 0;  // MODE 3: rows 2g, 2g+1 share the exponent of plane wave g
+    const int em = (m < mvalid) ? ea[MODE >= 3 ? (m >> 1) : m] : 0;  // MODE 3, 4: rows 2g, 2g+1 share the exponent of plane wave g
 #pragma unroll 1
     for (int n0 = 0; n0 < BN; n0 += 8) {
       double d[8];
@@ -190,7 +193,25 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           for (int j = 0; j < 8; ++j) d[j] = fma((double)(int)v[L][j], w, d[j]);
         }
       }
-      if (MODE >= 2) {  // real forms of the Gamma-only handle: one column per band
+      if (MODE == 4) {
+        const bool ok = m < mvalid;
+        const long long g = m >> 1;
+        const int c = (int)(m & 1);
+        const int mg = ok ? minus[g] : -1;
+#pragma unroll
+        for (int j = 0; j < 8; j += 2) {
+          const int col = q * BN + n0 + j;  // X column of band col / 2; nb = number of columns (even)
+          const bool cok = col < nb;
+          const double x = oz_scale(d[j], em, cok ? eb[col] : 0), y = oz_scale(d[j + 1], em, cok ? eb[col + 1] : 0);
+          const double yo = __shfl_xor_sync(0xffffffffu, y, 1);  // the other component of Y (lanes 2k, 2k+1 hold rows 2g, 2g+1)
+          if (ok && cok && mg != -1) {
+            double* row = reinterpret_cast<double*>(out + (size_t)(col >> 1) * ldo);
+            // c = 0: Re(G) += X_r - Y_i, Re(-G) += X_r + Y_i;   c = 1: Im(G) += X_i + Y_r, Im(-G) += Y_r - X_i
+            row[2 * g + c] += c == 0 ? x - yo : x + yo;
+            if (mg >= 0) row[2 * (long long)mg + c] += c == 0 ? x + yo : yo - x;
+          }
+        }
+      } else if (MODE >= 2) {  // real forms of the Gamma-only handle: one column per band
         if (m < mvalid) {
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
@@ -307,16 +328,18 @@ __device__ __forceinline__ void slice16(double (&r)[16], uint4 (&o)[S]) {
 template <int S>
 __global__ void __launch_bounds__(128)
 k_oz_slice(const double2* __restrict__ X, long long ldx, long long n, const int* __restrict__ e, int8_t* __restrict__ out,
-           long long kpad, long long slice_stride, int mode) {
+           long long kpad, long long slice_stride, int mode, const unsigned char* __restrict__ cls = nullptr) {
   const long long g0 = ((long long)blockIdx.x * 128 + threadIdx.x) * 8;
   if (g0 * 2 >= kpad) return;
   const int r = blockIdx.y;
   const int ex = -e[r];
+  const bool rot = cls != nullptr && cls[r] != 0;  // Gamma-symmetric mode: a class-1 row is sliced as i * x = (-im, re)
   double a[16], b2[16];
 #pragma unroll
   for (int t = 0; t < 8; ++t) {
     double2 v = make_double2(0.0, 0.0);
     if (g0 + t < n) v = X[(size_t)r * ldx + g0 + t];
+    if (rot) v = make_double2(-v.y, v.x);
     const double re = scalbn(v.x, ex), im = scalbn(v.y, ex);
     if (mode == 2) {
       a[2 * t] = re, a[2 * t + 1] = -im;
@@ -383,7 +406,7 @@ k_oz_slice_re(const double2* __restrict__ X, long long ldx, long long n, const i
 template <int S>
 __global__ void __launch_bounds__(128)
 k_oz_slice_tp(const double2* __restrict__ X, long long ldx, int rows, long long n, const int* __restrict__ e,
-              int8_t* __restrict__ out, long long kpad, long long slice_stride) {
+              int8_t* __restrict__ out, long long kpad, long long slice_stride, const unsigned char* __restrict__ cls = nullptr) {
   const long long g = (long long)blockIdx.x * 128 + threadIdx.x;
   if (g >= n) return;
   const int p0 = blockIdx.y * 16;
@@ -392,7 +415,10 @@ k_oz_slice_tp(const double2* __restrict__ X, long long ldx, int rows, long long 
 #pragma unroll
   for (int t = 0; t < 16; ++t) {
     double2 v = make_double2(0.0, 0.0);
-    if (p0 + t < rows) v = X[(size_t)(p0 + t) * ldx + g];
+    if (p0 + t < rows) {
+      v = X[(size_t)(p0 + t) * ldx + g];
+      if (cls != nullptr && cls[p0 + t] != 0) v = make_double2(-v.y, v.x);  // Gamma-symmetric mode: class-1 projector enters as i * beta
+    }
     re[t] = scalbn(v.x, ex);
     im[t] = scalbn(v.y, ex);
   }

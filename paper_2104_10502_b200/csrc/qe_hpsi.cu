@@ -130,6 +130,9 @@ struct qe_hpsi_handle {
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
   int sym_nsplit = 1, sym_ldc2 = 0;
+  std::vector<unsigned char> sym_cls_host;  // copy of sym_cls for qe_hpsi_set_s
+  bool sym_q_ok = false;                    // the q blocks of qe_hpsi_set_s couple equal classes only
+  std::vector<int> blk_off;                 // atom block table (for the same check)
   // QE_HPSI_PROJ_CERTIFY: a-posteriori check of the int8 nonlocal part + FP64 re-computation
   bool certify = false;
   double cert_tol = 1e-11;
@@ -859,27 +862,30 @@ bool oz_make_map(CUtensorMap* tm, void* base, long long kpad, long long rows, in
 template <int S>
 cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
   cudaError_t e = cudaSuccess;
-  const void* kern[4] = {(const void*)oz::k_oz_gemm<S, 0>, (const void*)oz::k_oz_gemm<S, 1>, (const void*)oz::k_oz_gemm<S, 2>,
-                         (const void*)oz::k_oz_gemm<S, 3>};
+  const void* kern[5] = {(const void*)oz::k_oz_gemm<S, 0>, (const void*)oz::k_oz_gemm<S, 1>, (const void*)oz::k_oz_gemm<S, 2>,
+                         (const void*)oz::k_oz_gemm<S, 3>, (const void*)oz::k_oz_gemm<S, 4>};
   for (const void* k : kern)
     if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem)) != cudaSuccess) return e;
   const long long k1 = h->oz_k1, k2 = h->oz_k2;
+  // Gamma-symmetric mode: the planes cover the leading sym_m sphere entries only, and rows of class 1 are sliced as i*beta
+  const long long ksph = h->sym ? h->sym_m : h->npw;
+  const unsigned char* cls = h->sym ? h->sym_cls : nullptr;
   // a6 operand: rows p scaled by 2^-ep[p]; a8 operand: rows g scaled by 2^-eg[g] (transposed beta)
-  oz::k_oz_rowexp<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep);
+  oz::k_oz_rowexp<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, ksph, h->oz_ep);
   if (h->oz_3m)
     oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k1c / 16 + 127) / 128), h->nproj), 128, 0, st>>>(
         h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1, h->oz_k1c, (long long)h->nproj * h->oz_k1c, 3LL * h->nproj * h->oz_k1c, -1.0);
   else
-    oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, h->npw, h->oz_ep, h->oz_a1,
-                                                                                      k1, (long long)h->nproj * k1, 0);
-  oz::k_oz_colexp<<<(unsigned)((h->npw + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg);
+    oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), h->nproj), 128, 0, st>>>(h->beta, h->ldbeta, ksph, h->oz_ep, h->oz_a1,
+                                                                                      k1, (long long)h->nproj * k1, 0, cls);
+  oz::k_oz_colexp<<<(unsigned)((ksph + 127) / 128), 128, 0, st>>>(h->beta, h->ldbeta, h->nproj, ksph, h->oz_eg);
   if (h->oz_3m8) {
     if ((e = cudaFuncSetAttribute(oz::k_oz_vnl3<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->oz_smem)) != cudaSuccess) return e;
     oz::k_oz_slice_t3<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(h->oz_k2c / 16)), 128, 0, st>>>(
         h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, h->oz_k2c, (long long)h->npw * h->oz_k2c, 3LL * h->npw * h->oz_k2c);
-  } else if (h->gamma)  // real form: rows 2g + c, K = p
-    oz::k_oz_slice_tp<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
-        h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, 2LL * h->npw * k2);
+  } else if (h->gamma || h->sym)  // real form: rows 2g + c, K = p
+    oz::k_oz_slice_tp<S><<<dim3((unsigned)((ksph + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
+        h->beta, h->ldbeta, h->nproj, ksph, h->oz_eg, h->oz_a2, k2, 2LL * ksph * k2, cls);
   else
     oz::k_oz_slice_t<S><<<dim3((unsigned)((h->npw + 127) / 128), (unsigned)(k2 / 16)), 128, 0, st>>>(
         h->beta, h->ldbeta, h->nproj, h->npw, h->oz_eg, h->oz_a2, k2, (long long)h->npw * k2);
@@ -890,6 +896,13 @@ cudaError_t oz_prepare_t(qe_hpsi_handle* h, cudaStream_t st) {
 template <int S>
 void oz_becp_slice_t(qe_hpsi_handle* h, const double2* psi, long long ldpsi, int nb, cudaStream_t st) {
   const long long k1 = h->oz_k1;
+  if (h->sym) {  // psi = u + i v: 2 nb real-wavefunction rows over the leading sym_m entries (sym_kernels.cuh), one B row each
+    sym::k_sym_merge<<<dim3((h->sym_m + 255) / 256, nb), 256, 0, st>>>(psi, ldpsi, h->sym_m, h->sym_minus, h->sym_u, h->sym_ldu);
+    oz::k_oz_rowexp<<<2 * nb, 256, 0, st>>>(h->sym_u, h->sym_ldu, h->sym_m, h->oz_eb);
+    oz::k_oz_slice<S><<<dim3((unsigned)((k1 / 16 + 127) / 128), 2 * nb), 128, 0, st>>>(h->sym_u, h->sym_ldu, h->sym_m, h->oz_eb, h->oz_b, k1,
+                                                                                     2LL * h->max_batch * k1, 0);
+    return;
+  }
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(psi, ldpsi, h->npw, h->oz_eb);
   if (h->oz_3m) {  // planes Re, Im, (Re + Im) / 2 of every band
     oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k1c / 16 + 127) / 128), nb), 128, 0, st>>>(
@@ -911,15 +924,28 @@ void oz_becp_gemm_t(qe_hpsi_handle* h, int nb, cudaStream_t st) {
                                                          h->oz_partial + (size_t)pl * h->oz_nsplit * slab, h->ldc, (long long)slab, 0);
     return;
   }
+  if (h->sym) {  // real form, 2 nb columns (u_b, v_b)
+    const dim3 gs((2 * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit);
+    oz::k_oz_gemm<S, 2><<<gs, oz::NT, h->oz_smem, st>>>(h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk,
+                                                       h->oz_ep, h->oz_eb, h->nproj, 2 * nb, h->oz_partial, h->sym_ldc2,
+                                                       (long long)h->nproj * h->sym_ldc2, 0);
+    return;
+  }
   const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (h->nproj + oz::BM - 1) / oz::BM, h->oz_nsplit);
   auto kern = h->gamma ? oz::k_oz_gemm<S, 2> : oz::k_oz_gemm<S, 0>;
   kern<<<grid, oz::NT, h->oz_smem, st>>>(h->oz_tm_a1, h->oz_tm_b1, h->oz_stages, (int)(h->oz_k1 / oz::KB), h->oz_kchunk, h->oz_ep,
-                                        h->oz_eb, h->nproj, nb, h->oz_partial, h->ldc, (long long)h->nproj * h->ldc, 0);
+                                        h->oz_eb, h->nproj, nb, h->oz_partial, h->ldc, (long long)h->nproj * h->ldc, 0, nullptr);
 }
 // a8 on int8 slices: hpsi[b][g] += sum_p beta[p][g] bT[b][p]
 template <int S>
 void oz_vnl_slice_t(qe_hpsi_handle* h, const double2* bT, int nb, cudaStream_t st) {
   const long long k2 = h->oz_k2;
+  if (h->sym) {  // rows (Re e, Im e) of every band from k_sym_coef (bT is ignored: the coefficients are in sym_e)
+    oz::k_oz_rowexp<<<2 * nb, 256, 0, st>>>(h->sym_e, h->ldp, h->nproj, h->oz_eb);
+    oz::k_oz_slice_re<S><<<dim3((unsigned)((k2 / 16 + 127) / 128), 2 * nb), 128, 0, st>>>(h->sym_e, h->ldp, h->nproj, h->oz_eb, h->oz_b, k2,
+                                                                                        2LL * h->max_batch * k2);
+    return;
+  }
   oz::k_oz_rowexp<<<nb, 256, 0, st>>>(bT, h->ldp, h->nproj, h->oz_eb);
   if (h->oz_3m8)  // planes Re, Im, (Re + Im) / 2 of dbecp^T, K = p
     oz::k_oz_slice3<S><<<dim3((unsigned)((h->oz_k2c / 16 + 127) / 128), nb), 128, 0, st>>>(
@@ -941,12 +967,20 @@ void oz_vnl_gemm_t(qe_hpsi_handle* h, double2* hpsi, long long ldh, int nb, cuda
         (int)(h->oz_k2c / oz::KB), h->oz_eg, h->oz_eb, h->npw, nb, hpsi, ldh);
     return;
   }
+  if (h->sym) {  // rows 2g + c over the leading sym_m entries, columns (X, Y) of every band; epilogue writes G and -G
+    const long long mr = 2LL * h->sym_m;
+    const dim3 gs((2 * nb + oz::BN - 1) / oz::BN, (unsigned)((mr + oz::BM - 1) / oz::BM), 1);
+    for (int ks = 0; ks * h->oz_kchunk2 < nkb; ++ks)
+      oz::k_oz_gemm<S, 4><<<gs, oz::NT, h->oz_smem, st>>>(h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, h->oz_kchunk2, h->oz_eg, h->oz_eb, mr,
+                                                         2 * nb, hpsi, ldh, 0, ks, h->sym_minus);
+    return;
+  }
   const long long mrows = (h->gamma ? 2LL : 1LL) * h->npw;  // Gamma-only: rows 2g + c of the planar transposed digits
   const dim3 grid(((h->gamma ? 1 : 2) * nb + oz::BN - 1) / oz::BN, (unsigned)((mrows + oz::BM - 1) / oz::BM), 1);
   auto kern = h->gamma ? oz::k_oz_gemm<S, 3> : oz::k_oz_gemm<S, 1>;
   for (int ks = 0; ks * h->oz_kchunk2 < nkb; ++ks)
     kern<<<grid, oz::NT, h->oz_smem, st>>>(h->oz_tm_a2, h->oz_tm_b2, h->oz_stages, nkb, h->oz_kchunk2, h->oz_eg, h->oz_eb, mrows, nb, hpsi,
-                                          ldh, 0, ks);
+                                          ldh, 0, ks, nullptr);
 }
 #define OZ_DISPATCH(S_, CALL)            \
   switch (S_) {                          \
@@ -963,7 +997,10 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, unsigned flags, cudaSt
   int S = (int)((flags >> 8) & 15u);
   if (S == 0) S = 7;
   cudaError_t e = cudaSuccess;
-  const long long k1 = round_up(2LL * h->npw, 128), k2 = round_up((h->gamma ? 1LL : 2LL) * h->nproj, 128);
+  // Gamma-symmetric mode (h->sym, sym_kernels.cuh): real forms over the leading sym_m sphere entries, like a Gamma-only handle
+  const bool realf = h->gamma || h->sym;
+  const long long ksph = h->sym ? h->sym_m : h->npw;  // sphere entries the digit planes cover
+  const long long k1 = round_up(2LL * ksph, 128), k2 = round_up((realf ? 1LL : 2LL) * h->nproj, 128);
   // K range per CTA: int32 level sums must not overflow (qe_hpsi_test_set_int8_kmax lowers it: the multi-range paths on small cases)
   const long long kmax_t = g_int8_kmax;
   const long long kmax = kmax_t >= oz::KB ? std::min<long long>(oz::max_k_per_cta(S), kmax_t / oz::KB * oz::KB) : oz::max_k_per_cta(S);
@@ -971,7 +1008,7 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, unsigned flags, cudaSt
   h->oz_k2 = k2;
   // 3M form of a6 (three real GEMMs instead of a real-form complex one: -25 % MMAs, three launches): pays from ~2^26 entries of beta
   const unsigned m3 = (flags >> 12) & 3u;  // 0 by size, 1 off, 2 a6 only, 3 a6 and a8 whatever the size
-  h->oz_3m = !h->gamma && (m3 == 0 ? (long long)h->nproj * h->npw >= (1LL << 26) : m3 >= 2);
+  h->oz_3m = !realf && (m3 == 0 ? (long long)h->nproj * h->npw >= (1LL << 26) : m3 >= 2);
   h->oz_k1c = round_up(h->npw, 128);
   h->oz_k2c = round_up(h->nproj, 128);
   // a8 in the 3M form: one exact-int32 K range, and enough K blocks per plane to amortise the three epilogues (measured: pays at
@@ -999,14 +1036,14 @@ cudaError_t setup_ozaki(qe_hpsi_handle* h, int max_batch, unsigned flags, cudaSt
   h->oz_kchunk = (int)((nkb + ns - 1) / ns);
   h->oz_nsplit = (nkb + h->oz_kchunk - 1) / h->oz_kchunk;
   h->oz_kchunk2 = (int)std::min<long long>(k2, kmax) / oz::KB;  // a8: sequential launches over K ranges of this many blocks
-  const long long a2rows = (h->gamma ? 2LL : 1LL) * h->npw;
+  const long long a2rows = (realf ? 2LL : 1LL) * ksph;
   const size_t a1 = h->oz_3m ? (size_t)S * 3 * h->nproj * h->oz_k1c : (size_t)S * h->nproj * k1, a2 = h->oz_3m8 ? (size_t)S * 3 * h->npw * h->oz_k2c : (size_t)S * a2rows * k2, bb = (size_t)S * 2 * max_batch * std::max(k1, k2);
-  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit * (h->oz_3m ? 3 : 1);
+  const size_t pc = (size_t)h->nproj * h->ldc * sizeof(double2) * h->oz_nsplit * (h->oz_3m ? 3 : (h->sym ? 2 : 1));
   if ((e = guarded_malloc(h, &h->oz_a1, a1)) != cudaSuccess || (e = guarded_malloc(h, &h->oz_a2, a2)) != cudaSuccess ||
       (e = guarded_malloc(h, &h->oz_b, bb)) != cudaSuccess || (e = guarded_malloc(h, &h->oz_partial, pc)) != cudaSuccess ||
       (e = guarded_malloc(h, &h->oz_ep, sizeof(int) * (size_t)h->nproj)) != cudaSuccess ||
       (e = guarded_malloc(h, &h->oz_eg, sizeof(int) * (size_t)h->npw)) != cudaSuccess ||
-      (e = guarded_malloc(h, &h->oz_eb, sizeof(int) * (size_t)max_batch)) != cudaSuccess) {
+      (e = guarded_malloc(h, &h->oz_eb, sizeof(int) * 2 * (size_t)max_batch)) != cudaSuccess) {
     // the digit planes do not fit (or another CUDA error): qe_hpsi_create fails with QE_HPSI_ENOMEM / QE_HPSI_ECUDA; the buffers
     // allocated so far are released by qe_hpsi_destroy
     return e;
@@ -1099,7 +1136,6 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
     CR_TRY(guarded_malloc(h, &h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
     CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
     h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
-    if (flags & QE_HPSI_PROJ_INT8) CR_TRY(setup_ozaki(h, max_batch, flags, st));
   #undef CR_TRY
   return cudaSuccess;
 }
@@ -1160,7 +1196,7 @@ cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
 // classifies every projector ON THE DEVICE by exact comparison, checks that D couples equal classes only, and allocates the
 // real-form operands.  Leaves h->sym = false (general complex contraction) whenever any check fails; only CUDA errors are errors.
 cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, const int nr[3], int nblocks,
-                            const int32_t* blk_off_host, const double* d_host, cudaStream_t st) {
+                            const int32_t* blk_off_host, const double* d_host, bool int8_path, cudaStream_t st) {
 #define CR_TRY(expr)                     \
   do {                                   \
     cudaError_t e__ = (expr);            \
@@ -1211,13 +1247,15 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
     CR_TRY(upload(&h->sym_cmask, cm, st));
     CR_TRY(cudaStreamSynchronize(st));  // cm leaves scope
   }
+  h->sym_cls_host = cls;
+  h->blk_off.assign(blk_off_host, blk_off_host + nblocks + 1);
   h->sym_wide = env_int("QE_HPSI_SYM_WIDE", 1);
   h->sym_m = M;
   h->sym_ldu = round_up(M, 8);
   h->sym_ldc2 = 2 * h->ldc;
   h->sym_nsplit = std::max(1, (M + h->kchunk - 1) / h->kchunk);
   const size_t ub = sizeof(double2) * 2 * (size_t)h->max_batch * h->sym_ldu, eb = sizeof(double2) * 2 * (size_t)h->max_batch * h->ldp;
-  const size_t pb = sizeof(double2) * (size_t)h->sym_nsplit * h->nproj * h->sym_ldc2;
+  const size_t pb = int8_path ? 16 : sizeof(double2) * (size_t)h->sym_nsplit * h->nproj * h->sym_ldc2;  // (the int8 path has its own)
   CR_TRY(guarded_malloc(h, &h->sym_u, ub));
   CR_TRY(guarded_malloc(h, &h->sym_e, eb));
   CR_TRY(guarded_malloc(h, &h->sym_partial, pb));
@@ -1560,9 +1598,9 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
   // ---- nonlocal ---------------------------------------------------------------------------------------
   if (nproj > 0)
     CR_TRY(setup_nonlocal(h, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
-  if (nproj > 0 && h->npw > 0 && !h->oz_s && !(flags & QE_HPSI_NO_GAMMA_SYM) && sg.kap[0] == 0.0 && sg.kap[1] == 0.0 &&
-      sg.kap[2] == 0.0)
-    CR_TRY(setup_symmetric(h, idx, nr, nblocks, blk_off_host, d_host, st));
+  if (nproj > 0 && h->npw > 0 && !(flags & QE_HPSI_NO_GAMMA_SYM) && sg.kap[0] == 0.0 && sg.kap[1] == 0.0 && sg.kap[2] == 0.0)
+    CR_TRY(setup_symmetric(h, idx, nr, nblocks, blk_off_host, d_host, (flags & QE_HPSI_PROJ_INT8) != 0, st));
+  if (nproj > 0 && (flags & QE_HPSI_PROJ_INT8)) CR_TRY(setup_ozaki(h, max_batch, flags, st));
   if ((flags & QE_HPSI_PROJ_CERTIFY) && h->oz_s) CR_TRY(setup_certify(h, st));
   // NEXT-3: split-K workspace of qe_hpsi_overlap; K slices depend on npw only, so an element's bits do not depend on how many
   // rows / columns a call has (chunks of 512 x 128)
@@ -1695,8 +1733,9 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
   const size_t t1 = prof_mark(h, st);
   prof_span(h, ts, t1, SLOT_BECP);
   const dim3 rg((nb + 127) / 128, h->nproj);
-  if (h->sym && !h->oz_s)
-    sym::k_sym_reduce<<<rg, 128, 0, st>>>(h->sym_partial, h->sym_nsplit, h->nproj, h->sym_ldc2, nb, h->sym_cls, h->becp, h->ldc);
+  if (h->sym)
+    sym::k_sym_reduce<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->sym_partial, h->oz_s ? h->oz_nsplit : h->sym_nsplit, h->nproj,
+                                          h->sym_ldc2, nb, h->sym_cls, h->becp, h->ldc);
   else if (h->gamma)
     k_becp_reduce_gamma<<<rg, 128, 0, st>>>(h->oz_s ? h->oz_partial : h->partial, h->oz_s ? h->oz_nsplit : h->nsplit, h->nproj, h->ldc, nb,
                                             h->beta, h->ldbeta, psi, ldpsi,
@@ -1708,7 +1747,7 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
                                       h->becp);
   k_dmul<<<rg, 128, 0, st>>>(h->becp, h->nproj, h->ldc, nb, h->proj_blk0, h->proj_nh, h->proj_doff, h->dpk, h->dbecp,
                             h->dbT, h->ldp);
-  if (h->sym && !h->oz_s)  // real coefficient rows (Re e, Im e) of the symmetric a8
+  if (h->sym)  // real coefficient rows (Re e, Im e) of the symmetric a8
     sym::k_sym_coef<<<rg, 128, 0, st>>>(h->dbecp, h->nproj, h->ldc, nb, h->sym_cls, h->sym_e, h->ldp);
   prof_span(h, t1, prof_mark(h, st), SLOT_DMUL);
   h->nb_last = nb;
@@ -1718,6 +1757,14 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 
 // a8
 int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
+  // Gamma-symmetric mode: the real coefficient rows of D becp are in sym_e already (launch_becp); for the q-term of
+  // qe_hpsi_apply_hs they are rebuilt from qbecp when q couples equal classes only (else: general contraction, FP64 path only)
+  bool use_sym = h->sym && bT == h->dbT;
+  if (h->sym && bT == h->qbT && h->sym_q_ok) {
+    sym::k_sym_coef<<<dim3((nb + 127) / 128, h->nproj), 128, 0, st>>>(h->qbecp, h->nproj, h->ldc, nb, h->sym_cls, h->sym_e, h->ldp);
+    use_sym = true;
+  }
+  if (h->sym && h->oz_s && !use_sym) return QE_HPSI_ESTATE;  // the int8 planes of a symmetric handle hold the real forms only
   if (h->oz_s) {
     const size_t t0 = prof_mark(h, st);
 #define OZ_CALL(S_) oz_vnl_slice_t<S_>(h, bT, nb, st)
@@ -1735,7 +1782,7 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
     if (mt > 0)
       k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
                                                                                 h->ldp, nb, hpsi, ldh);
-  } else if (h->sym && bT == h->dbT) {
+  } else if (use_sym) {
     // symmetric a8: X = sum_p b_p Re e_p, Y = sum_p b_p Im e_p over the half sphere; hpsi(G) += X + iY, hpsi(-G) += conj X + i conj Y
     auto go = [&](auto cfg) {
       using Cfg = decltype(cfg);
@@ -1856,6 +1903,22 @@ extern "C" int qe_hpsi_set_s(qe_hpsi_t h, const double* q_host) {
     CU_TRY(h, guarded_malloc(h, &h->qbT, (size_t)h->max_batch * h->ldp * sizeof(double2)));
     CU_TRY(h, cudaMemset(h->qbT, 0, (size_t)h->max_batch * h->ldp * sizeof(double2)));
     h->workspace_bytes += pc + (size_t)h->max_batch * h->ldp * sizeof(double2);
+  }
+  if (h->sym) {  // does q couple projectors of equal class only?  (needed by the symmetric real forms)
+    bool ok = true;
+    long long off = 0;
+    for (size_t a = 0; a + 1 < h->blk_off.size() && ok; ++a) {
+      const int q0 = h->blk_off[a], nh = h->blk_off[a + 1] - q0;
+      for (int i = 0; i < nh && ok; ++i)
+        for (int j = 0; j < nh; ++j)
+          if (q_host[off + (long long)i * nh + j] != 0.0 && h->sym_cls_host[(size_t)q0 + i] != h->sym_cls_host[(size_t)q0 + j]) {
+            ok = false;
+            break;
+          }
+      off += (long long)nh * nh;
+    }
+    if (!ok && h->oz_s) return QE_HPSI_EINVAL;  // see include/qe_hpsi.h: create such a handle with QE_HPSI_NO_GAMMA_SYM
+    h->sym_q_ok = ok;
   }
   CU_TRY(h, cudaMemcpy(h->qpk, q_host, sizeof(double) * (size_t)h->d_total, cudaMemcpyHostToDevice));
   return QE_HPSI_OK;
@@ -2252,6 +2315,7 @@ int gamma_create_impl(qe_hpsi_gamma_t* out, qe_hpsi_gamma_handle** live, const d
     g->nl->gamma = true;
     CG_TRY(set_kernel_attrs());
     CG_TRY(setup_nonlocal(g->nl, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
+    if (flags & QE_HPSI_PROJ_INT8) CG_TRY(setup_ozaki(g->nl, max_batch, flags, st));
   }
   CG_TRY(cudaStreamSynchronize(st));
 #undef CG_TRY
@@ -2423,6 +2487,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
     if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 : 4);
+    if (h->nproj > 0 && h->oz_s && h->sym) total += 2;  // merge and coefficient kernels of the symmetric real forms
     if (h->certify) total += 8;  // probe, decide, gather, the four FP64 kernels (empty grids when nothing failed), commit
   }
   return total;

@@ -491,8 +491,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         }
       }
     }
-    return;
-  }
+  } else {
   // a b = (P - Q) + i (R - P - Q)
 #pragma unroll
   for (int i = 0; i < TM; ++i) {
@@ -517,6 +516,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         }
       }
     }
+  }
   }
 }
 

@@ -22,6 +22,10 @@ def _qblocks(wl, seed):
 @pytest.mark.parametrize("flags", [0, _gpu.INT8, _gpu.INT8_S7])
 @pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
 def test_apply_hs_against_oracle(cfg, flags):
+    """q = random symmetric blocks coupling ALL projectors of an atom. At k = 0 the FP64 handle takes the Gamma-symmetric real
+    forms for H and the general contraction for the q-term; an int8 handle in that mode has real-form digit planes only and
+    must refuse such a q (QE_HPSI_EINVAL) -- it is then re-created with QE_HPSI_NO_GAMMA_SYM -- and accept a q that couples
+    equal parities only (second half of the test)."""
     h, inp = _gpu.make(cfg, flags=flags)
     wl = inp["wl"]
     sp = _gpu.oracle_sphere(wl)
@@ -29,6 +33,22 @@ def test_apply_hs_against_oracle(cfg, flags):
     nb = min(wl.nbands, 24)
     psi = _gpu.gen_psi_dev(inp, 0, nb)
     q = _qblocks(wl, 17)
+    if flags and h.info()["gamma_sym"]:
+        with pytest.raises(qe_hpsi.QeHpsiError) as e:
+            h.set_s(q)
+        assert e.value.status == qe_hpsi.QE_HPSI_EINVAL
+        qs = q * (np.asarray(inp["dblocks"]) != 0)  # the sparsity of D: equal l (hence equal parity) only
+        h.set_s(qs)
+        hs, ss = h.apply_hs(psi)
+        torch.cuda.synchronize()
+        beta = inp["beta"][:, :npw].cpu().numpy()
+        ph = psi[:, :npw].cpu().numpy()
+        assert _gpu.rel_l2(ss.cpu().numpy()[:, :npw], orc.spsi_of(beta, qs, ph)).max() <= TOL
+        assert _gpu.rel_l2(hs.cpu().numpy()[:, :npw], _gpu.oracle_hpsi(inp, sp, ph)).max() <= TOL
+        vq = (ss[:, :npw] - psi[:, :npw]).cpu().numpy()  # q-term alone (psi is O(1) and the q-term O(1e-2): 1e-13 of resolution left)
+        assert _gpu.rel_l2(vq, orc.vnl_psi(beta, qs, ph)).max() <= 1e-10
+        h.destroy()
+        h, inp = _gpu.make(cfg, flags=flags | qe_hpsi.QE_HPSI_NO_GAMMA_SYM, beta=inp["beta"])
     h.set_s(q)
     hpsi = torch.full_like(psi, 3.0)
     spsi = torch.full_like(psi, 5.0)

@@ -17,9 +17,10 @@ from tests import _gpu
 pytestmark = pytest.mark.gpu
 
 
-def _make_int8(key, digits=6, three_m=None, **kw):
-    """Handle on the int8 digit path with `digits` digits per operand (explicit create flag)."""
-    return _gpu.make(key, flags=harness.int8_flags(digits, three_m), **kw)
+def _make_int8(key, digits=6, three_m=None, nosym=False, **kw):
+    """Handle on the int8 digit path with `digits` digits per operand (explicit create flag). nosym: keep the general complex
+    contraction at k = 0 (QE_HPSI_NO_GAMMA_SYM), where the default is the Gamma-symmetric real form over the half sphere."""
+    return _gpu.make(key, flags=harness.int8_flags(digits, three_m) | (qe_hpsi.QE_HPSI_NO_GAMMA_SYM if nosym else 0), **kw)
 
 
 def _nonlocal(h, inp, nb):
@@ -40,20 +41,26 @@ def test_the_accuracy_class_is_what_the_create_flag_says_whatever_the_size():
         h.destroy()
         h, _ = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_PROJ_INT8)  # no digit field: 7 digits (55 bits)
         assert h.info()["ozaki_slices"] == 7 and h.info()["ozaki_nsplit"] >= 1 and h.info()["ozaki_3m"] == 0
+        assert h.info()["gamma_sym"] == 1  # k = 0, generator projectors: real forms over the half sphere
         h.destroy()
-    h, _ = _make_int8(1, 6, three_m=3)
-    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_3m"] == 2
+    h, _ = _make_int8(1, 6, three_m=3, nosym=True)
+    assert h.info()["ozaki_slices"] == 6 and h.info()["ozaki_3m"] == 2 and h.info()["gamma_sym"] == 0
     h.destroy()
 
 
 @pytest.mark.parametrize("digits", [6, 7])
-@pytest.mark.parametrize("three_m", [0, 2, 3])
+@pytest.mark.parametrize("three_m", [0, 2, 3, "sym"])
 @pytest.mark.parametrize("cfg", ["T1_general_k", "T2_radix5", "T5_odd_bands", 0, 1])
 def test_becp_and_vnl_against_oracle(cfg, three_m, digits):
-    """Both forms of a6 and a8: the real-form complex GEMMs and the integer 3M forms (three real GEMMs on planar digit planes;
-    QE_HPSI_PROJ_3M_A6: a6 only; QE_HPSI_PROJ_3M_ALL: a6 and a8 whatever the size), at 6 and 7 digits."""
-    h, inp = _make_int8(cfg, digits, three_m=three_m)
-    assert h.info()["ozaki_3m"] == {0: 0, 2: 1, 3: 2}[three_m]
+    """All forms of a6 and a8: the real-form complex GEMMs, the integer 3M forms (three real GEMMs on planar digit planes;
+    QE_HPSI_PROJ_3M_A6: a6 only; QE_HPSI_PROJ_3M_ALL: a6 and a8 whatever the size) -- all with QE_HPSI_NO_GAMMA_SYM so that the
+    k = 0 cases take them too -- and ("sym") the default: at k = 0 the Gamma-symmetric real forms over the half sphere."""
+    if three_m == "sym":
+        h, inp = _make_int8(cfg, digits)
+        assert h.info()["gamma_sym"] == (0 if cfg in ("T1_general_k", "T5_odd_bands") else 1) and h.info()["ozaki_3m"] == 0
+    else:
+        h, inp = _make_int8(cfg, digits, three_m=three_m, nosym=True)
+        assert h.info()["ozaki_3m"] == {0: 0, 2: 1, 3: 2}[three_m] and h.info()["gamma_sym"] == 0
     path = f"int8_s{digits}"
     wl = inp["wl"]
     npw = h.npw
@@ -152,18 +159,24 @@ def test_non_finite_operands_give_nan_not_finite_garbage():
 def test_k_ranges_of_a8_and_forced_splits_of_a6_give_the_same_result():
     """2 nproj beyond the exact-int32 K range makes a8 walk its K ranges launch by launch (and a6 split finer); forced here on
     config 1 by lowering the range (qe_hpsi_test_set_int8_kmax), checked against the default plan and the FP64 tensor path."""
-    h, inp = _make_int8(1, 6)
+    h, inp = _make_int8(1, 6, nosym=True)
     psi, ref, _ = _nonlocal(h, inp, 64)
     h.destroy()
     qe_hpsi.qe_hpsi_test_set_int8_kmax(384)
     try:
-        h2, inp2 = _make_int8(1, 6)
+        h2, inp2 = _make_int8(1, 6, nosym=True)
+        h3, inp3 = _make_int8(1, 6)  # the symmetric real forms: K of a8 is nproj = 512 -> 2 ranges
     finally:
         qe_hpsi.qe_hpsi_test_set_int8_kmax(0)
     assert h2.info()["ozaki_slices"] == 6
     assert h2.launch_count(64) == 5 + 7 + 3  # a1-a5, digit/reduce/a6 kernels, a8 in ceil(1024 / 384) = 3 launches
+    assert h3.info()["gamma_sym"] == 1 and h3.launch_count(64) == 5 + 9 + 2
     _, out, _ = _nonlocal(h2, inp2, 64)
+    _, out3, _ = _nonlocal(h3, inp3, 64)
     h2.destroy()
+    h3.destroy()
+    n3 = torch.linalg.vector_norm(out3 - ref, dim=1) / torch.linalg.vector_norm(ref, dim=1)
+    assert float(n3.max()) <= 1e-11  # other digits (half-sphere rows): agreement at the accuracy class, not bitwise
     num = torch.linalg.vector_norm(out - ref, dim=1)
     den = torch.linalg.vector_norm(ref, dim=1)
     assert float((num / den).max()) <= 1e-13  # same digits, same exact integer sums; only the FP64 order of the K ranges differs
