@@ -34,7 +34,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 // one mbarrier, and (two-pass kernel) the twiddle table tw[q*j] as [RA][RA+1] (RA <= 16)
 // (the mbarrier of the two-pass kernel lives in the unused [0][0] entry of its twiddle table; the three-pass kernel has no table)
 inline size_t fft2t_smem(int n, int P, bool two_pass, bool one_tile) {
-  return (one_tile ? 1 : 2) * (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)P * FFT_C * sizeof(double2) +
+  return (one_tile ? 1 : 2) * (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)(P + (two_pass ? 1 : 0)) * FFT_C * sizeof(double2) +
          (two_pass ? 16 * 17 * sizeof(double2) : 64);
 }
 
@@ -54,16 +54,17 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
   double2* tile1 = reinterpret_cast<double2*>(smem_raw);
   // one_tile: the tile is reused between the passes (two more barriers per band, 24 KB less per CTA at N = 192)
   double2* tile2 = one_tile ? tile1 : tile1 + N * FFT_C;
+  // both stages carry one extra row P: a zero row in the input stage (what an unpopulated plane reads) and a sink row in the
+  // output stage (what it writes), so the loads and stores of the radix-RA passes are unconditional: no branches around them
   double2* inb = tile2 + N * FFT_C;
   const int P = g.P;
-  double2* outb = inb + (size_t)P * FFT_C;
-  double2* twt = outb + (size_t)P * FFT_C;
+  double2* outb = inb + (size_t)(P + 1) * FFT_C;
+  double2* twt = outb + (size_t)(P + 1) * FFT_C;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(twt);  // entry [0][0] (tw = 1) is never read: the mbarrier lives there  // [RA][TWP]: tw[(q*j) % N] at j*TWP + q (odd pitch: 4 rows per warp, no conflicts)
   const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
   const bool io_thread = tid == (NW - 1) * 32;  // first lane of the last warp (idle in the radix-RA passes when RA > RB)
   const int i2 = blockIdx.x / g.ntz;
   const int z0 = (blockIdx.x - i2 * g.ntz) * FFT_C;
-  const double2 zero = make_double2(0.0, 0.0);
   double vv[RB];
 #pragma unroll
   for (int q = 0; q < RB; ++q) vv[q] = __ldg(&g.vs[((size_t)(j + q * RA) * g.n2 + i2) * g.ldz + z0 + c]);
@@ -71,8 +72,9 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
     const int jj = idx / RA, q = idx - jj * RA;
     if (q > 0) twt[jj * TWP + q] = __ldg(&g.ax1.tw[(q * jj) % N]);
   }
-  const int xhi = t.x_hi, xlo0 = N - t.x_lo, xsh = N - P;  // plane index of i1: i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : none)
+  const int xhi = t.x_hi, xlo0 = N - t.x_lo, xsh = N - P;  // plane index of i1: i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : row P)
   const double2* twj = twt + j * TWP;
+  if (tid < FFT_C) inb[(size_t)P * FFT_C + tid] = make_double2(0.0, 0.0);
   if (tid == 0) {
     mbar_init(full, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -103,8 +105,8 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
         const int i1 = j + q * RB;
-        const int p = i1 <= xhi ? i1 : i1 - xsh;
-        v[q] = (i1 <= xhi || i1 >= xlo0) ? in[p * FFT_C] : zero;
+        const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
+        v[q] = in[p * FFT_C];
       }
       pass_a_store<RA, +1>(v, tile1, j, c);
     }
@@ -143,8 +145,8 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
         const int i1 = j + q * RB;
-        if (i1 <= xhi) out[i1 * FFT_C] = v[q];
-        else if (i1 >= xlo0) out[(i1 - xsh) * FFT_C] = v[q];
+        const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
+        out[p * FFT_C] = v[q];
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the bulk store
     }

@@ -1527,7 +1527,7 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
     // gridDim.y only as far as needed to give every SM a few CTAs
     if (h->f2p[0] && h->f2p[0]->rb > 1 && h->P > 0 && h->P <= 256 && h->g2p.x_hi != -2 && env_int("QE_HPSI_X_TMA", 1)) {
       const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb, h->f2p[0]->smem_zy != 0);
-      h->x_one_tile = h->f2p[0]->smem_zy == 0 ? env_int("QE_HPSI_X_ONE_TILE", 0) : 0;
+      h->x_one_tile = h->f2p[0]->smem_zy == 0 ? env_int("QE_HPSI_X_ONE_TILE", 1) : 0;
       const size_t sm = fft2t_smem(nr[0], h->P, h->f2p[0]->smem_zy == 0, h->x_one_tile != 0);
       using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
