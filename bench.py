@@ -438,29 +438,39 @@ def int8_roofline(leg, stage, m, mp, hbm_peak, dmma, args, value, world):
     oz_s = info["ozaki_slices"]
     pairs = oz_s * (oz_s + 1) // 2
     m3 = info.get("ozaki_3m", 0)  # 1: a6 in the integer 3M form (3 real products per complex one), 2: a8 too
+    gsym = bool(info.get("gamma_sym"))  # Gamma-symmetric real forms over the half sphere: half of the real-form complex MACs
     t_becp, t_vnl = stage["a6_becp"][0], stage["a8_vnl_add"][0]
     a8_is_top = t_vnl >= t_becp
-    kname, t_k = (("k_oz_vnl3<S> (a8, 3M form)" if m3 == 2 else "k_oz_gemm<S,1> (a8)"), t_vnl) if a8_is_top else \
-        (("k_oz_gemm<S,2> x 3 (a6, 3M form)" if m3 else "k_oz_gemm<S,0> (a6)"), t_becp)
+    if gsym:
+        kname, t_k = ("k_oz_gemm<S,4> (a8, Gamma-symmetric real form)", t_vnl) if a8_is_top else ("k_oz_gemm<S,2> (a6, Gamma-symmetric real form)", t_becp)
+    else:
+        kname, t_k = (("k_oz_vnl3<S> (a8, 3M form)" if m3 == 2 else "k_oz_gemm<S,1> (a8)"), t_vnl) if a8_is_top else \
+            (("k_oz_gemm<S,2> x 3 (a6, 3M form)" if m3 else "k_oz_gemm<S,0> (a6)"), t_becp)
     flops_launch = 8.0 * wl.nproj * npw * nbc
     ops_launch = pairs * flops_launch  # 4 real MACs per complex MAC x 2 ops x pairs
-    if (a8_is_top and m3 == 2) or (not a8_is_top and m3 >= 1):
+    if gsym:
+        ops_launch *= 0.5
+    elif (a8_is_top and m3 == 2) or (not a8_is_top and m3 >= 1):
         ops_launch *= 0.75
     ach = ops_launch / (t_k * 1e-3) * 1e-12
     bf16_sus = float(mp.get("bf16_tflops_sustained", 0.0)) or 1414.0
     peak = 2.0 * bf16_sus
+    tkey = (("k_oz_gemm_a8_sym" if a8_is_top else "k_oz_gemm_a6_sym") if gsym else
+            (("k_oz_vnl3" if m3 == 2 else "k_oz_gemm_a8") if a8_is_top else ("k_oz_gemm_a6_3m" if m3 else "k_oz_gemm_a6")))
     roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
-                "traffic": committed_traffic(args.config, ("k_oz_vnl3" if m3 == 2 else "k_oz_gemm_a8") if a8_is_top else
-                                              ("k_oz_gemm_a6_3m" if m3 else "k_oz_gemm_a6")) if oz_s == 6 else None,
+                "traffic": committed_traffic(args.config, tkey) if oz_s == 6 else None,
                 "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; the "
                 "kernel runs inside a long, power-capped step). Against the chip's measured int8 burst (register-free UTCIMMA loop, "
-                "4540 TOP/s, profiles/r1g_int8.md) the same kernel is at " + f"{ach / 4540.0:.2f}" + "; ncu: tensor pipe ~41-47 % active, "
-                "shared-memory port 68-72 % (the limiter)", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
+                "4540 TOP/s, profiles/r1g_int8.md) the same kernel is at " + f"{ach / 4540.0:.2f}" + "; ncu (profiles/r2g_capture.md): tensor pipe 36-50 % active", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
                 "digit_pairs": pairs, "fp64_equivalent_tflops": flops_launch / (t_k * 1e-3) * 1e-12,
                 "digit_kernels_ms_per_launch": stage["a6_a8_int8_digits"][0]}
     units = (0.75 if m3 >= 1 else 1.0) + (0.75 if m3 == 2 else 1.0)  # integer 3M forms: 6 of the 8 tile-GEMM units each
+    if gsym:
+        units = 1.0  # two real forms over the half sphere: half of the real-form complex MACs each
     t_int8 = pairs * m["f_proj"] * 0.5 * units / (peak * 1e12)
     b_beta8 = (3 if m3 >= 1 else 2) * oz_s * wl.nproj * npw / wl.batch + (3 if m3 == 2 else 2) * oz_s * wl.nproj * npw / wl.batch
+    if gsym:
+        b_beta8 = 2.0 * oz_s * wl.nproj * npw / wl.batch  # half-sphere real-form planes, streamed once by a6 and once by a8
     roof8 = max((m["b_fft"] + b_beta8) / (hbm_peak * 1e9), t_int8)
     combined = {"bands_per_s": 1.0 / roof8, "frac": value / world * roof8, "int8_tops": peak, "bytes_per_band": m["b_fft"] + b_beta8,
                 "int8_ops_per_band": pairs * m["f_proj"] * 0.5 * units,
