@@ -43,6 +43,11 @@ int qe_hpsi_probe_fp64(double millis, double* dmma_tflops, double* dfma_tflops);
  * finer, a8 walking its K ranges launch by launch).  Process-wide; not for production use. */
 int qe_hpsi_test_set_int8_kmax(int64_t kmax);
 
+/* (testing) smallest nproj * npw from which the Gamma-symmetric projector mode (qe_hpsi.h, QE_HPSI_NO_GAMMA_SYM) is used by
+ * handles created from now on; default 2^20 (smaller steps are launch-latency bound; both forms are FP64), negative = default,
+ * 0 = always.  Lets the tests run the symmetric kernels on tiny cases the oracle can check with a dense H.  Process-wide. */
+int qe_hpsi_test_set_sym_min(int64_t entries);
+
 /* Guard bands (the pool's GPUs do not run compute-sanitizer): every device buffer a handle owns is allocated with a
  * pattern-filled tail of 256..511 bytes.  Synchronises the device and returns the number of buffers whose tail was
  * overwritten (0 = no kernel wrote past the end of a workspace since create), or a negative status. */

@@ -21,6 +21,11 @@ struct Fft2pGeom {
   // the populated i1 planes of a convex sphere are the wrapped interval [0..x_hi] u [N1-x_lo..N1-1] (x_hi = -1 / x_lo = 0:
   // that part is empty) in this order, so plane_of[i1] = i1, resp. i1 - (N1 - P); x_hi = -2 when the pattern does not hold
   int x_hi, x_lo;
+  // same rule per populated plane p for its sticks along i2: i2 in [0..y_hi[p]] u [N2-y_lo[p]..N2-1] are the plane's sticks
+  // plane_stick[p] + i2, resp. plane_stick[p] + i2 - (N2 - count); y_hi == nullptr when the pattern does not hold (table lookup)
+  const int* y_hi;
+  const int* y_lo;
+  const double2* zrow;  // ldz zeros: what an unpopulated (plane, i2) column reads, so that the loads need no branch
 };
 
 // shared tile [N][FFT_C] with the column XOR swizzle of fft_core.cuh (fft_phys)
@@ -177,10 +182,25 @@ __global__ void __launch_bounds__(RA* FFT_C) k2p_yinv(FftGeom g, Fft2pGeom t, co
   const int* col = t.col_of + (size_t)p * N;
   if (j < RB) {
     double2 v[RA];
+    if (t.y_hi != nullptr) {
+      // stick of column i2 by the wrapped-interval rule (three scalars per plane) instead of a dependent table lookup per
+      // column; unpopulated columns read the zero row: sixteen independent, unconditional loads
+      const int s0 = __ldg(&g.plane_stick[p]), yhi = __ldg(&t.y_hi[p]), ylo0 = N - __ldg(&t.y_lo[p]);
+      const int ysh = N - (__ldg(&g.plane_stick[p + 1]) - s0);
+      const double2* zr = t.zrow + z;
 #pragma unroll
-    for (int q = 0; q < RA; ++q) {
-      const int s = __ldg(&col[j + q * RB]);
-      v[q] = s >= 0 ? in[(size_t)s * g.ldz] : zero;
+      for (int q = 0; q < RA; ++q) {
+        const int i2 = j + q * RB;
+        const int s = s0 + (i2 <= yhi ? i2 : i2 - ysh);
+        const double2* src = (i2 <= yhi || i2 >= ylo0) ? in + (size_t)s * g.ldz : zr;
+        v[q] = *src;
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < RA; ++q) {
+        const int s = __ldg(&col[j + q * RB]);
+        v[q] = s >= 0 ? in[(size_t)s * g.ldz] : zero;
+      }
     }
     if constexpr (RB > 1) {
       pass_a_store<RA, +1>(v, tile, j, c);

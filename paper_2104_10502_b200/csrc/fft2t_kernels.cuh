@@ -362,6 +362,15 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_zfwd_gather(FftGeom g, Fft2pGeo
   }
   const double2* pb = psi + (size_t)b * ldpsi;
   double2* hb = hpsi + (size_t)b * ldh;
+  {
+    // the sphere entries of the tile's sticks are one contiguous chunk of psi / g2kin (canonical order): pull it towards L2 now,
+    // while the W1 rows are in flight, so that the kinetic-term reads after the transform do not pay a second DRAM latency
+    const int base = g.stick_start[s0], cnt = g.stick_start[min(s0 + FFT_C, g.S)] - base;
+    for (int i = tid * 8; i < cnt; i += RA * FFT_C * 8) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + base + i));
+      if ((i & 8) == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(g.g2kin + base + i));
+    }
+  }
   if (j < RB) {
     mbar_wait(full, 0);
     double2 v[RA];

@@ -76,6 +76,8 @@ struct qe_hpsi_handle {
   const Fft2pEntry* f2p[3] = {nullptr, nullptr, nullptr};  // per axis j = 0..2 (N1, N2, N3)
   Fft2pGeom g2p{};
   int *stick_lo = nullptr, *stick_hi = nullptr, *col_of = nullptr, *plane_of = nullptr;
+  int *plane_yhi = nullptr, *plane_ylo = nullptr;  // wrapped-interval rule of the sticks of a plane along i2
+  double2* zrow = nullptr;                          // ldz zeros
   size_t smem_x2p = 0;
   // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
   K2tX x_tma = nullptr;
@@ -561,6 +563,7 @@ constexpr int MAX_DEVICES = 64;
 bool g_attr_done[MAX_DEVICES] = {};
 std::mutex g_attr_mutex;
 long long g_int8_kmax = 0;  // qe_hpsi_test_set_int8_kmax
+long long g_sym_min = 1LL << 20;  // qe_hpsi_test_set_sym_min: entries of beta from which the Gamma-symmetric mode is used
 cudaError_t set_kernel_attrs() {
   int dev = 0, optin = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -639,6 +642,10 @@ extern "C" int64_t qe_hpsi_test_check_guards(qe_hpsi_t h) {
   }
   return bad;
 }
+extern "C" int qe_hpsi_test_set_sym_min(int64_t entries) {
+  g_sym_min = entries < 0 ? (1LL << 20) : entries;
+  return QE_HPSI_OK;
+}
 extern "C" int qe_hpsi_test_set_int8_kmax(int64_t kmax) {
   if (kmax < 0) return QE_HPSI_EINVAL;
   g_int8_kmax = kmax;
@@ -685,6 +692,9 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->stick_hi);
   cudaFree(h->col_of);
   cudaFree(h->plane_of);
+  cudaFree(h->plane_yhi);
+  cudaFree(h->plane_ylo);
+  cudaFree(h->zrow);
   cudaFree(h->vs);
   for (int j = 0; j < 3; ++j) cudaFree(h->tw[j]);
   cudaFree(h->w1);
@@ -1438,6 +1448,37 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
       h->g2p.x_hi = ok ? hi : -2;
       h->g2p.x_lo = ok ? lo : 0;
     }
+    // the same rule per plane along i2 (Fft2pGeom::y_hi / y_lo), verified against col_of
+    {
+      std::vector<int> yhi((size_t)std::max(h->P, 1), -1), ylo((size_t)std::max(h->P, 1), 0);
+      bool ok = true;
+      for (int p_ = 0; p_ < h->P && ok; ++p_) {
+        const int s0 = plane_stick[p_], cnt = plane_stick[p_ + 1] - s0;
+        int hi = -1, lo = 0;
+        for (int s_ = s0; s_ < s0 + cnt; ++s_) {
+          if (stick_i2[s_] < (n2 + 1) / 2) hi = std::max(hi, stick_i2[s_]);
+          else ++lo;
+        }
+        ok = (hi + 1) + lo == cnt;
+        for (int i2 = 0; i2 < n2 && ok; ++i2) {
+          const int want = i2 <= hi ? s0 + i2 : (i2 >= n2 - lo ? s0 + i2 - (n2 - cnt) : -1);
+          ok = col_of[(size_t)p_ * n2 + i2] == want;
+        }
+        yhi[(size_t)p_] = hi;
+        ylo[(size_t)p_] = lo;
+      }
+      h->g2p.y_hi = h->g2p.y_lo = nullptr;
+      if (ok) {
+        CR_TRY(upload(&h->plane_yhi, yhi, st));
+        CR_TRY(upload(&h->plane_ylo, ylo, st));
+        CR_TRY(cudaStreamSynchronize(st));  // the host vectors leave scope
+        h->g2p.y_hi = h->plane_yhi;
+        h->g2p.y_lo = h->plane_ylo;
+      }
+      CR_TRY(guarded_malloc(h, &h->zrow, sizeof(double2) * (size_t)h->ldz));
+      CR_TRY(cudaMemsetAsync(h->zrow, 0, sizeof(double2) * (size_t)h->ldz, st));
+      h->g2p.zrow = h->zrow;
+    }
   }
 
   // ---- FFT plan ---------------------------------------------------------------------------------------
@@ -1598,7 +1639,10 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
   // ---- nonlocal ---------------------------------------------------------------------------------------
   if (nproj > 0)
     CR_TRY(setup_nonlocal(h, nproj, beta_dev, ldbeta, nblocks, blk_off_host, d_host, d_total, max_batch, flags, st));
-  if (nproj > 0 && h->npw > 0 && !(flags & QE_HPSI_NO_GAMMA_SYM) && sg.kap[0] == 0.0 && sg.kap[1] == 0.0 && sg.kap[2] == 0.0)
+  // (below ~1e6 entries of beta the step is launch-latency bound and the two extra small kernels of the symmetric form cost more
+  // than the contraction saves: same FP64 arithmetic either way, so this size rule is a scheduling choice, not an accuracy one)
+  if (nproj > 0 && h->npw > 0 && !(flags & QE_HPSI_NO_GAMMA_SYM) && sg.kap[0] == 0.0 && sg.kap[1] == 0.0 && sg.kap[2] == 0.0 &&
+      (long long)nproj * h->npw >= g_sym_min)
     CR_TRY(setup_symmetric(h, idx, nr, nblocks, blk_off_host, d_host, (flags & QE_HPSI_PROJ_INT8) != 0, st));
   if (nproj > 0 && (flags & QE_HPSI_PROJ_INT8)) CR_TRY(setup_ozaki(h, max_batch, flags, st));
   if ((flags & QE_HPSI_PROJ_CERTIFY) && h->oz_s) CR_TRY(setup_certify(h, st));

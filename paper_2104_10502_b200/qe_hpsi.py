@@ -61,6 +61,7 @@ SIGNATURES = {
     "qe_hpsi_scale": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp]),
     # ---- include/qe_hpsi_test.h: measurement and test helpers, not the product boundary ----
     "qe_hpsi_test_set_int8_kmax": (_i32, [_i64]),
+    "qe_hpsi_test_set_sym_min": (_i32, [_i64]),
     "qe_hpsi_test_check_guards": (_i64, [_vp]),
     "qe_hpsi_probe_fp64": (_i32, [_dbl, _pd, _pd]),
     "qe_hpsi_profile": (_i32, [_vp, _i32]),
@@ -150,6 +151,11 @@ def qe_hpsi_gsphere(at, xk, ecutwfc, nr) -> np.ndarray:
 def qe_hpsi_test_set_int8_kmax(kmax: int):
     """(qe_hpsi_test.h) K range per CTA of the int8 GEMMs for handles created from now on; 0 = natural."""
     _check(load_library().qe_hpsi_test_set_int8_kmax(int(kmax)))
+
+
+def qe_hpsi_test_set_sym_min(entries: int):
+    """(qe_hpsi_test.h) smallest nproj * npw that takes the Gamma-symmetric projector mode; negative = default (2^20), 0 = always."""
+    _check(load_library().qe_hpsi_test_set_sym_min(int(entries)))
 
 
 def qe_hpsi_probe_fp64(millis=200.0):

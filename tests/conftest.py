@@ -27,7 +27,7 @@ def pytest_collection_modifyitems(config, items):
 
 
 @pytest.fixture(autouse=True)
-def _guard_bands_checked_at_destroy(monkeypatch):
+def _guard_bands_checked_at_destroy(monkeypatch, request):
     """Every handle a GPU test destroys first has its guard bands verified (qe_hpsi_test_check_guards): a kernel that wrote
     past the end of any workspace of the handle fails the test that used it. Stands in for compute-sanitizer memcheck, which
     the GPU pool does not run (profiles/r2_sanitizer.md)."""
@@ -44,4 +44,11 @@ def _guard_bands_checked_at_destroy(monkeypatch):
             orig(self)
 
     monkeypatch.setattr(qe_hpsi.Hpsi, "destroy", destroy)
+    # the Gamma-symmetric projector mode is a scheduling choice from 2^20 entries of beta on; the tests run it on the tiny cases too
+    import os
+    have = "gpu" in request.node.keywords and os.path.exists(qe_hpsi.LIB_PATH)
+    if have:
+        qe_hpsi.qe_hpsi_test_set_sym_min(0)
     yield
+    if have:
+        qe_hpsi.qe_hpsi_test_set_sym_min(-1)

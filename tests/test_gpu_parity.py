@@ -299,6 +299,16 @@ def test_gamma_symmetric_projector_mode_is_detected_and_matches_the_general_cont
     h3, _ = _gpu.make(0)
     assert h3.info()["gamma_sym"] == 1
     h3.destroy()
+    # outside the tests the mode starts at 2^20 entries of beta (config 0 has 17 k: launch-latency bound, general form)
+    qe_hpsi.qe_hpsi_test_set_sym_min(-1)
+    try:
+        h4, _ = _gpu.make(0)
+        h5, _ = _gpu.make(1)
+        assert h4.info()["gamma_sym"] == 0 and h5.info()["gamma_sym"] == 1
+        h4.destroy()
+        h5.destroy()
+    finally:
+        qe_hpsi.qe_hpsi_test_set_sym_min(0)
 
 
 def test_apply_host_matches_device_path():
