@@ -2176,7 +2176,10 @@ extern "C" int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, 
     const int n = std::min(h->fft_nb, nbands - b0);
     const double2* p = psi + (size_t)b0 * ldpsi;
     if (fast) {
-      ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
+      if (h->z_tma_inv)  // the bulk-staged a1 of the hot path
+        h->z_tma_inv<<<dim3(zt, n), ez->nthreads, h->smem_zt, st>>>(g, h->g2p, p, ldpsi, h->w1);
+      else
+        ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
       ey->yinv<<<dim3(yt, n), ey->nthreads, ey->smem_zy, st>>>(g, h->g2p, h->w1, h->w2);
       ex->rho<<<dim3(xt, 1), ex->nthreads, ex->smem_x, st>>>(g, h->g2p, h->w2, n, occ_dev + b0, scale, rho_dev);
     } else {
