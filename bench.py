@@ -47,7 +47,7 @@ def parse():
     ap.add_argument("--detail", action="store_true", help="extra pass with per-FFT-kernel events (stderr table)")
     ap.add_argument("--graph", type=int, default=-1, help="replay the step from a CUDA graph: 1 on, 0 off, -1 (default) only "
                     "for launch-latency-bound workloads (a step under 0.5 ms); stage timers are taken in a separate eager pass")
-    ap.add_argument("--path", default="fp64", choices=["fp64", "int8_s7", "int8_s6", "int8_s6_certified"],
+    ap.add_argument("--path", default="fp64", choices=["fp64", "fp64_general", "int8_s7", "int8_s6", "int8_s6_certified"],
                     help="arithmetic of the HEADLINE leg (default fp64 = the library default; the others for profiling runs)")
     ap.add_argument("--no-int8", action="store_true", help="skip the int8_paths legs")
     ap.add_argument("--no-next", action="store_true", help="skip the next_rows object (SURVEY 8(f) rows: apply_hs, overlap, "
@@ -305,9 +305,10 @@ def run_reference(args, wl, rank):
     print(json.dumps(line), flush=True)
 
 
-PATH_FLAGS = {"fp64": lambda hz: 0, "int8_s7": lambda hz: hz.int8_flags(7), "int8_s6": lambda hz: hz.int8_flags(6),
+PATH_FLAGS = {"fp64": lambda hz: 0, "fp64_general": lambda hz: 32,  # 32 = QE_HPSI_NO_GAMMA_SYM
+              "int8_s7": lambda hz: hz.int8_flags(7), "int8_s6": lambda hz: hz.int8_flags(6),
               "int8_s6_certified": lambda hz: hz.int8_flags(6, certify=True)}
-PATH_DTYPE = {"fp64": "f64",
+PATH_DTYPE = {"fp64": "f64", "fp64_general": "f64",
               "int8_s7": "f64 operands as 7 int8 digits (55-bit block fixed point) in the projector contractions, FP64 elsewhere",
               "int8_s6": "f64 operands as 6 int8 digits (47-bit block fixed point) in the projector contractions, FP64 elsewhere",
               "int8_s6_certified": "as int8_s6, each chunk checked a posteriori and failing bands re-computed in FP64"}
@@ -639,6 +640,29 @@ def main():
             if cnt:
                 sys.stderr.write(f"{k:18s} total {ms:10.3f} ms over {cnt} spans\n")
     leg.close()
+
+    # ---- the same FP64 step with the general complex contraction (QE_HPSI_NO_GAMMA_SYM): what k != 0 or unsymmetric projectors get
+    if wl.nproj and args.path == "fp64" and info.get("gamma_sym") and not args.no_int8 and world == 1:
+        lg = Leg("fp64_general", wl, inp, psi, hpsi, calls, None)
+        for _ in range(3):
+            lg.eager_step()
+        torch.cuda.synchronize()
+        k = max(2, min(args.steps, 3))
+        msg, _, clkg = lg.timed(k, 3, flush)
+        stg, _ = lg.stage_pass(1)
+        vg = nb / msg * 1e3
+        pb = psi[:min(batch, nb)]
+        got = lg.h.nonlocal_add(pb, torch.zeros_like(pb))
+        dg = torch.linalg.vector_norm(got[:, :npw] - ref_vnl[:, :npw], dim=1) / torch.linalg.vector_norm(ref_vnl[:, :npw], dim=1)
+        line["fp64_general_contraction"] = {
+            "value": vg, "unit": UNIT, "ms_per_step": msg, "steps": k, "dtype": "f64", "projector_path": "fp64 dmma (3M complex form)",
+            "combined_roofline_frac": vg * roof_t, "a6_becp_ms": stg["a6_becp"][0], "a8_vnl_add_ms": stg["a8_vnl_add"][0],
+            "executed_dmma_frac_a8": flops_launch / (stg["a8_vnl_add"][0] * 1e-3) * 1e-12 / dmma * 0.75, "clocks": clkg,
+            "max_rel_l2_nonlocal_part_vs_headline_leg": float(dg.max()),
+            "note": "the same step with create flag QE_HPSI_NO_GAMMA_SYM: 6 executed flops per complex MAC instead of 4; this is the "
+                    "form config 3 (general k) and unsymmetric projector sets run"}
+        del got, dg
+        lg.close()
 
     # ---- the opt-in int8 digit paths on the same inputs: named sub-objects, each with its measured error ---------------
     if wl.nproj and args.path == "fp64" and not args.no_int8 and world == 1:
