@@ -198,21 +198,45 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const long long g = m >> 1;
         const int c = (int)(m & 1);
         const int mg = ok ? minus[g] : -1;
+        // the loads of the four column pairs first, then the stores: the compiler cannot prove that the entries do not alias, so
+        // interleaved read-modify-writes would cost one global round trip each
+        double og[4], om[4], vg[4], vm[4];
+        bool wr[4];
 #pragma unroll
-        for (int j = 0; j < 8; j += 2) {
-          const int col = q * BN + n0 + j;  // X column of band col / 2; nb = number of columns (even)
+        for (int jp = 0; jp < 4; ++jp) {
+          const int col = q * BN + n0 + 2 * jp;  // X column of band col / 2; nb = number of columns (even)
           const bool cok = col < nb;
-          const double x = oz_scale(d[j], em, cok ? eb[col] : 0), y = oz_scale(d[j + 1], em, cok ? eb[col + 1] : 0);
+          const double x = oz_scale(d[2 * jp], em, cok ? eb[col] : 0), y = oz_scale(d[2 * jp + 1], em, cok ? eb[col + 1] : 0);
           const double yo = __shfl_xor_sync(0xffffffffu, y, 1);  // the other component of Y (lanes 2k, 2k+1 hold rows 2g, 2g+1)
-          if (ok && cok && mg != -1) {
-            double* row = reinterpret_cast<double*>(out + (size_t)(col >> 1) * ldo);
-            // c = 0: Re(G) += X_r - Y_i, Re(-G) += X_r + Y_i;   c = 1: Im(G) += X_i + Y_r, Im(-G) += Y_r - X_i
-            row[2 * g + c] += c == 0 ? x - yo : x + yo;
-            if (mg >= 0) row[2 * (long long)mg + c] += c == 0 ? x + yo : yo - x;
+          // c = 0: Re(G) += X_r - Y_i, Re(-G) += X_r + Y_i;   c = 1: Im(G) += X_i + Y_r, Im(-G) += Y_r - X_i
+          vg[jp] = c == 0 ? x - yo : x + yo;
+          vm[jp] = c == 0 ? x + yo : yo - x;
+          wr[jp] = ok && cok && mg != -1;
+          og[jp] = om[jp] = 0.0;
+          if (wr[jp]) {
+            const double* row = reinterpret_cast<const double*>(out + (size_t)(col >> 1) * ldo);
+            og[jp] = row[2 * g + c];
+            if (mg >= 0) om[jp] = row[2 * (long long)mg + c];
+          }
+        }
+#pragma unroll
+        for (int jp = 0; jp < 4; ++jp) {
+          if (wr[jp]) {
+            double* row = reinterpret_cast<double*>(out + (size_t)((q * BN + n0 + 2 * jp) >> 1) * ldo);
+            row[2 * g + c] = og[jp] + vg[jp];
+            if (mg >= 0) row[2 * (long long)mg + c] = om[jp] + vm[jp];
           }
         }
       } else if (MODE >= 2) {  // real forms of the Gamma-only handle: one column per band
         if (m < mvalid) {
+          double old8[8];
+          if (MODE == 3) {  // loads before stores (see MODE 4)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const int b = q * BN + n0 + j;
+              old8[j] = b < nb ? reinterpret_cast<const double*>(out + (size_t)b * ldo)[m] : 0.0;
+            }
+          }
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
             const int b = q * BN + n0 + j;
@@ -221,25 +245,28 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               if (MODE == 2)
                 out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(val, 0.0);
               else
-                reinterpret_cast<double*>(out + (size_t)b * ldo)[m] += val;  // m = 2g + c: component c of hpsi[b][g]
+                reinterpret_cast<double*>(out + (size_t)b * ldo)[m] = old8[j] + val;  // m = 2g + c: component c of hpsi[b][g]
             }
           }
         }
       } else if (m < mvalid) {
+        double2 old4[4];
+        if (MODE == 1) {  // loads before stores (see MODE 4)
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) {
+            const int b = (q * BN + n0) / 2 + jj;
+            old4[jj] = b < nb ? out[(size_t)b * ldo + m] : make_double2(0.0, 0.0);
+          }
+        }
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
           const int b = (q * BN + n0) / 2 + jj;
           if (b < nb) {
             const double re = oz_scale(d[2 * jj], em, eb[b]), im = oz_scale(d[2 * jj + 1], em, eb[b]);
-            if (MODE == 0) {
+            if (MODE == 0)
               out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(re, im);
-            } else {
-              double2* o = out + (size_t)b * ldo + m;
-              double2 t = *o;
-              t.x += re;
-              t.y += im;
-              *o = t;
-            }
+            else
+              out[(size_t)b * ldo + m] = make_double2(old4[jj].x + re, old4[jj].y + im);
           }
         }
       }
@@ -603,16 +630,23 @@ k_oz_vnl3(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUte
       asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&tfree)) : "memory");
       const double cr = pl == 0 ? 1.0 : pl == 1 ? -1.0 : 0.0, ci = pl == 2 ? 4.0 : -1.0;
       if (row_ok) {
+        // four loads in flight before their stores (the compiler cannot prove the entries distinct: interleaved
+        // read-modify-writes would cost one global round trip each)
 #pragma unroll
-        for (int j = 0; j < BN; ++j) {
-          const int b = q * BN + j;
-          if (b < nb) {
-            const double x = oz_scale(val[j], em, eb[b]);
-            double2* o = out + (size_t)b * ldo + m;
-            double2 t = *o;
-            t.x = fma(cr, x, t.x);
-            t.y = fma(ci, x, t.y);
-            *o = t;
+        for (int j0 = 0; j0 < BN; j0 += 4) {
+          double2 t[4];
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) {
+            const int b = q * BN + j0 + jj;
+            t[jj] = b < nb ? out[(size_t)b * ldo + m] : make_double2(0.0, 0.0);
+          }
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) {
+            const int b = q * BN + j0 + jj;
+            if (b < nb) {
+              const double x = oz_scale(val[j0 + jj], em, eb[b]);
+              out[(size_t)b * ldo + m] = make_double2(fma(cr, x, t[jj].x), fma(ci, x, t[jj].y));
+            }
           }
         }
       }

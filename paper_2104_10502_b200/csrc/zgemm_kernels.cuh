@@ -464,59 +464,66 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   }
   cp_async_wait<0>();
   if constexpr (SYM) {
-    // columns 2 fk, 2 fk + 1 of an 8-column block are (X, Y) of one band: X = (P, Q)[0], Y = (P, Q)[1]
+    // columns 2 fk, 2 fk + 1 of an 8-column block are (X, Y) of one band: X = (P, Q)[0], Y = (P, Q)[1].
+    // All loads of a row block are issued before its first store: the compiler cannot prove that hpsi[.][g] and hpsi[.][-g] do
+    // not alias, so interleaved read-modify-writes would serialise into one global round trip per entry.
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
       const int gg = m0 + wm0 + i * 8 + fr;
       if (gg >= npw) continue;
       const int mg = minus[gg];
       if (mg == -1) continue;
+      double2 v[TN], w[TN];
 #pragma unroll
       for (int j = 0; j < TN; ++j) {
         const int col = n0 + wn0 + j * 8 + 2 * fk;
-        if (col >= nb) continue;  // nb = number of columns = 2 x bands
-        const int b = col >> 1;
-        const double xr = P[i][j][0], xi = Q[i][j][0], yr = P[i][j][1], yi = Q[i][j][1];
-        double2* h = &hpsi[(size_t)b * ldh + gg];
-        double2 v = *h;
-        v.x += xr - yi;
-        v.y += xi + yr;
-        *h = v;
-        if (mg >= 0) {
-          double2* h2 = &hpsi[(size_t)b * ldh + mg];
-          double2 w = *h2;
-          w.x += xr + yi;
-          w.y += yr - xi;
-          *h2 = w;
+        v[j] = w[j] = make_double2(0.0, 0.0);
+        if (col < nb) {  // nb = number of columns = 2 x bands
+          v[j] = hpsi[(size_t)(col >> 1) * ldh + gg];
+          if (mg >= 0) w[j] = hpsi[(size_t)(col >> 1) * ldh + mg];
         }
+      }
+#pragma unroll
+      for (int j = 0; j < TN; ++j) {
+        const int col = n0 + wn0 + j * 8 + 2 * fk;
+        if (col >= nb) continue;
+        const double xr = P[i][j][0], xi = Q[i][j][0], yr = P[i][j][1], yi = Q[i][j][1];
+        hpsi[(size_t)(col >> 1) * ldh + gg] = make_double2(v[j].x + (xr - yi), v[j].y + (xi + yr));
+        if (mg >= 0) hpsi[(size_t)(col >> 1) * ldh + mg] = make_double2(w[j].x + (xr + yi), w[j].y + (yr - xi));
       }
     }
   } else {
-  // a b = (P - Q) + i (R - P - Q)
+    // a b = (P - Q) + i (R - P - Q); loads of a row block before its stores (see above)
 #pragma unroll
-  for (int i = 0; i < TM; ++i) {
-    const int gg = m0 + wm0 + i * 8 + fr;
-    if (gg >= npw) continue;
+    for (int i = 0; i < TM; ++i) {
+      const int gg = m0 + wm0 + i * 8 + fr;
+      if (gg >= npw) continue;
+      double2 v[TN][2];
 #pragma unroll
-    for (int j = 0; j < TN; ++j) {
+      for (int j = 0; j < TN; ++j)
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int b = n0 + wn0 + j * 8 + 2 * fk + e;
-        if (b < nb) {
-          double2* h = &hpsi[(size_t)b * ldh + gg];
-          double2 v = *h;
-          if constexpr (GAMMA) {
-            v.x += P[i][j][e];
-            v.y += Q[i][j][e];
-          } else {
-            v.x += P[i][j][e] - Q[i][j][e];
-            v.y += (R[i][j][e] - P[i][j][e]) - Q[i][j][e];
-          }
-          *h = v;
+        for (int e = 0; e < 2; ++e) {
+          const int b = n0 + wn0 + j * 8 + 2 * fk + e;
+          v[j][e] = b < nb ? hpsi[(size_t)b * ldh + gg] : make_double2(0.0, 0.0);
         }
-      }
+#pragma unroll
+      for (int j = 0; j < TN; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int b = n0 + wn0 + j * 8 + 2 * fk + e;
+          if (b < nb) {
+            double2 t = v[j][e];
+            if constexpr (GAMMA) {
+              t.x += P[i][j][e];
+              t.y += Q[i][j][e];
+            } else {
+              t.x += P[i][j][e] - Q[i][j][e];
+              t.y += (R[i][j][e] - P[i][j][e]) - Q[i][j][e];
+            }
+            hpsi[(size_t)b * ldh + gg] = t;
+          }
+        }
     }
-  }
   }
 }
 
