@@ -13,12 +13,14 @@ from paper_2104_10502_b200 import harness, inputs, qe_hpsi
 FP64 = 0
 INT8 = harness.int8_flags(6)       # 47-bit digits: north_star's 1e-11 of the nonlocal part holds empirically
 INT8_S7 = harness.int8_flags(7)    # 55-bit digits
-PATHS = {"fp64": FP64, "int8_s6": INT8, "int8_s7": INT8_S7}
+FP64_GENERAL = qe_hpsi.QE_HPSI_NO_GAMMA_SYM  # FP64 with the general complex contraction also at k = 0 (3M form)
+INT8_CERT = harness.int8_flags(6, certify=True)  # 47-bit digits, every chunk checked a posteriori, failing bands redone in FP64
+PATHS = {"fp64": FP64, "fp64_general": FP64_GENERAL, "int8_s6": INT8, "int8_s7": INT8_S7, "int8_s6_cert": INT8_CERT}
 # per-band relative L2 tolerance of the NONLOCAL PART ALONE against the oracle (the FP64 rows are the pre-c3f4fb3 values:
 # FP64 rounding of K <= 7.6e5 term sums; S = 6 keeps north_star's 1e-11 because DESIGN.md 5.6's truncation law puts it at
 # ~1e-12 on these operands; S = 7 is within a small factor of FP64)
-TOL_VNL = {"fp64": 1e-12, "int8_s7": 1e-12, "int8_s6": 1e-11}
-TOL_BECP = {"fp64": 1e-13, "int8_s7": 1e-13, "int8_s6": 5e-12}   # max-entry error relative to max |becp|
+TOL_VNL = {"fp64": 1e-12, "fp64_general": 1e-12, "int8_s7": 1e-12, "int8_s6": 1e-11, "int8_s6_cert": 1e-11}
+TOL_BECP = {"fp64": 1e-13, "fp64_general": 1e-13, "int8_s7": 1e-13, "int8_s6": 5e-12, "int8_s6_cert": 5e-12}   # max-entry error relative to max |becp|
 
 
 def make(key, max_batch=None, flags=0, beta=None):

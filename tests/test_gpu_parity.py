@@ -110,7 +110,7 @@ def test_batch_composition_and_chunking_do_not_change_bits():
     h.destroy()
 
 
-@pytest.mark.parametrize("path", ["fp64", "int8_s7", "int8_s6"])
+@pytest.mark.parametrize("path", ["fp64", "fp64_general", "int8_s7", "int8_s6", "int8_s6_cert"])
 def test_config1_all_bands(path):
     h, inp = _gpu.make(1, flags=_gpu.PATHS[path])
     wl = inp["wl"]
@@ -150,7 +150,7 @@ def _sample_bands(wl):
 @pytest.mark.parametrize("cfg", [2, 3, 4])
 def test_full_size_against_oracle_every_projector_path(cfg):
     """BASELINE.json's full sizes in the launch configuration bench.py times (calls of `batch` bands, beta borrowed), ALL
-    bands applied, for each projector path (FP64 default, int8 S = 7, int8 S = 6):
+    bands applied, for each projector path (FP64 default, FP64 with the general contraction, int8 S = 7, int8 S = 6):
       * sampled bands (first + last of every call, 8 random): H psi against oracle Level B, and the NONLOCAL PART ALONE
         (qe_hpsi_nonlocal on zeros) against the oracle's nonlocal part -- it is ~1e-5 of |H psi| here, so only this isolates
         a6 / a8 at their full-size shapes (23-37 K splits, 64 K blocks x 3 planes); becp of the sampled bands against orc.becp_of;
@@ -162,7 +162,10 @@ def test_full_size_against_oracle_every_projector_path(cfg):
     shared = {}
     report = {}
     for path, pflags in _gpu.PATHS.items():
+        if path == "fp64_general" and any(x != 0.0 for x in wl.xk):
+            continue  # at k != 0 the default FP64 path is the general contraction already
         h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA | pflags, beta=shared.get("beta"))
+        assert h.info()["gamma_sym"] == (0 if path == "fp64_general" or any(x != 0.0 for x in wl.xk) else 1)
         npw = h.npw
         if not shared:
             shared["beta"] = inp["beta"]
