@@ -66,7 +66,9 @@ typedef enum {
  * i.e. 8S-1 bits under the row exponent: S = 7 -> 55 bits, S = 6 -> 47 bits.  Digits: QE_HPSI_PROJ_DIGITS(4..7);
  * 0 = 7.  Costs 3 S bytes per complex entry of beta for a6 and 3 S for a8 of device memory (2 S each for small
  * problems) NEXT TO the FP64 beta: at S = 6 that is 2.25 x the size of beta (56 GB for the 25 GB beta of the
- * largest benchmark workload), 2.6 x at S = 7.  If those planes cannot be allocated qe_hpsi_create FAILS with
+ * largest benchmark workload), 2.6 x at S = 7; in the Gamma-symmetric mode (k = 0, see QE_HPSI_NO_GAMMA_SYM below) the
+ * planes hold real forms over the half sphere, 2 S bytes per complex entry of beta in all: 0.75 x the size of beta at
+ * S = 6 (19 GB for that workload).  If those planes cannot be allocated qe_hpsi_create FAILS with
  * QE_HPSI_ENOMEM; it never changes the arithmetic silently.  Non-finite operands give NaN for the affected
  * projector / band.  Needs an sm_100 device (tcgen05).
  * QE_HPSI_PROJ_CERTIFY (with QE_HPSI_PROJ_INT8) adds an a-posteriori check of every int8 result and the automatic
