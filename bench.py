@@ -459,7 +459,7 @@ def int8_roofline(leg, stage, m, mp, hbm_peak, dmma, args, value, world):
     tkey = (("k_oz_gemm_a8_sym" if a8_is_top else "k_oz_gemm_a6_sym") if gsym else
             (("k_oz_vnl3" if m3 == 2 else "k_oz_gemm_a8") if a8_is_top else ("k_oz_gemm_a6_3m" if m3 else "k_oz_gemm_a6")))
     roofline = {"bound": "tensor", "kernel": kname, "achieved": ach, "peak": peak, "unit": "TOP/s", "frac": ach / peak,
-                "traffic": committed_traffic(args.config, tkey) if oz_s == 6 else None,
+                "traffic": committed_traffic(args.config, tkey) if oz_s == 6 else (committed_traffic(args.config, tkey + "_s7") if oz_s == 7 and gsym else None),
                 "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; the "
                 "kernel runs inside a long, power-capped step). Against the chip's measured int8 burst (register-free UTCIMMA loop, "
                 "4540 TOP/s, profiles/r1g_int8.md) the same kernel is at " + f"{ach / 4540.0:.2f}" + "; ncu (profiles/r2g_capture.md): tensor pipe 36-50 % active", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
