@@ -205,7 +205,7 @@ int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const v
  * qe_hpsi_precond: r[b][G] /= (1 + x + sqrt(1 + (x-1)^2)) / 2, x = hdiag[G] - e[b] sdiag[G]; e_dev [nb] on the device,
  *                  sdiag_dev NULL means 1.
  * qe_hpsi_rotate:  y[k][G] (+)= sum_j coef[k][j] x[j][G], k < ny, j < nx, over the npw sphere entries; coef_dev complex128
- *                  [ny][ldcoef], ldcoef >= nx; accumulate = 0 overwrites y[k][0..npw).  Runs the DMMA kernel of step a8.
+ *                  [ny][ldcoef], ldcoef >= nx; accumulate = 0 overwrites y[k][0..npw) (store-only epilogue: y is not read).  Runs the DMMA kernel of step a8.
  *                  All arguments are validated before anything is written.
  * qe_hpsi_residual: r[b][G] = hx[b][G] - e[b] sx[b][G] for G < npw (r may be hx or sx), and rnorm2[b] = sum_G |r[b][G]|^2
  *                  (rnorm2_dev [nb] FP64 on the device, may be NULL; fixed summation order, bit-reproducible).

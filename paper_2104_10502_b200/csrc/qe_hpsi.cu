@@ -603,6 +603,8 @@ cudaError_t set_kernel_attrs() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_becp<ZgS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_vnl_add<ZgS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
 #undef SET_SMEM
   if (dev >= 0 && dev < MAX_DEVICES) g_attr_done[dev] = true;
   return cudaSuccess;
@@ -1757,10 +1759,13 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     OZ_DISPATCH(h->oz_s, OZ_CALL)
 #undef OZ_CALL
   } else if (h->gamma) {
-    using Cfg = ZgV0;
-    const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
-    k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
-                                                                                 h->npw, h->kchunk, h->partial, h->ldc);
+    auto go = [&](auto cfg) {
+      using Cfg = decltype(cfg);
+      const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+      k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
+                                                                                   h->npw, h->kchunk, h->partial, h->ldc);
+    };
+    if (nb > 64) go(ZgS{}); else go(ZgV0{});  // 64 x 128 tiles from 65 bands on (same sums in the same order: same bits)
   } else if (h->sym) {
     // Gamma-symmetric projector mode: psi = u + i v as 2 nb real-wavefunction columns over the leading sym_m sphere entries
     sym::k_sym_merge<<<dim3((h->sym_m + 255) / 256, nb), 256, 0, st>>>(psi, ldpsi, h->sym_m, h->sym_minus, h->sym_u, h->sym_ldu);
@@ -1821,11 +1826,14 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
 #undef OZ_CALL
     prof_span(h, ts, prof_mark(h, st), SLOT_VNL);
   } else if (h->gamma) {
-    using Cfg = ZgV0;
-    const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
-    if (mt > 0)
-      k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
-                                                                                h->ldp, nb, hpsi, ldh);
+    auto go = [&](auto cfg) {
+      using Cfg = decltype(cfg);
+      const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+      if (mt > 0)
+        k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
+                                                                                  h->ldp, nb, hpsi, ldh);
+    };
+    if (nb > 64) go(ZgS{}); else go(ZgV0{});
   } else if (use_sym) {
     // symmetric a8: X = sum_p b_p Re e_p, Y = sum_p b_p Im e_p over the half sphere; hpsi(G) += X + iY, hpsi(-G) += conj X + i conj Y
     auto go = [&](auto cfg) {
@@ -2096,7 +2104,7 @@ extern "C" int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int n
   if (nx > 0 && (!x_dev || !coef_dev || ldx < h->npw || ldcoef < nx)) return QE_HPSI_EINVAL;  // before anything is written
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double2* y = static_cast<double2*>(y_dev);
-  if (!accumulate)
+  if (!accumulate && nx == 0)
     CU_TRY(h, cudaMemset2DAsync(y, sizeof(double2) * (size_t)ldy, 0, sizeof(double2) * (size_t)h->npw, (size_t)ny, st));
   if (nx == 0) return QE_HPSI_OK;
   using Cfg = ZgV0;
@@ -2104,7 +2112,7 @@ extern "C" int qe_hpsi_rotate(qe_hpsi_t h, const void* x_dev, int64_t ldx, int n
   // y[k][g] += sum_j x[j][g] coef[k][j]: the a8 kernel with A = x (M-contiguous) and B = coef (K-contiguous)
   k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(static_cast<const double2*>(x_dev), ldx, nx, h->npw,
                                                                     static_cast<const double2*>(coef_dev), (int)ldcoef, ny, y,
-                                                                    ldy);
+                                                                    ldy, nullptr, nullptr, nullptr, accumulate ? 0 : 1);
   CU_TRY(h, cudaGetLastError());
   return QE_HPSI_OK;
 }

@@ -340,7 +340,8 @@ template <class Cfg, bool GAMMA = false, bool SYM = false>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_add(const double2* __restrict__ beta, long long ldb, int nproj, int npw, const double2* __restrict__ dbT,
               int ldp, int nb, double2* __restrict__ hpsi, long long ldh, const int* __restrict__ nb_dev = nullptr,
-              const unsigned* __restrict__ cmask = nullptr, const int* __restrict__ minus = nullptr) {
+              const unsigned* __restrict__ cmask = nullptr, const int* __restrict__ minus = nullptr, int overwrite = 0) {
+  // overwrite != 0 (general form only; qe_hpsi_rotate without accumulation): hpsi = product, nothing is read in the epilogue
   static_assert(!SYM || GAMMA, "the symmetric mode is a real form");
   static_assert(!SYM || Cfg::BK == 16, "cmask holds one 16-bit class mask per K tile of 16 projectors");
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
@@ -504,7 +505,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           const int b = n0 + wn0 + j * 8 + 2 * fk + e;
-          v[j][e] = b < nb ? hpsi[(size_t)b * ldh + gg] : make_double2(0.0, 0.0);
+          v[j][e] = (b < nb && !overwrite) ? hpsi[(size_t)b * ldh + gg] : make_double2(0.0, 0.0);
         }
 #pragma unroll
       for (int j = 0; j < TN; ++j)
