@@ -159,6 +159,95 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
 }
 
 
+// NEXT-4 (charge density) with the same staging: inverse FFT along i1 as the first half of k2t_x_vmul, the tile of W2
+// arriving by one TMA load per band (double-buffered: two input stages, loads issued one band ahead), then
+// rho[i1][i2][i3] += scale * sum_b occ[b] |psi_b(r)|^2.  One CTA owns its (i2, i3 tile) pencils for all bands of the launch
+// (gridDim.y must be 1): no atomics, bands summed in order, bit-reproducible.  Shared memory: fft2t_smem(n, P, true, true) + one stage.
+inline size_t fft2t_smem_rho(int n, int P) {
+  return (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)(P + 1) * FFT_C * sizeof(double2) + 16 * 17 * sizeof(double2) + 64;
+}
+template <int RA, int RB>
+__global__ void __launch_bounds__(RA* FFT_C, 3)
+k2t_x_rho(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb, const double* __restrict__ occ, double scale,
+          double* __restrict__ rho) {
+  static_assert(RB > 1 && RA >= RB && RA <= 16, "two-pass lengths with a [RA][RA+1] twiddle table");
+  constexpr int N = RA * RB, NT = RA * FFT_C, NW = (NT + 31) / 32, TWP = RA + 1;
+  constexpr unsigned ROWB = FFT_C * sizeof(double2);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double2* tile1 = reinterpret_cast<double2*>(smem_raw);
+  const int P = g.P;
+  double2* inb0 = tile1 + N * FFT_C;                   // two input stages of P + 1 rows (row P: zeros)
+  double2* inb1 = inb0 + (size_t)(P + 1) * FFT_C;
+  double2* twt = inb1 + (size_t)(P + 1) * FFT_C;
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(twt + RA * TWP);  // two mbarriers
+  const int tid = threadIdx.x, c = tid & (FFT_C - 1), j = tid / FFT_C;
+  const bool io_thread = tid == (NW - 1) * 32;
+  const int i2 = blockIdx.x / g.ntz;
+  const int z0 = (blockIdx.x - i2 * g.ntz) * FFT_C;
+  for (int idx = tid; idx < RA * RA; idx += NT) {
+    const int jj = idx / RA, q = idx - jj * RA;
+    twt[jj * TWP + q] = __ldg(&g.ax1.tw[(q * jj) % N]);
+  }
+  if (tid < 2 * FFT_C) (tid < FFT_C ? inb0 : inb1)[(size_t)P * FFT_C + (tid & (FFT_C - 1))] = make_double2(0.0, 0.0);
+  const int xhi = t.x_hi, xlo0 = N - t.x_lo, xsh = N - P;
+  const double2* twj = twt + j * TWP;
+  if (tid == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int cx = (i2 * g.ldz + z0) * 2;
+  auto issue_load = [&](int b) {
+    mbar_expect_tx(&full[b & 1], (unsigned)P * ROWB);
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     smem_u32((b & 1) ? inb1 : inb0)),
+                 "l"(&tmap), "r"(cx), "r"(0), "r"(b), "r"(smem_u32(&full[b & 1]))
+                 : "memory");
+  };
+  if (io_thread) {
+    if (nb > 0) issue_load(0);
+    if (nb > 1) issue_load(1);
+  }
+  double acc[RB];
+#pragma unroll
+  for (int q = 0; q < RB; ++q) acc[q] = 0.0;
+  for (int b = 0; b < nb; ++b) {
+    const double f = __ldg(&occ[b]);
+    if (j < RB) {
+      mbar_wait(&full[b & 1], (unsigned)(b >> 1) & 1u);
+      double2 v[RA];
+      const double2* in = ((b & 1) ? inb1 : inb0) + c;
+#pragma unroll
+      for (int q = 0; q < RA; ++q) {
+        const int i1 = j + q * RB;
+        const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
+        v[q] = in[p * FFT_C];
+      }
+      pass_a_store<RA, +1>(v, tile1, j, c);
+    }
+    __syncthreads();  // tile complete; the input stage of band b has been read by everybody
+    if (io_thread && b + 2 < nb) issue_load(b + 2);
+    double2 u[RB];
+#pragma unroll
+    for (int q = 0; q < RB; ++q) u[q] = tile1[fft_phys(j + q * RA, c)];
+#pragma unroll
+    for (int q = 1; q < RB; ++q) u[q] = cmul(u[q], twj[q]);
+    Dft<RB, +1>::run(u);
+#pragma unroll
+    for (int q = 0; q < RB; ++q) acc[q] += f * (u[q].x * u[q].x + u[q].y * u[q].y);
+    __syncthreads();  // the next band's first pass overwrites tile1
+  }
+  const int z = z0 + c;
+  if (z < g.n3) {
+#pragma unroll
+    for (int q = 0; q < RB; ++q) {
+      double* r = rho + ((size_t)(j + q * RA) * g.n2 + i2) * g.n3 + z;
+      *r += scale * acc[q];
+    }
+  }
+}
+
 // three-pass variant (lengths of fft3p_kernels.cuh): same staging, arithmetic of k3p_x_vmul
 template <int R1, int R2, int R3>
 __global__ void __launch_bounds__(P3<R1, R2, R3>::NT) k3t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap,
@@ -397,13 +486,15 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_zfwd_gather(FftGeom g, Fft2pGeo
 
 using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, int);
 
+using K2tRho = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, const double*, double, double*);
 struct Fft2tEntry {
   int n, ra, rb;
+  K2tRho rho;    // TMA-staged density kernel (two-pass lengths only)
   K2tX x;
   K2pZinv zinv;  // bulk-staged z stages (two-pass lengths only; null for the three-pass table)
   K2pZfwd zfwd;
 };
-#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
+#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_rho<RA, RB>, k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
 static const Fft2tEntry kFft2tTable[] = {
     QE_FFT2T_ENTRY(6, 3),   QE_FFT2T_ENTRY(5, 4),   QE_FFT2T_ENTRY(6, 6),   QE_FFT2T_ENTRY(8, 6),   QE_FFT2T_ENTRY(8, 8),
     QE_FFT2T_ENTRY(9, 8),   QE_FFT2T_ENTRY(10, 8),  QE_FFT2T_ENTRY(12, 8),  QE_FFT2T_ENTRY(10, 10), QE_FFT2T_ENTRY(12, 9),
@@ -412,7 +503,7 @@ static const Fft2tEntry kFft2tTable[] = {
 };
 #undef QE_FFT2T_ENTRY
 // three-pass lengths: ra = R1, rb = R2*R3 as in kFft3pTable
-#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
+#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), nullptr, k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
 static const Fft2tEntry kFft3tTable[] = {
     QE_FFT3T_ENTRY(5, 5, 5),  QE_FFT3T_ENTRY(6, 5, 5),  QE_FFT3T_ENTRY(8, 5, 5),  QE_FFT3T_ENTRY(6, 6, 6), QE_FFT3T_ENTRY(10, 5, 5),
     QE_FFT3T_ENTRY(8, 6, 6),  QE_FFT3T_ENTRY(10, 6, 5), QE_FFT3T_ENTRY(8, 8, 5),  QE_FFT3T_ENTRY(10, 6, 6), QE_FFT3T_ENTRY(8, 8, 6),

@@ -81,6 +81,8 @@ struct qe_hpsi_handle {
   size_t smem_x2p = 0;
   // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
   K2tX x_tma = nullptr;
+  K2tRho rho_tma = nullptr;  // TMA-staged density kernel (needs the unswizzled tensor map of x_tma)
+  size_t smem_rho = 0;
   int x_one_tile = 0;  // two-pass x stage with one shared tile (tuning knob QE_HPSI_X_ONE_TILE)
   K2pZinv z_tma_inv = nullptr;  // bulk-staged a1 / a5 (fft2t_kernels.cuh)
   K2pZfwd z_tma_fwd = nullptr;
@@ -1590,6 +1592,12 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
             cudaFuncSetAttribute((const void*)et->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess) {
           h->x_tma = et->x;
           h->smem_xt = sm;
+          const size_t smr = fft2t_smem_rho(nr[0], h->P);
+          if (et->rho && smr <= (size_t)110 * 1024 &&
+              cudaFuncSetAttribute((const void*)et->rho, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr) == cudaSuccess) {
+            h->rho_tma = et->rho;
+            h->smem_rho = smr;
+          }
         }
       }
       (void)cudaGetLastError();  // a failed probe falls back to k2p_x_vmul
@@ -2189,7 +2197,10 @@ extern "C" int qe_hpsi_density(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, 
       else
         ez->zinv<<<dim3(zt, n), ez->nthreads, ez->smem_zy, st>>>(g, h->g2p, p, ldpsi, h->w1);
       ey->yinv<<<dim3(yt, n), ey->nthreads, ey->smem_zy, st>>>(g, h->g2p, h->w1, h->w2);
-      ex->rho<<<dim3(xt, 1), ex->nthreads, ex->smem_x, st>>>(g, h->g2p, h->w2, n, occ_dev + b0, scale, rho_dev);
+      if (h->rho_tma)
+        h->rho_tma<<<dim3(xt, 1), ex->nthreads, h->smem_rho, st>>>(g, h->g2p, h->tmap_w2, n, occ_dev + b0, scale, rho_dev);
+      else
+        ex->rho<<<dim3(xt, 1), ex->nthreads, ex->smem_x, st>>>(g, h->g2p, h->w2, n, occ_dev + b0, scale, rho_dev);
     } else {
       k_scatter_zinv<<<dim3(zt, n), FFT_NT, h->smem_z, st>>>(g, p, ldpsi, h->w1);
       k_yinv<<<dim3(yt, n), FFT_NT, h->smem_y, st>>>(g, h->w1, h->w2);

@@ -136,14 +136,14 @@ def test_density_against_oracle(cfg, flags):
     h.destroy()
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 4])
-def test_density_full_size_properties_and_sampled_points(cfg):
+@pytest.mark.parametrize("cfg,nb", [(1, 1), (1, 2), (1, 3), (1, 8), (2, 8), (4, 8)])
+def test_density_full_size_properties_and_sampled_points(cfg, nb):
     """Full-size configs: Parseval (mean of rho = scale * sum occ |c|^2) and sampled grid points evaluated one by
-    one from the definition psi(r) = sum_G c(G) exp(2 pi i n.i/N)."""
+    one from the definition psi(r) = sum_G c(G) exp(2 pi i n.i/N).  nb = 1, 2, 3: start-up and drain of the two-stage
+    band pipeline of the TMA-staged kernel."""
     h, inp = _gpu.make(cfg, flags=qe_hpsi.QE_HPSI_BORROW_BETA)
     wl = inp["wl"]
     npw = h.npw
-    nb = 8
     psi = _gpu.gen_psi_dev(inp, 0, nb)
     occ = torch.linspace(2.0, 1.0, nb, dtype=torch.float64, device="cuda")
     rho = torch.zeros(tuple(wl.nr), dtype=torch.float64, device="cuda")
