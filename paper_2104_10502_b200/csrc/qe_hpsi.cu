@@ -34,16 +34,7 @@ constexpr int NUM_SMS_FALLBACK = 148;
 // ZGEMM tile configurations (see zgemm_kernels.cuh): BM, BN, warps along M, warps along N, BK, pipeline stages.
 // Variant 0 is the product default; the others exist for tuning runs (env QE_HPSI_ZG_VARIANT).
 using ZgV0 = ZgCfg<64, 64, 2, 4, 16, 4>;
-using ZgV1 = ZgCfg<64, 64, 4, 4, 16, 4>;
-using ZgV2 = ZgCfg<128, 32, 4, 2, 16, 4>;
-using ZgV3 = ZgCfg<64, 64, 2, 4, 8, 6>;
-using ZgV4 = ZgCfg<64, 64, 2, 4, 32, 3>;
-using ZgV5 = ZgCfg<64, 64, 2, 4, 16, 6>;
 using ZgS = ZgCfg<64, 128, 2, 4, 16, 4>;  // real forms of the Gamma-symmetric mode: 2 nb columns, 4 x 4 blocks per warp
-constexpr int ZG_NVARIANT = 6;
-constexpr int ZG_BM_TAB[ZG_NVARIANT] = {64, 64, 128, 64, 64, 64};
-constexpr int ZG_BN_TAB[ZG_NVARIANT] = {64, 64, 32, 64, 64, 64};
-constexpr int ZG_BK_TAB[ZG_NVARIANT] = {16, 16, 16, 8, 32, 16};
 
 struct DevBuf {
   void* p = nullptr;
@@ -100,7 +91,6 @@ struct qe_hpsi_handle {
   int max_batch = 0;
   int ldc = 0, ldp = 0;
   int nsplit = 1, kchunk = 0;
-  int zg_variant = 0;
   double2 *partial = nullptr, *becp = nullptr, *dbecp = nullptr, *dbT = nullptr;
   // projector contractions on tcgen05 int8 slices (ozaki_kernels.cuh): oz_s = slices per FP64 operand, 0 = FP64 DMMA path
   int oz_s = 0, oz_stages = 0, oz_nsplit = 1, oz_kchunk = 0, oz_kchunk2 = 0;  // K blocks per CTA of a6 / per launch of a8
@@ -583,29 +573,19 @@ cudaError_t set_kernel_attrs() {
   SET_SMEM(k_x_rho);
   SET_SMEM(k_yfwd);
   SET_SMEM(k_zfwd_gather);
-  SET_SMEM(k_becp<ZgV0>);
-  SET_SMEM(k_vnl_add<ZgV0>);
-  SET_SMEM(k_becp<ZgV1>);
-  SET_SMEM(k_vnl_add<ZgV1>);
-  SET_SMEM(k_becp<ZgV2>);
-  SET_SMEM(k_vnl_add<ZgV2>);
-  SET_SMEM(k_becp<ZgV3>);
-  SET_SMEM(k_vnl_add<ZgV3>);
-  SET_SMEM(k_becp<ZgV4>);
-  SET_SMEM(k_vnl_add<ZgV4>);
-  SET_SMEM(k_becp<ZgV5>);
-  SET_SMEM(k_vnl_add<ZgV5>);
-  e = cudaFuncSetAttribute(k_becp<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  // the DMMA kernels keep their mbarriers in static shared memory: ask for what the tile pipeline needs, not for the device maximum
+#define SET_ZG(Cfg, ...)                                                                                                 \
+  e = cudaFuncSetAttribute(k_becp<Cfg, ##__VA_ARGS__>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BECP); \
+  if (e != cudaSuccess) return e;                                                                                        \
+  e = cudaFuncSetAttribute(k_vnl_add<Cfg, ##__VA_ARGS__>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_VNL); \
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  SET_ZG(ZgV0);
+  SET_ZG(ZgV0, true);
+  SET_ZG(ZgS, true);
+#undef SET_ZG
+  e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgV0::SMEM_VNL);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_vnl_add<ZgS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_becp<ZgS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_vnl_add<ZgS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  e = cudaFuncSetAttribute(k_vnl_add<ZgS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_VNL);
   if (e != cudaSuccess) return e;
 #undef SET_SMEM
   if (dev >= 0 && dev < MAX_DEVICES) g_attr_done[dev] = true;
@@ -771,7 +751,7 @@ int env_int(const char* name, int dflt) {
 
 // choose the split-K count of a6 so that (M tiles x N tiles x nsplit) fills whole waves of CTAs
 void choose_split(qe_hpsi_handle* h) {
-  const int ZG_BM = ZG_BM_TAB[h->zg_variant], ZG_BN = ZG_BN_TAB[h->zg_variant], ZG_BK = ZG_BK_TAB[h->zg_variant];
+  constexpr int ZG_BM = ZgV0::BM, ZG_BN = ZgV0::BN, ZG_BK = ZgV0::BK;
   const int ntile = ((h->nproj + ZG_BM - 1) / ZG_BM) * ((h->max_batch + ZG_BN - 1) / ZG_BN);
   // slices of at least 512 plane waves, unless that cannot even fill two waves (few projectors, small sphere): then 128
   int ksmax = std::max(1, h->npw / 512);
@@ -819,24 +799,10 @@ void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, in
 // a6 on the FP64 tensor path (complex handles): split-K partials of conj(beta) psi.  nb_dev != nullptr: the band count is
 // min(nb, *nb_dev), read on the device (re-computation pass of QE_HPSI_PROJ_CERTIFY)
 void becp_fp64(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st, double2* partial, const int* nb_dev) {
-  switch (h->zg_variant) {
-    case 1: becp_launch<ZgV1>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-    case 2: becp_launch<ZgV2>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-    case 3: becp_launch<ZgV3>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-    case 4: becp_launch<ZgV4>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-    case 5: becp_launch<ZgV5>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-    default: becp_launch<ZgV0>(h, psi, ldpsi, nb, st, partial, nb_dev); break;
-  }
+  becp_launch<ZgV0>(h, psi, ldpsi, nb, st, partial, nb_dev);
 }
 void vnl_fp64(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
-  switch (h->zg_variant) {
-    case 1: vnl_launch<ZgV1>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-    case 2: vnl_launch<ZgV2>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-    case 3: vnl_launch<ZgV3>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-    case 4: vnl_launch<ZgV4>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-    case 5: vnl_launch<ZgV5>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-    default: vnl_launch<ZgV0>(h, bT, hpsi, ldh, nb, st, nb_dev); break;
-  }
+  vnl_launch<ZgV0>(h, bT, hpsi, ldh, nb, st, nb_dev);
 }
 // a6-a8 entirely on the FP64 tensor path of a complex handle: out[b] += V_NL psi[b] (used by the certified path's
 // re-computation and, at create, for its probe images)
@@ -1133,11 +1099,10 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
     CR_TRY(upload(&h->dpk, dv, st));
     h->ldc = (max_batch + 1) / 2 * 2;
     h->ldp = (nproj + 7) / 8 * 8;
-    h->zg_variant = std::min(std::max(env_int("QE_HPSI_ZG_VARIANT", 0), 0), ZG_NVARIANT - 1);
     choose_split(h);
     const int forced = env_int("QE_HPSI_NSPLIT", 0);
     if (forced > 0) {
-      const int ZG_BK = ZG_BK_TAB[h->zg_variant];
+      constexpr int ZG_BK = ZgV0::BK;
       int kchunk = (h->npw + forced - 1) / forced;
       kchunk = std::max(ZG_BK, (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK);
       h->kchunk = kchunk;

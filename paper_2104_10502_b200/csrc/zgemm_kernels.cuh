@@ -34,6 +34,41 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N));
 }
 
+// mbarrier pipeline of the DMMA kernels: every stage has a `full` barrier (all NT threads arrive through
+// cp.async.mbarrier.arrive.noinc once their own copies of the stage have landed) and an `empty` barrier (one arrive per warp
+// after its last fragment load of the stage).  No CTA-wide barrier in the K loop: a warp waits for DATA only, and may run up to
+// NSTAGE - 2 tiles ahead of the slowest one (the refill of a stage is issued two tiles after the stage was consumed).  Against
+// __syncthreads per tile: 0.83 -> 0.90 of the DMMA peak on the symmetric a8 kernel, same bits (profiles/r2j_dmma_pipeline.md).
+__device__ __forceinline__ void mb_init(unsigned bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mb_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tMBW_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra MBW_%=;\n\t}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mb_arrive(unsigned bar) {
+  asm volatile("{\n\t.reg .b64 t;\n\tmbarrier.arrive.shared::cta.b64 t, [%0];\n\t}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mb_cp_arrive(unsigned bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+// full[s] at mb0 + 8 s, empty[s] at mb0 + 8 (NSTAGE + s); ends with a CTA barrier
+template <int NSTAGE, int NT>
+__device__ __forceinline__ unsigned mb_setup(unsigned long long* mbar) {
+  const unsigned mb0 = static_cast<unsigned>(__cvta_generic_to_shared(mbar));
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NSTAGE; ++s) {
+      mb_init(mb0 + 8 * s, NT);
+      mb_init(mb0 + 8 * (NSTAGE + s), NT / 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  return mb0;
+}
+
 // K-contiguous operand tile: rows of BK complex; 16-byte column kc of odd rows is XOR-ed with 4 so that a
 // fragment load (quarter warp = 2 rows x 4 k) touches 8 distinct 16-byte bank groups.
 template <int BK>
@@ -51,7 +86,8 @@ struct ZgCfg {
   static constexpr int LDA_M = BM + 2;  // row stride of an M-contiguous [k][m] tile: (2k + m) mod 8 distinct per quarter warp
   static constexpr size_t SMEM_BECP = (size_t)NSTAGE * (BM + BN) * BK * sizeof(double2);
   static constexpr size_t SMEM_VNL = (size_t)NSTAGE * (BK * LDA_M + BN * BK) * sizeof(double2);
-  static_assert(BM % (WM * 8) == 0 && BN % (WN * 8) == 0 && BK % 4 == 0 && BK >= 8, "tile shape");
+  static constexpr int DIST = NSTAGE - 2;  // tiles in flight ahead of the one being consumed (mbarrier pipeline above)
+  static_assert(BM % (WM * 8) == 0 && BN % (WN * 8) == 0 && BK % 4 == 0 && BK >= 8 && NSTAGE >= 3, "tile shape");
 };
 
 // one k4 step of the 3M product on a TM x TN grid of 8x8 blocks
@@ -116,6 +152,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     nb = min(nb, *nb_dev);
     if (n0 >= nb) return;
   }
+  __shared__ __align__(8) unsigned long long mbar[2 * NSTAGE];
+  const unsigned mb0 = mb_setup<NSTAGE, NT>(mbar);
   const int ks = blockIdx.y;
   const int kb = ks * kchunk, ke = min(npw, kb + kchunk);
   const int nkt = (ke - kb + BK - 1) / BK;
@@ -144,6 +182,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   }
   const unsigned cdst = static_cast<unsigned>(__cvta_generic_to_shared(sm + swz_k<BK>(cr0, ckc)));
   auto load_stage = [&](int kt, int st) {
+    if (kt >= NSTAGE) mb_wait(mb0 + 8 * (NSTAGE + st), ((kt / NSTAGE) - 1) & 1);  // every warp is done with the stage's last tile
     const int koff = kt * BK;
     const bool kok = (kb + koff + ckc) < ke;
     const unsigned d0 = cdst + (unsigned)(st * STAGE * (int)sizeof(double2));
@@ -159,6 +198,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d0 + (unsigned)((BM + n * RPT) * BK * 16)),
                    "l"(bsrc[n] + koff), "r"(sz));
     }
+    mb_cp_arrive(mb0 + 8 * st);
   };
 
   double P[TM][TN][2], Q[TM][TN][2], R[TM][TN][2];
@@ -170,10 +210,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
       for (int e = 0; e < 2; ++e) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
 
 #pragma unroll
-  for (int s = 0; s < NSTAGE - 1; ++s) {
+  for (int s = 0; s < Cfg::DIST; ++s)
     if (s < nkt) load_stage(s, s);
-    cp_async_commit();
-  }
   const int fr = lane >> 2, fk = lane & 3;
   // Gamma-symmetric projector mode (cls != nullptr, GAMMA form): rows of class 1 (beta(-G) = -conj beta(G)) enter as i*beta =
   // (-a_i, a_r), so that every row is Hermitian and the real form applies; the fragment is only swapped to (a_i, a_r) and the
@@ -184,10 +222,9 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     const int p = m0 + wm0 + i * 8 + fr;
     swp[i] = GAMMA && cls != nullptr && p < nproj && cls[p] != 0;
   }
-  int st_c = 0, st_l = NSTAGE - 1;  // stage being consumed / stage being refilled
+  int st_c = 0, st_l = Cfg::DIST;  // stage being consumed / stage being refilled
   for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
+    mb_wait(mb0 + 8 * st_c, (kt / NSTAGE) & 1);  // the tile has landed (copies of all threads)
     const double2* As = sm + st_c * STAGE;
     const double2* Bs = As + BM * BK;
     double2 af[2][TM], bf[2][TN];
@@ -210,15 +247,15 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
         mma2r<TM, TN, true>(P, Q, af[kk & 1], bf[kk & 1]);
       } else
         mma3m<TM, TN, true>(P, Q, R, af[kk & 1], bf[kk & 1]);
-      if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
-        if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
-        cp_async_commit();
+      if (kk == 0) {  // refill the stage consumed two tiles ago, behind the first batch of DMMAs
+        if (kt + Cfg::DIST < nkt) load_stage(kt + Cfg::DIST, st_l);
       }
     }
+    __syncwarp();
+    if (lane == 0) mb_arrive(mb0 + 8 * (NSTAGE + st_c));  // this warp has read the stage
     st_c = (st_c + 1 == NSTAGE) ? 0 : st_c + 1;
     st_l = (st_l + 1 == NSTAGE) ? 0 : st_l + 1;
   }
-  cp_async_wait<0>();
   // C fragment: row = lane/4, columns 2*(lane%4) + {0,1};  conj(a) b = (P + Q) + i (R - P + Q)
   double2* out = partial + (size_t)ks * nproj * ldc;
 #pragma unroll
@@ -359,6 +396,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     if (n0 >= nb) return;
   }
   const int nkt = (nproj + BK - 1) / BK;
+  __shared__ __align__(8) unsigned long long mbar[2 * NSTAGE];
+  const unsigned mb0 = mb_setup<NSTAGE, NT>(mbar);
 
   // Per-thread copy plan (see k_becp).  A tile [BK][LDA]: thread owns column gc of rows ra, ra+RPA, ...; B tile
   // [BN][BK]: column ckc of rows cr0, cr0+RPT, ...
@@ -381,6 +420,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   }
   const unsigned bdst = static_cast<unsigned>(__cvta_generic_to_shared(sm + BK * LDA + swz_k<BK>(cr0, ckc)));
   auto load_stage = [&](int kt, int st) {
+    if (kt >= NSTAGE) mb_wait(mb0 + 8 * (NSTAGE + st), ((kt / NSTAGE) - 1) & 1);  // every warp is done with the stage's last tile
     const int k0 = kt * BK;
     const unsigned soff = (unsigned)(st * STAGE * (int)sizeof(double2));
     const double2* ap = asrc + (size_t)k0 * ldb;
@@ -398,6 +438,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(bdst + soff + (unsigned)(n * RPT * BK * 16)),
                    "l"(bsrc[n] + k0), "r"(sz));
     }
+    mb_cp_arrive(mb0 + 8 * st);
   };
 
   double P[TM][TN][2], Q[TM][TN][2], R[TM][TN][2];
@@ -409,15 +450,12 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
       for (int e = 0; e < 2; ++e) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
 
 #pragma unroll
-  for (int s = 0; s < NSTAGE - 1; ++s) {
+  for (int s = 0; s < Cfg::DIST; ++s)
     if (s < nkt) load_stage(s, s);
-    cp_async_commit();
-  }
   const int fr = lane >> 2, fk = lane & 3;
-  int st_c = 0, st_l = NSTAGE - 1;  // stage being consumed / stage being refilled
+  int st_c = 0, st_l = Cfg::DIST;  // stage being consumed / stage being refilled
   for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
+    mb_wait(mb0 + 8 * st_c, (kt / NSTAGE) & 1);  // the tile has landed (copies of all threads)
     const double2* As = sm + st_c * STAGE;
     const double2* Bs = As + BK * LDA;
     double2 af[2][TM], bf[2][TN];
@@ -455,15 +493,15 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
           mma2r<TM, TN, false>(P, Q, af[kk & 1], bf[kk & 1]);
       } else
         mma3m<TM, TN, false>(P, Q, R, af[kk & 1], bf[kk & 1]);
-      if (kk == 0) {  // refill the stage freed by the barrier above, behind the first batch of DMMAs
-        if (kt + NSTAGE - 1 < nkt) load_stage(kt + NSTAGE - 1, st_l);
-        cp_async_commit();
+      if (kk == 0) {  // refill the stage consumed two tiles ago, behind the first batch of DMMAs
+        if (kt + Cfg::DIST < nkt) load_stage(kt + Cfg::DIST, st_l);
       }
     }
+    __syncwarp();
+    if (lane == 0) mb_arrive(mb0 + 8 * (NSTAGE + st_c));  // this warp has read the stage
     st_c = (st_c + 1 == NSTAGE) ? 0 : st_c + 1;
     st_l = (st_l + 1 == NSTAGE) ? 0 : st_l + 1;
   }
-  cp_async_wait<0>();
   if constexpr (SYM) {
     // columns 2 fk, 2 fk + 1 of an 8-column block are (X, Y) of one band: X = (P, Q)[0], Y = (P, Q)[1].
     // All loads of a row block are issued before its first store: the compiler cannot prove that hpsi[.][g] and hpsi[.][-g] do
