@@ -198,6 +198,21 @@ int qe_hpsi_apply_hs(qe_hpsi_t h, const void* psi_dev, int64_t ldpsi, void* hpsi
 int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb,
                     void* out_dev, int64_t ldo, void* cuda_stream);
 
+/* The same reduced matrix for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): no handle, and neither set-up nor call uses cudaMalloc / cudaFree or an allocating library routine.  The
+ * split-K partials live in ONE file-scope device array of 8 MiB (32 slices x 128 x 128 complex128) that every GPU loading the
+ * library holds until exit.  Limits: na, nb <= QE_HPSI_OVERLAP_STATIC_MAX, npw < 2^31 - 4096; anything beyond returns
+ * QE_HPSI_EINVAL and launches nothing.  a_dev [na][lda], b_dev [nb][ldb], out_dev [na][ldo] as for qe_hpsi_overlap, summed over the
+ * leading npw entries of the rows; same K slices, kernel and reduction order, hence the same bits as qe_hpsi_overlap on a handle
+ * with that npw.  Asynchronous on cuda_stream.  ALL calls on a device share the array (it keeps the last call's partials;
+ * nothing in it has to start at zero): calls that can overlap on the GPU -- different streams, or graph branches -- race; order
+ * them.  qe_hpsi_overlap_static_init does the once-per-device set-up (device address of the array, kernel attributes) for the
+ * CURRENT device; the call does it on first use, so call init before a stream capture begins. */
+#define QE_HPSI_OVERLAP_STATIC_MAX 128
+int qe_hpsi_overlap_static_init(void);
+int qe_hpsi_overlap_static(const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb, int64_t npw,
+                           void* out_dev, int64_t ldo, void* cuda_stream);
+
 /* NEXT-3, the rest of the Davidson step:
  * qe_hpsi_hdiag:   hdiag[G] = |k+G|^2 + vbar + sum_p D_pp |beta_p(G)|^2  (vbar = mean of V(r), supplied by the caller)
  *                  sdiag[G] = 1 + sum_p q_pp |beta_p(G)|^2              (needs qe_hpsi_set_s when there are projectors)

@@ -2037,6 +2037,76 @@ extern "C" int qe_hpsi_overlap(qe_hpsi_t h, const void* a_dev, int64_t lda, int 
   return QE_HPSI_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// qe_hpsi_overlap_static: the same reduced matrix without a handle and without any allocation (qe_hpsi.h).  The split-K
+// partials live in a file-scope device array that every GPU loading the library holds until exit.
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+constexpr int OVS_MAX_N = QE_HPSI_OVERLAP_STATIC_MAX;  // rows and columns of one call
+constexpr int OVS_MAX_SPLIT = 32, OVS_LDC = 128;
+static __device__ __align__(256) double2 g_ovs_scratch[(size_t)OVS_MAX_SPLIT * OVS_MAX_N * OVS_LDC];  // 8 MiB
+// In host code g_ovs_scratch is only a stand-in for the symbol: the device address is asked for once per device, with that
+// device current, and that pointer is what the kernels get
+double2* g_ovs_ptr[MAX_DEVICES] = {};
+std::mutex g_ovs_mutex;
+int ovs_setup(double2** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess && (dev < 0 || dev >= MAX_DEVICES)) return QE_HPSI_EINVAL;
+  if (e == cudaSuccess) e = set_kernel_attrs();  // per device, allocates nothing
+  if (e == cudaSuccess) {
+    std::lock_guard<std::mutex> lock(g_ovs_mutex);
+    if (!g_ovs_ptr[dev]) {
+      double2* ptr = nullptr;
+      e = cudaGetSymbolAddress((void**)&ptr, g_ovs_scratch);
+      if (e == cudaSuccess) g_ovs_ptr[dev] = ptr;
+    }
+    if (e == cudaSuccess) *out = g_ovs_ptr[dev];
+  }
+  if (e != cudaSuccess) {
+    g_last_cuda = (int)e;
+    return QE_HPSI_ECUDA;
+  }
+  return QE_HPSI_OK;
+}
+}  // namespace
+
+extern "C" int qe_hpsi_overlap_static_init(void) {
+  double2* ptr = nullptr;
+  return ovs_setup(&ptr);
+}
+
+extern "C" int qe_hpsi_overlap_static(const void* a_dev, int64_t lda, int na, const void* b_dev, int64_t ldb, int nb, int64_t npw,
+                                      void* out_dev, int64_t ldo, void* cuda_stream) {
+  if (na < 0 || nb < 0 || npw < 0) return QE_HPSI_EINVAL;
+  if (na > OVS_MAX_N || nb > OVS_MAX_N || npw > (int64_t)INT32_MAX - 4096) return QE_HPSI_EINVAL;  // beyond the static scratch
+  if (na == 0 || nb == 0) return QE_HPSI_OK;
+  if (!a_dev || !b_dev || !out_dev || lda < npw || ldb < npw || ldo < nb) return QE_HPSI_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double2* out = static_cast<double2*>(out_dev);
+  qe_hpsi_handle* h = nullptr;
+  if (npw == 0) {
+    CU_TRY(h, cudaMemset2DAsync(out, sizeof(double2) * (size_t)ldo, 0, sizeof(double2) * (size_t)nb, (size_t)na, st));
+    return QE_HPSI_OK;
+  }
+  double2* scratch = nullptr;
+  const int rc = ovs_setup(&scratch);
+  if (rc != QE_HPSI_OK) return rc;
+  // the K slices of qe_hpsi_overlap (a function of npw only): the two entry points give the same bits
+  const int ns0 = std::max(1, std::min(OVS_MAX_SPLIT, (int)(npw / 2048)));
+  int kchunk = (int)((npw + ns0 - 1) / ns0);
+  kchunk = std::max(ZgV0::BK, (kchunk + ZgV0::BK - 1) / ZgV0::BK * ZgV0::BK);
+  const int ns = std::max(1, (int)((npw + kchunk - 1) / kchunk));
+  const int mt = (na + ZgV0::BM - 1) / ZgV0::BM, nt = (nb + ZgV0::BN - 1) / ZgV0::BN;
+  // every partial the reduction reads is written by this call's k_becp (slices are never empty), so nothing has to be cleared
+  k_becp<ZgV0><<<dim3(mt * nt, ns), ZgV0::NT, ZgV0::SMEM_BECP, st>>>(static_cast<const double2*>(a_dev), lda, na,
+                                                                     static_cast<const double2*>(b_dev), ldb, nb, (int)npw, kchunk,
+                                                                     scratch, OVS_LDC);
+  k_ovl_reduce<<<dim3((nb + 127) / 128, na), 128, 0, st>>>(scratch, ns, na, OVS_LDC, nb, out, ldo);
+  CU_TRY(h, cudaGetLastError());
+  return QE_HPSI_OK;
+}
+
 // NEXT-3, rest of the Davidson step: preconditioner diagonals, preconditioner, basis rotation (a8's kernel)
 extern "C" int qe_hpsi_hdiag(qe_hpsi_t h, double vbar, double* hdiag_dev, double* sdiag_dev, void* cuda_stream) {
   if (!h) return QE_HPSI_ESTATE;

@@ -71,6 +71,8 @@ SIGNATURES = {
     "qe_hpsi_set_s": (_i32, [_vp, _pd]),
     "qe_hpsi_apply_hs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i64, _i32, _vp]),
     "qe_hpsi_overlap": (_i32, [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _vp, _i64, _vp]),
+    "qe_hpsi_overlap_static_init": (_i32, []),
+    "qe_hpsi_overlap_static": (_i32, [_vp, _i64, _i32, _vp, _i64, _i32, _i64, _vp, _i64, _vp]),
     "qe_hpsi_density": (_i32, [_vp, _vp, _i64, _i32, _vp, _dbl, _vp, _vp]),
     "qe_hpsi_hdiag": (_i32, [_vp, _dbl, _vp, _vp, _vp]),
     "qe_hpsi_precond": (_i32, [_vp, _vp, _i64, _i32, _vp, _vp, _vp, _vp]),
@@ -156,6 +158,29 @@ def qe_hpsi_test_set_int8_kmax(kmax: int):
 def qe_hpsi_test_set_sym_min(entries: int):
     """(qe_hpsi_test.h) smallest nproj * npw that takes the Gamma-symmetric projector mode; negative = default (2^20), 0 = always."""
     _check(load_library().qe_hpsi_test_set_sym_min(int(entries)))
+
+
+QE_HPSI_OVERLAP_STATIC_MAX = 128
+
+
+def qe_hpsi_overlap_static_init():
+    """Once-per-device set-up of qe_hpsi_overlap_static for the current device (allocates nothing)."""
+    _check(load_library().qe_hpsi_overlap_static_init())
+
+
+def qe_hpsi_overlap_static(a, b, npw, out, stream=None):
+    """qe_hpsi_overlap_static: out[i][j] = <a_i|b_j> over the leading npw entries, without a handle and without any
+    allocation (split-K partials in the library's static device array; na, nb <= QE_HPSI_OVERLAP_STATIC_MAX; calls
+    that overlap on the GPU race).  The caller passes `out` ([na, >= nb] complex128 on the device)."""
+    for t in (a, b, out):
+        assert t.is_cuda and t.dtype == torch.complex128 and t.dim() == 2 and t.stride(1) == 1
+    na, nb = int(a.shape[0]), int(b.shape[0])
+    lda = int(a.stride(0)) if na > 1 else int(a.shape[1])
+    ldb = int(b.stride(0)) if nb > 1 else int(b.shape[1])
+    ldo = int(out.stride(0)) if na > 1 else int(out.shape[1])
+    _check(load_library().qe_hpsi_overlap_static(_vp(a.data_ptr()), lda, na, _vp(b.data_ptr()), ldb, nb, int(npw),
+                                                 _vp(out.data_ptr()), ldo, _stream_ptr(stream)))
+    return out
 
 
 def qe_hpsi_probe_fp64(millis=200.0):
