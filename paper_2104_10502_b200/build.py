@@ -12,7 +12,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libqe_hpsi.so")
 SOURCES = ["qe_hpsi.cu"]
-HEADERS = ["fft_core.cuh", "fft_kernels.cuh", "fft2p_kernels.cuh", "fft3p_kernels.cuh", "fft2t_kernels.cuh", "zgemm_kernels.cuh", "ozaki_kernels.cuh", "cert_kernels.cuh",
+HEADERS = ["fft_core.cuh", "fft_kernels.cuh", "fft2p_kernels.cuh", "fft3p_kernels.cuh", "fft2t_kernels.cuh", "zgemm_kernels.cuh", "zgemm_tma_kernels.cuh", "ozaki_kernels.cuh", "cert_kernels.cuh",
            os.path.join("..", "..", "include", "qe_hpsi.h"), os.path.join("..", "..", "include", "qe_hpsi_test.h")]
 
 NVCC_FLAGS = [

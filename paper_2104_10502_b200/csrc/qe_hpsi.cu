@@ -20,6 +20,7 @@
 #include "fft3p_kernels.cuh"
 #include "fft2t_kernels.cuh"
 #include "zgemm_kernels.cuh"
+#include "zgemm_tma_kernels.cuh"
 #include "ozaki_kernels.cuh"
 #include "cert_kernels.cuh"
 #include "sym_kernels.cuh"
@@ -121,6 +122,8 @@ struct qe_hpsi_handle {
   unsigned char* sym_cls = nullptr;   // [nproj] 0: beta(-G) = conj beta(G), 1: = -conj
   unsigned* sym_cmask = nullptr;      // [ceil(nproj / 16)] bit j: class of projector 16 t + j (K tiles of the symmetric a8)
   int sym_wide = 1;                   // 128-column tiles (ZgS) instead of ZgV0 (tuning knob QE_HPSI_SYM_WIDE)
+  bool sym_tma = false;               // operand tiles of the symmetric FP64 kernels by TMA (zgemm_tma_kernels.cuh; knob QE_HPSI_SYM_TMA)
+  CUtensorMap tm_a6_beta, tm_a6_u, tm_a8_beta, tm_a8_e;
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
   int sym_nsplit = 1, sym_ldc2 = 0;
@@ -583,6 +586,10 @@ cudaError_t set_kernel_attrs() {
   SET_ZG(ZgV0, true);
   SET_ZG(ZgS, true);
 #undef SET_ZG
+  e = cudaFuncSetAttribute(k_becp_sym_tma<ZgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_BECP + 1024);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_vnl_sym_tma<ZgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_VNL);
+  if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgV0::SMEM_VNL);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_vnl_add<ZgS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_VNL);
@@ -1171,6 +1178,29 @@ cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
   return cudaSuccess;
 }
 
+// FP64 matrix [rows][row_stride_bytes / 8] as a 2-D tensor map with boxes of box0 doubles x box1 rows, no swizzle, zero fill
+bool make_map_f64(CUtensorMap* tm, const void* base, long long dim0, long long rows, long long row_stride_bytes, int box0, int box1,
+                  bool swizzle128 = false) {
+  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn enc = nullptr;
+  if (!enc) {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      enc = nullptr;
+  }
+  if (!enc || dim0 <= 0 || rows <= 0 || (reinterpret_cast<uintptr_t>(base) & 15) || (row_stride_bytes & 15)) return false;
+  cuuint64_t dims[2] = {(cuuint64_t)dim0, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)row_stride_bytes};
+  cuuint32_t box[2] = {(cuuint32_t)box0, (cuuint32_t)box1};
+  cuuint32_t estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Gamma-symmetric projector mode (sym_kernels.cuh): at k = 0, FP64 path.  Builds the -G map of the leading sphere entries,
 // classifies every projector ON THE DEVICE by exact comparison, checks that D couples equal classes only, and allocates the
 // real-form operands.  Leaves h->sym = false (general complex contraction) whenever any check fails; only CUDA errors are errors.
@@ -1242,6 +1272,14 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
   CR_TRY(cudaMemsetAsync(h->sym_e, 0, eb, st));
   h->workspace_bytes += ub + eb + pb;
   h->sym = true;
+  // TMA-fed kernels of the FP64 path (64 x 128 tiles): beta and the two workspaces never move, so the maps are made once
+  if (!int8_path && h->sym_wide && env_int("QE_HPSI_SYM_TMA", 1)) {
+    const long long rb = (long long)h->ldbeta * 16;
+    h->sym_tma = make_map_f64(&h->tm_a6_beta, h->beta, 2LL * M, h->nproj, rb, 16, ZgS::BM, true) &&
+                 make_map_f64(&h->tm_a6_u, h->sym_u, 2LL * M, 2LL * h->max_batch, h->sym_ldu * 16, 16, ZgS::BN, true) &&
+                 make_map_f64(&h->tm_a8_beta, h->beta, 2LL * M, h->nproj, rb, 2 * ZgS::LDA_M, ZgS::BK) &&
+                 make_map_f64(&h->tm_a8_e, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgS::BN);
+  }
 #undef CR_TRY
   return cudaSuccess;
 }
@@ -1749,7 +1787,11 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
                                                                                        h->sym_ldu, 2 * nb, h->sym_m, h->kchunk,
                                                                                        h->sym_partial, h->sym_ldc2, nullptr, h->sym_cls);
     };
-    if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
+    if (h->sym_tma) {
+      const int mt = (h->nproj + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
+      k_becp_sym_tma<ZgS><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m,
+                                                                                         h->kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls);
+    } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);
   const size_t t1 = prof_mark(h, st);
@@ -1817,7 +1859,12 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
                                                                                         h->sym_e, h->ldp, 2 * nb, hpsi, ldh, nullptr,
                                                                                         h->sym_cmask, h->sym_minus);
     };
-    if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
+    if (h->sym_tma) {
+      const int mt = (h->sym_m + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
+      if (mt > 0)
+        k_vnl_sym_tma<ZgS><<<(unsigned)(mt * nt), ZgS::NT, ZgS::SMEM_VNL, st>>>(h->tm_a8_beta, h->tm_a8_e, h->nproj, h->sym_m, 2 * nb, hpsi,
+                                                                                ldh, h->sym_cmask, h->sym_minus);
+    } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     vnl_fp64(h, bT, hpsi, ldh, nb, st, nullptr);
   CU_TRY(h, cudaGetLastError());

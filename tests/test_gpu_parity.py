@@ -314,6 +314,33 @@ def test_gamma_symmetric_projector_mode_is_detected_and_matches_the_general_cont
         qe_hpsi.qe_hpsi_test_set_sym_min(0)
 
 
+@pytest.mark.parametrize("cfg,nb", [("T2_radix5", 3), ("T3_aliased", 5), (0, 16), (1, 37), (1, 64)])
+def test_tma_fed_symmetric_kernels_give_the_bits_of_the_cp_async_ones(cfg, nb, monkeypatch):
+    """zgemm_tma_kernels.cuh moves the operand tiles of the Gamma-symmetric FP64 a6 / a8 by TMA; tiles, DMMA order and epilogues
+    are those of k_becp / k_vnl_add, so becp and the nonlocal part must be bit-identical (ragged K tail, row tail, column
+    tail, and a second call with fewer bands over stale workspace columns)."""
+    h, inp = _gpu.make(cfg)
+    assert h.info()["gamma_sym"] == 1
+    monkeypatch.setenv("QE_HPSI_SYM_TMA", "0")
+    h0, _ = _gpu.make(cfg, beta=inp["beta"])
+    monkeypatch.delenv("QE_HPSI_SYM_TMA")
+    nb = min(nb, h.max_batch)
+    for band0, n in ((0, nb), (50, max(1, nb // 2))):
+        psi = _gpu.gen_psi_dev(inp, band0, n)
+        base = _gpu.gen_psi_dev(inp, 200, n)
+        a = h.nonlocal_add(psi, base.clone())
+        ba, da = h.becp(n)
+        b = h0.nonlocal_add(psi, base.clone())
+        bb, db = h0.becp(n)
+        torch.cuda.synchronize()
+        assert torch.equal(ba.view(torch.float64), bb.view(torch.float64))
+        assert torch.equal(da.view(torch.float64), db.view(torch.float64))
+        assert torch.equal(a.view(torch.float64), b.view(torch.float64))
+        assert not torch.equal(a, base)
+    h.destroy()
+    h0.destroy()
+
+
 def test_apply_host_matches_device_path():
     h, inp = _gpu.make(0, max_batch=6)
     psi = _gpu.gen_psi_dev(inp, 0, 16)
