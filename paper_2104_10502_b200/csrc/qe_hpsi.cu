@@ -124,6 +124,8 @@ struct qe_hpsi_handle {
   int sym_wide = 1;                   // 128-column tiles (ZgS) instead of ZgV0 (tuning knob QE_HPSI_SYM_WIDE)
   bool sym_tma = false;               // operand tiles of the symmetric FP64 kernels by TMA (zgemm_tma_kernels.cuh; knob QE_HPSI_SYM_TMA)
   CUtensorMap tm_a6_beta, tm_a6_u, tm_a8_beta, tm_a8_e;
+  bool zg_tma = false;                // the same for the general complex / Gamma-only kernels (knob QE_HPSI_ZG_TMA); beta maps over
+  CUtensorMap tm_g6_beta, tm_g8_beta; // the whole sphere made at create, the maps of psi / coefficient rows per call
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
   int sym_nsplit = 1, sym_ldc2 = 0;
@@ -586,10 +588,16 @@ cudaError_t set_kernel_attrs() {
   SET_ZG(ZgV0, true);
   SET_ZG(ZgS, true);
 #undef SET_ZG
-  e = cudaFuncSetAttribute(k_becp_sym_tma<ZgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_BECP + 1024);
+#define SET_ZT(Cfg, FORM)                                                                                                        \
+  e = cudaFuncSetAttribute(k_becp_tma<Cfg, FORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BECP + 1024); \
+  if (e != cudaSuccess) return e;                                                                                              \
+  e = cudaFuncSetAttribute(k_vnl_tma<Cfg, FORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_VNL);           \
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_vnl_sym_tma<ZgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_VNL);
-  if (e != cudaSuccess) return e;
+  SET_ZT(ZgV0, ZF_3M);
+  SET_ZT(ZgV0, ZF_GAMMA);
+  SET_ZT(ZgS, ZF_GAMMA);
+  SET_ZT(ZgS, ZF_SYM);
+#undef SET_ZT
   e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgV0::SMEM_VNL);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_vnl_add<ZgS, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgS::SMEM_VNL);
@@ -784,19 +792,67 @@ void choose_split(qe_hpsi_handle* h) {
   h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
 }
 
+// FP64 matrix [rows][row_stride_bytes / 8] as a 2-D tensor map with boxes of box0 doubles x box1 rows, no swizzle, zero fill
+bool make_map_f64(CUtensorMap* tm, const void* base, long long dim0, long long rows, long long row_stride_bytes, int box0, int box1,
+                  bool swizzle128 = false) {
+  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn enc = nullptr;
+  if (!enc) {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      enc = nullptr;
+  }
+  if (!enc || dim0 <= 0 || rows <= 0 || (reinterpret_cast<uintptr_t>(base) & 15) || (row_stride_bytes & 15)) return false;
+  cuuint64_t dims[2] = {(cuuint64_t)dim0, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)row_stride_bytes};
+  cuuint32_t box[2] = {(cuuint32_t)box0, (cuuint32_t)box1};
+  cuuint32_t estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // buffers of one a6-a7 pass on the FP64 tensor path: split-K partials, becp, dbecp, dbecp transposed
 struct NlBufs {
   double2 *partial, *becp, *dbecp, *dbT;
 };
 
+// TMA-fed a6 / a8 of the general complex and Gamma-only forms (zgemm_tma_kernels.cuh): beta maps from create, the map of the
+// K-contiguous B operand (psi [nb][ldpsi] or coefficient rows [nb][ldp]) encoded here, on the host, per call.  false = not
+// launched (maps unavailable): the caller launches the cp.async kernel
+template <class Cfg, int FORM>
+bool becp_tma_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st, double2* partial, const int* nb_dev) {
+  CUtensorMap tb;
+  if (!h->zg_tma || !make_map_f64(&tb, psi, 2LL * h->npw, nb, ldpsi * 16, 16, Cfg::BN, true)) return false;
+  const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  k_becp_tma<Cfg, FORM><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP + 1024, st>>>(h->tm_g6_beta, tb, h->nproj, nb, h->npw, h->kchunk,
+                                                                                          partial, h->ldc, nullptr, nb_dev);
+  return true;
+}
+template <class Cfg, int FORM>
+bool vnl_tma_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
+  CUtensorMap tb;
+  if (!h->zg_tma || !make_map_f64(&tb, bT, 2LL * h->nproj, nb, (long long)h->ldp * 16, 8, Cfg::BN)) return false;
+  const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
+  if (mt > 0)
+    k_vnl_tma<Cfg, FORM><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->tm_g8_beta, tb, h->nproj, h->npw, nb, hpsi, ldh, nb_dev,
+                                                                              nullptr, nullptr, 0);
+  return true;
+}
+
 template <class Cfg>
 void becp_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaStream_t st, double2* partial, const int* nb_dev) {
+  if (becp_tma_launch<Cfg, ZF_3M>(h, psi, ldpsi, nb, st, partial, nb_dev)) return;
   const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
   k_becp<Cfg><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
                                                                          h->npw, h->kchunk, partial, h->ldc, nb_dev);
 }
 template <class Cfg>
 void vnl_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
+  if (vnl_tma_launch<Cfg, ZF_3M>(h, bT, hpsi, ldh, nb, st, nb_dev)) return;
   const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
   if (mt == 0) return;
   k_vnl_add<Cfg><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT, h->ldp,
@@ -1122,6 +1178,11 @@ cudaError_t setup_nonlocal(qe_hpsi_handle* h, int nproj, const void* beta_dev, i
     CR_TRY(guarded_malloc(h, &h->dbT, (size_t)max_batch * h->ldp * sizeof(double2)));
     CR_TRY(cudaMemsetAsync(h->dbT, 0, (size_t)max_batch * h->ldp * sizeof(double2), st));
     h->workspace_bytes += pc * (h->nsplit + 2) + (size_t)max_batch * h->ldp * sizeof(double2);
+    // TMA-fed FP64 kernels: beta never moves, its two maps (K-contiguous tiles of a6, M-contiguous tiles of a8) are made once
+    if (h->npw > 0 && env_int("QE_HPSI_ZG_TMA", 1))
+      h->zg_tma = make_map_f64(&h->tm_g6_beta, h->beta, 2LL * h->npw, nproj, (long long)h->ldbeta * 16, 16, ZgV0::BM, true) &&
+                  make_map_f64(&h->tm_g8_beta, h->beta, 2LL * h->npw, nproj, (long long)h->ldbeta * 16, 2 * ZgV0::LDA_M, ZgV0::BK);
+    static_assert(ZgV0::BM == ZgS::BM && ZgV0::BK == ZgS::BK, "one set of beta maps serves both tile shapes");
   #undef CR_TRY
   return cudaSuccess;
 }
@@ -1178,28 +1239,6 @@ cudaError_t setup_certify(qe_hpsi_handle* h, cudaStream_t st) {
   return cudaSuccess;
 }
 
-// FP64 matrix [rows][row_stride_bytes / 8] as a 2-D tensor map with boxes of box0 doubles x box1 rows, no swizzle, zero fill
-bool make_map_f64(CUtensorMap* tm, const void* base, long long dim0, long long rows, long long row_stride_bytes, int box0, int box1,
-                  bool swizzle128 = false) {
-  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn enc = nullptr;
-  if (!enc) {
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
-        qres != cudaDriverEntryPointSuccess)
-      enc = nullptr;
-  }
-  if (!enc || dim0 <= 0 || rows <= 0 || (reinterpret_cast<uintptr_t>(base) & 15) || (row_stride_bytes & 15)) return false;
-  cuuint64_t dims[2] = {(cuuint64_t)dim0, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)row_stride_bytes};
-  cuuint32_t box[2] = {(cuuint32_t)box0, (cuuint32_t)box1};
-  cuuint32_t estr[2] = {1, 1};
-  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
 
 // Gamma-symmetric projector mode (sym_kernels.cuh): at k = 0, FP64 path.  Builds the -G map of the leading sphere entries,
 // classifies every projector ON THE DEVICE by exact comparison, checks that D couples equal classes only, and allocates the
@@ -1772,6 +1811,7 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
   } else if (h->gamma) {
     auto go = [&](auto cfg) {
       using Cfg = decltype(cfg);
+      if (becp_tma_launch<Cfg, ZF_GAMMA>(h, psi, ldpsi, nb, st, h->partial, nullptr)) return;
       const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
       k_becp<Cfg, true><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, psi, ldpsi, nb,
                                                                                    h->npw, h->kchunk, h->partial, h->ldc);
@@ -1789,8 +1829,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     };
     if (h->sym_tma) {
       const int mt = (h->nproj + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
-      k_becp_sym_tma<ZgS><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m,
-                                                                                         h->kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls);
+      k_becp_tma<ZgS, ZF_SYM><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(
+          h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr);
     } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);
@@ -1843,6 +1883,7 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
   } else if (h->gamma) {
     auto go = [&](auto cfg) {
       using Cfg = decltype(cfg);
+      if (vnl_tma_launch<Cfg, ZF_GAMMA>(h, bT, hpsi, ldh, nb, st, nullptr)) return;
       const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
       if (mt > 0)
         k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
@@ -1862,8 +1903,8 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
     if (h->sym_tma) {
       const int mt = (h->sym_m + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
       if (mt > 0)
-        k_vnl_sym_tma<ZgS><<<(unsigned)(mt * nt), ZgS::NT, ZgS::SMEM_VNL, st>>>(h->tm_a8_beta, h->tm_a8_e, h->nproj, h->sym_m, 2 * nb, hpsi,
-                                                                                ldh, h->sym_cmask, h->sym_minus);
+        k_vnl_tma<ZgS, ZF_SYM><<<(unsigned)(mt * nt), ZgS::NT, ZgS::SMEM_VNL, st>>>(h->tm_a8_beta, h->tm_a8_e, h->nproj, h->sym_m, 2 * nb,
+                                                                                    hpsi, ldh, nullptr, h->sym_cmask, h->sym_minus, 0);
     } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     vnl_fp64(h, bT, hpsi, ldh, nb, st, nullptr);

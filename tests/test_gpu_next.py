@@ -210,7 +210,7 @@ def test_gamma_apply_against_oracle(cfg, nb, flags):
     g.destroy()
 
 
-def test_gamma_matches_the_full_sphere_path_on_config_1():
+def test_gamma_matches_the_full_sphere_path_on_config_1(monkeypatch):
     """Full size (config 1, 64 atoms, 80^3): the Gamma path on the half sphere against the complex full-sphere library path
     AND the oracle on sampled bands, same real-wavefunction problem."""
     nb = 12
@@ -226,7 +226,23 @@ def test_gamma_matches_the_full_sphere_path_on_config_1():
                         blk, db, max_batch=nb)
     hf = full.apply(torch.from_numpy(orc.gamma_expand(psi, ip, im, npw)).cuda()).cpu().numpy()
     assert _gpu.rel_l2(got, hf[:, ip]).max() <= TOL
+    # TMA operand tiles (default) against the cp.async kernels: same bits, on 64 x 64 tiles (12 bands) and 64 x 128 (70 bands)
+    monkeypatch.setenv("QE_HPSI_ZG_TMA", "0")
+    g0 = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), torch.from_numpy(beta).cuda(), blk, db, max_batch=8)
+    monkeypatch.delenv("QE_HPSI_ZG_TMA")
+    assert np.array_equal(g0.apply(torch.from_numpy(psi).cuda()).cpu().numpy().view(np.float64), got.view(np.float64))
+    g0.destroy()
     g.destroy()
+    wide = torch.from_numpy(np.concatenate([psi] * 6)[:70]).cuda()
+    outs = []
+    for tma in ("1", "0"):
+        monkeypatch.setenv("QE_HPSI_ZG_TMA", tma)
+        gw = qe_hpsi.HpsiGamma(wl.at, wl.ecutwfc, wl.nr, vr.cuda(), torch.from_numpy(beta).cuda(), blk, db, max_batch=70)
+        outs.append(gw.apply(wide).cpu().numpy())
+        gw.destroy()
+    monkeypatch.delenv("QE_HPSI_ZG_TMA")
+    assert np.array_equal(outs[0].view(np.float64), outs[1].view(np.float64))
+    assert _gpu.rel_l2(outs[0][:12], got).max() <= 1e-13  # another max_batch: another split-K plan, rounding order only
     full.destroy()
 
 

@@ -341,6 +341,32 @@ def test_tma_fed_symmetric_kernels_give_the_bits_of_the_cp_async_ones(cfg, nb, m
     h0.destroy()
 
 
+@pytest.mark.parametrize("cfg,nb", [("T1_general_k", 5), ("T5_odd_bands", 3), ("T3_aliased", 5), (0, 16), (1, 37), (3, 24)])
+def test_tma_fed_general_kernels_give_the_bits_of_the_cp_async_ones(cfg, nb, monkeypatch):
+    """The general complex a6 / a8 (3M form; k != 0 or QE_HPSI_NO_GAMMA_SYM) with TMA operand tiles against the cp.async
+    kernels: becp, dbecp and the nonlocal part bit for bit, on two calls with different band counts."""
+    flags = qe_hpsi.QE_HPSI_NO_GAMMA_SYM
+    h, inp = _gpu.make(cfg, flags=flags)
+    monkeypatch.setenv("QE_HPSI_ZG_TMA", "0")
+    h0, _ = _gpu.make(cfg, flags=flags, beta=inp["beta"])
+    monkeypatch.delenv("QE_HPSI_ZG_TMA")
+    nb = min(nb, h.max_batch)
+    for band0, n in ((0, nb), (50, max(1, nb // 2))):
+        psi = _gpu.gen_psi_dev(inp, band0, n)
+        base = _gpu.gen_psi_dev(inp, 200, n)
+        a = h.nonlocal_add(psi, base.clone())
+        ba, da = h.becp(n)
+        b = h0.nonlocal_add(psi, base.clone())
+        bb, db = h0.becp(n)
+        torch.cuda.synchronize()
+        assert torch.equal(ba.view(torch.float64), bb.view(torch.float64))
+        assert torch.equal(da.view(torch.float64), db.view(torch.float64))
+        assert torch.equal(a.view(torch.float64), b.view(torch.float64))
+        assert not torch.equal(a, base)
+    h.destroy()
+    h0.destroy()
+
+
 def test_apply_host_matches_device_path():
     h, inp = _gpu.make(0, max_batch=6)
     psi = _gpu.gen_psi_dev(inp, 0, 16)
