@@ -572,7 +572,9 @@ def main():
         gsym = bool(info.get("gamma_sym"))
         ex = 0.5 if gsym else 0.75  # executed / algorithmic flops
         ach = flops_launch / (t_k * 1e-3) * 1e-12
-        roofline = {"bound": "tensor", "kernel": kname + ("<ZgS, GAMMA, SYM> (Gamma-symmetric real form)" if gsym else " (3M complex form)"),
+        kern = ("k_vnl_tma" if kname == "k_vnl_add" else "k_becp_tma") + ("<ZgS, ZF_SYM> (Gamma-symmetric real form, TMA-fed)" if gsym
+                                                                           else "<ZgV0, ZF_3M> (3M complex form, TMA-fed)")
+        roofline = {"bound": "tensor", "kernel": kern,
                     "achieved": ach, "peak": dmma, "unit": "TFLOP/s", "frac": ach / dmma,
                     "traffic": committed_traffic(args.config, kname + ("_sym" if gsym else "")),
                     "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-resident "
