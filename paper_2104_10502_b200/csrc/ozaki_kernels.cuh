@@ -72,8 +72,29 @@ __device__ __forceinline__ void mma_i8(uint32_t tmem_d, uint64_t da, uint64_t db
 __device__ __forceinline__ void mma_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// s8 x s8 -> s32, both operands K-major, M = 128, N = 64
-constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+// s8 x s8 -> s32, both operands K-major, M = 128, N = n (a multiple of 16, at most 256)
+__host__ __device__ constexpr uint32_t idesc_n(int n) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+// Digit products of one K block of 32: A_i x B_j accumulates into level i + j = TMEM columns [(i + j) BN, (i + j + 1) BN).  The B
+// slices j = 0..S-1 of a stage are adjacent in shared memory (64 rows x 64 B each, 8-row groups 512 B apart), so B_j0..B_j0+w-1 is
+// ONE K-major operand of w * 64 rows, and its product with A_i lands in the w consecutive levels i + j0 ..: one tcgen05.mma of
+// N = 64 w (w <= 4) instead of w of N = 64.  A 128 x 64 x 32 instruction reads 6 KB of shared memory for 0.52 Mop, more than the
+// 128 B / clk port delivers at the tensor rate (ncu: tensor pipe 50 % active, shared-memory operand cycles 61 %); at N = 256 it
+// reads 12 KB for 2.1 Mop.  S (S + 1) / 2 instructions per K block become about S (S + 7) / 8: 21 -> 8 at S = 6, 28 -> 11 at S = 7.
+template <int S>
+__device__ __forceinline__ void mma_digits(uint32_t tm, uint32_t sb, int kk, uint32_t first) {
+#pragma unroll
+  for (int i = 0; i < S; ++i) {
+    const uint64_t da = desc_sw64(sb + i * A_BYTES) + 2 * kk;
+#pragma unroll
+    for (int j0 = 0; j0 < S - i; j0 += 4) {
+      const int w = (S - i - j0) < 4 ? (S - i - j0) : 4;
+      const uint64_t db = desc_sw64(sb + S * A_BYTES + j0 * B_BYTES) + 2 * kk;
+      mma_i8(tm + (uint32_t)(i + j0) * BN, da, db, idesc_n(w * BN), (first | (uint32_t)i) ? 1u : 0u);
+    }
+  }
+}
 
 // MODE 0 (a6): out = partial[split][m][ldo] complex, written; MODE 1 (a8): out = hpsi[b][ldo] complex at column m, accumulated.
 // Gamma-only (real) forms, one column per band: MODE 2 (a6): partial[split][m][b] = (value, 0); MODE 3 (a8): row m = 2g + c
@@ -138,15 +159,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
 #pragma unroll
       for (int kk = 0; kk < KB / 32; ++kk) {
-#pragma unroll
-        for (int i = 0; i < S; ++i) {
-          const uint64_t da = desc_sw64(sb + i * A_BYTES) + 2 * kk;
-#pragma unroll
-          for (int j = 0; j < S - i; ++j) {
-            const uint64_t db = desc_sw64(sb + S * A_BYTES + j * B_BYTES) + 2 * kk;
-            mma_i8(tm + (uint32_t)(i + j) * BN, da, db, IDESC, (it | kk | i) ? 1u : 0u);
-          }
-        }
+        mma_digits<S>(tm, sb, kk, (uint32_t)(it | kk));
       }
       mma_commit(&empty[st]);
     }
@@ -578,15 +591,7 @@ k_oz_vnl3(const __grid_constant__ CUtensorMap tmA0, const __grid_constant__ CUte
         const uint32_t sb = sbase0 + (uint32_t)st * STAGE;
 #pragma unroll
         for (int kk = 0; kk < KB / 32; ++kk) {
-#pragma unroll
-          for (int i = 0; i < S; ++i) {
-            const uint64_t da = desc_sw64(sb + i * A_BYTES) + 2 * kk;
-#pragma unroll
-            for (int j = 0; j < S - i; ++j) {
-              const uint64_t db = desc_sw64(sb + S * A_BYTES + j * B_BYTES) + 2 * kk;
-              mma_i8(tm + (uint32_t)(i + j) * BN, da, db, IDESC, (it | kk | i) ? 1u : 0u);
-            }
-          }
+          mma_digits<S>(tm, sb, kk, (uint32_t)(it | kk));
         }
         mma_commit(&empty[st]);
       }
