@@ -792,19 +792,27 @@ void choose_split(qe_hpsi_handle* h) {
   h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda); looked up once, thread-safe
+// (handles may be created, and maps of psi encoded, from several host threads)
+using TmaEncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                 CUtensorMapFloatOOBfill);
+TmaEncodeFn tma_encoder() {
+  static const TmaEncodeFn enc = [] {
+    TmaEncodeFn f = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&f, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return f;
+  }();
+  return enc;
+}
+
 // FP64 matrix [rows][row_stride_bytes / 8] as a 2-D tensor map with boxes of box0 doubles x box1 rows, no swizzle, zero fill
 bool make_map_f64(CUtensorMap* tm, const void* base, long long dim0, long long rows, long long row_stride_bytes, int box0, int box1,
                   bool swizzle128 = false) {
-  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn enc = nullptr;
-  if (!enc) {
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
-        qres != cudaDriverEntryPointSuccess)
-      enc = nullptr;
-  }
+  const TmaEncodeFn enc = tma_encoder();
   if (!enc || dim0 <= 0 || rows <= 0 || (reinterpret_cast<uintptr_t>(base) & 15) || (row_stride_bytes & 15)) return false;
   cuuint64_t dims[2] = {(cuuint64_t)dim0, (cuuint64_t)rows};
   cuuint64_t strides[1] = {(cuuint64_t)row_stride_bytes};
@@ -883,16 +891,7 @@ long long round_up(long long x, long long m) { return (x + m - 1) / m * m; }
 
 // int8 planes [S][rows][kpad] as a 3-D tensor map (K bytes, rows, slice), SWIZZLE_64B boxes of box_rows x 64 bytes
 bool oz_make_map(CUtensorMap* tm, void* base, long long kpad, long long rows, int S, long long slice_stride, int box_rows) {
-  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn enc = nullptr;
-  if (!enc) {
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) != cudaSuccess ||
-        qres != cudaDriverEntryPointSuccess)
-      enc = nullptr;
-  }
+  const TmaEncodeFn enc = tma_encoder();
   if (!enc) return false;
   cuuint64_t dims[3] = {(cuuint64_t)kpad, (cuuint64_t)rows, (cuuint64_t)S};
   cuuint64_t strides[2] = {(cuuint64_t)kpad, (cuuint64_t)slice_stride};
@@ -1616,14 +1615,8 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
       const Fft2tEntry* et = fft2t_find(nr[0], h->f2p[0]->ra, h->f2p[0]->rb, h->f2p[0]->smem_zy != 0);
       h->x_one_tile = h->f2p[0]->smem_zy == 0 ? env_int("QE_HPSI_X_ONE_TILE", 1) : 0;
       const size_t sm = fft2t_smem(nr[0], h->P, h->f2p[0]->smem_zy == 0, h->x_one_tile != 0);
-      using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-      EncodeFn enc = nullptr;
-      cudaDriverEntryPointQueryResult qres;
-      if (et && sm <= (size_t)110 * 1024 &&
-          cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qres) == cudaSuccess && enc &&
-          qres == cudaDriverEntryPointSuccess) {
+      const TmaEncodeFn enc = tma_encoder();
+      if (et && sm <= (size_t)110 * 1024 && enc) {
         const cuuint64_t row = (cuuint64_t)nr[1] * h->ldz;  // complex elements per plane
         cuuint64_t dims[3] = {row * 2, (cuuint64_t)h->P, (cuuint64_t)h->fft_nb};
         cuuint64_t strides[2] = {row * sizeof(double2), row * sizeof(double2) * (cuuint64_t)h->P};
