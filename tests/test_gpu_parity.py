@@ -367,6 +367,46 @@ def test_tma_fed_general_kernels_give_the_bits_of_the_cp_async_ones(cfg, nb, mon
     h0.destroy()
 
 
+@pytest.mark.parametrize("cfg", ["T2_radix5", "T1_general_k", 0])
+@pytest.mark.parametrize("dmode", ["diag", "full"])
+def test_ragged_projector_blocks_and_tails(cfg, dmode):
+    """13 projectors in blocks of 5 and 8 (K tail of the 16-projector tiles, ldp padding, a ragged class mask), 5 bands: the
+    nonlocal part alone against becp_of / the block-diagonal D written out.  diag D keeps the Gamma-symmetric form at k = 0,
+    a full random block couples s with p and must take the general contraction."""
+    import scipy.linalg
+    h0, inp = _gpu.make(cfg)
+    wl = inp["wl"]
+    npw = h0.npw
+    h0.destroy()
+    if wl.nproj < 13:  # 8 rows: 5 more as combinations of rows of equal parity (s with s, p with p), so the symmetry classes stay exact
+        ia, ib = ([0, 1, 2, 3, 4], [1, 0, 3, 4, 2]) if wl.nh == 8 else ([0, 4, 1, 2, 3], [4, 0, 2, 3, 1])
+        beta = torch.cat([inp["beta"], inp["beta"][ia] * 0.7 + inp["beta"][ib] * 0.4]).contiguous()
+        assert beta.shape[0] == 13
+    else:
+        beta = inp["beta"][:13].contiguous()
+    rng = np.random.default_rng(11)
+    blocks = []
+    for n in (5, 8):
+        d = rng.standard_normal((n, n))
+        blocks.append(np.diag(np.diag(d)) if dmode == "diag" else (d + d.T) / 2)
+    h = qe_hpsi.Hpsi(wl.at, wl.ecutwfc, wl.xk, wl.nr, inp["vr"], beta, [0, 5, 13], blocks, max_batch=5)
+    k0 = all(x == 0.0 for x in wl.xk)
+    assert h.info()["gamma_sym"] == (1 if (k0 and dmode == "diag") else 0)
+    psi = _gpu.gen_psi_dev(inp, 0, 5)
+    got = h.nonlocal_add(psi, torch.zeros_like(psi))
+    ba, da = h.becp(5)
+    torch.cuda.synchronize()
+    bh, ph = beta[:, :npw].cpu().numpy(), psi[:, :npw].cpu().numpy()
+    becp = orc.becp_of(bh, ph)
+    dbecp = scipy.linalg.block_diag(*blocks) @ becp
+    ref = (bh.T @ dbecp).T
+    assert np.abs(ba.cpu().numpy() - becp).max() <= 1e-13 * np.abs(becp).max()
+    assert np.abs(da.cpu().numpy() - dbecp).max() <= 1e-13 * np.abs(dbecp).max()
+    assert _gpu.rel_l2(got.cpu().numpy()[:, :npw], ref).max() <= 1e-12
+    assert torch.equal(got[:, npw:], torch.zeros_like(got[:, npw:]))
+    h.destroy()
+
+
 def test_apply_host_matches_device_path():
     h, inp = _gpu.make(0, max_batch=6)
     psi = _gpu.gen_psi_dev(inp, 0, 16)
