@@ -149,7 +149,8 @@ int64_t qe_hpsi_nplanes(qe_hpsi_t h);        /* P: i1 planes holding >= 1 sphere
 int qe_hpsi_get_maps(qe_hpsi_t h, int32_t* miller_dev, int32_t* fftidx_dev, double* g2kin_dev, void* cuda_stream);
 /* info[0..15]: npw, S, P, fft band chunk, split-K count (FP64 path), workspace bytes, per axis j=0..2 the number of
  * generic FFT passes, K chunk, x split, SM count, [12] bit 0: two-pass FFT plan in use, bit 1: Gamma-symmetric projector mode of
- * the FP64 path in use; then the projector path: [13] digits per
+ * the FP64 path in use, bit 2: x stage of the FFT chain with quarter pruning (populated planes within the outer quarters of the
+ * axis); then the projector path: [13] digits per
  * FP64 operand of the int8 path (0 = FP64 tensor path), [14] its split-K count of a6, [15] 1 if a6 runs in the
  * integer 3M form, 2 if a8 does too, +4 if QE_HPSI_PROJ_CERTIFY is on. */
 int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]);

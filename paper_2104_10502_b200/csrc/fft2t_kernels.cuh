@@ -38,15 +38,58 @@ inline size_t fft2t_smem(int n, int P, bool two_pass, bool one_tile) {
          (two_pass ? 16 * 17 * sizeof(double2) : 64);
 }
 
+// Radix-R DFT (R = 4 Q) whose inputs Q .. 3Q - 1 are zero: the first stage of Dft<R> (4-point DFTs over v[b], v[Q + b], v[2Q + b],
+// v[3Q + b]) sees (t0, 0, 0, t3) and needs 4 complex additions instead of 8; the rest is Dft<R>.  Used by the x stage when the
+// populated planes lie in the outer quarters of the axis (HALF below): same sums as Dft<R> on zero-padded inputs up to the sign of
+// an exact zero.
+template <int R, int DIR>
+struct DftHalfIn {
+  static constexpr int Q = R / 4;
+  static_assert(R % 4 == 0, "quarter pruning needs a radix-4 first stage");
+  __device__ __forceinline__ static void run(double2 (&v)[R]) {
+    double2 y[Q][4];
+    static_for<Q>([&](auto b_) {
+      constexpr int b = decltype(b_)::value;
+      const double2 t0 = v[b], t3 = v[3 * Q + b];
+      const double2 d = cmul_i<DIR>(make_double2(-t3.x, -t3.y));
+      double2 t[4] = {cadd(t0, t3), cadd(t0, d), csub(t0, t3), csub(t0, d)};
+      static_for<4>([&](auto c_) {
+        constexpr int c = decltype(c_)::value;
+        y[b][c] = cmul_tw<b * c, R, DIR>(t[c]);
+      });
+    });
+    static_for<4>([&](auto c_) {
+      constexpr int c = decltype(c_)::value;
+      double2 u[Q];
+      static_for<Q>([&](auto b_) {
+        constexpr int b = decltype(b_)::value;
+        u[b] = y[b][c];
+      });
+      Dft<Q, DIR>::run(u);
+      static_for<Q>([&](auto d_) {
+        constexpr int d = decltype(d_)::value;
+        v[c + 4 * d] = u[d];
+      });
+    });
+  }
+};
+
 // tmap: W2 viewed as FP64 [nb][P][N2*ldz*2], box {16, P, 1}
 // Register diet (round 2): the second-pass twiddles tw[q*j] sit in a padded shared table instead of 64 registers, and the
 // populated-plane index comes from the wrapped-interval rule of Fft2pGeom (x_hi, x_lo) instead of a 16-entry register array:
 // 222 -> under 168 registers, three CTAs per SM instead of two, so the FP64 pipe has 12 warps to pick from across the
 // three barriers of a band (the stage is bound by FP64 issue, not HBM: DESIGN.md section 6).
-template <int RA, int RB>
+// HALF (RA = 4 QA): every populated plane has i1 < QA RB or i1 >= 3 QA RB, i.e. the inputs q in [QA, 3 QA) of every radix-RA
+// transform of the inverse pass are zero and the same outputs of the forward pass are not kept (true whenever the grid holds the
+// sphere twice over, x_hi < N / 4: the density-grid rule; checked on the host).  Those 2 QA of 4 QA shared-memory reads and
+// writes per thread are not made at all, the inverse butterfly is DftHalfIn, and the unused outputs of the forward butterfly
+// fall to dead-code elimination: the stage is bound by shared-memory traffic and FP64 issue, not by HBM.
+template <int RA, int RB, bool HALF = false>
 __global__ void __launch_bounds__(RA* FFT_C, 3)
 k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb, int one_tile) {
   static_assert(RB > 1, "single-pass lengths use k2p_x_vmul");
+  static_assert(!HALF || RA % 4 == 0, "quarter pruning");
+  constexpr int QA = RA / 4;
   static_assert(RA >= RB && RA <= 16, "twiddle table is [RA][RA+1]");
   constexpr int N = RA * RB, NT = RA * FFT_C, NW = (NT + 31) / 32, TWP = RA + 1;
   constexpr unsigned ROWB = FFT_C * sizeof(double2);  // 128 bytes per plane row of the tile
@@ -104,11 +147,17 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
       const double2* in = inb + c;
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
+        if (HALF && q >= QA && q < 3 * QA) continue;  // known zero
         const int i1 = j + q * RB;
         const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
         v[q] = in[p * FFT_C];
       }
-      pass_a_store<RA, +1>(v, tile1, j, c);
+      if constexpr (HALF) {
+        DftHalfIn<RA, +1>::run(v);
+#pragma unroll
+        for (int q = 0; q < RA; ++q) tile1[fft_phys(j * RA + q, c)] = v[q];
+      } else
+        pass_a_store<RA, +1>(v, tile1, j, c);
     }
     __syncthreads();
     if (io_thread) {
@@ -144,6 +193,7 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
       double2* out = outb + c;
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
+        if (HALF && q >= QA && q < 3 * QA) continue;  // not a populated plane: never computed
         const int i1 = j + q * RB;
         const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
         out[p * FFT_C] = v[q];
@@ -487,14 +537,22 @@ __global__ void __launch_bounds__(RA* FFT_C) k2t_zfwd_gather(FftGeom g, Fft2pGeo
 using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, int);
 
 using K2tRho = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, const double*, double, double*);
+template <int RA, int RB>
+constexpr K2tX x_half_kernel() {
+  if constexpr (RA % 4 == 0)
+    return k2t_x_vmul<RA, RB, true>;
+  else
+    return nullptr;
+}
 struct Fft2tEntry {
   int n, ra, rb;
   K2tRho rho;    // TMA-staged density kernel (two-pass lengths only)
+  K2tX xh;       // x stage with quarter pruning (RA % 4 == 0, populated planes in the outer quarters), else null
   K2tX x;
   K2pZinv zinv;  // bulk-staged z stages (two-pass lengths only; null for the three-pass table)
   K2pZfwd zfwd;
 };
-#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_rho<RA, RB>, k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
+#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_rho<RA, RB>, x_half_kernel<RA, RB>(), k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
 static const Fft2tEntry kFft2tTable[] = {
     QE_FFT2T_ENTRY(6, 3),   QE_FFT2T_ENTRY(5, 4),   QE_FFT2T_ENTRY(6, 6),   QE_FFT2T_ENTRY(8, 6),   QE_FFT2T_ENTRY(8, 8),
     QE_FFT2T_ENTRY(9, 8),   QE_FFT2T_ENTRY(10, 8),  QE_FFT2T_ENTRY(12, 8),  QE_FFT2T_ENTRY(10, 10), QE_FFT2T_ENTRY(12, 9),
@@ -503,7 +561,7 @@ static const Fft2tEntry kFft2tTable[] = {
 };
 #undef QE_FFT2T_ENTRY
 // three-pass lengths: ra = R1, rb = R2*R3 as in kFft3pTable
-#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), nullptr, k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
+#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), nullptr, nullptr, k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
 static const Fft2tEntry kFft3tTable[] = {
     QE_FFT3T_ENTRY(5, 5, 5),  QE_FFT3T_ENTRY(6, 5, 5),  QE_FFT3T_ENTRY(8, 5, 5),  QE_FFT3T_ENTRY(6, 6, 6), QE_FFT3T_ENTRY(10, 5, 5),
     QE_FFT3T_ENTRY(8, 6, 6),  QE_FFT3T_ENTRY(10, 6, 5), QE_FFT3T_ENTRY(8, 8, 5),  QE_FFT3T_ENTRY(10, 6, 6), QE_FFT3T_ENTRY(8, 8, 6),

@@ -73,6 +73,7 @@ struct qe_hpsi_handle {
   size_t smem_x2p = 0;
   // TMA-staged x stage (fft2t_kernels.cuh): tensor map over W2, used when the length has a two-pass plan with RB > 1
   K2tX x_tma = nullptr;
+  int x_half = 0;  // x stage with quarter pruning (k2t_x_vmul<RA, RB, true>)
   K2tRho rho_tma = nullptr;  // TMA-staged density kernel (needs the unswizzled tensor map of x_tma)
   size_t smem_rho = 0;
   int x_one_tile = 0;  // two-pass x stage with one shared tile (tuning knob QE_HPSI_X_ONE_TILE)
@@ -1626,6 +1627,13 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS &&
             cudaFuncSetAttribute((const void*)et->x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess) {
           h->x_tma = et->x;
+          // quarter pruning: every populated plane in [0, N/4) or [3N/4, N) (x_hi, x_lo of the wrapped-interval rule)
+          const int n1 = nr[0];
+          if (et->xh && h->f2p[0]->smem_zy == 0 && env_int("QE_HPSI_X_HALF", 1) && 4 * (h->g2p.x_hi + 1) <= n1 && 4 * h->g2p.x_lo <= n1 &&
+              cudaFuncSetAttribute((const void*)et->xh, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm) == cudaSuccess) {
+            h->x_tma = et->xh;
+            h->x_half = 1;
+          }
           h->smem_xt = sm;
           const size_t smr = fft2t_smem_rho(nr[0], h->P);
           if (et->rho && smr <= (size_t)110 * 1024 &&
@@ -2691,7 +2699,7 @@ extern "C" int qe_hpsi_info(qe_hpsi_t h, int64_t info[16]) {
   info[9] = h->kchunk;
   info[10] = h->x_split;
   info[11] = h->num_sms;
-  info[12] = (h->f2p[0] ? 1 : 0) | (h->sym ? 2 : 0);
+  info[12] = (h->f2p[0] ? 1 : 0) | (h->sym ? 2 : 0) | (h->x_half ? 4 : 0);
   info[13] = h->oz_s;
   info[14] = h->oz_nsplit;
   info[15] = (h->oz_3m ? (h->oz_3m8 ? 2 : 1) : 0) + (h->certify ? 4 : 0);

@@ -399,6 +399,7 @@ class Hpsi:
                 "x_split", "num_sms", "fft2p", "ozaki_slices", "ozaki_nsplit", "ozaki_3m"]
         d = {k: int(buf[i]) for i, k in enumerate(keys)}
         d["gamma_sym"] = (d["fft2p"] >> 1) & 1
+        d["x_half"] = (d["fft2p"] >> 2) & 1
         d["fft2p"] &= 1
         d["certify"] = d["ozaki_3m"] >> 2
         d["ozaki_3m"] &= 3

@@ -480,6 +480,42 @@ def test_local_term_for_every_fft_length(n):
         h.destroy()
 
 
+@pytest.mark.parametrize("n", [48, 64, 96, 108, 120, 128, 144, 160, 192, 240, 256])
+def test_x_stage_quarter_pruning(n, monkeypatch):
+    """Grids that hold the sphere twice over along x (x_hi < N1 / 4, the density-grid rule): the x stage skips the known-zero
+    half of its radix-RA inputs and the unused half of its outputs (k2t_x_vmul<RA, RB, HALF>).  Local + kinetic term against
+    oracle Level B, and against the unpruned kernel (same sums up to the sign of an exact zero)."""
+    ecut = 4.0
+    gen = torch.Generator().manual_seed(2000 + n)
+    nr = [n, 9, 10]
+    at = np.zeros((3, 3))
+    for j in range(3):
+        nmax = (nr[j] // 4 - 1) if j == 0 else (nr[j] - 1) // 2
+        at[j, j] = 2.0 * np.pi * (nmax + 0.4) / np.sqrt(ecut)
+    xk = np.zeros(3)
+    sp = orc.gsphere(at, xk, ecut, nr)
+    npw = sp["miller"].shape[0]
+    assert np.abs(sp["miller"][:, 0]).max() == n // 4 - 1
+    vr = torch.randn(tuple(nr), dtype=torch.float64, generator=gen)
+    nb = 3
+    psi = torch.zeros((nb, inputs.pad8(npw)), dtype=torch.complex128)
+    psi[:, :npw] = torch.randn((nb, npw), dtype=torch.complex128, generator=gen)
+    h = qe_hpsi.Hpsi(at, ecut, xk, nr, vr.cuda(), max_batch=2)
+    assert h.info()["x_half"] == 1
+    out = h.apply(psi.cuda())
+    monkeypatch.setenv("QE_HPSI_X_HALF", "0")
+    h0 = qe_hpsi.Hpsi(at, ecut, xk, nr, vr.cuda(), max_batch=2)
+    monkeypatch.delenv("QE_HPSI_X_HALF")
+    assert h0.info()["x_half"] == 0
+    out0 = h0.apply(psi.cuda())
+    torch.cuda.synchronize()
+    ref = orc.hpsi_dual(sp["fft_index"], sp["g2kin"], tuple(nr), vr.numpy(), psi[:, :npw].numpy(), None, None)
+    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], ref).max() <= TOL
+    assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], out0.cpu().numpy()[:, :npw]).max() <= 1e-15
+    h.destroy()
+    h0.destroy()
+
+
 def test_apply_can_be_captured_in_a_cuda_graph():
     """qe_hpsi_apply enqueues kernels only (no allocation, no host sync): it can be stream-captured and replayed, which
     is how a launch-latency-bound caller (config 0: 9 launches for 16 bands) should drive it. Replays must reproduce the
