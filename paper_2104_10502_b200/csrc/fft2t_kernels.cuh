@@ -216,7 +216,7 @@ k2t_x_vmul(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int
 inline size_t fft2t_smem_rho(int n, int P) {
   return (size_t)n * FFT_C * sizeof(double2) + 2 * (size_t)(P + 1) * FFT_C * sizeof(double2) + 16 * 17 * sizeof(double2) + 64;
 }
-template <int RA, int RB>
+template <int RA, int RB, bool HALF = false>
 __global__ void __launch_bounds__(RA* FFT_C, 3)
 k2t_x_rho(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int nb, const double* __restrict__ occ, double scale,
           double* __restrict__ rho) {
@@ -270,11 +270,17 @@ k2t_x_rho(FftGeom g, Fft2pGeom t, const __grid_constant__ CUtensorMap tmap, int 
       const double2* in = ((b & 1) ? inb1 : inb0) + c;
 #pragma unroll
       for (int q = 0; q < RA; ++q) {
+        if (HALF && q >= RA / 4 && q < 3 * (RA / 4)) continue;  // known zero (quarter pruning, see k2t_x_vmul)
         const int i1 = j + q * RB;
         const int p = i1 <= xhi ? i1 : (i1 >= xlo0 ? i1 - xsh : P);
         v[q] = in[p * FFT_C];
       }
-      pass_a_store<RA, +1>(v, tile1, j, c);
+      if constexpr (HALF) {
+        DftHalfIn<RA, +1>::run(v);
+#pragma unroll
+        for (int q = 0; q < RA; ++q) tile1[fft_phys(j * RA + q, c)] = v[q];
+      } else
+        pass_a_store<RA, +1>(v, tile1, j, c);
     }
     __syncthreads();  // tile complete; the input stage of band b has been read by everybody
     if (io_thread && b + 2 < nb) issue_load(b + 2);
@@ -538,6 +544,13 @@ using K2tX = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, int);
 
 using K2tRho = void (*)(FftGeom, Fft2pGeom, const CUtensorMap, int, const double*, double, double*);
 template <int RA, int RB>
+constexpr K2tRho rho_half_kernel() {
+  if constexpr (RA % 4 == 0)
+    return k2t_x_rho<RA, RB, true>;
+  else
+    return nullptr;
+}
+template <int RA, int RB>
 constexpr K2tX x_half_kernel() {
   if constexpr (RA % 4 == 0)
     return k2t_x_vmul<RA, RB, true>;
@@ -547,12 +560,13 @@ constexpr K2tX x_half_kernel() {
 struct Fft2tEntry {
   int n, ra, rb;
   K2tRho rho;    // TMA-staged density kernel (two-pass lengths only)
-  K2tX xh;       // x stage with quarter pruning (RA % 4 == 0, populated planes in the outer quarters), else null
+  K2tRho rhoh;   // the two with quarter pruning (RA % 4 == 0, populated planes in the outer quarters of the axis), else null
+  K2tX xh;
   K2tX x;
   K2pZinv zinv;  // bulk-staged z stages (two-pass lengths only; null for the three-pass table)
   K2pZfwd zfwd;
 };
-#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_rho<RA, RB>, x_half_kernel<RA, RB>(), k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
+#define QE_FFT2T_ENTRY(RA, RB) {(RA) * (RB), RA, RB, k2t_x_rho<RA, RB>, rho_half_kernel<RA, RB>(), x_half_kernel<RA, RB>(), k2t_x_vmul<RA, RB>, k2t_scatter_zinv<RA, RB>, k2t_zfwd_gather<RA, RB>}
 static const Fft2tEntry kFft2tTable[] = {
     QE_FFT2T_ENTRY(6, 3),   QE_FFT2T_ENTRY(5, 4),   QE_FFT2T_ENTRY(6, 6),   QE_FFT2T_ENTRY(8, 6),   QE_FFT2T_ENTRY(8, 8),
     QE_FFT2T_ENTRY(9, 8),   QE_FFT2T_ENTRY(10, 8),  QE_FFT2T_ENTRY(12, 8),  QE_FFT2T_ENTRY(10, 10), QE_FFT2T_ENTRY(12, 9),
@@ -561,7 +575,7 @@ static const Fft2tEntry kFft2tTable[] = {
 };
 #undef QE_FFT2T_ENTRY
 // three-pass lengths: ra = R1, rb = R2*R3 as in kFft3pTable
-#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), nullptr, nullptr, k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
+#define QE_FFT3T_ENTRY(R1, R2, R3) {(R1) * (R2) * (R3), R1, (R2) * (R3), nullptr, nullptr, nullptr, k3t_x_vmul<R1, R2, R3>, nullptr, nullptr}
 static const Fft2tEntry kFft3tTable[] = {
     QE_FFT3T_ENTRY(5, 5, 5),  QE_FFT3T_ENTRY(6, 5, 5),  QE_FFT3T_ENTRY(8, 5, 5),  QE_FFT3T_ENTRY(6, 6, 6), QE_FFT3T_ENTRY(10, 5, 5),
     QE_FFT3T_ENTRY(8, 6, 6),  QE_FFT3T_ENTRY(10, 6, 5), QE_FFT3T_ENTRY(8, 8, 5),  QE_FFT3T_ENTRY(10, 6, 6), QE_FFT3T_ENTRY(8, 8, 6),

@@ -1636,9 +1636,10 @@ int create_impl(qe_hpsi_t* out, qe_hpsi_handle** live, const double at[9], doubl
           }
           h->smem_xt = sm;
           const size_t smr = fft2t_smem_rho(nr[0], h->P);
-          if (et->rho && smr <= (size_t)110 * 1024 &&
-              cudaFuncSetAttribute((const void*)et->rho, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr) == cudaSuccess) {
-            h->rho_tma = et->rho;
+          const K2tRho kr = (h->x_half && et->rhoh) ? et->rhoh : et->rho;
+          if (kr && smr <= (size_t)110 * 1024 &&
+              cudaFuncSetAttribute((const void*)kr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smr) == cudaSuccess) {
+            h->rho_tma = kr;
             h->smem_rho = smr;
           }
         }

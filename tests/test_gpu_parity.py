@@ -512,6 +512,13 @@ def test_x_stage_quarter_pruning(n, monkeypatch):
     ref = orc.hpsi_dual(sp["fft_index"], sp["g2kin"], tuple(nr), vr.numpy(), psi[:, :npw].numpy(), None, None)
     assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], ref).max() <= TOL
     assert _gpu.rel_l2(out.cpu().numpy()[:, :npw], out0.cpu().numpy()[:, :npw]).max() <= 1e-15
+    # the density kernel shares the pruned inverse pass (k2t_x_rho<RA, RB, HALF>)
+    occ = torch.tensor([2.0, 1.0, 0.5], dtype=torch.float64, device="cuda")
+    rho = torch.full(tuple(nr), 0.25, dtype=torch.float64, device="cuda")
+    h.density(psi.cuda(), occ, 0.5, rho)
+    torch.cuda.synchronize()
+    rref = 0.25 + orc.density_of(sp["fft_index"], tuple(nr), psi[:, :npw].numpy(), occ.cpu().numpy(), 0.5)
+    assert np.abs(rho.cpu().numpy() - rref).max() <= 1e-12 * np.abs(rref).max()
     h.destroy()
     h0.destroy()
 
