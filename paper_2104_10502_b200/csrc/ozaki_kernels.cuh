@@ -168,22 +168,48 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     // ---- epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31; thread = row of the tile ----
     const int wq = warp & 3;
     const long long m = (long long)mt * BM + wq * 32 + lane;
-    if ((MODE == 1 || MODE == 3) && m < mvalid) {
-      // these warps idle while the MMAs run: pull the hpsi entries of the tile towards L2 for the read-modify-write below
-      const int ncol = MODE == 1 ? BN / 2 : BN;
-      for (int j = 0; j < ncol; ++j) {
-        const int b = q * ncol + j;
-        if (b < nb) {
-          const void* a = MODE == 1 ? (const void*)(out + (size_t)b * ldo + m)
-                                    : (const void*)(reinterpret_cast<const double*>(out + (size_t)b * ldo) + m);
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+    // the accumulating forms (MODE 1, 3, 4) fetch the hpsi entries this thread will update into registers NOW, while the MMAs run
+    // and these warps have nothing else to do: the epilogue below is then TMEM reads, FP64 recombination and stores, without a
+    // global round trip per column group.  Only this thread writes these entries (each (row, band) has one owner; K ranges are
+    // separate launches).
+    double pre[(MODE == 1 || MODE == 3) ? BN : 1];  // MODE 1: (re, im) of hpsi[b][m] for the BN / 2 bands; MODE 3: component m of the BN bands
+    if constexpr (MODE == 1) {
+#pragma unroll
+      for (int jj = 0; jj < BN / 2; ++jj) {
+        const int b = q * (BN / 2) + jj;
+        const double2 v = (m < mvalid && b < nb) ? out[(size_t)b * ldo + m] : make_double2(0.0, 0.0);
+        pre[2 * jj] = v.x;
+        pre[2 * jj + 1] = v.y;
+      }
+    } else if constexpr (MODE == 3) {
+#pragma unroll
+      for (int j = 0; j < BN; ++j) {
+        const int b = q * BN + j;
+        pre[j] = (m < mvalid && b < nb) ? reinterpret_cast<const double*>(out + (size_t)b * ldo)[m] : 0.0;
+      }
+    }
+    // MODE 4: component c of row g and of row -G, one pair per band of the tile
+    double pg[MODE == 4 ? BN / 2 : 1], pm[MODE == 4 ? BN / 2 : 1];
+    if constexpr (MODE == 4) {
+      const bool ok = m < mvalid;
+      const long long g = m >> 1;
+      const int c = (int)(m & 1);
+      const int mg = ok ? minus[g] : -1;
+#pragma unroll
+      for (int jp = 0; jp < BN / 2; ++jp) {
+        const int col = q * BN + 2 * jp;
+        pg[jp] = pm[jp] = 0.0;
+        if (ok && col < nb && mg != -1) {
+          const double* row = reinterpret_cast<const double*>(out + (size_t)(col >> 1) * ldo);
+          pg[jp] = row[2 * g + c];
+          if (mg >= 0) pm[jp] = row[2 * (long long)mg + c];
         }
       }
     }
     mbar_wait(&done, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int em = (m < mvalid) ? ea[MODE >= 3 ? (m >> 1) : m] : 0;  // MODE 3, 4: rows 2g, 2g+1 share the exponent of plane wave g
-#pragma unroll 1
+#pragma unroll(MODE == 1 || MODE >= 3 ? BN / 8 : 1)
     for (int n0 = 0; n0 < BN; n0 += 8) {
       double d[8];
 #pragma unroll
@@ -211,8 +237,6 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const long long g = m >> 1;
         const int c = (int)(m & 1);
         const int mg = ok ? minus[g] : -1;
-        // the loads of the four column pairs first, then the stores: the compiler cannot prove that the entries do not alias, so
-        // interleaved read-modify-writes would cost one global round trip each
         double og[4], om[4], vg[4], vm[4];
         bool wr[4];
 #pragma unroll
@@ -225,12 +249,8 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           vg[jp] = c == 0 ? x - yo : x + yo;
           vm[jp] = c == 0 ? x + yo : yo - x;
           wr[jp] = ok && cok && mg != -1;
-          og[jp] = om[jp] = 0.0;
-          if (wr[jp]) {
-            const double* row = reinterpret_cast<const double*>(out + (size_t)(col >> 1) * ldo);
-            og[jp] = row[2 * g + c];
-            if (mg >= 0) om[jp] = row[2 * (long long)mg + c];
-          }
+          og[jp] = pg[n0 / 2 + jp];  // fetched before the wait (see above)
+          om[jp] = pm[n0 / 2 + jp];
         }
 #pragma unroll
         for (int jp = 0; jp < 4; ++jp) {
@@ -242,14 +262,6 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         }
       } else if (MODE >= 2) {  // real forms of the Gamma-only handle: one column per band
         if (m < mvalid) {
-          double old8[8];
-          if (MODE == 3) {  // loads before stores (see MODE 4)
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const int b = q * BN + n0 + j;
-              old8[j] = b < nb ? reinterpret_cast<const double*>(out + (size_t)b * ldo)[m] : 0.0;
-            }
-          }
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
             const int b = q * BN + n0 + j;
@@ -258,19 +270,11 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               if (MODE == 2)
                 out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(val, 0.0);
               else
-                reinterpret_cast<double*>(out + (size_t)b * ldo)[m] = old8[j] + val;  // m = 2g + c: component c of hpsi[b][g]
+                reinterpret_cast<double*>(out + (size_t)b * ldo)[m] = pre[MODE == 3 ? n0 + j : 0] + val;  // m = 2g + c: component c of hpsi[b][g]
             }
           }
         }
       } else if (m < mvalid) {
-        double2 old4[4];
-        if (MODE == 1) {  // loads before stores (see MODE 4)
-#pragma unroll
-          for (int jj = 0; jj < 4; ++jj) {
-            const int b = (q * BN + n0) / 2 + jj;
-            old4[jj] = b < nb ? out[(size_t)b * ldo + m] : make_double2(0.0, 0.0);
-          }
-        }
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
           const int b = (q * BN + n0) / 2 + jj;
@@ -279,7 +283,7 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             if (MODE == 0)
               out[(size_t)ks * split_stride + (size_t)m * ldo + b] = make_double2(re, im);
             else
-              out[(size_t)b * ldo + m] = make_double2(old4[jj].x + re, old4[jj].y + im);
+              out[(size_t)b * ldo + m] = make_double2(pre[MODE == 1 ? n0 + 2 * jj : 0] + re, pre[MODE == 1 ? n0 + 2 * jj + 1 : 0] + im);
           }
         }
       }
