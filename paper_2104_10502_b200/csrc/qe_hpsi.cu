@@ -129,7 +129,7 @@ struct qe_hpsi_handle {
   CUtensorMap tm_g6_beta, tm_g8_beta; // the whole sphere made at create, the maps of psi / coefficient rows per call
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
-  int sym_nsplit = 1, sym_ldc2 = 0;
+  int sym_nsplit = 1, sym_ldc2 = 0, sym_kchunk = 0;
   std::vector<unsigned char> sym_cls_host;  // copy of sym_cls for qe_hpsi_set_s
   bool sym_q_ok = false;                    // the q blocks of qe_hpsi_set_s couple equal classes only
   std::vector<int> blk_off;                 // atom block table (for the same check)
@@ -766,19 +766,18 @@ int env_int(const char* name, int dflt) {
 }
 
 // choose the split-K count of a6 so that (M tiles x N tiles x nsplit) fills whole waves of CTAs
-void choose_split(qe_hpsi_handle* h) {
-  constexpr int ZG_BM = ZgV0::BM, ZG_BN = ZgV0::BN, ZG_BK = ZgV0::BK;
-  const int ntile = ((h->nproj + ZG_BM - 1) / ZG_BM) * ((h->max_batch + ZG_BN - 1) / ZG_BN);
+// split-K plan of an a6-type contraction: ntile output tiles, K entries; fills whole waves of the SMs where K allows
+void pick_split(int ntile, int klen, int num_sms, int bk, int* kchunk_out, int* nsplit_out) {
   // slices of at least 512 plane waves, unless that cannot even fill two waves (few projectors, small sphere): then 128
-  int ksmax = std::max(1, h->npw / 512);
-  if ((long long)ntile * ksmax < 2LL * h->num_sms) ksmax = std::max(1, h->npw / 128);
+  int ksmax = std::max(1, klen / 512);
+  if ((long long)ntile * ksmax < 2LL * num_sms) ksmax = std::max(1, klen / 128);
   int best = 1;
   double best_score = -1.0;
   for (int ks = 1; ks <= std::min(ksmax, 1024); ++ks) {
     const long long ctas = (long long)ntile * ks;
-    const long long waves = (ctas + h->num_sms - 1) / h->num_sms;
-    double eff = (double)ctas / (double)(waves * h->num_sms);
-    if (waves < 2) eff *= 0.5 + 0.25 * (double)ctas / h->num_sms;  // prefer at least two waves when K allows
+    const long long waves = (ctas + num_sms - 1) / num_sms;
+    double eff = (double)ctas / (double)(waves * num_sms);
+    if (waves < 2) eff *= 0.5 + 0.25 * (double)ctas / num_sms;  // prefer at least two waves when K allows
     const double score = eff - 1e-4 * ks;  // ties -> fewer splits (less partial traffic)
     if (score > best_score) {
       best_score = score;
@@ -786,11 +785,15 @@ void choose_split(qe_hpsi_handle* h) {
     }
     if (waves >= 16 && eff > 0.97) break;
   }
-  int kchunk = (h->npw + best - 1) / best;
-  kchunk = (kchunk + ZG_BK - 1) / ZG_BK * ZG_BK;
-  if (kchunk < ZG_BK) kchunk = ZG_BK;
-  h->kchunk = kchunk;
-  h->nsplit = std::max(1, (h->npw + kchunk - 1) / kchunk);
+  int kchunk = (klen + best - 1) / best;
+  kchunk = (kchunk + bk - 1) / bk * bk;
+  if (kchunk < bk) kchunk = bk;
+  *kchunk_out = kchunk;
+  *nsplit_out = std::max(1, (klen + kchunk - 1) / kchunk);
+}
+void choose_split(qe_hpsi_handle* h) {
+  const int ntile = ((h->nproj + ZgV0::BM - 1) / ZgV0::BM) * ((h->max_batch + ZgV0::BN - 1) / ZgV0::BN);
+  pick_split(ntile, h->npw, h->num_sms, ZgV0::BK, &h->kchunk, &h->nsplit);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda); looked up once, thread-safe
@@ -1301,7 +1304,18 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
   h->sym_m = M;
   h->sym_ldu = round_up(M, 8);
   h->sym_ldc2 = 2 * h->ldc;
-  h->sym_nsplit = std::max(1, (M + h->kchunk - 1) / h->kchunk);
+  {  // own split-K plan: 2 max_batch real columns on the tiles the symmetric kernels use, K = the half sphere
+    const int bn = h->sym_wide ? ZgS::BN : ZgV0::BN;
+    const int ntile = ((h->nproj + ZgS::BM - 1) / ZgS::BM) * ((2 * h->max_batch + bn - 1) / bn);
+    pick_split(ntile, M, h->num_sms, ZgS::BK, &h->sym_kchunk, &h->sym_nsplit);
+    const int forced = env_int("QE_HPSI_SYM_NSPLIT", 0);
+    if (forced > 0) {
+      int kc = (M + forced - 1) / forced;
+      kc = std::max((int)ZgS::BK, (kc + ZgS::BK - 1) / ZgS::BK * ZgS::BK);
+      h->sym_kchunk = kc;
+      h->sym_nsplit = std::max(1, (M + kc - 1) / kc);
+    }
+  }
   const size_t ub = sizeof(double2) * 2 * (size_t)h->max_batch * h->sym_ldu, eb = sizeof(double2) * 2 * (size_t)h->max_batch * h->ldp;
   const size_t pb = int8_path ? 16 : sizeof(double2) * (size_t)h->sym_nsplit * h->nproj * h->sym_ldc2;  // (the int8 path has its own)
   CR_TRY(guarded_malloc(h, &h->sym_u, ub));
@@ -1826,13 +1840,13 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
       using Cfg = decltype(cfg);
       const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (2 * nb + Cfg::BN - 1) / Cfg::BN;
       k_becp<Cfg, true><<<dim3(mt * nt, h->sym_nsplit), Cfg::NT, Cfg::SMEM_BECP, st>>>(h->beta, h->ldbeta, h->nproj, h->sym_u,
-                                                                                       h->sym_ldu, 2 * nb, h->sym_m, h->kchunk,
+                                                                                       h->sym_ldu, 2 * nb, h->sym_m, h->sym_kchunk,
                                                                                        h->sym_partial, h->sym_ldc2, nullptr, h->sym_cls);
     };
     if (h->sym_tma) {
       const int mt = (h->nproj + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
       k_becp_tma<ZgS, ZF_SYM><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(
-          h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr);
+          h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->sym_kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr);
     } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);
