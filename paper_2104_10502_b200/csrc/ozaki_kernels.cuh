@@ -116,6 +116,13 @@ k_oz_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const int q = blockIdx.x, mt = blockIdx.y, ks = ks_base + blockIdx.z;  // ks_base: a8 walks its K ranges launch by launch
   const int kb0 = ks * kchunk;
   const int nit = max(0, min(nkb, kb0 + kchunk) - kb0);
+  if constexpr (MODE == 4) {
+    // row tiles whose plane waves all belong to the other half of the sphere (minus = -1) have nothing to store: retire before
+    // any TMEM or pipeline set-up (see k_vnl_tma)
+    const long long r = (long long)mt * BM + threadIdx.x;
+    const bool dead = threadIdx.x >= BM || r >= mvalid || minus[r >> 1] == -1;
+    if (__syncthreads_and(dead)) return;
+  }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base)), "r"(TCOLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");

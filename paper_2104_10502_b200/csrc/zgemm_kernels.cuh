@@ -395,6 +395,11 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     nb = min(nb, *nb_dev);
     if (n0 >= nb) return;
   }
+  if constexpr (SYM) {  // row tiles with nothing to store retire at once (see k_vnl_tma)
+    const int r = m0 + (tid & (BM - 1));
+    const bool dead = tid >= BM || r >= npw || minus[r] == -1;
+    if (__syncthreads_and(dead)) return;
+  }
   const int nkt = (nproj + BK - 1) / BK;
   __shared__ __align__(8) unsigned long long mbar[2 * NSTAGE];
   const unsigned mb0 = mb_setup<NSTAGE, NT>(mbar);

@@ -205,6 +205,14 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     nb = min(nb, *nb_dev);
     if (n0 >= nb) return;
   }
+  if constexpr (FORM == ZF_SYM) {
+    // Row tiles whose entries all belong to the other half of the sphere (minus = -1: most of the n1 = 0, n2 < 0 half plane, a
+    // contiguous run in canonical order) would compute X, Y and store nothing: they retire here.  cfg 4: 98 of 6 074 tiles,
+    // which takes the launch from 41.04 waves of 148 CTAs to 40.4, i.e. one round less.
+    const int r = m0 + (tid & (BM - 1));
+    const bool dead = tid >= BM || r >= npw || minus[r] == -1;
+    if (__syncthreads_and(dead)) return;
+  }
   const int nkt = (nproj + BK - 1) / BK;
   const unsigned mb0 = mb_setup_tma<NSTAGE, NT>(mbar);
   const unsigned sm0 = static_cast<unsigned>(__cvta_generic_to_shared(sm));
