@@ -130,6 +130,7 @@ struct qe_hpsi_handle {
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
   int sym_nsplit = 1, sym_ldc2 = 0, sym_kchunk = 0;
+  int sym_dead0 = 0, sym_dead1 = 0;   // K tiles [dead0, dead1) of 16 rows of the half-sphere prefix hold rows of the other half only (U = 0 there)
   std::vector<unsigned char> sym_cls_host;  // copy of sym_cls for qe_hpsi_set_s
   bool sym_q_ok = false;                    // the q blocks of qe_hpsi_set_s couple equal classes only
   std::vector<int> blk_off;                 // atom block table (for the same check)
@@ -841,7 +842,7 @@ bool becp_tma_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, c
   if (!h->zg_tma || !make_map_f64(&tb, psi, 2LL * h->npw, nb, ldpsi * 16, 16, Cfg::BN, true)) return false;
   const int mt = (h->nproj + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
   k_becp_tma<Cfg, FORM><<<dim3(mt * nt, h->nsplit), Cfg::NT, Cfg::SMEM_BECP + 1024, st>>>(h->tm_g6_beta, tb, h->nproj, nb, h->npw, h->kchunk,
-                                                                                          partial, h->ldc, nullptr, nb_dev);
+                                                                                          partial, h->ldc, nullptr, nb_dev, 0, 0);
   return true;
 }
 template <class Cfg, int FORM>
@@ -1276,6 +1277,21 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
     minus[g] = (int)(it - idx.begin());
   }
   CR_TRY(upload(&h->sym_minus, minus, st));
+  {  // longest run of whole 16-row K tiles with minus = -1 only (the n1 = 0, n2 < 0 half plane): a6 skips it, U is zero there
+    int best0 = 0, best1 = 0, run0 = -1;
+    const int nt16 = M / ZgS::BK;
+    for (int t = 0; t <= nt16; ++t) {
+      bool dead = t < nt16;
+      for (int r = 0; dead && r < ZgS::BK; ++r) dead = minus[(size_t)t * ZgS::BK + r] == -1;
+      if (dead && run0 < 0) run0 = t;
+      if (!dead && run0 >= 0) {
+        if (t - run0 > best1 - best0) best0 = run0, best1 = t;
+        run0 = -1;
+      }
+    }
+    h->sym_dead0 = best0;
+    h->sym_dead1 = best1;
+  }
   CR_TRY(guarded_malloc(h, &h->sym_cls, (size_t)h->nproj));
   sym::k_sym_classify<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, M, h->sym_minus, h->sym_cls);
   std::vector<unsigned char> cls((size_t)h->nproj);
@@ -1846,7 +1862,8 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
     if (h->sym_tma) {
       const int mt = (h->nproj + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
       k_becp_tma<ZgS, ZF_SYM><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(
-          h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->sym_kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr);
+          h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->sym_kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr,
+          h->sym_dead0, h->sym_dead1);
     } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     becp_fp64(h, psi, ldpsi, nb, st, h->partial, nullptr);

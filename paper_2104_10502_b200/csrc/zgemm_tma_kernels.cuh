@@ -68,7 +68,7 @@ template <class Cfg, int FORM>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_becp_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nproj, int nb, int npw,
                int kchunk, double2* __restrict__ partial, int ldc, const unsigned char* __restrict__ cls,
-               const int* __restrict__ nb_dev) {
+               const int* __restrict__ nb_dev, int dead0, int dead1) {
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS;
   constexpr int STAGE = (BM + BN) * BK;  // complex elements per stage
@@ -87,7 +87,11 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   }
   const int ks = blockIdx.y;
   const int kb = ks * kchunk, ke = min(npw, kb + kchunk);  // kchunk is a multiple of BK: only the last slice has a ragged tile
-  const int nkt = (ke - kb + BK - 1) / BK;
+  // K tiles [dead0, dead1) (in units of BK entries) hold zeros in B (ZF_SYM: rows of the other half sphere, see k_vnl_tma): the
+  // slice walks [t0, ta) and [tb, t1) only.  Adding their exact zeros would not change a bit of the sums.
+  const int t0 = kb / BK, t1 = (ke + BK - 1) / BK;
+  const int ta = min(t1, max(t0, dead0)), tb = max(t0, min(t1, max(dead1, dead0)));
+  const int nk1 = ta - t0, nkt = nk1 + (t1 - tb);
   const unsigned mb0 = mb_setup_tma<NSTAGE, NT>(mbar);
   const unsigned sm0 = static_cast<unsigned>(__cvta_generic_to_shared(sm));
 
@@ -96,7 +100,7 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     const unsigned full = mb0 + 8 * st;
     const unsigned dst = sm0 + (unsigned)(st * STAGE * 16);
     mb_expect_tx(full, STAGE * 16);
-    const int k0 = 2 * (kb + kt * BK);
+    const int k0 = 2 * BK * (kt < nk1 ? t0 + kt : tb + (kt - nk1));
 #pragma unroll
     for (int hf = 0; hf < 2; ++hf) {
       tma_load_2d(dst + (unsigned)(hf * BM * 128), &tmA, k0 + 16 * hf, m0, full);
