@@ -462,7 +462,7 @@ def int8_roofline(leg, stage, m, mp, hbm_peak, dmma, args, value, world):
                 "traffic": committed_traffic(args.config, tkey) if oz_s == 6 else (committed_traffic(args.config, tkey + "_s7") if oz_s == 7 and gsym else None),
                 "peak_source": "int8 dense = 2 x MEASURED_PEAKS.json bf16_tflops_sustained (guide's nominal int8 : bf16 ratio; the "
                 "kernel runs inside a long, power-capped step). Against the chip's measured int8 burst (register-free UTCIMMA loop, "
-                "4540 TOP/s, profiles/r1g_int8.md) the same kernel is at " + f"{ach / 4540.0:.2f}" + "; ncu (profiles/r2g_capture.md): tensor pipe 36-50 % active", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
+                "4540 TOP/s, profiles/r1g_int8.md) the same kernel is at " + f"{ach / 4540.0:.2f}" + "; ncu (profiles/r2l_capture.md): tensor pipe 67-82 % of active cycles", "ms_per_launch": t_k, "ops_per_launch": ops_launch, "digits": oz_s,
                 "digit_pairs": pairs, "fp64_equivalent_tflops": flops_launch / (t_k * 1e-3) * 1e-12,
                 "digit_kernels_ms_per_launch": stage["a6_a8_int8_digits"][0]}
     units = (0.75 if m3 >= 1 else 1.0) + (0.75 if m3 == 2 else 1.0)  # integer 3M forms: 6 of the 8 tile-GEMM units each
