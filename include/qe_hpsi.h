@@ -45,7 +45,8 @@ typedef struct qe_hpsi_handle* qe_hpsi_t;
 
 typedef enum {
   QE_HPSI_OK = 0,
-  QE_HPSI_EINVAL = -1, /* null pointer, negative size, ld < npw, psi aliases hpsi, bad block table, bad flags */
+  QE_HPSI_EINVAL = -1, /* null pointer, negative size, ld < npw, psi aliases hpsi, bad block table, bad flags, */
+                       /* complex128 array not 16-byte aligned                                            */
   QE_HPSI_EGRID = -2,  /* N_j has a prime factor other than 2,3,5, exceeds QE_HPSI_MAX_N, or is smaller  */
                        /* than the sphere's index extent along j (the sphere itself would wrap)          */
   QE_HPSI_ENOMEM = -3, /* host or device allocation failed (including the digit planes of QE_HPSI_PROJ_INT8) */

@@ -1757,6 +1757,8 @@ int check_apply_args(qe_hpsi_t h, const void* psi, int64_t ldpsi, void* hpsi, in
   if (nbands < 0) return QE_HPSI_EINVAL;
   if (nbands == 0) return QE_HPSI_OK;
   if (!psi || !hpsi || ldpsi < h->npw || ldhpsi < h->npw) return QE_HPSI_EINVAL;
+  // complex128 rows are moved in 16-byte units (cp.async, TMA, double2 loads): a pointer that is only 8-byte aligned is an error
+  if ((reinterpret_cast<uintptr_t>(psi) | reinterpret_cast<uintptr_t>(hpsi)) & 15u) return QE_HPSI_EINVAL;
   const char* a0 = static_cast<const char*>(psi);
   const char* a1 = a0 + ((size_t)(nbands - 1) * ldpsi + h->npw) * sizeof(double2);
   const char* b0 = static_cast<const char*>(hpsi);

@@ -437,6 +437,16 @@ def test_argument_errors():
     assert e.value.status == qe_hpsi.QE_HPSI_EINVAL
     out = h.apply(torch.zeros((0, h.npw), dtype=torch.complex128, device="cuda"))  # empty input is fine
     assert out.shape[0] == 0
+    # a complex128 array that is only 8-byte aligned (a view into a float64 buffer at an odd offset)
+    import ctypes
+    big = torch.zeros((3, h.npw + 8), dtype=torch.complex128, device="cuda")
+    out2 = torch.zeros_like(big)
+    lib = qe_hpsi.load_library()
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = lib.qe_hpsi_apply(h._h, ctypes.c_void_p(big.data_ptr() + 8), h.npw + 8, ctypes.c_void_p(out2.data_ptr()), h.npw + 8, 2, st)
+    assert rc == qe_hpsi.QE_HPSI_EINVAL
+    rc = lib.qe_hpsi_apply(h._h, ctypes.c_void_p(big.data_ptr()), h.npw + 8, ctypes.c_void_p(out2.data_ptr() + 8), h.npw + 8, 2, st)
+    assert rc == qe_hpsi.QE_HPSI_EINVAL
     h.destroy()
 
 
