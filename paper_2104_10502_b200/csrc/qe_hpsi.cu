@@ -130,6 +130,10 @@ struct qe_hpsi_handle {
   double2 *sym_u = nullptr, *sym_e = nullptr, *sym_partial = nullptr;  // [2 max_batch][sym_ldu], [2 max_batch][ldp], [nsplit][nproj][ldc2]
   long long sym_ldu = 0;
   int sym_nsplit = 1, sym_ldc2 = 0, sym_kchunk = 0;
+  int* sym_live = nullptr;            // row tiles (64 rows) of the half-sphere prefix that have at least one row to store, ascending
+  int sym_nlive = 0;
+  CUtensorMap tm_a8_e64;              // E with 64-row boxes: the last partial wave of the symmetric a8 runs on 64 x 64 tiles
+  bool sym_tail = false;
   int sym_dead0 = 0, sym_dead1 = 0;   // K tiles [dead0, dead1) of 16 rows of the half-sphere prefix hold rows of the other half only (U = 0 there)
   std::vector<unsigned char> sym_cls_host;  // copy of sym_cls for qe_hpsi_set_s
   bool sym_q_ok = false;                    // the q blocks of qe_hpsi_set_s couple equal classes only
@@ -599,6 +603,7 @@ cudaError_t set_kernel_attrs() {
   SET_ZT(ZgV0, ZF_GAMMA);
   SET_ZT(ZgS, ZF_GAMMA);
   SET_ZT(ZgS, ZF_SYM);
+  SET_ZT(ZgV0, ZF_SYM);
 #undef SET_ZT
   e = cudaFuncSetAttribute(k_vnl_add<ZgV0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZgV0::SMEM_VNL);
   if (e != cudaSuccess) return e;
@@ -721,6 +726,7 @@ extern "C" int qe_hpsi_destroy(qe_hpsi_t h) {
   cudaFree(h->oz_eb);
   cudaFree(h->oz_partial);
   cudaFree(h->sym_minus);
+  cudaFree(h->sym_live);
   cudaFree(h->sym_cls);
   cudaFree(h->sym_cmask);
   cudaFree(h->sym_u);
@@ -1292,6 +1298,17 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
     h->sym_dead0 = best0;
     h->sym_dead1 = best1;
   }
+  {  // row tiles of the symmetric a8 that store something
+    std::vector<int> live;
+    for (int t = 0; t * ZgS::BM < M; ++t) {
+      bool any = false;
+      for (int r = t * ZgS::BM; !any && r < std::min(M, (t + 1) * ZgS::BM); ++r) any = minus[(size_t)r] != -1;
+      if (any) live.push_back(t);
+    }
+    h->sym_nlive = (int)live.size();
+    CR_TRY(upload(&h->sym_live, live, st));
+    CR_TRY(cudaStreamSynchronize(st));  // live leaves scope
+  }
   CR_TRY(guarded_malloc(h, &h->sym_cls, (size_t)h->nproj));
   sym::k_sym_classify<<<h->nproj, 256, 0, st>>>(h->beta, h->ldbeta, M, h->sym_minus, h->sym_cls);
   std::vector<unsigned char> cls((size_t)h->nproj);
@@ -1348,6 +1365,8 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
                  make_map_f64(&h->tm_a6_u, h->sym_u, 2LL * M, 2LL * h->max_batch, h->sym_ldu * 16, 16, ZgS::BN, true) &&
                  make_map_f64(&h->tm_a8_beta, h->beta, 2LL * M, h->nproj, rb, 2 * ZgS::LDA_M, ZgS::BK) &&
                  make_map_f64(&h->tm_a8_e, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgS::BN);
+    h->sym_tail = h->sym_tma && env_int("QE_HPSI_SYM_TAIL", 1) &&
+                  make_map_f64(&h->tm_a8_e64, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgV0::BN);
   }
 #undef CR_TRY
   return cudaSuccess;
@@ -1894,6 +1913,16 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
   return QE_HPSI_OK;
 }
 
+// symmetric a8 on the TMA kernels: number of live row tiles the 64 x 128 launch takes; the rest (the last, partly filled wave)
+// goes to a second launch on 64 x 64 tiles.  All of them when there is no tail worth splitting off.
+int sym_a8_main_tiles(qe_hpsi_t h, int nb) {
+  const int nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
+  const long long units = (long long)h->sym_nlive * nt;
+  const long long full = units / h->num_sms * h->num_sms, rem = units - full;
+  if (!h->sym_tail || full < 4LL * h->num_sms || rem == 0 || rem * 10 > 7LL * h->num_sms) return h->sym_nlive;
+  return (int)(full / nt);
+}
+
 // a8
 int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st) {
   // Gamma-symmetric mode: the real coefficient rows of D becp are in sym_e already (launch_becp); for the q-term of
@@ -1936,10 +1965,19 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
                                                                                         h->sym_cmask, h->sym_minus);
     };
     if (h->sym_tma) {
-      const int mt = (h->sym_m + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
-      if (mt > 0)
-        k_vnl_tma<ZgS, ZF_SYM><<<(unsigned)(mt * nt), ZgS::NT, ZgS::SMEM_VNL, st>>>(h->tm_a8_beta, h->tm_a8_e, h->nproj, h->sym_m, 2 * nb,
-                                                                                    hpsi, ldh, nullptr, h->sym_cmask, h->sym_minus, 0);
+      // live row tiles only; the last, partly filled wave of 64 x 128 tiles runs as 64 x 64 tiles instead (same sums, half the
+      // time of that round)
+      const int nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
+      const int ma = sym_a8_main_tiles(h, nb);
+      if (ma > 0)
+        k_vnl_tma<ZgS, ZF_SYM><<<(unsigned)(ma * nt), ZgS::NT, ZgS::SMEM_VNL, st>>>(h->tm_a8_beta, h->tm_a8_e, h->nproj, h->sym_m, 2 * nb,
+                                                                                    hpsi, ldh, nullptr, h->sym_cmask, h->sym_minus, 0,
+                                                                                    h->sym_live, 0);
+      if (ma < h->sym_nlive) {
+        const int nt64 = (2 * nb + ZgV0::BN - 1) / ZgV0::BN;
+        k_vnl_tma<ZgV0, ZF_SYM><<<(unsigned)((h->sym_nlive - ma) * nt64), ZgV0::NT, ZgV0::SMEM_VNL, st>>>(
+            h->tm_a8_beta, h->tm_a8_e64, h->nproj, h->sym_m, 2 * nb, hpsi, ldh, nullptr, h->sym_cmask, h->sym_minus, 0, h->sym_live, ma);
+      }
     } else if (h->sym_wide) go(ZgS{}); else go(ZgV0{});
   } else
     vnl_fp64(h, bT, hpsi, ldh, nb, st, nullptr);
@@ -2710,7 +2748,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 : 4);
+    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 + (h->sym_tma && sym_a8_main_tiles(h, nb) < h->sym_nlive ? 1 : 0) : 4);
     if (h->nproj > 0 && h->oz_s && h->sym) total += 2;  // merge and coefficient kernels of the symmetric real forms
     if (h->certify) total += 8;  // probe, decide, gather, the four FP64 kernels (empty grids when nothing failed), commit
   }

@@ -191,7 +191,7 @@ template <class Cfg, int FORM>
 __global__ void __launch_bounds__(Cfg::NT, 1)
     k_vnl_tma(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int nproj, int npw, int nb,
               double2* __restrict__ hpsi, long long ldh, const int* __restrict__ nb_dev, const unsigned* __restrict__ cmask,
-              const int* __restrict__ minus, int overwrite) {
+              const int* __restrict__ minus, int overwrite, const int* __restrict__ live = nullptr, int live0 = 0) {
   static_assert(FORM != ZF_SYM || Cfg::BK == 16, "cmask holds one 16-bit class mask per K tile of 16 projectors");
   constexpr int BM = Cfg::BM, BN = Cfg::BN, WM = Cfg::WM, WN = Cfg::WN, BK = Cfg::BK, NSTAGE = Cfg::NSTAGE;
   constexpr int NT = Cfg::NT, TM = Cfg::TM, TN = Cfg::TN, KSTEPS = Cfg::KSTEPS, LDA = Cfg::LDA_M;
@@ -204,15 +204,17 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / WN) * (BM / WM), wn0 = (warp % WN) * (BN / WN);
   const int ntn = (nb + BN - 1) / BN;
-  const int m0 = (blockIdx.x / ntn) * BM, n0 = (blockIdx.x % ntn) * BN;
+  // live != nullptr (ZF_SYM): row tile number live0 + blockIdx.x / ntn of the list of tiles that have something to store
+  const int m0 = (live ? live[live0 + blockIdx.x / ntn] : (int)(blockIdx.x / ntn)) * BM, n0 = (blockIdx.x % ntn) * BN;
   if (nb_dev) {  // see k_becp
     nb = min(nb, *nb_dev);
     if (n0 >= nb) return;
   }
-  if constexpr (FORM == ZF_SYM) {
+  if (FORM == ZF_SYM && live == nullptr) {
     // Row tiles whose entries all belong to the other half of the sphere (minus = -1: most of the n1 = 0, n2 < 0 half plane, a
-    // contiguous run in canonical order) would compute X, Y and store nothing: they retire here.  cfg 4: 98 of 6 074 tiles,
-    // which takes the launch from 41.04 waves of 148 CTAs to 40.4, i.e. one round less.
+    // contiguous run in canonical order) would compute X, Y and store nothing: they retire here (or are not launched at all
+    // when the host passes the list of live tiles).  cfg 4: 98 of 6 074 tiles, which takes the launch from 41.04 waves of
+    // 148 CTAs to 40.4, i.e. one round less.
     const int r = m0 + (tid & (BM - 1));
     const bool dead = tid >= BM || r >= npw || minus[r] == -1;
     if (__syncthreads_and(dead)) return;
