@@ -799,7 +799,9 @@ void pick_split(int ntile, int klen, int num_sms, int bk, int* kchunk_out, int* 
   *nsplit_out = std::max(1, (klen + kchunk - 1) / kchunk);
 }
 void choose_split(qe_hpsi_handle* h) {
-  const int ntile = ((h->nproj + ZgV0::BM - 1) / ZgV0::BM) * ((h->max_batch + ZgV0::BN - 1) / ZgV0::BN);
+  // the Gamma-only handle contracts more than 64 bands on 64 x 128 tiles
+  const int bn = (h->gamma && h->max_batch > ZgV0::BN) ? ZgS::BN : ZgV0::BN;
+  const int ntile = ((h->nproj + ZgV0::BM - 1) / ZgV0::BM) * ((h->max_batch + bn - 1) / bn);
   pick_split(ntile, h->npw, h->num_sms, ZgV0::BK, &h->kchunk, &h->nsplit);
 }
 
@@ -852,13 +854,15 @@ bool becp_tma_launch(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, c
   return true;
 }
 template <class Cfg, int FORM>
-bool vnl_tma_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev) {
+bool vnl_tma_launch(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh, int nb, cudaStream_t st, const int* nb_dev,
+                    int mt0 = 0, int mt1 = -1) {  // row tiles [mt0, mt1) of Cfg::BM rows; mt1 < 0: to the end
   CUtensorMap tb;
   if (!h->zg_tma || !make_map_f64(&tb, bT, 2LL * h->nproj, nb, (long long)h->ldp * 16, 8, Cfg::BN)) return false;
   const int mt = (h->npw + Cfg::BM - 1) / Cfg::BM, nt = (nb + Cfg::BN - 1) / Cfg::BN;
-  if (mt > 0)
-    k_vnl_tma<Cfg, FORM><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->tm_g8_beta, tb, h->nproj, h->npw, nb, hpsi, ldh, nb_dev,
-                                                                              nullptr, nullptr, 0);
+  if (mt1 < 0) mt1 = mt;
+  if (mt1 > mt0)
+    k_vnl_tma<Cfg, FORM><<<(unsigned)((mt1 - mt0) * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->tm_g8_beta, tb, h->nproj, h->npw, nb, hpsi, ldh,
+                                                                                       nb_dev, nullptr, nullptr, 0, nullptr, mt0);
   return true;
 }
 
@@ -1953,7 +1957,13 @@ int launch_vnl_add(qe_hpsi_t h, const double2* bT, double2* hpsi, long long ldh,
         k_vnl_add<Cfg, true><<<(unsigned)(mt * nt), Cfg::NT, Cfg::SMEM_VNL, st>>>(h->beta, h->ldbeta, h->nproj, h->npw, bT,
                                                                                   h->ldp, nb, hpsi, ldh);
     };
-    if (nb > 64) go(ZgS{}); else go(ZgV0{});
+    // 64 x 128 tiles from 65 bands on; a partly filled last wave of them runs on 64 x 64 tiles (see the symmetric form below)
+    const int mtg = (h->npw + ZgS::BM - 1) / ZgS::BM, ntg = (nb + ZgS::BN - 1) / ZgS::BN;
+    const long long ug = (long long)mtg * ntg, fullg = ug / h->num_sms * h->num_sms, remg = ug - fullg;
+    if (nb > 64 && h->zg_tma && fullg >= 4LL * h->num_sms && remg > 0 && remg * 10 <= 7LL * h->num_sms &&
+        vnl_tma_launch<ZgS, ZF_GAMMA>(h, bT, hpsi, ldh, nb, st, nullptr, 0, (int)(fullg / ntg))) {
+      if (!vnl_tma_launch<ZgV0, ZF_GAMMA>(h, bT, hpsi, ldh, nb, st, nullptr, (int)(fullg / ntg), mtg)) return QE_HPSI_ECUDA;
+    } else if (nb > 64) go(ZgS{}); else go(ZgV0{});
   } else if (use_sym) {
     // symmetric a8: X = sum_p b_p Re e_p, Y = sum_p b_p Im e_p over the half sphere; hpsi(G) += X + iY, hpsi(-G) += conj X + i conj Y
     auto go = [&](auto cfg) {

@@ -204,8 +204,9 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm0 = (warp / WN) * (BM / WM), wn0 = (warp % WN) * (BN / WN);
   const int ntn = (nb + BN - 1) / BN;
-  // live != nullptr (ZF_SYM): row tile number live0 + blockIdx.x / ntn of the list of tiles that have something to store
-  const int m0 = (live ? live[live0 + blockIdx.x / ntn] : (int)(blockIdx.x / ntn)) * BM, n0 = (blockIdx.x % ntn) * BN;
+  // row tile live0 + blockIdx.x / ntn, taken from the list of tiles that have something to store when there is one (ZF_SYM)
+  const int mtile = live0 + (int)(blockIdx.x / ntn);
+  const int m0 = (live ? live[mtile] : mtile) * BM, n0 = (blockIdx.x % ntn) * BN;
   if (nb_dev) {  // see k_becp
     nb = min(nb, *nb_dev);
     if (n0 >= nb) return;
