@@ -533,6 +533,41 @@ def test_x_stage_quarter_pruning(n, monkeypatch):
     h0.destroy()
 
 
+def test_handles_created_and_applied_from_two_host_threads():
+    """Two host threads, each with its own stream and handle (per-device kernel attributes under a mutex, the tensor-map
+    encoder looked up once, maps of psi encoded per call): same bits as the single-threaded result."""
+    import threading
+    h0, inp = _gpu.make(1)
+    psi = _gpu.gen_psi_dev(inp, 0, 24)
+    ref = h0.apply(psi).clone()
+    torch.cuda.synchronize()
+    h0.destroy()
+    results, errors = {}, []
+
+    def work(tag, flags):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for _ in range(3):
+                    h, _ = _gpu.make(1, flags=flags, beta=inp["beta"])
+                    out = h.apply(psi)
+                    st.synchronize()
+                    h.destroy()
+                results[tag] = out
+        except Exception as e:  # noqa: BLE001
+            errors.append((tag, repr(e)))
+
+    ts = [threading.Thread(target=work, args=("sym", 0)), threading.Thread(target=work, args=("gen", qe_hpsi.QE_HPSI_NO_GAMMA_SYM))]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errors, errors
+    assert torch.equal(results["sym"].view(torch.float64), ref.view(torch.float64))
+    npw = inp["miller"].shape[0]
+    assert _gpu.rel_l2(results["gen"].cpu().numpy()[:, :npw], ref.cpu().numpy()[:, :npw]).max() <= 1e-13
+
+
 def test_apply_can_be_captured_in_a_cuda_graph():
     """qe_hpsi_apply enqueues kernels only (no allocation, no host sync): it can be stream-captured and replayed, which
     is how a launch-latency-bound caller (config 0: 9 launches for 16 bands) should drive it. Replays must reproduce the
