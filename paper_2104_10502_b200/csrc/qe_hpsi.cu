@@ -132,7 +132,8 @@ struct qe_hpsi_handle {
   int sym_nsplit = 1, sym_ldc2 = 0, sym_kchunk = 0;
   int* sym_live = nullptr;            // row tiles (64 rows) of the half-sphere prefix that have at least one row to store, ascending
   int sym_nlive = 0;
-  CUtensorMap tm_a8_e64;              // E with 64-row boxes: the last partial wave of the symmetric a8 runs on 64 x 64 tiles
+  CUtensorMap tm_a8_e64, tm_a6_u64;   // E / U with 64-row boxes: the last partial wave of the symmetric a8, and calls of at most
+                                      // 32 bands (64 real columns), run on 64 x 64 tiles
   bool sym_tail = false;
   int sym_dead0 = 0, sym_dead1 = 0;   // K tiles [dead0, dead1) of 16 rows of the half-sphere prefix hold rows of the other half only (U = 0 there)
   std::vector<unsigned char> sym_cls_host;  // copy of sym_cls for qe_hpsi_set_s
@@ -1370,7 +1371,8 @@ cudaError_t setup_symmetric(qe_hpsi_handle* h, const std::vector<int>& idx, cons
                  make_map_f64(&h->tm_a8_beta, h->beta, 2LL * M, h->nproj, rb, 2 * ZgS::LDA_M, ZgS::BK) &&
                  make_map_f64(&h->tm_a8_e, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgS::BN);
     h->sym_tail = h->sym_tma && env_int("QE_HPSI_SYM_TAIL", 1) &&
-                  make_map_f64(&h->tm_a8_e64, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgV0::BN);
+                  make_map_f64(&h->tm_a8_e64, h->sym_e, 2LL * h->nproj, 2LL * h->max_batch, (long long)h->ldp * 16, 8, ZgV0::BN) &&
+                  make_map_f64(&h->tm_a6_u64, h->sym_u, 2LL * M, 2LL * h->max_batch, h->sym_ldu * 16, 16, ZgV0::BN, true);
   }
 #undef CR_TRY
   return cudaSuccess;
@@ -1884,7 +1886,12 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
                                                                                        h->sym_ldu, 2 * nb, h->sym_m, h->sym_kchunk,
                                                                                        h->sym_partial, h->sym_ldc2, nullptr, h->sym_cls);
     };
-    if (h->sym_tma) {
+    if (h->sym_tma && h->sym_tail && 2 * nb <= ZgV0::BN) {  // at most 32 bands: one 64-column tile instead of a half-empty 128-column one
+      const int mt = (h->nproj + ZgV0::BM - 1) / ZgV0::BM;
+      k_becp_tma<ZgV0, ZF_SYM><<<dim3(mt, h->sym_nsplit), ZgV0::NT, ZgV0::SMEM_BECP + 1024, st>>>(
+          h->tm_a6_beta, h->tm_a6_u64, h->nproj, 2 * nb, h->sym_m, h->sym_kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr,
+          h->sym_dead0, h->sym_dead1);
+    } else if (h->sym_tma) {
       const int mt = (h->nproj + ZgS::BM - 1) / ZgS::BM, nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
       k_becp_tma<ZgS, ZF_SYM><<<dim3(mt * nt, h->sym_nsplit), ZgS::NT, ZgS::SMEM_BECP + 1024, st>>>(
           h->tm_a6_beta, h->tm_a6_u, h->nproj, 2 * nb, h->sym_m, h->sym_kchunk, h->sym_partial, h->sym_ldc2, h->sym_cls, nullptr,
@@ -1920,6 +1927,7 @@ int launch_becp(qe_hpsi_t h, const double2* psi, long long ldpsi, int nb, cudaSt
 // symmetric a8 on the TMA kernels: number of live row tiles the 64 x 128 launch takes; the rest (the last, partly filled wave)
 // goes to a second launch on 64 x 64 tiles.  All of them when there is no tail worth splitting off.
 int sym_a8_main_tiles(qe_hpsi_t h, int nb) {
+  if (h->sym_tail && 2 * nb <= ZgV0::BN) return 0;  // at most 32 bands: every tile on 64 x 64
   const int nt = (2 * nb + ZgS::BN - 1) / ZgS::BN;
   const long long units = (long long)h->sym_nlive * nt;
   const long long full = units / h->num_sms * h->num_sms, rem = units - full;
@@ -2693,13 +2701,15 @@ extern "C" int qe_hpsi_apply_host(qe_hpsi_t h, const void* psi_host, int64_t ldp
   // chunks of max_batch bands, except that the first and the last chunk are halved (down to a 64-band ZGEMM tile) when
   // there are several: the H2D copy of the first chunk and the D2H copy of the last one are the only transfers that do
   // not overlap compute
-  const int half = (h->max_batch >= 128 && nbands > h->max_batch) ? (h->max_batch / 2 + 63) / 64 * 64 : h->max_batch;
+  // (32 bands where the projector kernels have a 64-column tile for them: the Gamma-symmetric TMA kernels; else 64)
+  const int small = (h->sym_tma && h->sym_tail) ? 32 : 64;
+  const int half = (h->max_batch >= 128 && nbands > h->max_batch) ? small : h->max_batch;
   int ci = 0;
   for (int b0 = 0, nb = 0; b0 < nbands; b0 += nb, ++ci) {
     const int left = nbands - b0;
     nb = std::min(h->max_batch, left);
     if (ci == 0) nb = std::min(half, left);
-    else if (left > h->max_batch && left < h->max_batch + half) nb = left - half;  // leave exactly `half` for the last chunk
+    else if (left > half && left < h->max_batch + half) nb = std::min(h->max_batch, left - half);  // leave exactly `half` for the last chunk
     const int u = ci & 1;
     if (ci >= 2) CU_TRY(h, cudaStreamWaitEvent(h->st_in, h->ev_comp[u], 0));  // compute of chunk ci-2 read psi buf u
     if (width)
@@ -2758,7 +2768,7 @@ extern "C" int64_t qe_hpsi_launch_count(qe_hpsi_t h, int nbands) {
   for (int b0 = 0; b0 < nbands; b0 += h->max_batch) {
     const int nb = std::min(h->max_batch, nbands - b0);
     total += 5 * (int64_t)((nb + h->fft_nb - 1) / h->fft_nb);
-    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 + (h->sym_tma && sym_a8_main_tiles(h, nb) < h->sym_nlive ? 1 : 0) : 4);
+    if (h->nproj > 0) total += h->oz_s ? 7 + (h->oz_3m ? 2 : 0) + (h->oz_3m8 ? 1 : (int)((h->oz_k2 / oz::KB + h->oz_kchunk2 - 1) / h->oz_kchunk2)) : (h->sym ? 6 + (h->sym_tma && sym_a8_main_tiles(h, nb) > 0 && sym_a8_main_tiles(h, nb) < h->sym_nlive ? 1 : 0) : 4);
     if (h->nproj > 0 && h->oz_s && h->sym) total += 2;  // merge and coefficient kernels of the symmetric real forms
     if (h->certify) total += 8;  // probe, decide, gather, the four FP64 kernels (empty grids when nothing failed), commit
   }
